@@ -1,0 +1,204 @@
+"""ctypes binding of liboracle.so (TEST INFRASTRUCTURE; see tpcca_oracle.cpp header)."""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+
+import numpy as np
+
+from . import build as _build
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("n_rows", C.c_int32),
+        ("row_x", _dp), ("grid_y_lo", _dp), ("grid_inv_bin_y", _dp), ("grid_ny", _ip),
+        ("grid_z_lo", C.c_double), ("grid_inv_bin_z", _dp), ("grid_nz", _ip),
+        ("nf_hy_up", _dp), ("nf_hz_up", _dp), ("nf_hy_dn", _dp), ("nf_hz_dn", _dp), ("nf_cut", _dp),
+        ("kappa_per_qpt", C.c_double), ("err2_y", C.c_double), ("err2_z", C.c_double),
+        ("init_cov", C.c_double * 5),
+        ("tc_win_y", C.c_double), ("tc_win_z", C.c_double), ("tc_gate", C.c_double),
+        ("max_sinphi", C.c_double), ("grid_margin", C.c_double),
+        ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32),
+    ]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(_build.build())
+        lib.oracle_create.restype = C.c_void_p
+        lib.oracle_create.argtypes = [C.POINTER(_Params), C.c_int]
+        lib.oracle_destroy.argtypes = [C.c_void_p]
+        lib.oracle_load.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.oracle_run.argtypes = [C.c_void_p, C.c_uint32, C.c_int]
+        lib.oracle_sizes.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+        lib.oracle_get_grid.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        lib.oracle_get_links.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+        lib.oracle_get_tracks.argtypes = [C.c_void_p] + [C.c_void_p] * 8
+        lib.oracle_kf_propagate.argtypes = [C.c_void_p, _dp, C.c_double]
+        lib.oracle_kf_propagate.restype = C.c_int
+        lib.oracle_kf_update.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
+        lib.oracle_kf_dist2.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
+        lib.oracle_kf_dist2.restype = C.c_double
+        lib.oracle_score.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 6
+        lib.oracle_score.restype = C.c_double
+        _lib = lib
+    return _lib
+
+
+@dataclasses.dataclass
+class OracleResult:
+    """Outputs of one sector.  Index space: sorted positions (after S1); order: sorted -> original."""
+    n: int
+    order: np.ndarray = None
+    sy: np.ndarray = None
+    sz: np.ndarray = None
+    bin_start: np.ndarray = None
+    row_start: np.ndarray = None
+    link_up_raw: np.ndarray = None
+    link_dn_raw: np.ndarray = None
+    link_up: np.ndarray = None
+    link_dn: np.ndarray = None
+    start_hit: np.ndarray = None
+    x_ref: np.ndarray = None
+    z_ref: np.ndarray = None
+    par: np.ndarray = None       # [n_tracks, 5]
+    cov: np.ndarray = None       # [n_tracks, 15]
+    chi2: np.ndarray = None
+    n_hits: np.ndarray = None
+    n_fit: np.ndarray = None
+    first_row: np.ndarray = None
+    last_row: np.ndarray = None
+    trk_start_hit: np.ndarray = None
+    hit_offset: np.ndarray = None
+    hit_idx: np.ndarray = None
+
+    @property
+    def n_tracks(self) -> int:
+        return 0 if self.x_ref is None else int(self.x_ref.shape[0])
+
+
+def _d(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+class Oracle:
+    """One oracle instance = one set of tables; `run` processes one sector."""
+
+    def __init__(self, params, precision: str = "f32"):
+        lib = _load()
+        self._lib = lib
+        self.precision = {"f32": 0, "f64": 1}[precision]
+        self.n_rows = int(params.n_rows)
+        self._keep = dict(
+            row_x=_d(params.row_x), grid_y_lo=_d(params.grid_y_lo),
+            grid_inv_bin_y=_d(params.grid_inv_bin_y), grid_inv_bin_z=_d(params.grid_inv_bin_z),
+            nf_hy_up=_d(params.nf_hy_up), nf_hz_up=_d(params.nf_hz_up),
+            nf_hy_dn=_d(params.nf_hy_dn), nf_hz_dn=_d(params.nf_hz_dn), nf_cut=_d(params.nf_cut),
+            grid_ny=np.ascontiguousarray(params.grid_ny, dtype=np.int32),
+            grid_nz=np.ascontiguousarray(params.grid_nz, dtype=np.int32))
+        k = self._keep
+        p = _Params()
+        p.n_rows = self.n_rows
+        for name in ("row_x", "grid_y_lo", "grid_inv_bin_y", "grid_inv_bin_z", "nf_hy_up", "nf_hz_up",
+                     "nf_hy_dn", "nf_hz_dn", "nf_cut"):
+            setattr(p, name, k[name].ctypes.data_as(_dp))
+        p.grid_ny = k["grid_ny"].ctypes.data_as(_ip)
+        p.grid_nz = k["grid_nz"].ctypes.data_as(_ip)
+        p.grid_z_lo = float(params.grid_z_lo)
+        p.kappa_per_qpt = float(params.kappa_per_qpt)
+        p.err2_y = float(params.err2_y)
+        p.err2_z = float(params.err2_z)
+        for i in range(5):
+            p.init_cov[i] = float(params.init_cov[i])
+        p.tc_win_y = float(params.tc_win_y); p.tc_win_z = float(params.tc_win_z)
+        p.tc_gate = float(params.tc_gate); p.max_sinphi = float(params.max_sinphi)
+        p.grid_margin = float(params.grid_margin)
+        p.tc_max_gap = int(params.tc_max_gap); p.tc_min_hits = int(params.tc_min_hits)
+        self._h = lib.oracle_create(C.byref(p), self.precision)
+        if not self._h:
+            raise RuntimeError("oracle_create failed")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    # ------------------------------------------------------------------------------
+    def run(self, y, z, row, stage_mask: int = 0x1F, brute: bool = False, want=("grid", "links", "tracks")) -> OracleResult:
+        ft = np.float32 if self.precision == 0 else np.float64
+        y = np.ascontiguousarray(y, dtype=ft)
+        z = np.ascontiguousarray(z, dtype=ft)
+        row = np.ascontiguousarray(row, dtype=np.uint16)
+        n = int(y.shape[0])
+        rc = self._lib.oracle_load(self._h, n, y.ctypes.data, z.ctypes.data, row.ctypes.data)
+        if rc != 0:
+            raise ValueError(f"oracle_load failed: {rc}")
+        self._lib.oracle_run(self._h, stage_mask, int(brute))
+        sizes = (C.c_int64 * 5)()
+        self._lib.oracle_sizes(self._h, sizes)
+        _, n_start, n_trk, n_hit, n_bins = (int(v) for v in sizes)
+        res = OracleResult(n=n)
+        if "grid" in want and (stage_mask & 1):
+            res.order = np.empty(n, np.int32); res.sy = np.empty(n, np.float64); res.sz = np.empty(n, np.float64)
+            res.bin_start = np.empty(n_bins + 1, np.uint32); res.row_start = np.empty(self.n_rows + 1, np.int32)
+            self._lib.oracle_get_grid(self._h, res.order.ctypes.data, res.sy.ctypes.data, res.sz.ctypes.data,
+                                      res.bin_start.ctypes.data, res.row_start.ctypes.data)
+        if "links" in want:
+            def arr(cond):
+                return np.empty(n, np.int32) if cond else None
+            res.link_up_raw = arr(stage_mask & 2); res.link_dn_raw = arr(stage_mask & 2)
+            res.link_up = arr(stage_mask & 4); res.link_dn = arr(stage_mask & 4)
+            res.start_hit = np.empty(n_start, np.int32) if (stage_mask & 8) else None
+            ptr = lambda a: a.ctypes.data if a is not None else None
+            self._lib.oracle_get_links(self._h, ptr(res.link_up_raw), ptr(res.link_dn_raw), ptr(res.link_up),
+                                       ptr(res.link_dn), ptr(res.start_hit))
+        if "tracks" in want and (stage_mask & 16):
+            res.x_ref = np.empty(n_trk); res.z_ref = np.empty(n_trk); res.chi2 = np.empty(n_trk)
+            res.par = np.empty((n_trk, 5)); res.cov = np.empty((n_trk, 15))
+            ints = np.empty((n_trk, 5), np.int32)
+            res.hit_offset = np.empty(n_trk + 1, np.int32); res.hit_idx = np.empty(n_hit, np.int32)
+            self._lib.oracle_get_tracks(self._h, res.x_ref.ctypes.data, res.z_ref.ctypes.data, res.par.ctypes.data,
+                                        res.cov.ctypes.data, res.chi2.ctypes.data, ints.ctypes.data,
+                                        res.hit_offset.ctypes.data, res.hit_idx.ctypes.data)
+            res.n_hits, res.n_fit, res.first_row, res.last_row, res.trk_start_hit = (
+                np.ascontiguousarray(ints[:, i]) for i in range(5))
+        return res
+
+    # ---- unit entry points (pins) ---------------------------------------------------
+    def kf_propagate(self, state, x2):
+        st = np.ascontiguousarray(state, dtype=np.float64).copy()
+        ok = self._lib.oracle_kf_propagate(self._h, st.ctypes.data_as(_dp), float(x2))
+        return bool(ok), st
+
+    def kf_update(self, state, ym, zm):
+        st = np.ascontiguousarray(state, dtype=np.float64).copy()
+        self._lib.oracle_kf_update(self._h, st.ctypes.data_as(_dp), float(ym), float(zm))
+        return st
+
+    def kf_dist2(self, state, ym, zm):
+        st = np.ascontiguousarray(state, dtype=np.float64)
+        return float(self._lib.oracle_kf_dist2(self._h, st.ctypes.data_as(_dp), float(ym), float(zm)))
+
+    def score(self, r, yc, zc, yu, zu, yd, zd):
+        return float(self._lib.oracle_score(self._h, int(r), yc, zc, yu, zu, yd, zd))
+
+
+def run_timeframe(tf, sectors=None, precision="f32", stage_mask=0x1F, brute=False):
+    """Run the oracle over the sectors of a tpcsynth.Timeframe (independent units)."""
+    orc = Oracle(tf.params, precision)
+    out = {}
+    for s in (range(tf.n_sectors) if sectors is None else sectors):
+        out[s] = orc.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=stage_mask, brute=brute)
+    orc.close()
+    return out

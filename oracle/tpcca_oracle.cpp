@@ -1,0 +1,601 @@
+// =========================================================================================
+// tpcca_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, slow, single-threaded CPU statement of the five-stage cellular-automaton TPC
+// sector tracker that BASELINE.json:5 (north_star) names and SURVEY.md section 8(c) /
+// DESIGN.md section 3 define step by step.  The paper itself (section 1) only
+// names the task ("full online track reconstruction of the TPC data ... the most
+// computing-intense part of the synchronous processing"); it prints no algorithm and no
+// numbers, so the result is a heuristic *defined by its algorithm* and this file follows
+// that algorithm in DESIGN.md's order and notation, one IEEE operation per written
+// operation, no blocking, no fusion, no reordering.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
+// may load this library.  It shares no code, header, table generator or helper with the
+// CUDA path (paper_2208_07412_b200/csrc); inputs and data tables come from tpcsynth/.
+//
+// Build: g++ -O2 -ffp-contract=off -fno-fast-math -shared -fPIC  (see oracle/build.py).
+//   Real = float  : the parity reference (north_star fixes fp32 arithmetic);
+//   Real = double : same source, used only by the pins (P4, P6, P7).
+//
+// Pins (tests/test_oracle_pins.py): P1 grid invariants, P2 brute-force all-pairs neighbour
+// search, P3 bin-size / mirror metamorphic, P4 exact straight-track recovery (dyadic
+// geometry, score == 0), P5 link invariants, P6 noise-free helix recovery 1e-5 (double),
+// P7 textbook weighted-least-squares reduction, P8 pulls / chi2, P9 covariance sanity,
+// P10 generator truth (efficiency / fake), P11 determinism, P12 z-translation, plus a
+// finite-difference pin of the transport Jacobian.  Nothing can be pinned to values the
+// paper prints (it prints none): S5's heuristic choices (gate, gap, passes) are pinned
+// only by P4/P6/P7/P8/P10 -- "parity unpinned to the paper" in that sense.
+// =========================================================================================
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+extern "C" {
+struct oracle_params {      // all tables are double arrays holding the (fp32-representable) data
+  int32_t n_rows;
+  const double* row_x;
+  const double* grid_y_lo;
+  const double* grid_inv_bin_y;
+  const int32_t* grid_ny;
+  double grid_z_lo;
+  const double* grid_inv_bin_z;
+  const int32_t* grid_nz;
+  const double* nf_hy_up;
+  const double* nf_hz_up;
+  const double* nf_hy_dn;
+  const double* nf_hz_dn;
+  const double* nf_cut;
+  double kappa_per_qpt, err2_y, err2_z;
+  double init_cov[5];
+  double tc_win_y, tc_win_z, tc_gate, max_sinphi, grid_margin;
+  int32_t tc_max_gap, tc_min_hits;
+};
+}
+
+namespace {
+
+constexpr int MAX_ROWS = 1024;
+
+// lower-triangle index, i >= j
+inline int tri(int i, int j) { return i * (i + 1) / 2 + j; }
+
+template <class R>
+struct KFState {
+  R x;        // plane
+  R p[5];     // y, z_rel, sin(phi), dz/ds, q/pT
+  R C[15];    // lower triangle
+  R chi2;
+  int n;
+  R c(int i, int j) const { return i >= j ? C[tri(i, j)] : C[tri(j, i)]; }
+};
+
+template <class R>
+struct Track {
+  R x_ref, z_ref, p[5], C[15], chi2;
+  int32_t n_hits, n_fit, first_row, last_row, start_hit;
+};
+
+template <class R>
+class Oracle {
+ public:
+  explicit Oracle(const oracle_params& q) {
+    n_rows = q.n_rows;
+    auto cp = [&](std::vector<R>& v, const double* s) {
+      v.resize(n_rows);
+      for (int i = 0; i < n_rows; ++i) v[i] = (R)s[i];
+    };
+    cp(row_x, q.row_x); cp(grid_y_lo, q.grid_y_lo); cp(inv_bin_y, q.grid_inv_bin_y);
+    cp(inv_bin_z, q.grid_inv_bin_z); cp(hy_up, q.nf_hy_up); cp(hz_up, q.nf_hz_up);
+    cp(hy_dn, q.nf_hy_dn); cp(hz_dn, q.nf_hz_dn); cp(nf_cut, q.nf_cut);
+    ny.assign(q.grid_ny, q.grid_ny + n_rows);
+    nz.assign(q.grid_nz, q.grid_nz + n_rows);
+    grid_z_lo = (R)q.grid_z_lo;
+    Bc = (R)q.kappa_per_qpt; err2_y = (R)q.err2_y; err2_z = (R)q.err2_z;
+    for (int i = 0; i < 5; ++i) init_cov[i] = (R)q.init_cov[i];
+    win_y = (R)q.tc_win_y; win_z = (R)q.tc_win_z; gate = (R)q.tc_gate;
+    max_sinphi = (R)q.max_sinphi; margin = (R)q.grid_margin;
+    max_gap = q.tc_max_gap; min_hits = q.tc_min_hits;
+    row_bin_base.resize(n_rows + 1);
+    row_bin_base[0] = 0;
+    for (int r = 0; r < n_rows; ++r) row_bin_base[r + 1] = row_bin_base[r] + (int64_t)ny[r] * nz[r];
+    c24 = (R)(1.0 / 24.0); c640 = (R)(3.0 / 640.0); c12 = (R)(1.0 / 12.0);
+  }
+
+  // ----------------------------------------------------------------------------- S1
+  // by = clamp(floor((y - grid_y_lo_r) * inv_bin_y_r), 0, ny_r - 1), same for
+  // z; bin = bz * ny_r + by (y fastest).
+  int bin_y(int r, R y) const {
+    R t = (y - grid_y_lo[r]) * inv_bin_y[r];
+    R f = std::floor(t);
+    if (f < (R)0) f = (R)0;
+    R hi = (R)(ny[r] - 1);
+    if (f > hi) f = hi;
+    return (int)f;
+  }
+  int bin_z(int r, R z) const {
+    R t = (z - grid_z_lo) * inv_bin_z[r];
+    R f = std::floor(t);
+    if (f < (R)0) f = (R)0;
+    R hi = (R)(nz[r] - 1);
+    if (f > hi) f = hi;
+    return (int)f;
+  }
+
+  int load(int64_t n_, const R* y_, const R* z_, const uint16_t* row_) {
+    n = n_;
+    for (int64_t i = 0; i < n; ++i)
+      if (row_[i] >= n_rows) return -5;
+    y.assign(y_, y_ + n); z.assign(z_, z_ + n); row.assign(row_, row_ + n);
+    return 0;
+  }
+
+  // sorted order = ascending (row, bin, original index); bin_start = exclusive prefix of the
+  // per-bin counts (sector-local sorted positions), row_start[r] = first position of row r.
+  void build_grid() {
+    std::vector<uint64_t> key(n);      // global bin id of the sector
+    for (int64_t i = 0; i < n; ++i) {
+      int r = row[i];
+      int by = bin_y(r, y[i]);
+      int bz = bin_z(r, z[i]);
+      key[i] = (uint64_t)(row_bin_base[r] + (int64_t)bz * ny[r] + by);
+    }
+    order.resize(n);
+    for (int64_t i = 0; i < n; ++i) order[i] = (int32_t)i;
+    std::sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+      if (key[a] != key[b]) return key[a] < key[b];
+      return a < b;
+    });
+    int64_t nb = row_bin_base[n_rows];
+    bin_start.assign(nb + 1, 0);
+    for (int64_t i = 0; i < n; ++i) bin_start[key[i] + 1]++;
+    for (int64_t b = 0; b < nb; ++b) bin_start[b + 1] += bin_start[b];
+    sy.resize(n); sz.resize(n); srow.resize(n);
+    for (int64_t p = 0; p < n; ++p) {
+      sy[p] = y[order[p]]; sz[p] = z[order[p]]; srow[p] = row[order[p]];
+    }
+    row_start.assign(n_rows + 1, 0);
+    for (int r = 0; r <= n_rows; ++r) row_start[r] = (int32_t)bin_start[row_bin_base[r]];
+  }
+
+  // ----------------------------------------------------------------------------- S2
+  // candidates of row r2 inside the window |y - yc| <= hy and |z - zc| <= hz; brute = whole row
+  void window(int r2, R yc, R zc, R hy, R hz, bool brute, std::vector<int32_t>& out) const {
+    out.clear();
+    if (brute) {
+      for (int32_t c = row_start[r2]; c < row_start[r2 + 1]; ++c) {
+        R dy = sy[c] - yc, dz = sz[c] - zc;
+        if (std::fabs(dy) <= hy && std::fabs(dz) <= hz) out.push_back(c);
+      }
+      return;
+    }
+    // the grid is only an accelerator: visit a superset of the window, then the exact test
+    R my = hy + margin, mz = hz + margin;
+    int by0 = bin_y(r2, yc - my), by1 = bin_y(r2, yc + my);
+    int bz0 = bin_z(r2, zc - mz), bz1 = bin_z(r2, zc + mz);
+    for (int bz = bz0; bz <= bz1; ++bz) {
+      int64_t b0 = row_bin_base[r2] + (int64_t)bz * ny[r2];
+      for (uint32_t c = bin_start[b0 + by0]; c < bin_start[b0 + by1 + 1]; ++c) {
+        R dy = sy[c] - yc, dz = sz[c] - zc;
+        if (std::fabs(dy) <= hy && std::fabs(dz) <= hz) out.push_back((int32_t)c);
+      }
+    }
+  }
+
+  // score of the triplet (d, c, u)
+  R score(int r, R yc, R zc, R yu, R zu, R yd, R zd) const {
+    R dxu = row_x[r + 1] - row_x[r];
+    R dxd = row_x[r] - row_x[r - 1];
+    R ay = (yu - yc) * dxd - (yc - yd) * dxu;
+    R az = (zu - zc) * dxd - (zc - zd) * dxu;
+    return ay * ay + az * az;
+  }
+
+  void find_neighbours(bool brute) {
+    link_up.assign(n, -1); link_dn.assign(n, -1);
+    std::vector<int32_t> U, D;
+    for (int64_t c = 0; c < n; ++c) {
+      int r = srow[c];
+      if (r < 1 || r > n_rows - 2) continue;
+      R yc = sy[c], zc = sz[c];
+      window(r + 1, yc, zc, hy_up[r], hz_up[r], brute, U);
+      if (U.empty()) continue;
+      window(r - 1, yc, zc, hy_dn[r], hz_dn[r], brute, D);
+      if (D.empty()) continue;
+      bool have = false;
+      R best = 0; int32_t bu = -1, bd = -1;
+      for (int32_t u : U)
+        for (int32_t d : D) {
+          R s = score(r, yc, zc, sy[u], sz[u], sy[d], sz[d]);
+          bool better;
+          if (!have) better = true;
+          else if (s < best) better = true;
+          else if (s == best) {
+            // ties: smallest original id of u, then of d
+            if (order[u] != order[bu]) better = order[u] < order[bu];
+            else better = order[d] < order[bd];
+          } else better = false;
+          if (better) { have = true; best = s; bu = u; bd = d; }
+        }
+      if (have && best <= nf_cut[r]) { link_up[c] = bu; link_dn[c] = bd; }
+    }
+  }
+
+  // ----------------------------------------------------------------------------- S3 / S4
+  void clean_links() {
+    link_up_c.assign(n, -1); link_dn_c.assign(n, -1);
+    for (int64_t c = 0; c < n; ++c) {
+      int32_t u = link_up[c], d = link_dn[c];
+      if (u >= 0 && link_dn[u] == (int32_t)c) link_up_c[c] = u;
+      if (d >= 0 && link_up[d] == (int32_t)c) link_dn_c[c] = d;
+    }
+  }
+  void select_start_hits() {
+    start_hit.clear();
+    for (int64_t c = 0; c < n; ++c)
+      if (link_dn_c[c] == -1 && link_up_c[c] >= 0) start_hit.push_back((int32_t)c);
+  }
+
+  // ----------------------------------------------------------------------------- S5: Kalman
+  // DESIGN.md 3.5 "Propagate to x2".  Returns false (state untouched) on failure.
+  bool propagate(KFState<R>& s, R x2) const {
+    R dx = x2 - s.x;
+    if (dx == (R)0) return true;
+    R k = s.p[4] * Bc;
+    R ey = s.p[2];
+    R ey2 = ey + k * dx;
+    if (!(std::fabs(ey) <= max_sinphi) || !(std::fabs(ey2) <= max_sinphi)) return false;
+    R ex = std::sqrt((R)1 - ey * ey);
+    R ex2 = std::sqrt((R)1 - ey2 * ey2);
+    R sx = ex + ex2;
+    R sY = ey + ey2;
+    R tg = sY / sx;
+    R dy = dx * tg;
+    R d2 = dx * dx + dy * dy;
+    R d = std::sqrt(d2);
+    if (dx < (R)0) d = -d;
+    R tt = (k * k) * d2;
+    R dS = d * ((R)1 + tt * (c24 + tt * c640));
+    R cc = (R)1 + (ex * ex2 + ey * ey2);
+    R n02 = (dx * cc) / ((sx * ex) * ex2);
+    R j4 = ((dx * dx) * cc) / (ex2 * (sx * sx));
+    R n04 = Bc * j4;
+    R n12 = s.p[3] * ((dx * tg) / (ex * ex2));
+    R n13 = dS;
+    R n14 = (s.p[3] * Bc) * ((dy / d) * j4 + ((k * d) * d2) * c12);
+    R n24 = Bc * dx;
+    s.p[0] = s.p[0] + dy;
+    s.p[1] = s.p[1] + s.p[3] * dS;
+    s.p[2] = ey2;
+    s.x = x2;
+    // A = J*C (all 25), then C' = A*J^T (lower triangle); terms added left to right
+    R A[5][5];
+    for (int j = 0; j < 5; ++j) {
+      A[0][j] = s.c(0, j) + n02 * s.c(2, j) + n04 * s.c(4, j);
+      A[1][j] = s.c(1, j) + n12 * s.c(2, j) + n13 * s.c(3, j) + n14 * s.c(4, j);
+      A[2][j] = s.c(2, j) + n24 * s.c(4, j);
+      A[3][j] = s.c(3, j);
+      A[4][j] = s.c(4, j);
+    }
+    for (int i = 0; i < 5; ++i) {
+      s.C[tri(i, 0)] = A[i][0] + A[i][2] * n02 + A[i][4] * n04;
+      if (i >= 1) s.C[tri(i, 1)] = A[i][1] + A[i][2] * n12 + A[i][3] * n13 + A[i][4] * n14;
+      if (i >= 2) s.C[tri(i, 2)] = A[i][2] + A[i][4] * n24;
+      if (i >= 3) s.C[tri(i, 3)] = A[i][3];
+      if (i >= 4) s.C[tri(i, 4)] = A[i][4];
+    }
+    return true;
+  }
+
+  // gate distance on the predicted state
+  R dist2(const KFState<R>& s, R ym, R zm) const {
+    R ry = ym - s.p[0];
+    R rz = zm - s.p[1];
+    return (ry * ry) / (s.C[tri(0, 0)] + err2_y) + (rz * rz) / (s.C[tri(1, 1)] + err2_z);
+  }
+
+  // one scalar update of component m (0 = y, 1 = z) with variance e2
+  void update1(KFState<R>& s, int m, R meas, R e2) const {
+    R r = meas - s.p[m];
+    R w = (R)1 / (s.C[tri(m, m)] + e2);
+    R col[5], kk[5];
+    for (int i = 0; i < 5; ++i) col[i] = s.c(i, m);
+    for (int i = 0; i < 5; ++i) { kk[i] = col[i] * w; s.p[i] = s.p[i] + kk[i] * r; }
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j <= i; ++j) s.C[tri(i, j)] = s.C[tri(i, j)] - kk[i] * col[j];
+    s.chi2 = s.chi2 + (r * r) * w;
+  }
+  void update(KFState<R>& s, R ym, R zm) const {
+    update1(s, 0, ym, err2_y);
+    update1(s, 1, zm, err2_z);
+    s.n++;
+  }
+
+  // Search(row r): best cluster inside the tc window around the prediction; ties -> smallest id
+  int32_t search(const KFState<R>& s, int r, R z_ref, R& best_d2) const {
+    R yc = s.p[0];
+    R zc = z_ref + s.p[1];
+    R my = win_y + margin, mz = win_z + margin;
+    int by0 = bin_y(r, yc - my), by1 = bin_y(r, yc + my);
+    int bz0 = bin_z(r, zc - mz), bz1 = bin_z(r, zc + mz);
+    R wy = s.C[tri(0, 0)] + err2_y;
+    R wz = s.C[tri(1, 1)] + err2_z;
+    int32_t best = -1;
+    for (int bz = bz0; bz <= bz1; ++bz) {
+      int64_t b0 = row_bin_base[r] + (int64_t)bz * ny[r];
+      for (uint32_t c = bin_start[b0 + by0]; c < bin_start[b0 + by1 + 1]; ++c) {
+        R ry = sy[c] - s.p[0];
+        R rz = (sz[c] - z_ref) - s.p[1];
+        if (!(std::fabs(ry) <= win_y && std::fabs(rz) <= win_z)) continue;
+        R d2 = (ry * ry) / wy + (rz * rz) / wz;
+        if (best < 0 || d2 < best_d2 || (d2 == best_d2 && order[c] < order[best])) {
+          best = (int32_t)c; best_d2 = d2;
+        }
+      }
+    }
+    return best;
+  }
+
+  void reset_cov(KFState<R>& s) const {
+    for (int i = 0; i < 15; ++i) s.C[i] = (R)0;
+    for (int i = 0; i < 5; ++i) s.C[tri(i, i)] = init_cov[i];
+    s.chi2 = (R)0;
+    s.n = 0;
+  }
+
+  // seed, phase A (follow links), phase B (extrapolate up), phase C (refit down)
+  bool construct_tracklet(int32_t c0, Track<R>& out, std::vector<int32_t>& hit) const {
+    int r0 = srow[c0];
+    int32_t c1 = link_up_c[c0];
+    R z_ref = sz[c0];
+    KFState<R> s;
+    {
+      R dx = row_x[r0 + 1] - row_x[r0];
+      R dy = sy[c1] - sy[c0];
+      R dz = sz[c1] - z_ref;
+      R d = std::sqrt(dx * dx + dy * dy);
+      s.x = row_x[r0];
+      s.p[0] = sy[c0]; s.p[1] = (R)0; s.p[2] = dy / d; s.p[3] = dz / d; s.p[4] = (R)0;
+      reset_cov(s);
+    }
+    hit.assign(n_rows, -1);
+    int top = r0;
+    bool failed = false;
+    // ---- phase A
+    int32_t cur = c0;
+    int last = r0;
+    while (cur != -1) {
+      int r = srow[cur];
+      if (!propagate(s, row_x[r])) { failed = true; break; }
+      R ym = sy[cur], zm = sz[cur] - z_ref;
+      if (s.n >= 2 && dist2(s, ym, zm) > gate) break;
+      update(s, ym, zm);
+      hit[r] = cur; last = r; top = r;
+      cur = link_up_c[cur];
+    }
+    // ---- phase B
+    if (!failed) {
+      int gap = 0;
+      for (int r = last + 1; r < n_rows; ++r) {
+        if (!propagate(s, row_x[r])) break;
+        R d2 = (R)0;
+        int32_t b = search(s, r, z_ref, d2);
+        if (b >= 0 && d2 <= gate) {
+          update(s, sy[b], sz[b] - z_ref);
+          hit[r] = b; top = r; gap = 0;
+        } else {
+          if (++gap > max_gap) break;
+        }
+      }
+    }
+    // ---- phase C: start at the highest row holding a hit (reading R2)
+    reset_cov(s);
+    int gap = 0;
+    bool have_snap = false;
+    KFState<R> snap = s;
+    for (int r = top; r >= 0; --r) {
+      if (!propagate(s, row_x[r])) break;
+      if (hit[r] != -1) {
+        int32_t c = hit[r];
+        update(s, sy[c], sz[c] - z_ref);
+        snap = s; have_snap = true;
+      } else {
+        bool took = false;
+        if (s.n >= 2) {   // reading R3: no search before two hits constrain the direction
+          R d2 = (R)0;
+          int32_t b = search(s, r, z_ref, d2);
+          if (b >= 0 && d2 <= gate) {
+            update(s, sy[b], sz[b] - z_ref);
+            hit[r] = b; snap = s; have_snap = true; gap = 0; took = true;
+          }
+        }
+        if (!took && r < r0) {
+          if (++gap > max_gap) break;
+        }
+      }
+    }
+    int nh = 0, first = -1, lastr = -1;
+    for (int r = 0; r < n_rows; ++r)
+      if (hit[r] != -1) { if (first < 0) first = r; lastr = r; ++nh; }
+    if (nh < min_hits || !have_snap) return false;
+    out.x_ref = snap.x; out.z_ref = z_ref;
+    for (int i = 0; i < 5; ++i) out.p[i] = snap.p[i];
+    for (int i = 0; i < 15; ++i) out.C[i] = snap.C[i];
+    out.chi2 = snap.chi2; out.n_fit = snap.n; out.n_hits = nh;
+    out.first_row = first; out.last_row = lastr; out.start_hit = c0;
+    return true;
+  }
+
+  void construct_tracklets() {
+    tracks.clear(); hit_offset.assign(1, 0); hit_idx.clear();
+    std::vector<int32_t> hit;
+    for (int32_t c0 : start_hit) {
+      Track<R> t;
+      if (!construct_tracklet(c0, t, hit)) continue;
+      tracks.push_back(t);
+      for (int r = 0; r < n_rows; ++r)
+        if (hit[r] != -1) hit_idx.push_back(hit[r]);
+      hit_offset.push_back((int32_t)hit_idx.size());
+    }
+  }
+
+  void run(uint32_t stage_mask, bool brute) {
+    if (stage_mask & 1u) build_grid();
+    if (stage_mask & 2u) find_neighbours(brute);
+    if (stage_mask & 4u) clean_links();
+    if (stage_mask & 8u) select_start_hits();
+    if (stage_mask & 16u) construct_tracklets();
+  }
+
+  // tables
+  int n_rows;
+  std::vector<R> row_x, grid_y_lo, inv_bin_y, inv_bin_z, hy_up, hz_up, hy_dn, hz_dn, nf_cut;
+  std::vector<int32_t> ny, nz;
+  std::vector<int64_t> row_bin_base;
+  R grid_z_lo, Bc, err2_y, err2_z, init_cov[5], win_y, win_z, gate, max_sinphi, margin;
+  R c24, c640, c12;
+  int max_gap, min_hits;
+  // data
+  int64_t n = 0;
+  std::vector<R> y, z, sy, sz;
+  std::vector<uint16_t> row, srow;
+  std::vector<int32_t> order, row_start;
+  std::vector<uint32_t> bin_start;
+  std::vector<int32_t> link_up, link_dn, link_up_c, link_dn_c, start_hit;
+  std::vector<Track<R>> tracks;
+  std::vector<int32_t> hit_offset, hit_idx;
+};
+
+struct Handle {
+  int precision;           // 0 = float, 1 = double
+  Oracle<float>* f = nullptr;
+  Oracle<double>* d = nullptr;
+};
+
+template <class V>
+void copy_out(double* dst, const V& v) { for (size_t i = 0; i < v.size(); ++i) dst[i] = (double)v[i]; }
+
+// state = [x, p0..p4, C0..C14, chi2] (22 doubles), in/out
+template <class R>
+void st_in(KFState<R>& s, const double* st) {
+  s.x = (R)st[0];
+  for (int i = 0; i < 5; ++i) s.p[i] = (R)st[1 + i];
+  for (int i = 0; i < 15; ++i) s.C[i] = (R)st[6 + i];
+  s.chi2 = (R)st[21]; s.n = 0;
+}
+template <class R>
+void st_out(const KFState<R>& s, double* st) {
+  st[0] = (double)s.x;
+  for (int i = 0; i < 5; ++i) st[1 + i] = (double)s.p[i];
+  for (int i = 0; i < 15; ++i) st[6 + i] = (double)s.C[i];
+  st[21] = (double)s.chi2;
+}
+
+}  // namespace
+
+#define DISPATCH(h, expr_f, expr_d) (((Handle*)(h))->precision == 0 ? (expr_f) : (expr_d))
+
+extern "C" {
+
+void* oracle_create(const oracle_params* q, int precision) {
+  if (!q || q->n_rows < 3 || q->n_rows > MAX_ROWS) return nullptr;
+  Handle* h = new Handle;
+  h->precision = precision;
+  if (precision == 0) h->f = new Oracle<float>(*q); else h->d = new Oracle<double>(*q);
+  return h;
+}
+void oracle_destroy(void* hv) {
+  Handle* h = (Handle*)hv;
+  if (!h) return;
+  delete h->f; delete h->d; delete h;
+}
+// y, z: float* if precision 0, double* if precision 1.  One sector.
+int oracle_load(void* hv, int64_t n, const void* y, const void* z, const uint16_t* row) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) return h->f->load(n, (const float*)y, (const float*)z, row);
+  return h->d->load(n, (const double*)y, (const double*)z, row);
+}
+// stage_mask bit i = stage i+1; brute != 0: S2 scans whole rows r+-1 instead of the grid
+int oracle_run(void* hv, uint32_t stage_mask, int brute) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) h->f->run(stage_mask, brute != 0); else h->d->run(stage_mask, brute != 0);
+  return 0;
+}
+// out[0..4] = n_clusters, n_start, n_tracks, n_hits, n_bins
+void oracle_sizes(void* hv, int64_t* out) {
+  Handle* h = (Handle*)hv;
+#define SZ(o) do { out[0] = (o)->n; out[1] = (int64_t)(o)->start_hit.size(); \
+    out[2] = (int64_t)(o)->tracks.size(); out[3] = (int64_t)(o)->hit_idx.size(); \
+    out[4] = (o)->row_bin_base[(o)->n_rows]; } while (0)
+  if (h->precision == 0) SZ(h->f); else SZ(h->d);
+#undef SZ
+}
+void oracle_get_grid(void* hv, int32_t* order, double* sy, double* sz, uint32_t* bin_start, int32_t* row_start) {
+  Handle* h = (Handle*)hv;
+#define GG(o) do { \
+    if (order) std::copy((o)->order.begin(), (o)->order.end(), order); \
+    if (sy) copy_out(sy, (o)->sy); \
+    if (sz) copy_out(sz, (o)->sz); \
+    if (bin_start) std::copy((o)->bin_start.begin(), (o)->bin_start.end(), bin_start); \
+    if (row_start) std::copy((o)->row_start.begin(), (o)->row_start.end(), row_start); } while (0)
+  if (h->precision == 0) GG(h->f); else GG(h->d);
+#undef GG
+}
+void oracle_get_links(void* hv, int32_t* up_raw, int32_t* dn_raw, int32_t* up, int32_t* dn, int32_t* start) {
+  Handle* h = (Handle*)hv;
+#define GL(o) do { \
+    if (up_raw) std::copy((o)->link_up.begin(), (o)->link_up.end(), up_raw); \
+    if (dn_raw) std::copy((o)->link_dn.begin(), (o)->link_dn.end(), dn_raw); \
+    if (up) std::copy((o)->link_up_c.begin(), (o)->link_up_c.end(), up); \
+    if (dn) std::copy((o)->link_dn_c.begin(), (o)->link_dn_c.end(), dn); \
+    if (start) std::copy((o)->start_hit.begin(), (o)->start_hit.end(), start); } while (0)
+  if (h->precision == 0) GL(h->f); else GL(h->d);
+#undef GL
+}
+// par: [n_tracks][5], cov: [n_tracks][15] (row-major per track), ints: [n_tracks][5] =
+// n_hits, n_fit, first_row, last_row, start_hit
+void oracle_get_tracks(void* hv, double* x_ref, double* z_ref, double* par, double* cov, double* chi2,
+                       int32_t* ints, int32_t* hit_offset, int32_t* hit_idx) {
+  Handle* h = (Handle*)hv;
+#define GT(o) do { \
+    for (size_t t = 0; t < (o)->tracks.size(); ++t) { \
+      const auto& T = (o)->tracks[t]; \
+      x_ref[t] = (double)T.x_ref; z_ref[t] = (double)T.z_ref; chi2[t] = (double)T.chi2; \
+      for (int i = 0; i < 5; ++i) par[t * 5 + i] = (double)T.p[i]; \
+      for (int i = 0; i < 15; ++i) cov[t * 15 + i] = (double)T.C[i]; \
+      ints[t * 5 + 0] = T.n_hits; ints[t * 5 + 1] = T.n_fit; ints[t * 5 + 2] = T.first_row; \
+      ints[t * 5 + 3] = T.last_row; ints[t * 5 + 4] = T.start_hit; } \
+    std::copy((o)->hit_offset.begin(), (o)->hit_offset.end(), hit_offset); \
+    std::copy((o)->hit_idx.begin(), (o)->hit_idx.end(), hit_idx); } while (0)
+  if (h->precision == 0) GT(h->f); else GT(h->d);
+#undef GT
+}
+
+// ---- unit entry points for the pins ---------------------------------------------------
+// state = [x, p0..p4, C0..C14, chi2] (22 doubles), in/out
+int oracle_kf_propagate(void* hv, double* st, double x2) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) { KFState<float> s; st_in(s, st); bool ok = h->f->propagate(s, (float)x2); st_out(s, st); return ok; }
+  KFState<double> s; st_in(s, st); bool ok = h->d->propagate(s, x2); st_out(s, st); return ok;
+}
+void oracle_kf_update(void* hv, double* st, double ym, double zm) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) { KFState<float> s; st_in(s, st); h->f->update(s, (float)ym, (float)zm); st_out(s, st); return; }
+  KFState<double> s; st_in(s, st); h->d->update(s, ym, zm); st_out(s, st);
+}
+double oracle_kf_dist2(void* hv, const double* st, double ym, double zm) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) { KFState<float> s; st_in(s, st); return (double)h->f->dist2(s, (float)ym, (float)zm); }
+  KFState<double> s; st_in(s, st); return h->d->dist2(s, ym, zm);
+}
+// S2 score of the triplet (d, c, u) around row r with the oracle's arithmetic (reading N4)
+double oracle_score(void* hv, int r, double yc, double zc, double yu, double zu, double yd, double zd) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0)
+    return (double)h->f->score(r, (float)yc, (float)zc, (float)yu, (float)zu, (float)yd, (float)zd);
+  return h->d->score(r, yc, zc, yu, zu, yd, zd);
+}
+
+}  // extern "C"
