@@ -1,0 +1,25 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box via gpurun)")
+
+
+@pytest.fixture(scope="session")
+def cfg0():
+    import tpcsynth
+    return tpcsynth.generate(0)
+
+
+@pytest.fixture(scope="session")
+def cfg1_small():
+    """Config-1 kinematics at 1500 tracks (36 sectors): seconds for the oracle."""
+    import tpcsynth
+    return tpcsynth.generate(1, n_tracks=1500)
