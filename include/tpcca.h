@@ -1,0 +1,203 @@
+/* =========================================================================================
+ * tpcca.h -- C-ABI boundary of the B200-native TPC sector cellular-automaton (CA) tracker.
+ *
+ * What the library computes: the hot path PAPER.md:21 (section 1, "the EPNs perform full online
+ * track reconstruction of the TPC data. This is the most computing-intense part of the
+ * synchronous processing ... The full TPC processing happens on the GPUs") names and
+ * BASELINE.json:5 (north_star) fixes as five stages, defined step by step in DESIGN.md
+ * section 3 (= SURVEY.md section 8(c)):
+ *   S1 per-row y/z grid binning of clusters
+ *   S2 neighbour finder: best up/down link pair
+ *   S3 mutual-link confirmation ("link cleaner")
+ *   S4 start-hit selection, ordered compaction
+ *   S5 tracklet construction + fp32 Kalman helix fit   (Bz = 0.5 T)
+ * "clusters per sector and pad row in, links and fitted tracks out" (BASELINE.json:5).
+ *
+ * Every stage runs in hand-written CUDA kernels for sm_100a; there is NO CPU fallback: every
+ * entry point that needs the device fails with TPCCA_E_CUDA when no usable device exists.
+ *
+ * Conventions
+ *  - every call returns 0 (TPCCA_OK) or a negative code; no exceptions, no exit(), no stdout;
+ *    tpcca_last_error(ctx) gives a human-readable message for the last failing call.
+ *  - plain pointers and sizes only.  Each pointer argument says whether it is HOST or DEVICE.
+ *  - a context is not thread-safe; use one context per host thread / per stream.
+ *  - index space of all outputs: "sorted position" = position of a cluster inside its sector
+ *    after S1 (ascending (row, bin, original index)); order[] maps sorted -> original index.
+ *    All cluster indices stored in outputs are SECTOR-LOCAL sorted positions; -1 = none.
+ *  - arithmetic: every + - * / sqrt is one IEEE-754 binary32 round-to-nearest operation, no
+ *    FMA contraction, no flush-to-zero; inputs containing NaN/Inf are
+ *    undefined behaviour.
+ * ========================================================================================= */
+#ifndef TPCCA_H_
+#define TPCCA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPCCA_OK            0
+#define TPCCA_E_ARG        -1   /* NULL / out-of-range argument                                  */
+#define TPCCA_E_STATE      -2   /* wrong call order (e.g. run before all sectors were loaded)   */
+#define TPCCA_E_CUDA       -3   /* CUDA runtime error or no usable device (message has details) */
+#define TPCCA_E_WORKSPACE  -4   /* caller's workspace too small, or a device-side capacity       */
+                                /* (max_start_hits) overflowed: nothing is silently truncated   */
+#define TPCCA_E_RANGE      -5   /* a cluster's row >= n_rows (detected on the device in S1)      */
+
+#define TPCCA_MAX_ROWS     256  /* n_rows limit of this build (the ALICE TPC has 152)            */
+#define TPCCA_MAX_SECTORS  64   /* n_sectors limit (the ALICE TPC has 36)                        */
+
+#define TPCCA_MEM_HOST          0  /* pointer is HOST memory, the library copies                  */
+#define TPCCA_MEM_DEVICE        1  /* pointer is DEVICE memory, the library copies (D2D)          */
+#define TPCCA_MEM_DEVICE_BORROW 2  /* DEVICE memory, used in place; must stay valid until the     */
+                                   /* next load of the same sector or destroy (load only)        */
+
+#define TPCCA_STAGE_GRID       0x01u
+#define TPCCA_STAGE_NEIGHBOURS 0x02u
+#define TPCCA_STAGE_CLEAN      0x04u
+#define TPCCA_STAGE_START      0x08u
+#define TPCCA_STAGE_TRACKLETS  0x10u
+#define TPCCA_STAGE_ALL        0x1Fu
+
+typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
+
+/* Tracker tables (DESIGN.md 3 "Derived tables").  All table pointers are HOST arrays of length
+ * n_rows, owned by the caller and copied by tpcca_create.  The tables are DATA: geometry, grid,
+ * windows and cuts are never hard-coded in the kernels. */
+typedef struct {
+  int32_t n_sectors;               /* 1 .. TPCCA_MAX_SECTORS; sectors are independent units       */
+  int32_t n_rows;                  /* 3 .. TPCCA_MAX_ROWS pad rows                                */
+  const float   *row_x;            /* pad-row plane x [cm], strictly increasing                   */
+  const float   *grid_y_lo;        /* S1: lower y edge of the grid of row r                       */
+  const float   *grid_inv_bin_y;   /* S1: 1 / bin size in y                                       */
+  const int32_t *grid_ny;          /* S1: number of y bins (>= 1)                                 */
+  float          grid_z_lo;        /* S1: lower z edge (all rows)                                 */
+  const float   *grid_inv_bin_z;   /* S1: 1 / bin size in z                                       */
+  const int32_t *grid_nz;          /* S1: number of z bins (>= 1)                                 */
+  const float   *nf_hy_up, *nf_hz_up;   /* S2: window half-widths towards row r+1                */
+  const float   *nf_hy_dn, *nf_hz_dn;   /* S2: window half-widths towards row r-1                */
+  const float   *nf_cut;           /* S2: upper cut on the best score                             */
+  float kappa_per_qpt;             /* S5: d sin(phi)/dx = kappa_per_qpt * (q/pT); 0.2998e-3*Bz[kG] */
+  float err2_y, err2_z;            /* S5: measurement variances                                   */
+  float init_cov[5];               /* S5: diagonal of the reset covariance                        */
+  float tc_win_y, tc_win_z;        /* S5: search window half-widths                               */
+  float tc_gate;                   /* S5: chi2-like gate on dist2                                 */
+  float max_sinphi;                /* S5: propagation fails beyond this |sin(phi)|                */
+  float grid_margin;               /* S2/S5: safety margin when turning a window into a bin range */
+  int32_t tc_max_gap;              /* S5: consecutive rows without a hit before stopping          */
+  int32_t tc_min_hits;             /* S5: minimum hits of an emitted track                        */
+} tpcca_params;
+
+/* Outputs of ONE sector.  With mem_space == TPCCA_MEM_DEVICE the pointers are DEVICE pointers
+ * into the caller's workspace; with TPCCA_MEM_HOST they are HOST pointers to buffers owned by
+ * the context (the library did the D2H copies).  Either way they stay valid until the next
+ * tpcca_run / tpcca_load_clusters / tpcca_get_* (HOST) / tpcca_destroy on this context.
+ * Arrays of stages that were not run are NULL with their counts 0. */
+typedef struct {
+  int64_t n_clusters;      /* clusters loaded for the sector                                     */
+  int64_t n_bins;          /* grid bins of a sector = sum_r ny_r * nz_r                          */
+  int64_t n_start;         /* S4 start hits                                                      */
+  int64_t n_tracks;        /* S5 emitted tracks                                                  */
+  int64_t n_hits;          /* S5 total hits of the emitted tracks                                */
+  int64_t trk_stride;      /* elements between consecutive planes of par[] and cov[]             */
+  /* S1 */
+  const int32_t  *order;      /* [n_clusters] sorted position -> original index                  */
+  const float    *syz;        /* [n_clusters][2] bin-sorted (y, z) pairs, interleaved            */
+  const uint32_t *bin_start;  /* [n_bins + 1] first sorted position of each bin; last = n        */
+  const int32_t  *row_start;  /* [n_rows + 1] first sorted position of each row                  */
+  /* S2: raw links */
+  const int32_t  *link_up_raw, *link_dn_raw;   /* [n_clusters]                                   */
+  /* S3: reciprocal links */
+  const int32_t  *link_up, *link_dn;           /* [n_clusters]                                   */
+  /* S4 */
+  const int32_t  *start_hit;  /* [n_start] ascending sorted positions                            */
+  /* S5: tracks in start-hit order */
+  const float    *x_ref;      /* [n_tracks] plane of the reference state                         */
+  const float    *z_ref;      /* [n_tracks] z of the start hit; absolute z = z_ref + par[1]      */
+  const float    *par;        /* par[i * trk_stride + t], i < 5: y, z_rel, sin(phi), dz/ds, q/pT */
+  const float    *cov;        /* cov[k * trk_stride + t], k < 15: lower triangle, k = i(i+1)/2+j */
+  const float    *chi2;       /* [n_tracks]                                                      */
+  const int32_t  *n_hits_trk; /* [n_tracks] number of attached clusters                          */
+  const int32_t  *n_fit;      /* [n_tracks] clusters used by the final (downward) fit            */
+  const int32_t  *first_row, *last_row, *trk_start_hit;   /* [n_tracks]                          */
+  const int32_t  *hit_offset; /* [n_tracks + 1] CSR offsets into hit_idx, hit_offset[0] = 0      */
+  const int32_t  *hit_idx;    /* [n_hits] sorted positions, ascending row inside a track         */
+} tpcca_tracks_view;
+
+/* Bytes of DEVICE workspace that tpcca_create needs for at most `max_clusters_total` clusters
+ * over all sectors and at most `max_start_hits` S4 start hits over all sectors
+ * (max_start_hits <= 0: a default of max_clusters_total / 8 + 1024; the hard bound is
+ * max_clusters_total / 2).  HOST call, no device needed.  Errors: TPCCA_E_ARG. */
+int tpcca_workspace_bytes(const tpcca_params *params, int64_t max_clusters_total,
+                          int64_t max_start_hits, size_t *out_bytes);
+
+/* Create a context on CUDA device `cuda_device`.  `cuda_stream` is a cudaStream_t of that device
+ * (NULL = the legacy default stream) on which every kernel and copy of this context is issued.
+ * `workspace` is a DEVICE buffer of `workspace_bytes` bytes (256-byte aligned), owned by the
+ * caller and used by the context until tpcca_destroy.  The capacities are the ones passed to
+ * tpcca_workspace_bytes.  Errors: TPCCA_E_ARG (bad tables), TPCCA_E_CUDA (no device: there is no
+ * CPU path), TPCCA_E_WORKSPACE (buffer too small; message names the required size). */
+int tpcca_create(const tpcca_params *params, int cuda_device, void *cuda_stream,
+                 void *workspace, size_t workspace_bytes,
+                 int64_t max_clusters_total, int64_t max_start_hits, tpcca_ctx **out_ctx);
+
+/* Hand the clusters of one sector to the context (BASELINE.json:5 "clusters per sector and pad
+ * row in").  SoA arrays of length n: y, z fp32 local coordinates [cm], row = pad-row index.
+ * x (= row_x[row]) and charge are part of the cluster record (BASELINE.json:7) but S1-S5 do not
+ * read them: either may be NULL; when given they are only validated for nullness, never copied.
+ * mem_space says where x, y, z, charge, row live (TPCCA_MEM_*).  Copies are asynchronous on the
+ * context's stream; HOST arrays must stay valid until the stream has passed the copy (pinned
+ * memory makes it truly asynchronous).  Sectors accumulate until tpcca_reset; sectors never
+ * loaded are empty; loading a sector twice without a reset is TPCCA_E_STATE.  The sum of n over
+ * sectors must not exceed max_clusters_total (TPCCA_E_WORKSPACE).  Loading invalidates the
+ * outputs of earlier runs.  Errors: TPCCA_E_ARG, TPCCA_E_STATE, TPCCA_E_WORKSPACE, TPCCA_E_CUDA. */
+int tpcca_load_clusters(tpcca_ctx *ctx, int sector, int64_t n, const float *x, const float *y,
+                        const float *z, const float *charge, const uint16_t *row, int mem_space);
+
+/* Start a new time frame: forget all loaded sectors and all outputs (no device work). */
+int tpcca_reset(tpcca_ctx *ctx);
+
+/* Run the stages in `stage_mask` (bit i = stage i+1) over all sectors, asynchronously on the
+ * context's stream.  A stage needs the outputs of the stages before it from this or an earlier
+ * run on the same clusters (TPCCA_E_STATE otherwise).  Device-side failures (row out of range,
+ * start-hit capacity overflow) are reported by the next tpcca_get_* / tpcca_sync call.
+ * Errors: TPCCA_E_STATE, TPCCA_E_CUDA. */
+int tpcca_run(tpcca_ctx *ctx, uint32_t stage_mask);
+
+/* Wait for the stream and report device-side failures of the last run (TPCCA_E_RANGE,
+ * TPCCA_E_WORKSPACE) or TPCCA_E_CUDA. */
+int tpcca_sync(tpcca_ctx *ctx);
+
+/* Outputs of one sector (BASELINE.json:5 "links and fitted tracks out").  Synchronises the
+ * stream.  mem_space: TPCCA_MEM_DEVICE (pointers into the workspace, no copy) or TPCCA_MEM_HOST
+ * (copies into context-owned host buffers; par/cov are packed with trk_stride = n_tracks).
+ * Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
+int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, tpcca_tracks_view *out);
+
+/* Totals over all sectors after a run: out[0..4] = n_clusters, n_start, n_tracks, n_hits,
+ * n_bins (per sector).  Synchronises the stream.  Errors as tpcca_sync. */
+int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[5]);
+
+/* Device time of each stage of the last run [ms], from CUDA events on the context's stream;
+ * ms[5] = whole run.  Synchronises the stream. */
+int tpcca_get_timings(tpcca_ctx *ctx, float ms[6]);
+
+/* Number of kernels the last tpcca_run launched (for bench.py's "gpu_launches"). */
+int tpcca_get_launch_count(const tpcca_ctx *ctx, int64_t *out);
+
+/* Message of the last failing call on this context ("" if none).  Never NULL.  With ctx == NULL:
+ * the message of the last failing tpcca_create / tpcca_workspace_bytes of this thread. */
+const char *tpcca_last_error(const tpcca_ctx *ctx);
+
+/* Release the context (not the workspace, not borrowed inputs).  NULL is allowed. */
+void tpcca_destroy(tpcca_ctx *ctx);
+
+/* Library version string, e.g. "tpcca 0.1 (sm_100a)". */
+const char *tpcca_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif  /* TPCCA_H_ */

@@ -1,0 +1,433 @@
+// S5 tracklet construction + fp32 Kalman helix fit.
+// One tracklet per thread; the three phases (A follow links, B extrapolate up, C refit down) are
+// folded into ONE loop over row steps so that the lanes of a warp, which sit in different phases,
+// still share the propagate / search / update instruction stream.
+#pragma once
+#include "k_links.cuh"
+
+namespace tpcca {
+
+// Kalman state: plane x, parameters p = (y, z_rel, sin phi, dz/ds, q/pT), covariance lower
+// triangle c_ij (i >= j).  Every operation below is one IEEE binary32 operation in exactly the
+// order DESIGN.md 3.5 writes it (the library is compiled with --fmad=false; the _rn intrinsics
+// are used where a contraction would otherwise be tempting for the compiler).
+struct KF {
+  float x;
+  float p0, p1, p2, p3, p4;
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+  float chi2;
+  int n;
+};
+
+struct KFConst {
+  float Bc, err2_y, err2_z, max_sinphi, c24, c640, c12;
+  float ic0, ic1, ic2, ic3, ic4;
+};
+
+__device__ __forceinline__ void kf_reset_cov(KF& s, const KFConst& k) {
+  s.c00 = k.ic0; s.c10 = 0.f; s.c11 = k.ic1; s.c20 = 0.f; s.c21 = 0.f; s.c22 = k.ic2;
+  s.c30 = 0.f; s.c31 = 0.f; s.c32 = 0.f; s.c33 = k.ic3;
+  s.c40 = 0.f; s.c41 = 0.f; s.c42 = 0.f; s.c43 = 0.f; s.c44 = k.ic4;
+  s.chi2 = 0.f; s.n = 0;
+}
+
+// DESIGN.md 3.5 "Propagate to x2".  false (state untouched) if |sin phi| would exceed the limit.
+__device__ __forceinline__ bool kf_propagate(KF& s, float x2, const KFConst& K) {
+  const float dx = x2 - s.x;
+  if (dx == 0.0f) return true;
+  const float k = s.p4 * K.Bc;
+  const float ey = s.p2;
+  const float ey2 = ey + k * dx;
+  if (!(fabsf(ey) <= K.max_sinphi) || !(fabsf(ey2) <= K.max_sinphi)) return false;
+  const float ex = sqrtf(1.0f - ey * ey);
+  const float ex2 = sqrtf(1.0f - ey2 * ey2);
+  const float sx = ex + ex2;
+  const float sY = ey + ey2;
+  const float tg = sY / sx;
+  const float dy = dx * tg;
+  const float d2 = dx * dx + dy * dy;
+  float d = sqrtf(d2);
+  if (dx < 0.0f) d = -d;
+  const float tt = (k * k) * d2;
+  const float dS = d * (1.0f + tt * (K.c24 + tt * K.c640));
+  const float cc = 1.0f + (ex * ex2 + ey * ey2);
+  const float n02 = (dx * cc) / ((sx * ex) * ex2);
+  const float j4 = ((dx * dx) * cc) / (ex2 * (sx * sx));
+  const float n04 = K.Bc * j4;
+  const float n12 = s.p3 * ((dx * tg) / (ex * ex2));
+  const float n13 = dS;
+  const float n14 = (s.p3 * K.Bc) * ((dy / d) * j4 + ((k * d) * d2) * K.c12);
+  const float n24 = K.Bc * dx;
+  s.p0 = s.p0 + dy;
+  s.p1 = s.p1 + s.p3 * dS;
+  s.p2 = ey2;
+  s.x = x2;
+  // A = J*C (rows 0..2 differ from C), C' = A*J^T (lower triangle); terms left to right.
+  const float A00 = s.c00 + n02 * s.c20 + n04 * s.c40;
+  const float A02 = s.c20 + n02 * s.c22 + n04 * s.c42;
+  const float A04 = s.c40 + n02 * s.c42 + n04 * s.c44;
+  const float A10 = s.c10 + n12 * s.c20 + n13 * s.c30 + n14 * s.c40;
+  const float A11 = s.c11 + n12 * s.c21 + n13 * s.c31 + n14 * s.c41;
+  const float A12 = s.c21 + n12 * s.c22 + n13 * s.c32 + n14 * s.c42;
+  const float A13 = s.c31 + n12 * s.c32 + n13 * s.c33 + n14 * s.c43;
+  const float A14 = s.c41 + n12 * s.c42 + n13 * s.c43 + n14 * s.c44;
+  const float A20 = s.c20 + n24 * s.c40;
+  const float A21 = s.c21 + n24 * s.c41;
+  const float A22 = s.c22 + n24 * s.c42;
+  const float A23 = s.c32 + n24 * s.c43;
+  const float A24 = s.c42 + n24 * s.c44;
+  const float A30 = s.c30, A31 = s.c31, A32 = s.c32, A33 = s.c33, A34 = s.c43;
+  const float A40 = s.c40, A41 = s.c41, A42 = s.c42, A43 = s.c43, A44 = s.c44;
+  s.c00 = A00 + A02 * n02 + A04 * n04;
+  s.c10 = A10 + A12 * n02 + A14 * n04;
+  s.c20 = A20 + A22 * n02 + A24 * n04;
+  s.c30 = A30 + A32 * n02 + A34 * n04;
+  s.c40 = A40 + A42 * n02 + A44 * n04;
+  s.c11 = A11 + A12 * n12 + A13 * n13 + A14 * n14;
+  s.c21 = A21 + A22 * n12 + A23 * n13 + A24 * n14;
+  s.c31 = A31 + A32 * n12 + A33 * n13 + A34 * n14;
+  s.c41 = A41 + A42 * n12 + A43 * n13 + A44 * n14;
+  s.c22 = A22 + A24 * n24;
+  s.c32 = A32 + A34 * n24;
+  s.c42 = A42 + A44 * n24;
+  s.c33 = A33;
+  s.c43 = A43;
+  s.c44 = A44;
+  return true;
+}
+
+// DESIGN.md 3.5 "Update": two scalar updates, y (component 0) then z (component 1).
+__device__ __forceinline__ void kf_update(KF& s, float ym, float zm, const KFConst& K) {
+  {
+    const float r = ym - s.p0;
+    const float w = 1.0f / (s.c00 + K.err2_y);
+    const float q0 = s.c00, q1 = s.c10, q2 = s.c20, q3 = s.c30, q4 = s.c40;
+    const float k0 = q0 * w, k1 = q1 * w, k2 = q2 * w, k3 = q3 * w, k4 = q4 * w;
+    s.p0 = s.p0 + k0 * r; s.p1 = s.p1 + k1 * r; s.p2 = s.p2 + k2 * r;
+    s.p3 = s.p3 + k3 * r; s.p4 = s.p4 + k4 * r;
+    s.c00 = s.c00 - k0 * q0;
+    s.c10 = s.c10 - k1 * q0; s.c11 = s.c11 - k1 * q1;
+    s.c20 = s.c20 - k2 * q0; s.c21 = s.c21 - k2 * q1; s.c22 = s.c22 - k2 * q2;
+    s.c30 = s.c30 - k3 * q0; s.c31 = s.c31 - k3 * q1; s.c32 = s.c32 - k3 * q2; s.c33 = s.c33 - k3 * q3;
+    s.c40 = s.c40 - k4 * q0; s.c41 = s.c41 - k4 * q1; s.c42 = s.c42 - k4 * q2; s.c43 = s.c43 - k4 * q3;
+    s.c44 = s.c44 - k4 * q4;
+    s.chi2 = s.chi2 + (r * r) * w;
+  }
+  {
+    const float r = zm - s.p1;
+    const float w = 1.0f / (s.c11 + K.err2_z);
+    const float q0 = s.c10, q1 = s.c11, q2 = s.c21, q3 = s.c31, q4 = s.c41;
+    const float k0 = q0 * w, k1 = q1 * w, k2 = q2 * w, k3 = q3 * w, k4 = q4 * w;
+    s.p0 = s.p0 + k0 * r; s.p1 = s.p1 + k1 * r; s.p2 = s.p2 + k2 * r;
+    s.p3 = s.p3 + k3 * r; s.p4 = s.p4 + k4 * r;
+    s.c00 = s.c00 - k0 * q0;
+    s.c10 = s.c10 - k1 * q0; s.c11 = s.c11 - k1 * q1;
+    s.c20 = s.c20 - k2 * q0; s.c21 = s.c21 - k2 * q1; s.c22 = s.c22 - k2 * q2;
+    s.c30 = s.c30 - k3 * q0; s.c31 = s.c31 - k3 * q1; s.c32 = s.c32 - k3 * q2; s.c33 = s.c33 - k3 * q3;
+    s.c40 = s.c40 - k4 * q0; s.c41 = s.c41 - k4 * q1; s.c42 = s.c42 - k4 * q2; s.c43 = s.c43 - k4 * q3;
+    s.c44 = s.c44 - k4 * q4;
+    s.chi2 = s.chi2 + (r * r) * w;
+  }
+  s.n++;
+}
+
+// Per-row tables staged in shared memory (lanes of a warp sit on different rows in S5).
+struct RowTab {
+  float x, y_lo, inv_by, ny_hi, inv_bz, nz_hi;
+  int32_t ny, bin_base;
+};
+
+// slot-space scratch of S5 (SoA with stride cap): 24 float planes + 4 int planes
+constexpr int kTrkF = 24;   // x_ref, z_ref, p0..p4, c[15], chi2, (pad)
+constexpr int kTrkI = 4;    // n_hits (0 = rejected), n_fit, first_row, last_row
+
+// ---- K5a ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
+            DevStatus* __restrict__ st, const float2* __restrict__ syz,
+            const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
+            const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
+            const int32_t* __restrict__ start_hit, int32_t cap,
+            int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
+            int32_t* __restrict__ trk_i /*[kTrkI][cap]*/) {
+  __shared__ RowTab tab[kMaxRows];
+  __shared__ int s_start_off[kMaxSectors + 1];
+  __shared__ int s_work[4];
+  const int n_rows = T->n_rows, ns = T->n_sectors;
+  for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
+    RowTab t;
+    t.x = T->row_x[r]; t.y_lo = T->y_lo[r]; t.inv_by = T->inv_by[r]; t.ny_hi = T->ny_hi[r];
+    t.inv_bz = T->inv_bz[r]; t.nz_hi = T->nz_hi[r]; t.ny = T->ny[r]; t.bin_base = T->bin_base[r];
+    tab[r] = t;
+  }
+  for (int i = threadIdx.x; i <= ns; i += blockDim.x) s_start_off[i] = st->start_off[i];
+  __syncthreads();
+  if (st->err_capacity) return;
+  const int n_start = st->n_start;
+  KFConst K;
+  K.Bc = T->Bc; K.err2_y = T->err2_y; K.err2_z = T->err2_z; K.max_sinphi = T->max_sinphi;
+  K.c24 = (float)(1.0 / 24.0); K.c640 = (float)(3.0 / 640.0); K.c12 = (float)(1.0 / 12.0);
+  K.ic0 = T->init_cov[0]; K.ic1 = T->init_cov[1]; K.ic2 = T->init_cov[2]; K.ic3 = T->init_cov[3];
+  K.ic4 = T->init_cov[4];
+  const float win_y = T->win_y, win_z = T->win_z, gate = T->gate, margin = T->margin;
+  const float grid_z_lo = T->grid_z_lo;
+  const int max_gap = T->tc_max_gap, min_hits = T->tc_min_hits;
+  const float my = win_y + margin, mz = win_z + margin;
+  const size_t nbp1 = (size_t)T->bins_per_sector + 1;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+  for (;;) {
+    // dynamic work distribution: one warp takes 32 consecutive start hits
+    if (lane == 0) s_work[wid] = atomicAdd(&st->work_counter, 32);
+    __syncwarp();
+    const int slot = s_work[wid] + lane;
+    __syncwarp();
+    if (slot - lane >= n_start) break;
+    if (slot >= n_start) continue;
+
+    // sector of the slot
+    int s = 0;
+    {
+      int lo = 0, hi = ns - 1;
+      while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (s_start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
+      s = lo;
+    }
+    const int off = sec[s].off;
+    const float2* yz = syz + off;
+    const int32_t* ord = order + off;
+    const int32_t* lup = link_up + off;
+    const uint32_t* bs = bin_start + (size_t)s * nbp1;
+    const int32_t* rs = row_start + s * (n_rows + 1);
+    const int c0 = start_hit[slot];
+    const int r0 = row_search(rs, n_rows, c0);
+    const int c1 = lup[c0];
+    const float2 h0 = yz[c0], h1 = yz[c1];
+    const float z_ref = h0.y;
+    KF f;
+    {
+      const float dx = tab[r0 + 1].x - tab[r0].x;
+      const float dy = h1.x - h0.x;
+      const float dz = h1.y - z_ref;
+      const float d = sqrtf(dx * dx + dy * dy);
+      f.x = tab[r0].x;
+      f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
+      kf_reset_cov(f, K);
+    }
+    // search: best cluster of row r in the tc window around the prediction
+    auto search = [&](int r, float& best_d2) -> int {
+      const RowTab t = tab[r];
+      const float yc = f.p0;
+      const float zc = z_ref + f.p1;
+      const int by0 = bin_coord(yc - my, t.y_lo, t.inv_by, t.ny_hi), by1 = bin_coord(yc + my, t.y_lo, t.inv_by, t.ny_hi);
+      const int bz0 = bin_coord(zc - mz, grid_z_lo, t.inv_bz, t.nz_hi), bz1 = bin_coord(zc + mz, grid_z_lo, t.inv_bz, t.nz_hi);
+      const float wy = f.c00 + K.err2_y;
+      const float wz = f.c11 + K.err2_z;
+      int best = -1;
+      for (int bz = bz0; bz <= bz1; ++bz) {
+        const int b0 = t.bin_base + bz * t.ny;
+        const uint32_t e = __ldg(&bs[b0 + by1 + 1]);
+        for (uint32_t c = __ldg(&bs[b0 + by0]); c < e; ++c) {
+          const float2 h = __ldg(&yz[c]);
+          const float ry = h.x - f.p0;
+          const float rz = (h.y - z_ref) - f.p1;
+          if (!(fabsf(ry) <= win_y && fabsf(rz) <= win_z)) continue;
+          const float d2 = (ry * ry) / wy + (rz * rz) / wz;
+          if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
+            best = (int)c; best_d2 = d2;
+          }
+        }
+      }
+      return best;
+    };
+
+    // ---- unified phase loop --------------------------------------------------------------------
+    enum { PH_A = 0, PH_B = 1, PH_C = 2, PH_DONE = 3 };
+    int phase = PH_A;
+    int r = r0, cur = c0, top = r0, gap = 0;
+    int n_hits = 0, first = r0;
+    bool have_snap = false;
+    KF snap = f;
+    int32_t* hcol = hits + slot;
+    while (phase != PH_DONE) {
+      // phase transitions that need no propagation
+      if (phase == PH_A && cur == -1) { phase = PH_B; gap = 0; }          // r == last + 1 already
+      if (phase == PH_B && r >= n_rows) { phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; }
+      if (phase == PH_C && r < 0) { phase = PH_DONE; break; }
+      if (!kf_propagate(f, tab[r].x, K)) {
+        if (phase == PH_C) { phase = PH_DONE; break; }
+        // rows (top, r] of the up pass that were never decided hold no hit
+        phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top;
+        continue;
+      }
+      int take = -1;          // cluster to update with
+      bool is_new = false;    // hit[r] was empty before
+      if (phase == PH_A) {
+        const float2 h = yz[cur];
+        const float ym = h.x, zm = h.y - z_ref;
+        bool ok = true;
+        if (f.n >= 2) {
+          const float ry = ym - f.p0, rz = zm - f.p1;
+          const float d2 = (ry * ry) / (f.c00 + K.err2_y) + (rz * rz) / (f.c11 + K.err2_z);
+          ok = !(d2 > gate);
+        }
+        if (!ok) { phase = PH_B; gap = 0; continue; }   // state already sits on row r (dx = 0 next)
+        take = cur; is_new = true;
+      } else if (phase == PH_B) {
+        float d2 = 0.f;
+        const int b = search(r, d2);
+        if (b >= 0 && d2 <= gate) { take = b; is_new = true; }
+      } else {
+        const int hr = (r >= r0 && r <= top) ? hcol[(size_t)r * cap] : -1;
+        if (hr != -1) { take = hr; }
+        else if (f.n >= 2) {
+          float d2 = 0.f;
+          const int b = search(r, d2);
+          if (b >= 0 && d2 <= gate) { take = b; is_new = true; }
+        }
+      }
+      if (take >= 0) {
+        const float2 h = yz[take];
+        kf_update(f, h.x, h.y - z_ref, K);
+        if (is_new) { hcol[(size_t)r * cap] = take; ++n_hits; }
+        if (phase == PH_C) {
+          snap = f; have_snap = true;
+          if (is_new) { gap = 0; if (r < first) first = r; }
+        } else {
+          top = r; gap = 0;
+        }
+      } else {
+        if (phase == PH_B) {
+          hcol[(size_t)r * cap] = -1;
+          if (++gap > max_gap) { phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; continue; }
+        } else {   // PH_C, nothing taken
+          if (r < r0) {
+            hcol[(size_t)r * cap] = -1;
+            if (++gap > max_gap) { phase = PH_DONE; break; }
+          }
+        }
+      }
+      if (phase == PH_A) { cur = lup[cur]; ++r; }
+      else if (phase == PH_B) ++r;
+      else --r;
+    }
+    // ---- emit into slot space --------------------------------------------------------------------
+    const bool accept = (n_hits >= min_hits) && have_snap;
+    trk_i[0 * (size_t)cap + slot] = accept ? n_hits : 0;
+    if (accept) {
+      trk_i[1 * (size_t)cap + slot] = snap.n;
+      trk_i[2 * (size_t)cap + slot] = first;
+      trk_i[3 * (size_t)cap + slot] = top;
+      float* o = trk_f + slot;
+      const size_t cs = (size_t)cap;
+      o[0 * cs] = snap.x; o[1 * cs] = z_ref;
+      o[2 * cs] = snap.p0; o[3 * cs] = snap.p1; o[4 * cs] = snap.p2; o[5 * cs] = snap.p3; o[6 * cs] = snap.p4;
+      o[7 * cs] = snap.c00; o[8 * cs] = snap.c10; o[9 * cs] = snap.c11; o[10 * cs] = snap.c20;
+      o[11 * cs] = snap.c21; o[12 * cs] = snap.c22; o[13 * cs] = snap.c30; o[14 * cs] = snap.c31;
+      o[15 * cs] = snap.c32; o[16 * cs] = snap.c33; o[17 * cs] = snap.c40; o[18 * cs] = snap.c41;
+      o[19 * cs] = snap.c42; o[20 * cs] = snap.c43; o[21 * cs] = snap.c44; o[22 * cs] = snap.chi2;
+    }
+  }
+}
+
+// ---- K5b: per-tile (1024 slots) sums of (accepted, n_hits) ------------------------------------
+__global__ void __launch_bounds__(1024)
+k_track_tile_sums(const DevStatus* __restrict__ st, const int32_t* __restrict__ trk_i, int2* __restrict__ tile_cnt) {
+  __shared__ int ws[33];
+  const int n_start = st->err_capacity ? 0 : st->n_start;
+  const int slot = blockIdx.x * 1024 + threadIdx.x;
+  const int nh = slot < n_start ? trk_i[slot] : 0;
+  int ta, tb;
+  block_exclusive_scan<int>(nh > 0 ? 1 : 0, ws, ta);
+  block_exclusive_scan<int>(nh, ws, tb);
+  if (threadIdx.x == 0) tile_cnt[blockIdx.x] = make_int2(ta, tb);
+}
+
+// ---- K5c': sector bases of the track table and of the hit CSR ---------------------------------
+__global__ void k_track_sector_bases(const DevTables* __restrict__ T, DevStatus* __restrict__ st,
+                                     const int32_t* __restrict__ trk_i, const longlong2* __restrict__ tile_off,
+                                     const int64_t* __restrict__ tot) {
+  const int ns = T->n_sectors;
+  const int s = threadIdx.x;
+  if (s > ns) return;
+  const int n_start = st->err_capacity ? 0 : st->n_start;
+  const int slot = st->err_capacity ? 0 : st->start_off[s];
+  if (slot >= n_start) { st->trk_off[s] = (int32_t)tot[0]; st->hit_off[s] = tot[1]; return; }
+  const int t = slot >> 10;
+  long long a = tile_off[t].x, b = tile_off[t].y;
+  for (int q = t << 10; q < slot; ++q) { const int nh = trk_i[q]; a += nh > 0; b += nh; }
+  st->trk_off[s] = (int32_t)a;
+  st->hit_off[s] = b;
+}
+
+// ---- K5d: gather accepted tracklets into the track table + hit CSR (start-hit order) ----------
+struct TrackOut {
+  float *x_ref, *z_ref, *par, *cov, *chi2;
+  int32_t *n_hits, *n_fit, *first_row, *last_row, *start_hit, *hit_offset, *hit_idx;
+};
+
+__global__ void __launch_bounds__(1024)
+k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st,
+               const int32_t* __restrict__ start_hit, int32_t cap, const int32_t* __restrict__ hits,
+               const float* __restrict__ trk_f, const int32_t* __restrict__ trk_i,
+               const longlong2* __restrict__ tile_off, TrackOut o) {
+  __shared__ int ws[33];
+  const int ns = T->n_sectors;
+  const int n_start = st->err_capacity ? 0 : st->n_start;
+  const int slot = blockIdx.x * 1024 + threadIdx.x;
+  const int nh = slot < n_start ? trk_i[slot] : 0;
+  int ta, tb;
+  const int ea = block_exclusive_scan<int>(nh > 0 ? 1 : 0, ws, ta);
+  const int eb = block_exclusive_scan<int>(nh, ws, tb);
+  if (slot >= n_start) return;
+  // sector of the slot
+  int s = 0;
+  {
+    int lo = 0, hi = ns - 1;
+    while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (st->start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
+    s = lo;
+  }
+  const long long t = tile_off[blockIdx.x].x + ea;       // global track index
+  const long long h = tile_off[blockIdx.x].y + eb;       // global hit index
+  const long long hloc = h - st->hit_off[s];
+  // hit_offset of sector s lives at [trk_off[s] + s, trk_off[s+1] + s + 1)
+  if (nh > 0) {
+    const size_t cs = (size_t)cap;
+    o.hit_offset[t + s] = (int32_t)hloc;
+    o.x_ref[t] = trk_f[0 * cs + slot];
+    o.z_ref[t] = trk_f[1 * cs + slot];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) o.par[i * cs + t] = trk_f[(2 + i) * cs + slot];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) o.cov[i * cs + t] = trk_f[(7 + i) * cs + slot];
+    o.chi2[t] = trk_f[22 * cs + slot];
+    o.n_hits[t] = nh;
+    o.n_fit[t] = trk_i[1 * cs + slot];
+    const int first = trk_i[2 * cs + slot], last = trk_i[3 * cs + slot];
+    o.first_row[t] = first;
+    o.last_row[t] = last;
+    o.start_hit[t] = start_hit[slot];
+    long long w = h;
+    for (int r = first; r <= last; ++r) {
+      const int c = hits[(size_t)r * cs + slot];
+      if (c != -1) o.hit_idx[w++] = c;
+    }
+  }
+  // closing entry of each sector's hit_offset: written by the last slot of the sector
+  if (slot + 1 == st->start_off[s + 1] || slot + 1 == n_start) {
+    // all later sectors that are empty share the same closing value pattern: handle each sector
+    // whose slot range ends here (this one) -- empty sectors are closed by k_track_close_empty.
+    const long long tend = t + (nh > 0 ? 1 : 0);
+    o.hit_offset[tend + s] = (int32_t)(hloc + nh);
+  }
+}
+
+// sectors without start hits still own a one-entry hit_offset = {0}
+__global__ void k_track_close_empty(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, TrackOut o) {
+  const int ns = T->n_sectors;
+  const int s = threadIdx.x;
+  if (s >= ns) return;
+  const bool bad = st->err_capacity != 0;
+  if (bad || st->start_off[s] == st->start_off[s + 1]) o.hit_offset[(bad ? 0 : st->trk_off[s]) + s] = 0;
+}
+
+}  // namespace tpcca

@@ -1,0 +1,557 @@
+// Host side of the tpcca C-ABI (include/tpcca.h): workspace carving, stage scheduling on the
+// caller's stream, per-stage CUDA events, error mapping.  No torch types, no CPU compute path:
+// every stage of the hot path runs in the kernels of k_grid.cuh / k_links.cuh / k_tracklets.cuh.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "k_tracklets.cuh"
+
+using namespace tpcca;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+// ---- workspace layout -------------------------------------------------------------
+struct Layout {
+  size_t tables, sec, status, tot;
+  size_t in_y, in_z, in_row;
+  size_t syz, order, bin_start, row_start, multi_list, bin_tile_sum;
+  size_t up_raw, dn_raw, up, dn;
+  size_t tile_cnt, tile_off;
+  size_t start_hit, hits, trk_f, trk_i;
+  size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
+  size_t total;
+  int64_t n_bin_tiles, n_tiles_max, multi_cap;
+};
+
+int64_t bins_per_sector(const tpcca_params* p) {
+  int64_t nb = 0;
+  for (int r = 0; r < p->n_rows; ++r) nb += (int64_t)p->grid_ny[r] * p->grid_nz[r];
+  return nb;
+}
+
+Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
+  Layout L{};
+  size_t cur = 0;
+  auto take = [&](size_t bytes) { size_t o = cur; cur = align_up(cur + bytes); return o; };
+  const int64_t ns = p->n_sectors, nr = p->n_rows, nb = bins_per_sector(p);
+  L.n_bin_tiles = ns * ((nb + kScanTile - 1) / kScanTile);
+  L.n_tiles_max = std::max<int64_t>(N / 2048 + ns + 1, CS / 1024 + 2);
+  L.multi_cap = N / 2 + 1;
+  L.tables = take(sizeof(DevTables));
+  L.sec = take(sizeof(SectorDesc) * (kMaxSectors + 1));
+  L.status = take(sizeof(DevStatus));
+  L.tot = take(sizeof(int64_t) * 4);
+  const size_t n_in = (size_t)N + 8 * kMaxSectors;   // every sector's copy starts 8-element aligned
+  L.in_y = take(4 * n_in);
+  L.in_z = take(4 * n_in);
+  L.in_row = take(2 * n_in);
+  L.syz = take(8 * (size_t)N);
+  L.order = take(4 * (size_t)N);
+  L.bin_start = take(4 * (size_t)(ns * (nb + 1)));
+  L.row_start = take(4 * (size_t)(ns * (nr + 1)));
+  L.multi_list = take(4 * (size_t)L.multi_cap);
+  L.bin_tile_sum = take(4 * (size_t)(L.n_bin_tiles + 1));
+  L.up_raw = take(4 * (size_t)N);
+  L.dn_raw = take(4 * (size_t)N);
+  L.up = take(4 * (size_t)N);
+  L.dn = take(4 * (size_t)N);
+  L.tile_cnt = take(sizeof(int2) * (size_t)L.n_tiles_max);
+  L.tile_off = take(sizeof(longlong2) * (size_t)L.n_tiles_max);
+  L.start_hit = take(4 * (size_t)CS);
+  L.hits = take(4 * (size_t)(nr * CS));
+  L.trk_f = take(4 * (size_t)(kTrkF * CS));
+  L.trk_i = take(4 * (size_t)(kTrkI * CS));
+  L.o_x_ref = take(4 * (size_t)CS);
+  L.o_z_ref = take(4 * (size_t)CS);
+  L.o_chi2 = take(4 * (size_t)CS);
+  L.o_par = take(4 * (size_t)(5 * CS));
+  L.o_cov = take(4 * (size_t)(15 * CS));
+  L.o_n_hits = take(4 * (size_t)CS);
+  L.o_n_fit = take(4 * (size_t)CS);
+  L.o_first = take(4 * (size_t)CS);
+  L.o_last = take(4 * (size_t)CS);
+  L.o_start = take(4 * (size_t)CS);
+  L.o_hit_offset = take(4 * (size_t)(CS + ns + 1));
+  L.o_hit_idx = take(4 * (size_t)(nr * CS));
+  L.total = cur;
+  return L;
+}
+
+int check_params(const tpcca_params* p, std::string& err) {
+  auto fail = [&](const char* m) { err = m; return TPCCA_E_ARG; };
+  if (!p) return fail("params is NULL");
+  if (p->n_sectors < 1 || p->n_sectors > TPCCA_MAX_SECTORS) return fail("n_sectors out of range");
+  if (p->n_rows < 3 || p->n_rows > TPCCA_MAX_ROWS) return fail("n_rows out of range (3..TPCCA_MAX_ROWS)");
+  if (!p->row_x || !p->grid_y_lo || !p->grid_inv_bin_y || !p->grid_ny || !p->grid_inv_bin_z || !p->grid_nz ||
+      !p->nf_hy_up || !p->nf_hz_up || !p->nf_hy_dn || !p->nf_hz_dn || !p->nf_cut)
+    return fail("a table pointer is NULL");
+  int64_t nb = 0;
+  for (int r = 0; r < p->n_rows; ++r) {
+    if (p->grid_ny[r] < 1 || p->grid_nz[r] < 1) return fail("grid_ny / grid_nz must be >= 1");
+    if (p->grid_ny[r] >= (1 << 24) || p->grid_nz[r] >= (1 << 24)) return fail("grid_ny / grid_nz must be < 2^24");
+    if (r > 0 && !(p->row_x[r] > p->row_x[r - 1])) return fail("row_x must be strictly increasing");
+    nb += (int64_t)p->grid_ny[r] * p->grid_nz[r];
+  }
+  if ((nb + 1) * (int64_t)p->n_sectors >= (int64_t)0xFFFFFFF0u) return fail("too many grid bins (n_sectors * (bins + 1) must fit 32 bits)");
+  if (nb >= 0x7FFFFFF0) return fail("too many grid bins per sector");
+  return TPCCA_OK;
+}
+
+int64_t default_cap(int64_t N, int64_t CS) {
+  if (CS <= 0) CS = N / 8 + 1024;
+  if (CS > N / 2 + 1) CS = N / 2 + 1;
+  if (CS < 1) CS = 1;
+  return CS;
+}
+
+}  // namespace
+
+struct tpcca_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  char* ws = nullptr;
+  size_t ws_bytes = 0;
+  int64_t N = 0, CS = 0;
+  int ns = 0, nr = 0;
+  int64_t nb = 0;
+  Layout L{};
+  DevTables tab{};
+  // sectors
+  struct Sec { bool loaded = false; int64_t n = 0; const float* y = nullptr; const float* z = nullptr; const uint16_t* row = nullptr; };
+  std::vector<Sec> sec;
+  int64_t in_used = 0;
+  std::vector<SectorDesc> desc;       // as uploaded by the last run
+  int64_t n_total = 0;
+  int n_tiles256 = 0, n_tiles2048 = 0;
+  uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
+  bool desc_valid = false;
+  cudaEvent_t ev[7]{};
+  bool ev_valid[7]{};
+  int64_t launches = 0;
+  DevStatus status{};
+  bool status_valid = false;
+  std::vector<std::vector<char>> host_bufs;
+  std::string err;
+
+  template <class Tp> Tp* at(size_t off) const { return reinterpret_cast<Tp*>(ws + off); }
+};
+
+namespace {
+
+int set_err(tpcca_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf; else g_last_error = buf;
+  return code;
+}
+
+#define CU(c, call)                                                                             \
+  do {                                                                                          \
+    cudaError_t e_ = (call);                                                                    \
+    if (e_ != cudaSuccess) return set_err((c), TPCCA_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+int fetch_status(tpcca_ctx* c) {
+  CU(c, cudaStreamSynchronize(c->stream));
+  CU(c, cudaMemcpy(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost));
+  c->status_valid = true;
+  if (c->status.err_range) return set_err(c, TPCCA_E_RANGE, "a cluster has row >= n_rows (%d)", c->nr);
+  if (c->status.err_capacity)
+    return set_err(c, TPCCA_E_WORKSPACE, "start-hit capacity exceeded: %d start hits > max_start_hits %lld",
+                   c->status.n_start, (long long)c->CS);
+  if (c->status.n_multi > (uint32_t)c->L.multi_cap) return set_err(c, TPCCA_E_WORKSPACE, "internal: multi-bin list overflow");
+  return TPCCA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tpcca_version(void) { return "tpcca 0.1 (sm_100a)"; }
+
+const char* tpcca_last_error(const tpcca_ctx* ctx) { return ctx ? ctx->err.c_str() : g_last_error.c_str(); }
+
+int tpcca_workspace_bytes(const tpcca_params* params, int64_t max_clusters_total, int64_t max_start_hits,
+                          size_t* out_bytes) {
+  std::string e;
+  int rc = check_params(params, e);
+  if (rc) return set_err(nullptr, rc, "%s", e.c_str());
+  if (!out_bytes || max_clusters_total < 0 || max_clusters_total >= 0x7FFFFF00)
+    return set_err(nullptr, TPCCA_E_ARG, "max_clusters_total must be in [0, 2^31)");
+  const int64_t N = std::max<int64_t>(max_clusters_total, 1);
+  *out_bytes = make_layout(params, N, default_cap(N, max_start_hits)).total;
+  return TPCCA_OK;
+}
+
+int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void* workspace, size_t workspace_bytes,
+                 int64_t max_clusters_total, int64_t max_start_hits, tpcca_ctx** out_ctx) {
+  if (!out_ctx) return set_err(nullptr, TPCCA_E_ARG, "out_ctx is NULL");
+  *out_ctx = nullptr;
+  std::string e;
+  int rc = check_params(p, e);
+  if (rc) return set_err(nullptr, rc, "%s", e.c_str());
+  if (max_clusters_total < 0 || max_clusters_total >= 0x7FFFFF00)
+    return set_err(nullptr, TPCCA_E_ARG, "max_clusters_total must be in [0, 2^31)");
+  int n_dev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&n_dev);
+  if (ce != cudaSuccess || n_dev <= 0)
+    return set_err(nullptr, TPCCA_E_CUDA, "no usable CUDA device (%s); tpcca has no CPU path",
+                   ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0");
+  if (cuda_device < 0 || cuda_device >= n_dev) return set_err(nullptr, TPCCA_E_ARG, "cuda_device out of range");
+  CU(nullptr, cudaSetDevice(cuda_device));
+  cudaDeviceProp prop;
+  CU(nullptr, cudaGetDeviceProperties(&prop, cuda_device));
+  if (prop.major != 10)
+    return set_err(nullptr, TPCCA_E_CUDA, "device %d is sm_%d%d; this library holds sm_100a code only", cuda_device,
+                   prop.major, prop.minor);
+  const int64_t N = std::max<int64_t>(max_clusters_total, 1);
+  const int64_t CS = default_cap(N, max_start_hits);
+  Layout L = make_layout(p, N, CS);
+  if (!workspace || ((uintptr_t)workspace & (kAlign - 1))) return set_err(nullptr, TPCCA_E_ARG, "workspace must be a 256-byte aligned device pointer");
+  if (workspace_bytes < L.total)
+    return set_err(nullptr, TPCCA_E_WORKSPACE, "workspace too small: %zu bytes given, %zu required", workspace_bytes, L.total);
+
+  tpcca_ctx* c = new tpcca_ctx;
+  c->device = cuda_device;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->ws = (char*)workspace;
+  c->ws_bytes = workspace_bytes;
+  c->N = N; c->CS = CS; c->ns = p->n_sectors; c->nr = p->n_rows; c->nb = bins_per_sector(p);
+  c->L = L;
+  c->sec.resize(c->ns);
+  DevTables& t = c->tab;
+  memset(&t, 0, sizeof t);
+  t.n_rows = p->n_rows; t.n_sectors = p->n_sectors; t.bins_per_sector = (int32_t)c->nb;
+  t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits;
+  t.grid_z_lo = p->grid_z_lo; t.Bc = p->kappa_per_qpt; t.err2_y = p->err2_y; t.err2_z = p->err2_z;
+  for (int i = 0; i < 5; ++i) t.init_cov[i] = p->init_cov[i];
+  t.win_y = p->tc_win_y; t.win_z = p->tc_win_z; t.gate = p->tc_gate; t.max_sinphi = p->max_sinphi;
+  t.margin = p->grid_margin;
+  int32_t base = 0;
+  for (int r = 0; r < p->n_rows; ++r) {
+    t.row_x[r] = p->row_x[r]; t.y_lo[r] = p->grid_y_lo[r]; t.inv_by[r] = p->grid_inv_bin_y[r];
+    t.inv_bz[r] = p->grid_inv_bin_z[r]; t.ny[r] = p->grid_ny[r]; t.nz[r] = p->grid_nz[r];
+    t.ny_hi[r] = (float)(p->grid_ny[r] - 1); t.nz_hi[r] = (float)(p->grid_nz[r] - 1);
+    t.bin_base[r] = base; base += p->grid_ny[r] * p->grid_nz[r];
+    t.hy_up[r] = p->nf_hy_up[r]; t.hz_up[r] = p->nf_hz_up[r]; t.hy_dn[r] = p->nf_hy_dn[r];
+    t.hz_dn[r] = p->nf_hz_dn[r]; t.nf_cut[r] = p->nf_cut[r];
+  }
+  t.bin_base[p->n_rows] = base;
+  cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
+  if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
+  for (int i = 0; i < 7 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[i]);
+  if (e1 != cudaSuccess) {
+    set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
+    delete c;
+    return TPCCA_E_CUDA;
+  }
+  *out_ctx = c;
+  return TPCCA_OK;
+}
+
+int tpcca_reset(tpcca_ctx* c) {
+  if (!c) return TPCCA_E_ARG;
+  for (auto& s : c->sec) s = tpcca_ctx::Sec();
+  c->in_used = 0;
+  c->done_mask = 0;
+  c->desc_valid = false;
+  c->status_valid = false;
+  return TPCCA_OK;
+}
+
+int tpcca_load_clusters(tpcca_ctx* c, int sector, int64_t n, const float* x, const float* y, const float* z,
+                        const float* charge, const uint16_t* row, int mem_space) {
+  (void)x; (void)charge;   // part of the cluster record, not read by S1-S5 (tpcca.h)
+  if (!c) return TPCCA_E_ARG;
+  if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
+  if (n < 0 || (n > 0 && (!y || !z || !row))) return set_err(c, TPCCA_E_ARG, "n < 0 or y/z/row NULL");
+  if (mem_space < 0 || mem_space > 2) return set_err(c, TPCCA_E_ARG, "bad mem_space");
+  if (c->sec[sector].loaded) return set_err(c, TPCCA_E_STATE, "sector %d already loaded; call tpcca_reset first", sector);
+  int64_t tot = n;
+  for (auto& s : c->sec) if (s.loaded) tot += s.n;
+  if (tot > c->N) return set_err(c, TPCCA_E_WORKSPACE, "%lld clusters exceed max_clusters_total %lld", (long long)tot, (long long)c->N);
+  auto& S = c->sec[sector];
+  if (mem_space == TPCCA_MEM_DEVICE_BORROW || n == 0) {
+    S.y = y; S.z = z; S.row = row;
+  } else {
+    // 8-element alignment keeps every sector's copy 16-byte aligned
+    const int64_t o = c->in_used;
+    float* dy = c->at<float>(c->L.in_y) + o;
+    float* dz = c->at<float>(c->L.in_z) + o;
+    uint16_t* dr = c->at<uint16_t>(c->L.in_row) + o;
+    const cudaMemcpyKind k = mem_space == TPCCA_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    CU(c, cudaMemcpyAsync(dy, y, 4 * (size_t)n, k, c->stream));
+    CU(c, cudaMemcpyAsync(dz, z, 4 * (size_t)n, k, c->stream));
+    CU(c, cudaMemcpyAsync(dr, row, 2 * (size_t)n, k, c->stream));
+    S.y = dy; S.z = dz; S.row = dr;
+    c->in_used += (n + 7) / 8 * 8;   // (fits: the total check above bounds the sum of n by N)
+  }
+  S.n = n; S.loaded = true;
+  c->done_mask = 0;
+  c->desc_valid = false;
+  c->status_valid = false;
+  return TPCCA_OK;
+}
+
+int tpcca_run(tpcca_ctx* c, uint32_t mask) {
+  if (!c) return TPCCA_E_ARG;
+  mask &= TPCCA_STAGE_ALL;
+  if (!mask) return set_err(c, TPCCA_E_ARG, "empty stage mask");
+  // a stage needs everything before it
+  for (int i = 0; i < 5; ++i)
+    if (mask & (1u << i)) {
+      const uint32_t need = (1u << i) - 1u;
+      if ((need & ~(c->done_mask | mask)) != 0)
+        return set_err(c, TPCCA_E_STATE, "stage %d needs the outputs of earlier stages (done 0x%x, asked 0x%x)", i + 1, c->done_mask, mask);
+    }
+  CU(c, cudaSetDevice(c->device));
+  const Layout& L = c->L;
+  cudaStream_t st = c->stream;
+  c->launches = 0;
+  c->status_valid = false;
+  c->host_bufs.clear();
+  // ---- sector descriptors
+  if (!c->desc_valid) {
+    c->desc.assign(kMaxSectors + 1, SectorDesc{});
+    int64_t off = 0, t256 = 0, t2048 = 0, bt = 0;
+    const int64_t bin_tiles = (c->nb + kScanTile - 1) / kScanTile;
+    for (int s = 0; s <= c->ns; ++s) {
+      SectorDesc& d = c->desc[s];
+      const int64_t n = s < c->ns ? c->sec[s].n : 0;
+      if (s < c->ns) { d.y = c->sec[s].y; d.z = c->sec[s].z; d.row = c->sec[s].row; }
+      d.n = (int32_t)n; d.off = (int32_t)off; d.tile256 = (int32_t)t256; d.tile2048 = (int32_t)t2048; d.bin_tile = (int32_t)bt;
+      off += n; t256 += (n + 255) / 256; t2048 += (n + 2047) / 2048; bt += bin_tiles;
+    }
+    c->n_total = off; c->n_tiles256 = (int)t256; c->n_tiles2048 = (int)t2048;
+    CU(c, cudaMemcpyAsync(c->at<SectorDesc>(L.sec), c->desc.data(), sizeof(SectorDesc) * (kMaxSectors + 1), cudaMemcpyHostToDevice, st));
+    c->desc_valid = true;
+  }
+  const DevTables* T = c->at<DevTables>(L.tables);
+  const SectorDesc* sec = c->at<SectorDesc>(L.sec);
+  DevStatus* status = c->at<DevStatus>(L.status);
+  int64_t* tot = c->at<int64_t>(L.tot);
+  float2* syz = c->at<float2>(L.syz);
+  int32_t* order = c->at<int32_t>(L.order);
+  uint32_t* bin_start = c->at<uint32_t>(L.bin_start);
+  int32_t* row_start = c->at<int32_t>(L.row_start);
+  int2* tile_cnt = c->at<int2>(L.tile_cnt);
+  longlong2* tile_off = c->at<longlong2>(L.tile_off);
+  int32_t* start_hit = c->at<int32_t>(L.start_hit);
+  const int32_t cap = (int32_t)c->CS;
+  for (int i = 0; i < 7; ++i) c->ev_valid[i] = false;
+  auto mark = [&](int i) { cudaEventRecord(c->ev[i], st); c->ev_valid[i] = true; };
+  mark(0);
+
+  if (mask & TPCCA_STAGE_GRID) {
+    CU(c, cudaMemsetAsync(status, 0, sizeof(DevStatus), st));
+    CU(c, cudaMemsetAsync(bin_start, 0, 4 * (size_t)c->ns * (size_t)(c->nb + 1), st));
+    uint32_t* multi = c->at<uint32_t>(L.multi_list);
+    uint32_t* tsum = c->at<uint32_t>(L.bin_tile_sum);
+    if (c->n_tiles256 > 0) {
+      k_grid_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, bin_start, multi, (uint32_t)L.multi_cap, status);
+      ++c->launches;
+    }
+    k_scan_tile_sums<<<(unsigned)L.n_bin_tiles, 256, 0, st>>>(T, sec, bin_start, tsum);
+    k_scan_sector_tiles<<<c->ns, 1024, 0, st>>>(sec, tsum);
+    k_scan_apply<<<(unsigned)L.n_bin_tiles, 256, 0, st>>>(T, sec, bin_start, tsum);
+    c->launches += 3;
+    if (c->n_tiles256 > 0) {
+      k_grid_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, bin_start, syz, order);
+      k_grid_fixup<<<148 * 8, 256, 0, st>>>(T, sec, bin_start, multi, status, syz, order);
+      c->launches += 2;
+    }
+    k_row_start<<<c->ns, 256, 0, st>>>(T, bin_start, row_start);
+    ++c->launches;
+  }
+  mark(1);
+  if ((mask & TPCCA_STAGE_NEIGHBOURS) && c->n_tiles256 > 0) {
+    k_neighbours<<<c->n_tiles256, 256, 0, st>>>(T, sec, syz, bin_start, row_start, order, c->at<int32_t>(L.up_raw),
+                                               c->at<int32_t>(L.dn_raw));
+    ++c->launches;
+  }
+  mark(2);
+  if ((mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
+    k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
+                                                 c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt);
+    ++c->launches;
+  }
+  mark(3);
+  if (mask & TPCCA_STAGE_START) {
+    // tile_cnt is S3's by-product; if S3 ran in an earlier call S5's scans may have reused the
+    // buffer, so S4 on its own recounts through S3's kernel (cheap, idempotent).
+    if (!(mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
+      k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
+                                                   c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt);
+      ++c->launches;
+    }
+    k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, c->n_tiles2048, tot);
+    k_start_offsets<<<1, kMaxSectors + 1, 0, st>>>(T, sec, tile_off, tot, c->n_tiles2048, cap, status);
+    c->launches += 2;
+    if (c->n_tiles2048 > 0) {
+      k_start_hits<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_off, cap, start_hit);
+      ++c->launches;
+    }
+  }
+  mark(4);
+  if (mask & TPCCA_STAGE_TRACKLETS) {
+    TrackOut o;
+    o.x_ref = c->at<float>(L.o_x_ref); o.z_ref = c->at<float>(L.o_z_ref); o.par = c->at<float>(L.o_par);
+    o.cov = c->at<float>(L.o_cov); o.chi2 = c->at<float>(L.o_chi2); o.n_hits = c->at<int32_t>(L.o_n_hits);
+    o.n_fit = c->at<int32_t>(L.o_n_fit); o.first_row = c->at<int32_t>(L.o_first); o.last_row = c->at<int32_t>(L.o_last);
+    o.start_hit = c->at<int32_t>(L.o_start); o.hit_offset = c->at<int32_t>(L.o_hit_offset); o.hit_idx = c->at<int32_t>(L.o_hit_idx);
+    int32_t* hits = c->at<int32_t>(L.hits);
+    float* trk_f = c->at<float>(L.trk_f);
+    int32_t* trk_i = c->at<int32_t>(L.trk_i);
+    const int cap_tiles = (int)((c->CS + 1023) / 1024);
+    CU(c, cudaMemsetAsync(&status->work_counter, 0, sizeof(int32_t), st));
+    k_tracklets<<<148 * 8, 128, 0, st>>>(T, sec, status, syz, bin_start, row_start, order, c->at<int32_t>(L.up), start_hit,
+                                         cap, hits, trk_f, trk_i);
+    k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
+    k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
+    k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
+    k_track_gather<<<cap_tiles, 1024, 0, st>>>(T, status, start_hit, cap, hits, trk_f, trk_i, tile_off, o);
+    k_track_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, o);
+    c->launches += 6;
+  }
+  mark(5);
+  CU(c, cudaGetLastError());
+  c->done_mask |= mask;
+  return TPCCA_OK;
+}
+
+int tpcca_sync(tpcca_ctx* c) {
+  if (!c) return TPCCA_E_ARG;
+  return fetch_status(c);
+}
+
+int tpcca_get_counts(tpcca_ctx* c, int64_t out[5]) {
+  if (!c || !out) return TPCCA_E_ARG;
+  int rc = fetch_status(c);
+  if (rc) return rc;
+  out[0] = c->n_total;
+  out[1] = (c->done_mask & TPCCA_STAGE_START) ? c->status.n_start : 0;
+  out[2] = (c->done_mask & TPCCA_STAGE_TRACKLETS) ? c->status.trk_off[c->ns] : 0;
+  out[3] = (c->done_mask & TPCCA_STAGE_TRACKLETS) ? c->status.hit_off[c->ns] : 0;
+  out[4] = c->nb;
+  return TPCCA_OK;
+}
+
+int tpcca_get_timings(tpcca_ctx* c, float ms[6]) {
+  if (!c || !ms) return TPCCA_E_ARG;
+  CU(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < 6; ++i) ms[i] = 0.f;
+  if (!c->ev_valid[0] || !c->ev_valid[5]) return set_err(c, TPCCA_E_STATE, "nothing was run");
+  for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[i], c->ev[i + 1]));
+  CU(c, cudaEventElapsedTime(&ms[5], c->ev[0], c->ev[5]));
+  return TPCCA_OK;
+}
+
+int tpcca_get_launch_count(const tpcca_ctx* c, int64_t* out) {
+  if (!c || !out) return TPCCA_E_ARG;
+  *out = c->launches;
+  return TPCCA_OK;
+}
+
+int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, tpcca_tracks_view* v) {
+  if (!c || !v) return TPCCA_E_ARG;
+  if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
+  if (mem_space != TPCCA_MEM_HOST && mem_space != TPCCA_MEM_DEVICE) return set_err(c, TPCCA_E_ARG, "bad mem_space");
+  if (!c->done_mask || !c->desc_valid) return set_err(c, TPCCA_E_STATE, "nothing was run");
+  int rc = fetch_status(c);
+  if (rc) return rc;
+  memset(v, 0, sizeof *v);
+  const Layout& L = c->L;
+  const DevStatus& S = c->status;
+  const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
+  const uint32_t done = c->done_mask;
+  v->n_clusters = n;
+  v->n_bins = c->nb;
+  const bool host = mem_space == TPCCA_MEM_HOST;
+  if (host) c->host_bufs.clear();
+  cudaError_t cerr = cudaSuccess;
+  auto out = [&](const void* dev, size_t bytes) -> const void* {
+    if (!host) return dev;
+    c->host_bufs.emplace_back(bytes ? bytes : 1);
+    if (bytes) {
+      cudaError_t e = cudaMemcpy(c->host_bufs.back().data(), dev, bytes, cudaMemcpyDeviceToHost);
+      if (e != cudaSuccess) cerr = e;
+    }
+    return c->host_bufs.back().data();
+  };
+  if (done & TPCCA_STAGE_GRID) {
+    v->order = (const int32_t*)out(c->at<int32_t>(L.order) + off, 4 * (size_t)n);
+    v->syz = (const float*)out(c->at<float2>(L.syz) + off, 8 * (size_t)n);
+    v->bin_start = (const uint32_t*)out(c->at<uint32_t>(L.bin_start) + (size_t)sector * (c->nb + 1), 4 * (size_t)(c->nb + 1));
+    v->row_start = (const int32_t*)out(c->at<int32_t>(L.row_start) + (size_t)sector * (c->nr + 1), 4 * (size_t)(c->nr + 1));
+  }
+  if (done & TPCCA_STAGE_NEIGHBOURS) {
+    v->link_up_raw = (const int32_t*)out(c->at<int32_t>(L.up_raw) + off, 4 * (size_t)n);
+    v->link_dn_raw = (const int32_t*)out(c->at<int32_t>(L.dn_raw) + off, 4 * (size_t)n);
+  }
+  if (done & TPCCA_STAGE_CLEAN) {
+    v->link_up = (const int32_t*)out(c->at<int32_t>(L.up) + off, 4 * (size_t)n);
+    v->link_dn = (const int32_t*)out(c->at<int32_t>(L.dn) + off, 4 * (size_t)n);
+  }
+  if (done & TPCCA_STAGE_START) {
+    const int64_t s0 = S.start_off[sector], s1 = S.start_off[sector + 1];
+    v->n_start = s1 - s0;
+    v->start_hit = (const int32_t*)out(c->at<int32_t>(L.start_hit) + s0, 4 * (size_t)(s1 - s0));
+  }
+  if (done & TPCCA_STAGE_TRACKLETS) {
+    const int64_t t0 = S.trk_off[sector], t1 = S.trk_off[sector + 1], nt = t1 - t0;
+    const int64_t h0 = S.hit_off[sector], h1 = S.hit_off[sector + 1];
+    v->n_tracks = nt;
+    v->n_hits = h1 - h0;
+    v->x_ref = (const float*)out(c->at<float>(L.o_x_ref) + t0, 4 * (size_t)nt);
+    v->z_ref = (const float*)out(c->at<float>(L.o_z_ref) + t0, 4 * (size_t)nt);
+    v->chi2 = (const float*)out(c->at<float>(L.o_chi2) + t0, 4 * (size_t)nt);
+    v->n_hits_trk = (const int32_t*)out(c->at<int32_t>(L.o_n_hits) + t0, 4 * (size_t)nt);
+    v->n_fit = (const int32_t*)out(c->at<int32_t>(L.o_n_fit) + t0, 4 * (size_t)nt);
+    v->first_row = (const int32_t*)out(c->at<int32_t>(L.o_first) + t0, 4 * (size_t)nt);
+    v->last_row = (const int32_t*)out(c->at<int32_t>(L.o_last) + t0, 4 * (size_t)nt);
+    v->trk_start_hit = (const int32_t*)out(c->at<int32_t>(L.o_start) + t0, 4 * (size_t)nt);
+    v->hit_offset = (const int32_t*)out(c->at<int32_t>(L.o_hit_offset) + t0 + sector, 4 * (size_t)(nt + 1));
+    v->hit_idx = (const int32_t*)out(c->at<int32_t>(L.o_hit_idx) + h0, 4 * (size_t)(h1 - h0));
+    if (!host) {
+      v->trk_stride = c->CS;
+      v->par = c->at<float>(L.o_par) + t0;
+      v->cov = c->at<float>(L.o_cov) + t0;
+    } else {
+      v->trk_stride = nt;
+      c->host_bufs.emplace_back(4 * (size_t)std::max<int64_t>(5 * nt, 1));
+      char* hp = c->host_bufs.back().data();
+      c->host_bufs.emplace_back(4 * (size_t)std::max<int64_t>(15 * nt, 1));
+      char* hc = c->host_bufs.back().data();
+      if (nt > 0) {
+        cudaError_t e = cudaMemcpy2D(hp, 4 * (size_t)nt, c->at<float>(L.o_par) + t0, 4 * (size_t)c->CS, 4 * (size_t)nt, 5, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) cerr = e;
+        e = cudaMemcpy2D(hc, 4 * (size_t)nt, c->at<float>(L.o_cov) + t0, 4 * (size_t)c->CS, 4 * (size_t)nt, 15, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) cerr = e;
+      }
+      v->par = (const float*)hp;
+      v->cov = (const float*)hc;
+    }
+  }
+  if (cerr != cudaSuccess) return set_err(c, TPCCA_E_CUDA, "D2H copy failed: %s", cudaGetErrorString(cerr));
+  return TPCCA_OK;
+}
+
+void tpcca_destroy(tpcca_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  for (int i = 0; i < 7; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  delete c;
+}
+
+}  // extern "C"

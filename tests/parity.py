@@ -1,0 +1,128 @@
+"""Element-by-element comparison of the CUDA path (paper_2208_07412_b200.SectorOutput) with the
+CPU oracle (oracle.OracleResult).  Used by the -m gpu parity tests, smoke() and bench.py's check.
+
+The bar (BASELINE.json:5 north_star, readings N4/N5 of DESIGN.md 3.8):
+  * grid, links, start hits, track membership: bit-exact.  Link exception: clusters whose link pair
+    differs are allowed iff the oracle-rescored scores of the two pairs agree to 1e-5 relative,
+    and such clusters are <= 0.1 % of the oracle's linked clusters;
+  * fitted parameters: |a-b| <= 1e-4 * max(|a|,|b|,floor_i), floors (1 cm, 1 cm, 0.1, 0.1, 0.1/GeV);
+    covariances: |dC_ij| <= 1e-4 * sqrt(C_ii C_jj); chi2: 1e-4 relative (floor 1e-3).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+PAR_FLOOR = np.array([1.0, 1.0, 0.1, 0.1, 0.1])
+TRI = [(i, j) for i in range(5) for j in range(i + 1)]   # k = i(i+1)/2 + j
+
+
+class ParityError(AssertionError):
+    pass
+
+
+def _eq(name, a, b, report):
+    a = np.asarray(a); b = np.asarray(b)
+    if a.shape != b.shape:
+        raise ParityError(f"{name}: shape {a.shape} (gpu) vs {b.shape} (oracle)")
+    if not np.array_equal(a, b):
+        bad = np.nonzero(a != b)[0]
+        raise ParityError(f"{name}: {bad.size} of {a.size} differ; first at {bad[0]}: gpu {a[bad[0]]} oracle {b[bad[0]]}")
+    report[name] = "bit-exact"
+
+
+def compare_sector(gpu, orc, oracle_obj=None, srow=None, stages=0x1F) -> dict:
+    """Raise ParityError on any violation of the bar; return a small report dict."""
+    rep = {}
+    if gpu.n != orc.n:
+        raise ParityError(f"n_clusters {gpu.n} vs {orc.n}")
+    if stages & 1:
+        _eq("order", gpu.order, orc.order, rep)
+        _eq("sy", gpu.sy, orc.sy.astype(np.float32), rep)
+        _eq("sz", gpu.sz, orc.sz.astype(np.float32), rep)
+        _eq("bin_start", gpu.bin_start, orc.bin_start, rep)
+        _eq("row_start", gpu.row_start, orc.row_start, rep)
+    if stages & 2:
+        du = gpu.link_up_raw != orc.link_up_raw
+        dd = gpu.link_dn_raw != orc.link_dn_raw
+        diff = np.nonzero(du | dd)[0]
+        rep["links_differing"] = int(diff.size)
+        if diff.size:
+            # reading N4: rescore both pairs with the oracle's arithmetic
+            if oracle_obj is None or srow is None:
+                raise ParityError(f"raw links differ at {diff.size} clusters (first {diff[0]})")
+            n_linked = max(int((orc.link_up_raw >= 0).sum()), 1)
+            for c in diff:
+                gu, gd, ou, od = gpu.link_up_raw[c], gpu.link_dn_raw[c], orc.link_up_raw[c], orc.link_dn_raw[c]
+                if min(gu, gd, ou, od) < 0:
+                    raise ParityError(f"raw link of cluster {c}: gpu ({gu},{gd}) oracle ({ou},{od})")
+                r = int(srow[c])
+                sg = oracle_obj.score(r, orc.sy[c], orc.sz[c], orc.sy[gu], orc.sz[gu], orc.sy[gd], orc.sz[gd])
+                so = oracle_obj.score(r, orc.sy[c], orc.sz[c], orc.sy[ou], orc.sz[ou], orc.sy[od], orc.sz[od])
+                if abs(sg - so) > 1e-5 * max(sg, so, 1e-12):
+                    raise ParityError(f"raw link of cluster {c}: scores {sg} (gpu pair) vs {so} (oracle pair)")
+            if diff.size > 1e-3 * n_linked:
+                raise ParityError(f"{diff.size} differing links > 0.1 % of {n_linked}")
+        else:
+            rep["link_up_raw"] = rep["link_dn_raw"] = "bit-exact"
+    if stages & 4:
+        _eq("link_up", gpu.link_up, orc.link_up, rep)
+        _eq("link_dn", gpu.link_dn, orc.link_dn, rep)
+    if stages & 8:
+        _eq("start_hit", gpu.start_hit, orc.start_hit, rep)
+    if stages & 16:
+        if gpu.n_tracks != orc.n_tracks:
+            raise ParityError(f"n_tracks {gpu.n_tracks} (gpu) vs {orc.n_tracks} (oracle)")
+        _eq("trk_start_hit", gpu.trk_start_hit, orc.trk_start_hit, rep)
+        _eq("n_hits", gpu.n_hits, orc.n_hits, rep)
+        _eq("hit_offset", gpu.hit_offset, orc.hit_offset, rep)
+        _eq("hit_idx", gpu.hit_idx, orc.hit_idx, rep)
+        _eq("n_fit", gpu.n_fit, orc.n_fit, rep)
+        _eq("first_row", gpu.first_row, orc.first_row, rep)
+        _eq("last_row", gpu.last_row, orc.last_row, rep)
+        _eq("x_ref", gpu.x_ref, orc.x_ref.astype(np.float32), rep)
+        _eq("z_ref", gpu.z_ref, orc.z_ref.astype(np.float32), rep)
+        if orc.n_tracks:
+            gp = gpu.par.astype(np.float64); op = orc.par
+            tol = 1e-4 * np.maximum(np.maximum(np.abs(gp), np.abs(op)), PAR_FLOOR[None, :])
+            bad = np.abs(gp - op) > tol
+            if bad.any():
+                t, i = np.argwhere(bad)[0]
+                raise ParityError(f"par[{t},{i}]: gpu {gp[t, i]} oracle {op[t, i]}")
+            gc = gpu.cov.astype(np.float64); oc = orc.cov
+            diag = np.stack([oc[:, i * (i + 1) // 2 + i] for i in range(5)], axis=1)
+            for k, (i, j) in enumerate(TRI):
+                lim = 1e-4 * np.sqrt(np.abs(diag[:, i] * diag[:, j]))
+                b = np.abs(gc[:, k] - oc[:, k]) > lim
+                if b.any():
+                    t = np.nonzero(b)[0][0]
+                    raise ParityError(f"cov[{t},{k}]: gpu {gc[t, k]} oracle {oc[t, k]}")
+            g2 = gpu.chi2.astype(np.float64)
+            b = np.abs(g2 - orc.chi2) > 1e-4 * np.maximum(np.maximum(np.abs(g2), np.abs(orc.chi2)), 1e-3)
+            if b.any():
+                t = np.nonzero(b)[0][0]
+                raise ParityError(f"chi2[{t}]: gpu {g2[t]} oracle {orc.chi2[t]}")
+            rep["par_bit_exact"] = bool(np.array_equal(gpu.par, op.astype(np.float32)))
+            rep["cov_bit_exact"] = bool(np.array_equal(gpu.cov, oc.astype(np.float32)))
+            rep["chi2_bit_exact"] = bool(np.array_equal(gpu.chi2, orc.chi2.astype(np.float32)))
+        rep["n_tracks"] = int(orc.n_tracks)
+    return rep
+
+
+def compare_timeframe(tracker, tf, oracle_obj, sectors=None, stages=0x1F) -> dict:
+    """Compare every (or the given) sector of an already-run Tracker against the oracle."""
+    tot = dict(sectors=0, n_clusters=0, n_tracks=0, links_differing=0, par_bit_exact=True, cov_bit_exact=True)
+    for s in (range(tf.n_sectors) if sectors is None else sectors):
+        g = tracker.get_tracks(s)
+        o = oracle_obj.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=stages)
+        srow = tf.row[s][o.order] if o.order is not None else None
+        try:
+            rep = compare_sector(g, o, oracle_obj, srow, stages)
+        except ParityError as e:
+            raise ParityError(f"sector {s}: {e}") from None
+        tot["sectors"] += 1
+        tot["n_clusters"] += o.n
+        tot["n_tracks"] += rep.get("n_tracks", 0)
+        tot["links_differing"] += rep.get("links_differing", 0)
+        tot["par_bit_exact"] &= rep.get("par_bit_exact", True)
+        tot["cov_bit_exact"] &= rep.get("cov_bit_exact", True)
+    return tot

@@ -1,0 +1,283 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle, element by element.
+
+Run on the B200 box: python -m pytest tests -m gpu.  Inputs are the seeded synthetic generators of
+tpcsynth (BASELINE.json:7-11 recipes), never values produced by the CUDA path.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import tpcsynth
+from oracle import Oracle
+from parity import ParityError, compare_sector, compare_timeframe
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device is visible")
+    import paper_2208_07412_b200 as p
+    p.load_library()
+    return p
+
+
+def run_gpu(pkg, tf, stages=0x1F, max_start_hits=0):
+    n = max(tf.n_clusters, 1)
+    trk = pkg.Tracker(tf.params, max_clusters=n, max_start_hits=max_start_hits)
+    trk.load_timeframe(tf)
+    trk.run(stages)
+    trk.sync()
+    return trk
+
+
+class ArrTF:
+    """Minimal time-frame-like holder for hand-made inputs."""
+    def __init__(self, params, secs):
+        self.params = params
+        self.y = [np.asarray(s[0], np.float32) for s in secs]
+        self.z = [np.asarray(s[1], np.float32) for s in secs]
+        self.row = [np.asarray(s[2], np.uint16) for s in secs]
+        self.x = [params.row_x[r] for r in self.row]
+        self.q = [np.ones(len(r), np.float32) for r in self.row]
+
+    @property
+    def n_sectors(self):
+        return len(self.y)
+
+    @property
+    def n_clusters(self):
+        return int(sum(len(a) for a in self.y))
+
+
+def check(pkg, tf, stages=0x1F, sectors=None, **kw):
+    trk = run_gpu(pkg, tf, stages, **kw)
+    orc = Oracle(tf.params)
+    rep = compare_timeframe(trk, tf, orc, sectors=sectors, stages=stages)
+    trk.close()
+    return rep
+
+
+# ------------------------------------------------------------------------------------------------
+def test_config0_full_pipeline(pkg, cfg0):
+    rep = check(pkg, cfg0)
+    assert rep["n_tracks"] > 100 and rep["links_differing"] == 0
+
+
+def test_config1_small_36_sectors(pkg, cfg1_small):
+    rep = check(pkg, cfg1_small)
+    assert rep["sectors"] == 36 and rep["n_tracks"] > 1000 and rep["links_differing"] == 0
+
+
+def test_config4_small_stress(pkg):
+    tf = tpcsynth.generate(4, n_tracks=1500)
+    rep = check(pkg, tf)
+    assert rep["n_tracks"] > 500 and rep["links_differing"] == 0
+
+
+def test_timeframe_slice_small(pkg):
+    """Config-2 recipe at 2 orbits: several collisions shifted along z (reading G9)."""
+    tf = tpcsynth.generate(2, n_orbits=2, mult_scale=0.3)
+    assert tf.coll_t.shape[0] >= 3
+    rep = check(pkg, tf)
+    assert rep["n_tracks"] > 300 and rep["links_differing"] == 0
+
+
+def test_stage_by_stage_equals_all_at_once(pkg, cfg0):
+    tf = cfg0
+    a = run_gpu(pkg, tf, 0x1F)
+    b = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+    b.load_timeframe(tf)
+    for m in (1, 2, 4, 8, 16):
+        b.run(m)
+    b.sync()
+    ga, gb = a.get_tracks(0), b.get_tracks(0)
+    for f in ("order", "sy", "sz", "bin_start", "row_start", "link_up_raw", "link_dn_raw", "link_up", "link_dn",
+              "start_hit", "par", "cov", "chi2", "hit_offset", "hit_idx", "trk_start_hit"):
+        assert np.array_equal(getattr(ga, f), getattr(gb, f)), f
+    # partial masks are compared with the oracle as well
+    orc = Oracle(tf.params)
+    for m in (1, 3, 7, 15):
+        c = run_gpu(pkg, tf, m)
+        compare_timeframe(c, tf, orc, stages=m)
+        c.close()
+    a.close(); b.close()
+
+
+def test_determinism_and_context_reuse(pkg, cfg1_small):
+    """P11: same input twice -> byte-identical outputs; a context is reusable after reset."""
+    tf = cfg1_small
+    trk = run_gpu(pkg, tf)
+    first = [trk.get_tracks(s) for s in (0, 5, 20)]
+    trk.load_timeframe(tf)      # reset + reload
+    trk.run()
+    second = [trk.get_tracks(s) for s in (0, 5, 20)]
+    for a, b in zip(first, second):
+        for f in ("order", "bin_start", "link_up_raw", "link_dn", "start_hit", "par", "cov", "chi2", "hit_idx"):
+            assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    trk.close()
+
+
+def test_empty_and_tiny_inputs(pkg):
+    P = tpcsynth.default_params(n_sectors=3)
+    e = (np.empty(0, np.float32), np.empty(0, np.float32), np.empty(0, np.uint16))
+    # all empty
+    rep = check(pkg, ArrTF(P, [e, e, e]))
+    assert rep["n_tracks"] == 0
+    # one cluster; a sector in the middle empty; clusters outside the grid (reading N9)
+    one = (np.array([0.5], np.float32), np.array([10.0], np.float32), np.array([7], np.uint16))
+    out = (np.array([-1e3, 1e3, 0.0, 0.0], np.float32), np.array([10.0, 10.0, -50.0, 1e6], np.float32),
+           np.array([5, 5, 5, 5], np.uint16))
+    check(pkg, ArrTF(P, [one, e, out]))
+    # rows 0 and n_rows-1 only
+    edge = (np.zeros(6, np.float32), np.arange(6, dtype=np.float32), np.array([0, 0, 151, 151, 0, 151], np.uint16))
+    check(pkg, ArrTF(P, [edge, one, e]))
+
+
+def test_ties_and_duplicates(pkg):
+    """Reading N7: duplicated clusters; ties go to the smallest original id (needs order[] on the GPU)."""
+    P = tpcsynth.default_params(n_sectors=1)
+    y = np.array([0.0, 0.5, -0.5, 0.5, -0.5], np.float32)
+    z = np.array([10.0, 10.5, 9.5, 10.5, 9.5], np.float32)
+    row = np.array([10, 11, 9, 11, 9], np.uint16)
+    check(pkg, ArrTF(P, [(y, z, row)]))
+    # many exact duplicates on three rows, shuffled ids
+    rng = np.random.default_rng(3)
+    yy = np.repeat(np.array([0.0, 0.25, 0.5], np.float32), 40)
+    zz = np.repeat(np.array([20.0, 20.5, 21.0], np.float32), 40)
+    rr = np.repeat(np.array([20, 21, 22], np.uint16), 40)
+    p = rng.permutation(120)
+    check(pkg, ArrTF(P, [(yy[p], zz[p], rr[p])]))
+
+
+@pytest.mark.parametrize("seed,n,zmax", [(1, 2000, 30.0), (2, 6000, 12.0)])
+def test_dense_random_windows(pkg, seed, n, zmax):
+    """Dense uniform clusters: many candidates per window (overflows the shared-memory candidate
+    cache at the denser setting), many occupied bins, S5 searches with several candidates."""
+    P = tpcsynth.default_params(n_sectors=1)
+    rng = np.random.default_rng(seed)
+    row = rng.integers(0, 12, n).astype(np.uint16)
+    y = (rng.random(n) * 16.0 - 8.0).astype(np.float32)
+    z = (rng.random(n) * zmax).astype(np.float32)
+    check(pkg, ArrTF(P, [(y, z, row)]))
+
+
+def test_grid_variants(pkg):
+    """P3 on the GPU: other bin sizes / margins (bin ranges spanning more than 3 bins)."""
+    tf = tpcsynth.generate(1, n_tracks=600)
+    for bs, gm in ((0.5, 0.01), (1.7, 0.01), (3.0, 0.5)):
+        P2 = tpcsynth.default_params(n_sectors=2, bin_scale=bs, grid_margin=gm)
+        check(pkg, ArrTF(P2, [(tf.y[s], tf.z[s], tf.row[s]) for s in (3, 4)]))
+
+
+def test_toy_worked_example(pkg):
+    path = os.path.join(os.path.dirname(__file__), "golden", "toy_links.txt")
+    rows, ys, zs, exp = [], [], [], []
+    exp_start = None
+    for line in open(path):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        if line.startswith("start"):
+            exp_start = [int(v) for v in line.split()[1:]]
+            continue
+        f = line.split()
+        rows.append(int(f[1])); ys.append(float(f[2])); zs.append(float(f[3]))
+        exp.append([int(v) for v in f[4:8]])
+    exp = np.array(exp)
+    P = tpcsynth.default_params(n_sectors=1, row_x=64.0 + 1.0 * np.arange(8), sigma=0.125)
+    tf = ArrTF(P, [(ys, zs, rows)])
+    trk = run_gpu(pkg, tf, 0xF)
+    g = trk.get_tracks(0)
+    o = g.order.astype(np.int64)
+
+    def to_orig(a):
+        out = np.full(g.n, -1, np.int64)
+        m = a >= 0
+        out[o[m]] = o[a[m]]
+        return out
+    assert to_orig(g.link_up_raw).tolist() == exp[:, 0].tolist()
+    assert to_orig(g.link_dn_raw).tolist() == exp[:, 1].tolist()
+    assert to_orig(g.link_up).tolist() == exp[:, 2].tolist()
+    assert to_orig(g.link_dn).tolist() == exp[:, 3].tolist()
+    assert sorted(o[g.start_hit].tolist()) == sorted(exp_start)
+    trk.close()
+
+
+def test_straight_tracks_dyadic(pkg):
+    """P4 on the GPU: exact recovery, 152-hit tracks, rows 0 and 151 attached by the search."""
+    row_x = 64.0 + 0.75 * np.arange(152)
+    P = tpcsynth.default_params(n_sectors=1, row_x=row_x)
+    nt = 12
+    row, y, z, trk_id = tpcsynth.straight_tracks(row_x, -6.0 + np.arange(nt), (np.arange(nt) - 6) / 64.0,
+                                                 8.0 + 16.0 * np.arange(nt), (np.arange(nt) - 4) / 8.0)
+    perm = np.random.default_rng(5).permutation(row.shape[0])
+    tf = ArrTF(P, [(y[perm], z[perm], row[perm])])
+    trk = run_gpu(pkg, tf)
+    g = trk.get_tracks(0)
+    assert g.n_tracks == nt and np.all(g.n_hits == 152) and np.all(g.first_row == 0) and np.all(g.last_row == 151)
+    compare_timeframe(trk, tf, Oracle(P))
+    trk.close()
+
+
+def test_error_paths(pkg, cfg0):
+    tf = cfg0
+    P = tf.params
+    # row out of range -> TPCCA_E_RANGE at sync
+    trk = pkg.Tracker(P, max_clusters=16)
+    trk.load_clusters(0, np.zeros(3, np.float32), np.ones(3, np.float32), np.array([1, 2, 999], np.uint16))
+    trk.run()
+    with pytest.raises(pkg.TpccaError) as e:
+        trk.sync()
+    assert e.value.code == -5
+    # loading a sector twice -> E_STATE; too many clusters -> E_WORKSPACE
+    trk.reset()
+    trk.load_clusters(0, np.zeros(3, np.float32), np.ones(3, np.float32), np.array([1, 2, 3], np.uint16))
+    with pytest.raises(pkg.TpccaError) as e:
+        trk.load_clusters(0, np.zeros(3, np.float32), np.ones(3, np.float32), np.array([1, 2, 3], np.uint16))
+    assert e.value.code == -2
+    trk.reset()
+    with pytest.raises(pkg.TpccaError) as e:
+        trk.load_clusters(0, np.zeros(30, np.float32), np.ones(30, np.float32), np.zeros(30, np.uint16))
+    assert e.value.code == -4
+    # S2 before S1 -> E_STATE
+    trk.reset()
+    trk.load_clusters(0, np.zeros(3, np.float32), np.ones(3, np.float32), np.array([1, 2, 3], np.uint16))
+    with pytest.raises(pkg.TpccaError) as e:
+        trk.run(2)
+    assert e.value.code == -2
+    trk.close()
+    # start-hit capacity overflow is reported, never silently truncated
+    trk = pkg.Tracker(P, max_clusters=tf.n_clusters, max_start_hits=5)
+    trk.load_timeframe(tf)
+    trk.run()
+    with pytest.raises(pkg.TpccaError) as e:
+        trk.sync()
+    assert e.value.code == -4
+    trk.close()
+
+
+def test_device_inputs_and_borrow(pkg, cfg0):
+    """Clusters already resident in HBM (torch CUDA tensors): copy and borrow modes."""
+    import torch
+    tf = cfg0
+    y = torch.from_numpy(tf.y[0]).cuda(); z = torch.from_numpy(tf.z[0]).cuda()
+    row = torch.from_numpy(tf.row[0].astype(np.int16)).cuda().view(torch.uint16)
+    orc = Oracle(tf.params)
+    for borrow in (False, True):
+        trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+        trk.load_clusters(0, y, z, row, borrow=borrow)
+        trk.run()
+        compare_timeframe(trk, tf, orc)
+        trk.close()
+
+
+def test_config1_full_size(pkg):
+    """BASELINE.json config 1 at full size (10k tracks, ~1.5M clusters): every sector, every output."""
+    tf = tpcsynth.generate(1)
+    assert tf.n_clusters > 1_000_000
+    rep = check(pkg, tf)
+    assert rep["n_tracks"] > 20000 and rep["links_differing"] == 0
