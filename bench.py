@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TPC sector CA tracker hot path (S1-S5) on B200.
+
+Contract: `python bench.py --gpus N --steps K --warmup W [--impl reference]` prints ONE JSON line.
+A step = one pass of the whole hot path (tpcca_run(S1..S5)) over one synthetic time frame.
+Workload at N=1: BASELINE.json configs[3] (128-orbit 50 kHz Pb-Pb-like time frame, seeded synthetic,
+tpcsynth recipe of DESIGN.md 6).  N>1: one time frame per GPU (the paper's own scheme, PAPER.md:21
+"different collisions are distributed over the EPNs"): replicas, no data-path collective, weak scaling.
+
+  value     : clusters/s, inputs resident in HBM before the timed region (device-timed, max over ranks)
+  e2e       : same metric through the C-ABI with HOST (pinned) buffers: H2D of the clusters and D2H of
+              order + cleaned links + start hits + track table + hit CSR inside the timed region
+  roofline  : neighbour finder (S2; the stage BASELINE.json's metric names) vs the measured HBM peak;
+  roofline_dominant : the stage that takes the most time (S5 tracklets), plain-ALU bound
+  cpu_baseline : the oracle as it stands on one host core over sector 0 of the same time frame
+                 (also used as a full-size parity check of that sector)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "TPC clusters tracked/sec per B200 (full timeframe)"
+UNIT = "clusters/s"
+
+# fp32 operations of one call, counted from DESIGN.md 3.5 (every + - * / sqrt is one operation)
+FLOPS_PROPAGATE = 157   # 55 transport + 52 (A = J C) + 50 (C' = A J^T)
+FLOPS_UPDATE = 102      # 2 x (1 + 2 + 5 + 10 + 30 + 3)
+FLOPS_GATE = 9
+FLOPS_SEARCH = 23       # bin range + weights
+FLOPS_CANDIDATE = 10
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.lines = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for t, line in self.lines:
+            if t < t0 - 0.05 or t > t1 + 0.15:
+                continue
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+
+
+def make_timeframe(args, rank):
+    import tpcsynth
+    t0 = time.time()
+    seed = None if rank == 0 and args.seed is None else (args.seed or (tpcsynth.generator.BASE_SEED + args.config)) + 1000 * rank
+    tf = tpcsynth.generate(args.config, seed=seed, mult_scale=args.mult_scale)
+    return tf, time.time() - t0
+
+
+def sample_sector(tf, sector, z_frac):
+    """Bounded sample of the workload: clusters of one sector with z below z_frac of the z range."""
+    y, z, row = tf.y[sector], tf.z[sector], tf.row[sector]
+    if z_frac >= 1.0:
+        return y, z, row
+    m = z < np.float32(z_frac * tf.params.z_hi)
+    return np.ascontiguousarray(y[m]), np.ascontiguousarray(z[m]), np.ascontiguousarray(row[m])
+
+
+def workload_name(args, tf):
+    import tpcsynth
+    return (f"BASELINE.json configs[{args.config}] ({tpcsynth.CONFIGS[args.config]['name']}), seed {tf.seed}, "
+            f"mult_scale {args.mult_scale}")
+
+
+# --------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The oracle (CPU, one core) on bounded samples of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import Oracle
+    tf, gen_s = make_timeframe(args, 0)
+    y, z, row = sample_sector(tf, 0, args.ref_z_frac)
+    orc = Oracle(tf.params)
+    for _ in range(args.warmup):
+        orc.run(y, z, row, want=())
+    t0 = time.time()
+    for _ in range(args.steps):
+        orc.run(y, z, row, want=())
+    dt = time.time() - t0
+    n = int(y.shape[0])
+    value = n * args.steps / dt
+    sample = f"sector 0 of {tf.n_sectors}, z < {args.ref_z_frac:g} of the z range: {n} of {tf.n_clusters} clusters per step"
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f32", data="synthetic",
+                config=dict(workload=workload_name(args, tf), n_clusters=tf.n_clusters, sample=sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=1, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0, generate_s=gen_s)
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+def run_tpcca(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2208_07412_b200 as pkg
+    from paper_2208_07412_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: tpcca has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(v):
+        if world == 1:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    peaks = load_peaks()
+    tf, gen_s = make_timeframe(args, rank)
+    N = tf.n_clusters
+    cap = args.max_start_hits or (N // 8 + 1024)
+    trk = pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local)
+
+    # ---- device-resident inputs (borrowed: no copy inside the timed region) ------------------------
+    host = []
+    for s in range(tf.n_sectors):
+        hy = torch.from_numpy(tf.y[s]).pin_memory()
+        hz = torch.from_numpy(tf.z[s]).pin_memory()
+        hr = torch.from_numpy(tf.row[s].view(np.int16)).pin_memory().view(torch.uint16)
+        host.append((hy, hz, hr))
+    devin = [(a.to(dev), b.to(dev), c.to(dev)) for a, b, c in host]
+    trk.reset()
+    for s, (a, b, c) in enumerate(devin):
+        trk.load_clusters(s, a, b, c, borrow=True)
+
+    for _ in range(args.warmup):
+        trk.run()
+    trk.sync()
+    launches_per_step = trk.launch_count()
+    counts = trk.counts()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall0 = time.time()
+    ev0.record()
+    for _ in range(args.steps):
+        trk.run()
+    ev1.record()
+    torch.cuda.synchronize()
+    t_wall1 = time.time()
+    barrier()
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    clocks = sampler.stop(t_wall0, t_wall1)
+    trk.sync()
+    n_all = sum_over_ranks(float(N))
+    value = n_all * args.steps / (ms_total * 1e-3)
+
+    # per-stage device times of the timed steps (events recorded inside tpcca_run on the same stream)
+    k = min(args.steps, 16)
+    stage_ms = np.mean([trk.timings(i) for i in range(k)], axis=0)
+    work = trk.work_counters()
+    n_bins_total = counts["n_bins"] * tf.n_sectors
+    s2_bytes = 16.0 * N + 4.0 * n_bins_total
+    s2_gbs = s2_bytes / (stage_ms[1] * 1e-3) / 1e9
+    flops = (work["propagations"] * FLOPS_PROPAGATE + work["updates"] * FLOPS_UPDATE + work["gates"] * FLOPS_GATE
+             + work["searches"] * FLOPS_SEARCH + work["candidates"] * FLOPS_CANDIDATE)
+    alu_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12       # T fp32 op/s without FMA
+    s5_tops = flops / (stage_ms[4] * 1e-3) / 1e12
+
+    # ---- end to end: host buffers in, host buffers out, through the public API ---------------------
+    what = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START | B.OUT_TRACKS
+    h2d = int(10 * N)
+    d2h = 0
+
+    def e2e_step():
+        nonlocal d2h
+        trk.reset()
+        for s, (a, b, c) in enumerate(host):
+            trk.load_clusters(s, a, b, c)
+        trk.run()
+        out = 0
+        for s in range(tf.n_sectors):
+            v = trk.get_tracks_view(s, B.MEM_HOST, what)
+            out += 12 * v.n_clusters + 4 * v.n_start + 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
+        d2h = int(out)
+
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    e2e_step()   # warm-up: grows the pinned arena
+    barrier()
+    ev0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
+    e2e_value = n_all * e2e_steps / (e2e_ms * 1e-3)
+
+    # ---- CPU baseline = the oracle on one core over sector 0 (rank 0, N = 1 only); parity check ----
+    cpu = None
+    parity = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sys.path.insert(0, os.path.join(ROOT, "tests"))
+        from oracle import Oracle
+        from parity import compare_sector
+        y, z, row = sample_sector(tf, 0, 1.0)
+        orc = Oracle(tf.params)
+        t0 = time.time()
+        orc.run(y, z, row, want=())
+        dt = time.time() - t0
+        cpu = dict(value=float(y.shape[0] / dt), unit=UNIT, cores=1, kind="oracle",
+                   sample=f"sector 0 of {tf.n_sectors}: {int(y.shape[0])} of {N} clusters, S1-S5, {dt:.1f} s")
+        o = orc.run(y, z, row)
+        g = trk.get_tracks(0)
+        try:
+            rep = compare_sector(g, o, orc, row[o.order])
+            parity = dict(sector=0, n_clusters=int(o.n), n_tracks=int(o.n_tracks), links_differing=rep["links_differing"],
+                          membership="bit-exact", par_bit_exact=rep.get("par_bit_exact"), status="pass")
+        except AssertionError as e:
+            parity = dict(sector=0, status="FAIL", error=str(e)[:300])
+
+    if rank == 0:
+        line = dict(
+            metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+            ms_per_step=ms_total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+            dtype="f32", data="synthetic",
+            config=dict(workload=workload_name(args, tf), n_clusters_per_gpu=N, n_sectors=tf.n_sectors,
+                        n_start=counts["n_start"], n_tracks=counts["n_tracks"], n_hits=counts["n_hits"],
+                        grid_bins=n_bins_total, parallelism=f"replicas x{world} (one time frame per GPU)",
+                        l2="inputs larger than L2 (no flush needed)", inputs="device-resident, borrowed"),
+            stage_ms=dict(zip(("S1_grid", "S2_neighbours", "S3_clean", "S4_start", "S5_tracklets", "total"),
+                              (round(float(v), 4) for v in stage_ms))),
+            roofline=dict(kernel="k_neighbours (S2)", bound="hbm", achieved=s2_gbs, peak=peaks["hbm_gbs"], unit="GB/s",
+                          frac=s2_gbs / peaks["hbm_gbs"], frac_of_nominal_8000=s2_gbs / 8000.0, traffic=None,
+                          algorithmic_bytes=s2_bytes, peak_source=peaks["source"]),
+            roofline_dominant=dict(kernel="k_tracklets (S5)", bound="alu", achieved=s5_tops, peak=alu_peak,
+                                   unit="Tfp32op/s (no FMA)", frac=s5_tops / alu_peak, traffic=None, flops=flops,
+                                   work=work),
+            e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
+                     ms_per_step=e2e_ms / e2e_steps),
+            gpu_launches=int(launches_per_step * args.steps),
+            clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1),
+        )
+        print(json.dumps(line), flush=True)
+    trk.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="tpcca", choices=["tpcca", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--mult-scale", type=float, default=1.0)
+    ap.add_argument("--seed", type=int, default=None)
+    ap.add_argument("--max-start-hits", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-z-frac", type=float, default=0.25)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "tpcca":
+        args.warmup = 3        # timing rule: W >= 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_tpcca(args)
+
+
+if __name__ == "__main__":
+    main()

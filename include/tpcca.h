@@ -61,6 +61,15 @@ extern "C" {
 #define TPCCA_STAGE_TRACKLETS  0x10u
 #define TPCCA_STAGE_ALL        0x1Fu
 
+/* which output groups tpcca_get_tracks delivers (HOST: copies) */
+#define TPCCA_OUT_ORDER      0x01u  /* order                                      (S1)            */
+#define TPCCA_OUT_GRID       0x02u  /* syz, bin_start, row_start                  (S1)            */
+#define TPCCA_OUT_LINKS_RAW  0x04u  /* link_up_raw, link_dn_raw                   (S2)            */
+#define TPCCA_OUT_LINKS      0x08u  /* link_up, link_dn                           (S3)            */
+#define TPCCA_OUT_START      0x10u  /* start_hit                                  (S4)            */
+#define TPCCA_OUT_TRACKS     0x20u  /* track table + hit CSR                      (S5)            */
+#define TPCCA_OUT_ALL        0x3Fu
+
 typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
 
 /* Tracker tables (DESIGN.md 3 "Derived tables").  All table pointers are HOST arrays of length
@@ -172,17 +181,27 @@ int tpcca_sync(tpcca_ctx *ctx);
 
 /* Outputs of one sector (BASELINE.json:5 "links and fitted tracks out").  Synchronises the
  * stream.  mem_space: TPCCA_MEM_DEVICE (pointers into the workspace, no copy) or TPCCA_MEM_HOST
- * (copies into context-owned host buffers; par/cov are packed with trk_stride = n_tracks).
- * Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
-int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, tpcca_tracks_view *out);
+ * (asynchronous D2H copies on the context's stream into a context-owned PINNED host arena, then
+ * one synchronise; par/cov are packed with trk_stride = n_tracks).  `what` selects the output
+ * groups (TPCCA_OUT_*); groups not selected, or whose stage was not run, are NULL.  Counts are
+ * always filled.  Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
+int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, uint32_t what, tpcca_tracks_view *out);
 
 /* Totals over all sectors after a run: out[0..4] = n_clusters, n_start, n_tracks, n_hits,
  * n_bins (per sector).  Synchronises the stream.  Errors as tpcca_sync. */
 int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[5]);
 
-/* Device time of each stage of the last run [ms], from CUDA events on the context's stream;
- * ms[5] = whole run.  Synchronises the stream. */
-int tpcca_get_timings(tpcca_ctx *ctx, float ms[6]);
+/* Device time of each stage [ms] of the run `runs_back` runs ago (0 = the last tpcca_run; the
+ * context keeps the events of its last 16 runs), from CUDA events recorded on the context's
+ * stream around the stages; ms[5] = whole run.  Synchronises the stream.
+ * Errors: TPCCA_E_ARG (runs_back outside 0..15), TPCCA_E_STATE (no such run). */
+int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[6]);
+
+/* Work counters of the last run's S5 kernel, for the ALU roofline:
+ * out[0] = Kalman propagations that moved the state, out[1] = Kalman updates,
+ * out[2] = gate evaluations (phase A), out[3] = searches, out[4] = search candidates scored.
+ * Synchronises the stream. */
+int tpcca_get_work_counters(tpcca_ctx *ctx, int64_t out[5]);
 
 /* Number of kernels the last tpcca_run launched (for bench.py's "gpu_launches"). */
 int tpcca_get_launch_count(const tpcca_ctx *ctx, int64_t *out);

@@ -23,8 +23,9 @@ _up = C.POINTER(C.c_uint32)
 
 #: every symbol include/tpcca.h declares
 ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "tpcca_reset", "tpcca_run",
-               "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings",
+               "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
                "tpcca_get_launch_count", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
+OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
 
 
 class TpccaError(RuntimeError):
@@ -83,9 +84,10 @@ def load_library():
     lib.tpcca_reset.argtypes = [C.c_void_p]
     lib.tpcca_run.argtypes = [C.c_void_p, C.c_uint32]
     lib.tpcca_sync.argtypes = [C.c_void_p]
-    lib.tpcca_get_tracks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(_View)]
+    lib.tpcca_get_tracks.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_uint32, C.POINTER(_View)]
     lib.tpcca_get_counts.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
-    lib.tpcca_get_timings.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    lib.tpcca_get_timings.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_float)]
+    lib.tpcca_get_work_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_last_error.argtypes = [C.c_void_p]
     lib.tpcca_last_error.restype = C.c_char_p
@@ -284,34 +286,41 @@ class Tracker:
         return dict(n_clusters=int(out[0]), n_start=int(out[1]), n_tracks=int(out[2]), n_hits=int(out[3]),
                     n_bins=int(out[4]))
 
-    def timings(self):
-        """Per-stage device ms of the last run: [S1, S2, S3, S4, S5, total]."""
+    def timings(self, runs_back: int = 0):
+        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, total]."""
         out = (C.c_float * 6)()
-        self._check(self._lib.tpcca_get_timings(self._h, out))
+        self._check(self._lib.tpcca_get_timings(self._h, int(runs_back), out))
         return [float(v) for v in out]
+
+    def work_counters(self) -> dict:
+        """S5 work counters of the last run (tpcca_get_work_counters)."""
+        out = (C.c_int64 * 5)()
+        self._check(self._lib.tpcca_get_work_counters(self._h, out))
+        return dict(zip(("propagations", "updates", "gates", "searches", "candidates"), (int(v) for v in out)))
 
     def launch_count(self) -> int:
         out = C.c_int64(0)
         self._check(self._lib.tpcca_get_launch_count(self._h, C.byref(out)))
         return int(out.value)
 
-    def get_tracks_view(self, sector: int, mem_space: int = MEM_DEVICE) -> _View:
-        """Raw tpcca_tracks_view (device pointers by default)."""
+    def get_tracks_view(self, sector: int, mem_space: int = MEM_DEVICE, what: int = OUT_ALL) -> _View:
+        """Raw tpcca_tracks_view (device pointers by default; HOST pointers live in the context's pinned
+        arena until the next call)."""
         v = _View()
-        self._check(self._lib.tpcca_get_tracks(self._h, int(sector), int(mem_space), C.byref(v)))
+        self._check(self._lib.tpcca_get_tracks(self._h, int(sector), int(mem_space), int(what), C.byref(v)))
         return v
 
-    def get_tracks(self, sector: int) -> SectorOutput:
+    def get_tracks(self, sector: int, what: int = OUT_ALL) -> SectorOutput:
         """tpcca_get_tracks(HOST) -> numpy copies."""
-        v = self.get_tracks_view(sector, MEM_HOST)
+        v = self.get_tracks_view(sector, MEM_HOST, what)
         n, nt = int(v.n_clusters), int(v.n_tracks)
         o = SectorOutput(n=n, n_bins=int(v.n_bins))
         o.order = _np(v.order, n, np.int32)
         if v.syz:
             syz = _np(v.syz, 2 * n, np.float32).reshape(n, 2)
             o.sy, o.sz = np.ascontiguousarray(syz[:, 0]), np.ascontiguousarray(syz[:, 1])
-        o.bin_start = _np(v.bin_start, int(v.n_bins) + 1, np.uint32)
-        o.row_start = _np(v.row_start, self.n_rows + 1, np.int32)
+        o.bin_start = _np(v.bin_start, int(v.n_bins) + 1, np.uint32) if v.bin_start else None
+        o.row_start = _np(v.row_start, self.n_rows + 1, np.int32) if v.row_start else None
         o.link_up_raw = _np(v.link_up_raw, n, np.int32); o.link_dn_raw = _np(v.link_dn_raw, n, np.int32)
         o.link_up = _np(v.link_up, n, np.int32); o.link_dn = _np(v.link_dn, n, np.int32)
         o.start_hit = _np(v.start_hit, int(v.n_start), np.int32)

@@ -175,6 +175,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   const float my = win_y + margin, mz = win_z + margin;
   const size_t nbp1 = (size_t)T->bins_per_sector + 1;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned w_prop = 0, w_upd = 0, w_gate = 0, w_search = 0, w_cand = 0;   // work counters
 
   for (;;) {
     // dynamic work distribution: one warp takes 32 consecutive start hits
@@ -223,6 +224,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       const float wy = f.c00 + K.err2_y;
       const float wz = f.c11 + K.err2_z;
       int best = -1;
+      ++w_search;
       for (int bz = bz0; bz <= bz1; ++bz) {
         const int b0 = t.bin_base + bz * t.ny;
         const uint32_t e = __ldg(&bs[b0 + by1 + 1]);
@@ -232,6 +234,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
           const float rz = (h.y - z_ref) - f.p1;
           if (!(fabsf(ry) <= win_y && fabsf(rz) <= win_z)) continue;
           const float d2 = (ry * ry) / wy + (rz * rz) / wz;
+          ++w_cand;
           if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
             best = (int)c; best_d2 = d2;
           }
@@ -253,6 +256,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       if (phase == PH_A && cur == -1) { phase = PH_B; gap = 0; }          // r == last + 1 already
       if (phase == PH_B && r >= n_rows) { phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; }
       if (phase == PH_C && r < 0) { phase = PH_DONE; break; }
+      w_prop += (tab[r].x != f.x) ? 1u : 0u;
       if (!kf_propagate(f, tab[r].x, K)) {
         if (phase == PH_C) { phase = PH_DONE; break; }
         // rows (top, r] of the up pass that were never decided hold no hit
@@ -266,6 +270,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
         const float ym = h.x, zm = h.y - z_ref;
         bool ok = true;
         if (f.n >= 2) {
+          ++w_gate;
           const float ry = ym - f.p0, rz = zm - f.p1;
           const float d2 = (ry * ry) / (f.c00 + K.err2_y) + (rz * rz) / (f.c11 + K.err2_z);
           ok = !(d2 > gate);
@@ -288,6 +293,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       if (take >= 0) {
         const float2 h = yz[take];
         kf_update(f, h.x, h.y - z_ref, K);
+        ++w_upd;
         if (is_new) { hcol[(size_t)r * cap] = take; ++n_hits; }
         if (phase == PH_C) {
           snap = f; have_snap = true;
@@ -326,6 +332,15 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       o[15 * cs] = snap.c32; o[16 * cs] = snap.c33; o[17 * cs] = snap.c40; o[18 * cs] = snap.c41;
       o[19 * cs] = snap.c42; o[20 * cs] = snap.c43; o[21 * cs] = snap.c44; o[22 * cs] = snap.chi2;
     }
+  }
+  // work counters: one atomic per warp and counter
+  unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};
+#pragma unroll
+  for (int i = 0; i < 5; ++i) {
+    unsigned long long v = w[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0 && v) atomicAdd(&st->work[i], v);
   }
 }
 

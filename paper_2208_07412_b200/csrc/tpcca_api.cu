@@ -133,12 +133,15 @@ struct tpcca_ctx {
   int n_tiles256 = 0, n_tiles2048 = 0;
   uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
   bool desc_valid = false;
-  cudaEvent_t ev[7]{};
-  bool ev_valid[7]{};
+  static constexpr int kRing = 16;
+  cudaEvent_t ev[kRing][6]{};
+  uint32_t ev_mask[kRing]{};          // stage mask of the run that used the slot (0 = unused)
+  int64_t run_count = 0;
+  char* arena = nullptr;              // pinned host arena of tpcca_get_tracks(HOST)
+  size_t arena_bytes = 0;
   int64_t launches = 0;
   DevStatus status{};
   bool status_valid = false;
-  std::vector<std::vector<char>> host_bufs;
   std::string err;
 
   template <class Tp> Tp* at(size_t off) const { return reinterpret_cast<Tp*>(ws + off); }
@@ -250,7 +253,8 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   t.bin_base[p->n_rows] = base;
   cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
-  for (int i = 0; i < 7 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[i]);
+  for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
+    for (int i = 0; i < 6 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
     delete c;
@@ -320,7 +324,6 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   cudaStream_t st = c->stream;
   c->launches = 0;
   c->status_valid = false;
-  c->host_bufs.clear();
   // ---- sector descriptors
   if (!c->desc_valid) {
     c->desc.assign(kMaxSectors + 1, SectorDesc{});
@@ -349,8 +352,9 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   longlong2* tile_off = c->at<longlong2>(L.tile_off);
   int32_t* start_hit = c->at<int32_t>(L.start_hit);
   const int32_t cap = (int32_t)c->CS;
-  for (int i = 0; i < 7; ++i) c->ev_valid[i] = false;
-  auto mark = [&](int i) { cudaEventRecord(c->ev[i], st); c->ev_valid[i] = true; };
+  const int slot_ev = (int)(c->run_count % tpcca_ctx::kRing);
+  c->ev_mask[slot_ev] = 0;
+  auto mark = [&](int i) { cudaEventRecord(c->ev[slot_ev][i], st); };
   mark(0);
 
   if (mask & TPCCA_STAGE_GRID) {
@@ -415,6 +419,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     int32_t* trk_i = c->at<int32_t>(L.trk_i);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
     CU(c, cudaMemsetAsync(&status->work_counter, 0, sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(status->work, 0, sizeof(status->work), st));
     k_tracklets<<<148 * 8, 128, 0, st>>>(T, sec, status, syz, bin_start, row_start, order, c->at<int32_t>(L.up), start_hit,
                                          cap, hits, trk_f, trk_i);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
@@ -426,6 +431,8 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   }
   mark(5);
   CU(c, cudaGetLastError());
+  c->ev_mask[slot_ev] = mask;
+  ++c->run_count;
   c->done_mask |= mask;
   return TPCCA_OK;
 }
@@ -447,13 +454,24 @@ int tpcca_get_counts(tpcca_ctx* c, int64_t out[5]) {
   return TPCCA_OK;
 }
 
-int tpcca_get_timings(tpcca_ctx* c, float ms[6]) {
+int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[6]) {
   if (!c || !ms) return TPCCA_E_ARG;
-  CU(c, cudaStreamSynchronize(c->stream));
+  if (runs_back < 0 || runs_back >= tpcca_ctx::kRing) return set_err(c, TPCCA_E_ARG, "runs_back must be in 0..15");
   for (int i = 0; i < 6; ++i) ms[i] = 0.f;
-  if (!c->ev_valid[0] || !c->ev_valid[5]) return set_err(c, TPCCA_E_STATE, "nothing was run");
-  for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[i], c->ev[i + 1]));
-  CU(c, cudaEventElapsedTime(&ms[5], c->ev[0], c->ev[5]));
+  if (runs_back >= c->run_count) return set_err(c, TPCCA_E_STATE, "no such run");
+  const int k = (int)((c->run_count - 1 - runs_back) % tpcca_ctx::kRing);
+  if (!c->ev_mask[k]) return set_err(c, TPCCA_E_STATE, "no such run");
+  CU(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[k][i], c->ev[k][i + 1]));
+  CU(c, cudaEventElapsedTime(&ms[5], c->ev[k][0], c->ev[k][5]));
+  return TPCCA_OK;
+}
+
+int tpcca_get_work_counters(tpcca_ctx* c, int64_t out[5]) {
+  if (!c || !out) return TPCCA_E_ARG;
+  int rc = fetch_status(c);
+  if (rc) return rc;
+  for (int i = 0; i < 5; ++i) out[i] = (int64_t)c->status.work[i];
   return TPCCA_OK;
 }
 
@@ -463,7 +481,7 @@ int tpcca_get_launch_count(const tpcca_ctx* c, int64_t* out) {
   return TPCCA_OK;
 }
 
-int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, tpcca_tracks_view* v) {
+int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpcca_tracks_view* v) {
   if (!c || !v) return TPCCA_E_ARG;
   if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
   if (mem_space != TPCCA_MEM_HOST && mem_space != TPCCA_MEM_DEVICE) return set_err(c, TPCCA_E_ARG, "bad mem_space");
@@ -475,82 +493,87 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, tpcca_tracks_view*
   const DevStatus& S = c->status;
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
   const uint32_t done = c->done_mask;
+  const bool host = mem_space == TPCCA_MEM_HOST;
   v->n_clusters = n;
   v->n_bins = c->nb;
-  const bool host = mem_space == TPCCA_MEM_HOST;
-  if (host) c->host_bufs.clear();
-  cudaError_t cerr = cudaSuccess;
-  auto out = [&](const void* dev, size_t bytes) -> const void* {
-    if (!host) return dev;
-    c->host_bufs.emplace_back(bytes ? bytes : 1);
-    if (bytes) {
-      cudaError_t e = cudaMemcpy(c->host_bufs.back().data(), dev, bytes, cudaMemcpyDeviceToHost);
-      if (e != cudaSuccess) cerr = e;
-    }
-    return c->host_bufs.back().data();
-  };
-  if (done & TPCCA_STAGE_GRID) {
-    v->order = (const int32_t*)out(c->at<int32_t>(L.order) + off, 4 * (size_t)n);
-    v->syz = (const float*)out(c->at<float2>(L.syz) + off, 8 * (size_t)n);
-    v->bin_start = (const uint32_t*)out(c->at<uint32_t>(L.bin_start) + (size_t)sector * (c->nb + 1), 4 * (size_t)(c->nb + 1));
-    v->row_start = (const int32_t*)out(c->at<int32_t>(L.row_start) + (size_t)sector * (c->nr + 1), 4 * (size_t)(c->nr + 1));
-  }
-  if (done & TPCCA_STAGE_NEIGHBOURS) {
-    v->link_up_raw = (const int32_t*)out(c->at<int32_t>(L.up_raw) + off, 4 * (size_t)n);
-    v->link_dn_raw = (const int32_t*)out(c->at<int32_t>(L.dn_raw) + off, 4 * (size_t)n);
-  }
-  if (done & TPCCA_STAGE_CLEAN) {
-    v->link_up = (const int32_t*)out(c->at<int32_t>(L.up) + off, 4 * (size_t)n);
-    v->link_dn = (const int32_t*)out(c->at<int32_t>(L.dn) + off, 4 * (size_t)n);
-  }
-  if (done & TPCCA_STAGE_START) {
-    const int64_t s0 = S.start_off[sector], s1 = S.start_off[sector + 1];
-    v->n_start = s1 - s0;
-    v->start_hit = (const int32_t*)out(c->at<int32_t>(L.start_hit) + s0, 4 * (size_t)(s1 - s0));
-  }
+  int64_t s0 = 0, s1 = 0, t0 = 0, nt = 0, h0 = 0, h1 = 0;
+  if (done & TPCCA_STAGE_START) { s0 = S.start_off[sector]; s1 = S.start_off[sector + 1]; v->n_start = s1 - s0; }
   if (done & TPCCA_STAGE_TRACKLETS) {
-    const int64_t t0 = S.trk_off[sector], t1 = S.trk_off[sector + 1], nt = t1 - t0;
-    const int64_t h0 = S.hit_off[sector], h1 = S.hit_off[sector + 1];
-    v->n_tracks = nt;
-    v->n_hits = h1 - h0;
-    v->x_ref = (const float*)out(c->at<float>(L.o_x_ref) + t0, 4 * (size_t)nt);
-    v->z_ref = (const float*)out(c->at<float>(L.o_z_ref) + t0, 4 * (size_t)nt);
-    v->chi2 = (const float*)out(c->at<float>(L.o_chi2) + t0, 4 * (size_t)nt);
-    v->n_hits_trk = (const int32_t*)out(c->at<int32_t>(L.o_n_hits) + t0, 4 * (size_t)nt);
-    v->n_fit = (const int32_t*)out(c->at<int32_t>(L.o_n_fit) + t0, 4 * (size_t)nt);
-    v->first_row = (const int32_t*)out(c->at<int32_t>(L.o_first) + t0, 4 * (size_t)nt);
-    v->last_row = (const int32_t*)out(c->at<int32_t>(L.o_last) + t0, 4 * (size_t)nt);
-    v->trk_start_hit = (const int32_t*)out(c->at<int32_t>(L.o_start) + t0, 4 * (size_t)nt);
-    v->hit_offset = (const int32_t*)out(c->at<int32_t>(L.o_hit_offset) + t0 + sector, 4 * (size_t)(nt + 1));
-    v->hit_idx = (const int32_t*)out(c->at<int32_t>(L.o_hit_idx) + h0, 4 * (size_t)(h1 - h0));
-    if (!host) {
-      v->trk_stride = c->CS;
-      v->par = c->at<float>(L.o_par) + t0;
-      v->cov = c->at<float>(L.o_cov) + t0;
-    } else {
-      v->trk_stride = nt;
-      c->host_bufs.emplace_back(4 * (size_t)std::max<int64_t>(5 * nt, 1));
-      char* hp = c->host_bufs.back().data();
-      c->host_bufs.emplace_back(4 * (size_t)std::max<int64_t>(15 * nt, 1));
-      char* hc = c->host_bufs.back().data();
-      if (nt > 0) {
-        cudaError_t e = cudaMemcpy2D(hp, 4 * (size_t)nt, c->at<float>(L.o_par) + t0, 4 * (size_t)c->CS, 4 * (size_t)nt, 5, cudaMemcpyDeviceToHost);
-        if (e != cudaSuccess) cerr = e;
-        e = cudaMemcpy2D(hc, 4 * (size_t)nt, c->at<float>(L.o_cov) + t0, 4 * (size_t)c->CS, 4 * (size_t)nt, 15, cudaMemcpyDeviceToHost);
-        if (e != cudaSuccess) cerr = e;
-      }
-      v->par = (const float*)hp;
-      v->cov = (const float*)hc;
-    }
+    t0 = S.trk_off[sector]; nt = S.trk_off[sector + 1] - t0; h0 = S.hit_off[sector]; h1 = S.hit_off[sector + 1];
+    v->n_tracks = nt; v->n_hits = h1 - h0;
   }
-  if (cerr != cudaSuccess) return set_err(c, TPCCA_E_CUDA, "D2H copy failed: %s", cudaGetErrorString(cerr));
+  // the arrays to deliver: (destination field, device source, bytes); par / cov are strided planes
+  struct Item { const void** dst; const void* src; size_t bytes; int planes; };
+  std::vector<Item> items;
+  auto add = [&](const void* const* dst, const void* src, size_t bytes, int planes = 1) {
+    items.push_back(Item{(const void**)dst, src, bytes, planes});
+  };
+  if ((what & TPCCA_OUT_ORDER) && (done & TPCCA_STAGE_GRID))
+    add((const void* const*)&v->order, c->at<int32_t>(L.order) + off, 4 * (size_t)n);
+  if ((what & TPCCA_OUT_GRID) && (done & TPCCA_STAGE_GRID)) {
+    add((const void* const*)&v->syz, c->at<float2>(L.syz) + off, 8 * (size_t)n);
+    add((const void* const*)&v->bin_start, c->at<uint32_t>(L.bin_start) + (size_t)sector * (c->nb + 1), 4 * (size_t)(c->nb + 1));
+    add((const void* const*)&v->row_start, c->at<int32_t>(L.row_start) + (size_t)sector * (c->nr + 1), 4 * (size_t)(c->nr + 1));
+  }
+  if ((what & TPCCA_OUT_LINKS_RAW) && (done & TPCCA_STAGE_NEIGHBOURS)) {
+    add((const void* const*)&v->link_up_raw, c->at<int32_t>(L.up_raw) + off, 4 * (size_t)n);
+    add((const void* const*)&v->link_dn_raw, c->at<int32_t>(L.dn_raw) + off, 4 * (size_t)n);
+  }
+  if ((what & TPCCA_OUT_LINKS) && (done & TPCCA_STAGE_CLEAN)) {
+    add((const void* const*)&v->link_up, c->at<int32_t>(L.up) + off, 4 * (size_t)n);
+    add((const void* const*)&v->link_dn, c->at<int32_t>(L.dn) + off, 4 * (size_t)n);
+  }
+  if ((what & TPCCA_OUT_START) && (done & TPCCA_STAGE_START))
+    add((const void* const*)&v->start_hit, c->at<int32_t>(L.start_hit) + s0, 4 * (size_t)(s1 - s0));
+  if ((what & TPCCA_OUT_TRACKS) && (done & TPCCA_STAGE_TRACKLETS)) {
+    add((const void* const*)&v->x_ref, c->at<float>(L.o_x_ref) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->z_ref, c->at<float>(L.o_z_ref) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->chi2, c->at<float>(L.o_chi2) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->par, c->at<float>(L.o_par) + t0, 4 * (size_t)nt, 5);
+    add((const void* const*)&v->cov, c->at<float>(L.o_cov) + t0, 4 * (size_t)nt, 15);
+    add((const void* const*)&v->n_hits_trk, c->at<int32_t>(L.o_n_hits) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->n_fit, c->at<int32_t>(L.o_n_fit) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->first_row, c->at<int32_t>(L.o_first) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->last_row, c->at<int32_t>(L.o_last) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->trk_start_hit, c->at<int32_t>(L.o_start) + t0, 4 * (size_t)nt);
+    add((const void* const*)&v->hit_offset, c->at<int32_t>(L.o_hit_offset) + t0 + sector, 4 * (size_t)(nt + 1));
+    add((const void* const*)&v->hit_idx, c->at<int32_t>(L.o_hit_idx) + h0, 4 * (size_t)(h1 - h0));
+    v->trk_stride = host ? nt : c->CS;
+  }
+  if (!host) {
+    for (auto& it : items) *it.dst = it.src;
+    return TPCCA_OK;
+  }
+  size_t need = 256;
+  for (auto& it : items) need += align_up(it.bytes * it.planes + 4);
+  if (need > c->arena_bytes) {
+    if (c->arena) cudaFreeHost(c->arena);
+    c->arena = nullptr; c->arena_bytes = 0;
+    const size_t want = need + need / 4;
+    cudaError_t e = cudaMallocHost((void**)&c->arena, want);
+    if (e != cudaSuccess) return set_err(c, TPCCA_E_CUDA, "cudaMallocHost(%zu) failed: %s", want, cudaGetErrorString(e));
+    c->arena_bytes = want;
+  }
+  size_t cur = 0;
+  for (auto& it : items) {
+    char* dst = c->arena + cur;
+    if (it.bytes) {
+      if (it.planes == 1) CU(c, cudaMemcpyAsync(dst, it.src, it.bytes, cudaMemcpyDeviceToHost, c->stream));
+      else CU(c, cudaMemcpy2DAsync(dst, it.bytes, it.src, 4 * (size_t)c->CS, it.bytes, it.planes, cudaMemcpyDeviceToHost, c->stream));
+    }
+    *it.dst = dst;
+    cur += align_up(it.bytes * it.planes + 4);
+  }
+  CU(c, cudaStreamSynchronize(c->stream));
   return TPCCA_OK;
 }
 
 void tpcca_destroy(tpcca_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->stream);
-  for (int i = 0; i < 7; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+  for (int k = 0; k < tpcca_ctx::kRing; ++k)
+    for (int i = 0; i < 6; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
+  if (c->arena) cudaFreeHost(c->arena);
   delete c;
 }
 

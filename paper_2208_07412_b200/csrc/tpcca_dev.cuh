@@ -55,6 +55,7 @@ struct DevStatus {
   int32_t start_off[kMaxSectors + 1];   // first start-hit slot of each sector
   int32_t trk_off[kMaxSectors + 1];     // first track of each sector
   int64_t hit_off[kMaxSectors + 1];     // first hit of each sector (global CSR base)
+  unsigned long long work[5];           // S5 work counters: propagations, updates, gates, searches, candidates
 };
 
 // ---- S1 key: by = clamp(floor((y - y_lo) * inv_bin_y), 0, ny - 1) ------------
