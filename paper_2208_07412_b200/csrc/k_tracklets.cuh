@@ -131,207 +131,252 @@ __device__ __forceinline__ void kf_update(KF& s, float ym, float zm, const KFCon
   s.n++;
 }
 
-// Per-row tables staged in shared memory (lanes of a warp sit on different rows in S5).
-struct RowTab {
-  float x, y_lo, inv_by, ny_hi, inv_bz, nz_hi;
-  int32_t ny, bin_base;
-};
-
 // slot-space scratch of S5 (SoA with stride cap): 24 float planes + 4 int planes
 constexpr int kTrkF = 24;   // x_ref, z_ref, p0..p4, c[15], chi2, (pad)
 constexpr int kTrkI = 4;    // n_hits (0 = rejected), n_fit, first_row, last_row
 
+constexpr int kS5Threads = 128;   // threads per block of k_tracklets
+constexpr int kS5BlocksPerSM = 6;  // resident blocks per SM the kernel is compiled for (persistent grid)
+constexpr int kS5Refill = 4;      // idle lanes of a warp that trigger a refill from the work counter
+constexpr int kSnapF = 22;        // floats of a saved Kalman state: x, p[5], c[15], chi2
+
+// scalars of S5, passed by value (constant bank: no registers)
+struct S5Params {
+  float Bc, err2_y, err2_z, max_sinphi;
+  float ic0, ic1, ic2, ic3, ic4;
+  float win_y, win_z, gate, margin, grid_z_lo;
+  int32_t n_rows, n_sectors, max_gap, min_hits, bins_per_sector;
+};
+
 // ---- K5a ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128)
+// One tracklet per thread.  The three phases (A follow links, B extrapolate up, C refit down) are
+// folded into ONE loop over row steps, so lanes in different phases share the propagate / search /
+// update instruction stream.  A lane that finishes its tracklet goes idle; as soon as kS5Refill
+// lanes of the warp are idle (or no lane is active) the warp takes that many new start hits from
+// the global work counter, so warps never wait for their longest tracklet.
+// The phase-C snapshot ("state right after the last update") lives in registers while it equals
+// the running state and is parked in shared memory the moment the running state moves on without
+// an update, which keeps the register count at one Kalman state per lane.
+__global__ void __launch_bounds__(kS5Threads, kS5BlocksPerSM)
 k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-            DevStatus* __restrict__ st, const float2* __restrict__ syz,
+            DevStatus* __restrict__ st, const S5Params P, const float2* __restrict__ syz,
             const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
             const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
             const int32_t* __restrict__ start_hit, int32_t cap,
             int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
             int32_t* __restrict__ trk_i /*[kTrkI][cap]*/) {
-  __shared__ RowTab tab[kMaxRows];
+  __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_nyh[kMaxRows], t_ibz[kMaxRows], t_nzh[kMaxRows];
+  __shared__ int32_t t_ny[kMaxRows], t_base[kMaxRows];
   __shared__ int s_start_off[kMaxSectors + 1];
-  __shared__ int s_work[4];
-  const int n_rows = T->n_rows, ns = T->n_sectors;
+  __shared__ int s_sec_off[kMaxSectors + 1];
+  __shared__ float s_snap[kSnapF][kS5Threads];
+  const int n_rows = P.n_rows, ns = P.n_sectors;
   for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
-    RowTab t;
-    t.x = T->row_x[r]; t.y_lo = T->y_lo[r]; t.inv_by = T->inv_by[r]; t.ny_hi = T->ny_hi[r];
-    t.inv_bz = T->inv_bz[r]; t.nz_hi = T->nz_hi[r]; t.ny = T->ny[r]; t.bin_base = T->bin_base[r];
-    tab[r] = t;
+    t_x[r] = T->row_x[r]; t_ylo[r] = T->y_lo[r]; t_iby[r] = T->inv_by[r]; t_nyh[r] = T->ny_hi[r];
+    t_ibz[r] = T->inv_bz[r]; t_nzh[r] = T->nz_hi[r]; t_ny[r] = T->ny[r]; t_base[r] = T->bin_base[r];
   }
-  for (int i = threadIdx.x; i <= ns; i += blockDim.x) s_start_off[i] = st->start_off[i];
+  for (int i = threadIdx.x; i <= ns; i += blockDim.x) { s_start_off[i] = st->start_off[i]; s_sec_off[i] = sec[i].off; }
   __syncthreads();
   if (st->err_capacity) return;
   const int n_start = st->n_start;
   KFConst K;
-  K.Bc = T->Bc; K.err2_y = T->err2_y; K.err2_z = T->err2_z; K.max_sinphi = T->max_sinphi;
+  K.Bc = P.Bc; K.err2_y = P.err2_y; K.err2_z = P.err2_z; K.max_sinphi = P.max_sinphi;
   K.c24 = (float)(1.0 / 24.0); K.c640 = (float)(3.0 / 640.0); K.c12 = (float)(1.0 / 12.0);
-  K.ic0 = T->init_cov[0]; K.ic1 = T->init_cov[1]; K.ic2 = T->init_cov[2]; K.ic3 = T->init_cov[3];
-  K.ic4 = T->init_cov[4];
-  const float win_y = T->win_y, win_z = T->win_z, gate = T->gate, margin = T->margin;
-  const float grid_z_lo = T->grid_z_lo;
-  const int max_gap = T->tc_max_gap, min_hits = T->tc_min_hits;
-  const float my = win_y + margin, mz = win_z + margin;
-  const size_t nbp1 = (size_t)T->bins_per_sector + 1;
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  K.ic0 = P.ic0; K.ic1 = P.ic1; K.ic2 = P.ic2; K.ic3 = P.ic3; K.ic4 = P.ic4;
+  const float my = P.win_y + P.margin, mz = P.win_z + P.margin;
+  const size_t nbp1 = (size_t)P.bins_per_sector + 1;
+  const int lane = threadIdx.x & 31;
+  const int tid = threadIdx.x;
   unsigned w_prop = 0, w_upd = 0, w_gate = 0, w_search = 0, w_cand = 0;   // work counters
 
-  for (;;) {
-    // dynamic work distribution: one warp takes 32 consecutive start hits
-    if (lane == 0) s_work[wid] = atomicAdd(&st->work_counter, 32);
-    __syncwarp();
-    const int slot = s_work[wid] + lane;
-    __syncwarp();
-    if (slot - lane >= n_start) break;
-    if (slot >= n_start) continue;
+  enum { PH_A = 0, PH_B = 1, PH_C = 2, PH_IDLE = 3 };
+  // ---- per-lane tracklet state ---------------------------------------------------------------
+  int phase = PH_IDLE;
+  bool drained = false;      // warp-uniform: the work counter ran out
+  int slot = 0, r = 0, cur = -1, top = 0, top_hit = -1, gap = 0, n_hits = 0, first = 0, r0 = 0;
+  bool fresh = false;        // running state == snapshot (last operation was a phase-C update)
+  bool saved = false;        // snapshot parked in shared memory
+  float z_ref = 0.f;
+  const float2* yz = syz;
+  const int32_t* lup = link_up;
+  const int32_t* ord = order;
+  const uint32_t* bs = bin_start;
+  KF f;
+  f.x = 0.f; f.p0 = f.p1 = f.p2 = f.p3 = f.p4 = 0.f;
+  kf_reset_cov(f, K);
 
-    // sector of the slot
-    int s = 0;
-    {
-      int lo = 0, hi = ns - 1;
-      while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (s_start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
-      s = lo;
-    }
-    const int off = sec[s].off;
-    const float2* yz = syz + off;
-    const int32_t* ord = order + off;
-    const int32_t* lup = link_up + off;
-    const uint32_t* bs = bin_start + (size_t)s * nbp1;
-    const int32_t* rs = row_start + s * (n_rows + 1);
-    const int c0 = start_hit[slot];
-    const int r0 = row_search(rs, n_rows, c0);
-    const int c1 = lup[c0];
-    const float2 h0 = yz[c0], h1 = yz[c1];
-    const float z_ref = h0.y;
-    KF f;
-    {
-      const float dx = tab[r0 + 1].x - tab[r0].x;
-      const float dy = h1.x - h0.x;
-      const float dz = h1.y - z_ref;
-      const float d = sqrtf(dx * dx + dy * dy);
-      f.x = tab[r0].x;
-      f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
-      kf_reset_cov(f, K);
-    }
-    // search: best cluster of row r in the tc window around the prediction
-    auto search = [&](int r, float& best_d2) -> int {
-      const RowTab t = tab[r];
-      const float yc = f.p0;
-      const float zc = z_ref + f.p1;
-      const int by0 = bin_coord(yc - my, t.y_lo, t.inv_by, t.ny_hi), by1 = bin_coord(yc + my, t.y_lo, t.inv_by, t.ny_hi);
-      const int bz0 = bin_coord(zc - mz, grid_z_lo, t.inv_bz, t.nz_hi), bz1 = bin_coord(zc + mz, grid_z_lo, t.inv_bz, t.nz_hi);
-      const float wy = f.c00 + K.err2_y;
-      const float wz = f.c11 + K.err2_z;
-      int best = -1;
-      ++w_search;
-      for (int bz = bz0; bz <= bz1; ++bz) {
-        const int b0 = t.bin_base + bz * t.ny;
-        const uint32_t e = __ldg(&bs[b0 + by1 + 1]);
-        for (uint32_t c = __ldg(&bs[b0 + by0]); c < e; ++c) {
-          const float2 h = __ldg(&yz[c]);
-          const float ry = h.x - f.p0;
-          const float rz = (h.y - z_ref) - f.p1;
-          if (!(fabsf(ry) <= win_y && fabsf(rz) <= win_z)) continue;
-          const float d2 = (ry * ry) / wy + (rz * rz) / wz;
-          ++w_cand;
-          if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
-            best = (int)c; best_d2 = d2;
-          }
-        }
-      }
-      return best;
-    };
-
-    // ---- unified phase loop --------------------------------------------------------------------
-    enum { PH_A = 0, PH_B = 1, PH_C = 2, PH_DONE = 3 };
-    int phase = PH_A;
-    int r = r0, cur = c0, top = r0, gap = 0;
-    int n_hits = 0, first = r0;
-    bool have_snap = false;
-    KF snap = f;
-    int32_t* hcol = hits + slot;
-    while (phase != PH_DONE) {
-      // phase transitions that need no propagation
-      if (phase == PH_A && cur == -1) { phase = PH_B; gap = 0; }          // r == last + 1 already
-      if (phase == PH_B && r >= n_rows) { phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; }
-      if (phase == PH_C && r < 0) { phase = PH_DONE; break; }
-      w_prop += (tab[r].x != f.x) ? 1u : 0u;
-      if (!kf_propagate(f, tab[r].x, K)) {
-        if (phase == PH_C) { phase = PH_DONE; break; }
-        // rows (top, r] of the up pass that were never decided hold no hit
-        phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top;
-        continue;
-      }
-      int take = -1;          // cluster to update with
-      bool is_new = false;    // hit[r] was empty before
-      if (phase == PH_A) {
-        const float2 h = yz[cur];
-        const float ym = h.x, zm = h.y - z_ref;
-        bool ok = true;
-        if (f.n >= 2) {
-          ++w_gate;
-          const float ry = ym - f.p0, rz = zm - f.p1;
-          const float d2 = (ry * ry) / (f.c00 + K.err2_y) + (rz * rz) / (f.c11 + K.err2_z);
-          ok = !(d2 > gate);
-        }
-        if (!ok) { phase = PH_B; gap = 0; continue; }   // state already sits on row r (dx = 0 next)
-        take = cur; is_new = true;
-      } else if (phase == PH_B) {
-        float d2 = 0.f;
-        const int b = search(r, d2);
-        if (b >= 0 && d2 <= gate) { take = b; is_new = true; }
-      } else {
-        const int hr = (r >= r0 && r <= top) ? hcol[(size_t)r * cap] : -1;
-        if (hr != -1) { take = hr; }
-        else if (f.n >= 2) {
-          float d2 = 0.f;
-          const int b = search(r, d2);
-          if (b >= 0 && d2 <= gate) { take = b; is_new = true; }
-        }
-      }
-      if (take >= 0) {
-        const float2 h = yz[take];
-        kf_update(f, h.x, h.y - z_ref, K);
-        ++w_upd;
-        if (is_new) { hcol[(size_t)r * cap] = take; ++n_hits; }
-        if (phase == PH_C) {
-          snap = f; have_snap = true;
-          if (is_new) { gap = 0; if (r < first) first = r; }
-        } else {
-          top = r; gap = 0;
-        }
-      } else {
-        if (phase == PH_B) {
-          hcol[(size_t)r * cap] = -1;
-          if (++gap > max_gap) { phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; continue; }
-        } else {   // PH_C, nothing taken
-          if (r < r0) {
-            hcol[(size_t)r * cap] = -1;
-            if (++gap > max_gap) { phase = PH_DONE; break; }
-          }
-        }
-      }
-      if (phase == PH_A) { cur = lup[cur]; ++r; }
-      else if (phase == PH_B) ++r;
-      else --r;
-    }
-    // ---- emit into slot space --------------------------------------------------------------------
-    const bool accept = (n_hits >= min_hits) && have_snap;
+  auto save_snap = [&]() {
+    s_snap[0][tid] = f.x; s_snap[1][tid] = f.p0; s_snap[2][tid] = f.p1; s_snap[3][tid] = f.p2;
+    s_snap[4][tid] = f.p3; s_snap[5][tid] = f.p4;
+    s_snap[6][tid] = f.c00; s_snap[7][tid] = f.c10; s_snap[8][tid] = f.c11; s_snap[9][tid] = f.c20;
+    s_snap[10][tid] = f.c21; s_snap[11][tid] = f.c22; s_snap[12][tid] = f.c30; s_snap[13][tid] = f.c31;
+    s_snap[14][tid] = f.c32; s_snap[15][tid] = f.c33; s_snap[16][tid] = f.c40; s_snap[17][tid] = f.c41;
+    s_snap[18][tid] = f.c42; s_snap[19][tid] = f.c43; s_snap[20][tid] = f.c44; s_snap[21][tid] = f.chi2;
+  };
+  int snap_n = 0;            // f.n at the time of the snapshot
+  // emit the tracklet of this lane into slot space and go idle
+  auto finish = [&]() {
+    if (fresh) { save_snap(); snap_n = f.n; saved = true; }
+    const bool accept = (n_hits >= P.min_hits) && saved;
     trk_i[0 * (size_t)cap + slot] = accept ? n_hits : 0;
     if (accept) {
-      trk_i[1 * (size_t)cap + slot] = snap.n;
+      trk_i[1 * (size_t)cap + slot] = snap_n;
       trk_i[2 * (size_t)cap + slot] = first;
       trk_i[3 * (size_t)cap + slot] = top;
       float* o = trk_f + slot;
       const size_t cs = (size_t)cap;
-      o[0 * cs] = snap.x; o[1 * cs] = z_ref;
-      o[2 * cs] = snap.p0; o[3 * cs] = snap.p1; o[4 * cs] = snap.p2; o[5 * cs] = snap.p3; o[6 * cs] = snap.p4;
-      o[7 * cs] = snap.c00; o[8 * cs] = snap.c10; o[9 * cs] = snap.c11; o[10 * cs] = snap.c20;
-      o[11 * cs] = snap.c21; o[12 * cs] = snap.c22; o[13 * cs] = snap.c30; o[14 * cs] = snap.c31;
-      o[15 * cs] = snap.c32; o[16 * cs] = snap.c33; o[17 * cs] = snap.c40; o[18 * cs] = snap.c41;
-      o[19 * cs] = snap.c42; o[20 * cs] = snap.c43; o[21 * cs] = snap.c44; o[22 * cs] = snap.chi2;
+      o[0 * cs] = s_snap[0][tid]; o[1 * cs] = z_ref;
+#pragma unroll
+      for (int k = 1; k < kSnapF; ++k) o[(k + 1) * cs] = s_snap[k][tid];
     }
+    phase = PH_IDLE;
+  };
+  auto to_phase_c = [&]() {
+    phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; cur = top_hit; fresh = false; saved = false;
+  };
+
+  for (;;) {
+    // ---- refill idle lanes from the work counter ---------------------------------------------
+    const unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
+    if (idle == 0xffffffffu && drained) break;
+    if (!drained && (__popc(idle) >= kS5Refill || idle == 0xffffffffu)) {
+      const int n_idle = __popc(idle);
+      int base = 0;
+      if (lane == 0) base = atomicAdd(&st->work_counter, n_idle);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (base + n_idle >= n_start) drained = true;
+      if (phase == PH_IDLE) {
+        const int my_slot = base + __popc(idle & ((1u << lane) - 1u));
+        if (my_slot < n_start) {
+          slot = my_slot;
+          int s = 0;
+          {
+            int lo = 0, hi = ns - 1;
+            while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (s_start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
+            s = lo;
+          }
+          const int off = s_sec_off[s];
+          yz = syz + off; ord = order + off; lup = link_up + off;
+          bs = bin_start + (size_t)s * nbp1;
+          const int32_t* rs = row_start + s * (n_rows + 1);
+          const int c0 = start_hit[slot];
+          r0 = row_search(rs, n_rows, c0);
+          const int c1 = lup[c0];
+          const float2 h0 = yz[c0], h1 = yz[c1];
+          z_ref = h0.y;
+          const float dx = t_x[r0 + 1] - t_x[r0];
+          const float dy = h1.x - h0.x;
+          const float dz = h1.y - z_ref;
+          const float d = sqrtf(dx * dx + dy * dy);
+          f.x = t_x[r0];
+          f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
+          kf_reset_cov(f, K);
+          phase = PH_A; r = r0; cur = c0; top = r0; top_hit = c0; gap = 0; n_hits = 0; first = r0;
+          fresh = false; saved = false;
+        }
+      }
+    }
+    if (phase == PH_IDLE) continue;
+
+    // ---- one row step ---------------------------------------------------------------------------
+    int32_t* hcol = hits + slot;
+    int cand = cur;                       // >= 0: cluster to use on this row; -1: none known
+    float2 h = make_float2(0.f, 0.f);
+    if (cand >= 0) h = __ldg(&yz[cand]);
+    int nxt = -1;                         // candidate of the next row (loaded early)
+    if (phase == PH_A) nxt = __ldg(&lup[cand]);
+    else if (phase == PH_C && r - 1 >= r0) nxt = hcol[(size_t)(r - 1) * cap];
+    const float xr = t_x[r];
+    if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
+    w_prop += (xr != f.x) ? 1u : 0u;
+    if (!kf_propagate(f, xr, K)) {
+      if (phase == PH_C) finish(); else to_phase_c();
+      continue;
+    }
+    bool took = false, is_new = false;
+    if (phase == PH_A) {
+      bool ok = true;
+      if (f.n >= 2) {
+        ++w_gate;
+        const float ry = h.x - f.p0, rz = (h.y - z_ref) - f.p1;
+        const float d2 = (ry * ry) / (f.c00 + K.err2_y) + (rz * rz) / (f.c11 + K.err2_z);
+        ok = !(d2 > P.gate);
+      }
+      if (!ok) { phase = PH_B; gap = 0; cur = -1; continue; }   // state already sits on row r (dx = 0 next)
+      took = true; is_new = true;
+    } else if (cand >= 0) {
+      took = true;                        // phase C, row already holds a hit: no gate
+    } else if (phase == PH_B || f.n >= 2) {
+      // search: best cluster of row r in the tc window around the prediction
+      const float yc = f.p0;
+      const float zc = z_ref + f.p1;
+      const float ylo = t_ylo[r], iby = t_iby[r], nyh = t_nyh[r], ibz = t_ibz[r], nzh = t_nzh[r];
+      const int by0 = bin_coord(yc - my, ylo, iby, nyh), by1 = bin_coord(yc + my, ylo, iby, nyh);
+      const int bz0 = bin_coord(zc - mz, P.grid_z_lo, ibz, nzh), bz1 = bin_coord(zc + mz, P.grid_z_lo, ibz, nzh);
+      const float wy = f.c00 + K.err2_y;
+      const float wz = f.c11 + K.err2_z;
+      const int ny = t_ny[r];
+      const uint32_t* bp = bs + t_base[r] + bz0 * ny;
+      int best = -1;
+      float best_d2 = 0.f;
+      float2 best_h = make_float2(0.f, 0.f);
+      ++w_search;
+      // bounds of the first three z slices are fetched together (a tc window spans <= 3 bins with
+      // the default tables); further slices, if any, are walked one by one
+      const int nsl = bz1 - bz0 + 1;
+      uint32_t c = __ldg(&bp[by0]), e = __ldg(&bp[by1 + 1]);
+      uint32_t c1 = 0, e1 = 0, c2 = 0, e2 = 0;
+      if (nsl > 1) { c1 = __ldg(&bp[ny + by0]); e1 = __ldg(&bp[ny + by1 + 1]); }
+      if (nsl > 2) { c2 = __ldg(&bp[2 * ny + by0]); e2 = __ldg(&bp[2 * ny + by1 + 1]); }
+      int k = 0;
+      for (;;) {
+        if (c >= e) {
+          ++k;
+          if (k >= nsl) break;
+          if (k == 1) { c = c1; e = e1; }
+          else if (k == 2) { c = c2; e = e2; }
+          else { c = __ldg(&bp[k * ny + by0]); e = __ldg(&bp[k * ny + by1 + 1]); }
+          continue;
+        }
+        const float2 hc = __ldg(&yz[c]);
+        const float ry = hc.x - f.p0;
+        const float rz = (hc.y - z_ref) - f.p1;
+        if (fabsf(ry) <= P.win_y && fabsf(rz) <= P.win_z) {
+          const float d2 = (ry * ry) / wy + (rz * rz) / wz;
+          ++w_cand;
+          if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
+            best = (int)c; best_d2 = d2; best_h = hc;
+          }
+        }
+        ++c;
+      }
+      if (best >= 0 && best_d2 <= P.gate) { cand = best; h = best_h; took = true; is_new = true; }
+    }
+    if (took) {
+      kf_update(f, h.x, h.y - z_ref, K);
+      ++w_upd;
+      if (is_new) { hcol[(size_t)r * cap] = cand; ++n_hits; }
+      if (phase == PH_C) {
+        fresh = true; saved = false;
+        if (is_new) { gap = 0; if (r < first) first = r; }
+      } else {
+        top = r; top_hit = cand; gap = 0;
+      }
+    } else {
+      if (phase == PH_B) {
+        hcol[(size_t)r * cap] = -1;
+        if (++gap > P.max_gap) { to_phase_c(); continue; }
+      } else if (r < r0) {                // phase C below the start hit
+        hcol[(size_t)r * cap] = -1;
+        if (++gap > P.max_gap) { finish(); continue; }
+      }
+    }
+    // ---- advance to the next row -------------------------------------------------------------
+    if (phase == PH_A) { cur = nxt; ++r; if (cur == -1) { phase = PH_B; gap = 0; } }
+    else if (phase == PH_B) ++r;
+    else { cur = nxt; --r; }
+    if (phase == PH_B && r >= n_rows) to_phase_c();
+    if (phase == PH_C && r < 0) finish();
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};

@@ -116,6 +116,7 @@ int64_t default_cap(int64_t N, int64_t CS) {
 
 struct tpcca_ctx {
   int device = 0;
+  int sm_count = 148;
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   size_t ws_bytes = 0;
@@ -227,6 +228,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
 
   tpcca_ctx* c = new tpcca_ctx;
   c->device = cuda_device;
+  c->sm_count = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
   c->stream = (cudaStream_t)cuda_stream;
   c->ws = (char*)workspace;
   c->ws_bytes = workspace_bytes;
@@ -420,8 +422,15 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
     CU(c, cudaMemsetAsync(&status->work_counter, 0, sizeof(int32_t), st));
     CU(c, cudaMemsetAsync(status->work, 0, sizeof(status->work), st));
-    k_tracklets<<<148 * 8, 128, 0, st>>>(T, sec, status, syz, bin_start, row_start, order, c->at<int32_t>(L.up), start_hit,
-                                         cap, hits, trk_f, trk_i);
+    const DevTables& t = c->tab;
+    S5Params sp;
+    sp.Bc = t.Bc; sp.err2_y = t.err2_y; sp.err2_z = t.err2_z; sp.max_sinphi = t.max_sinphi;
+    sp.ic0 = t.init_cov[0]; sp.ic1 = t.init_cov[1]; sp.ic2 = t.init_cov[2]; sp.ic3 = t.init_cov[3]; sp.ic4 = t.init_cov[4];
+    sp.win_y = t.win_y; sp.win_z = t.win_z; sp.gate = t.gate; sp.margin = t.margin; sp.grid_z_lo = t.grid_z_lo;
+    sp.n_rows = t.n_rows; sp.n_sectors = t.n_sectors; sp.max_gap = t.tc_max_gap; sp.min_hits = t.tc_min_hits;
+    sp.bins_per_sector = t.bins_per_sector;
+    k_tracklets<<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order,
+                                                                     c->at<int32_t>(L.up), start_hit, cap, hits, trk_f, trk_i);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
