@@ -175,14 +175,48 @@ k_grid_fixup(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
   }
 }
 
-// ---- K1g: row_start[s][r] = bin_start[s][bin_base[r]] ------------------------------------------
-__global__ void k_row_start(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_start,
-                            int32_t* __restrict__ row_start) {
-  const int s = blockIdx.x;
-  const int nr = T->n_rows;
+// ---- K1g: row_start[s][r] = bin_start[s][bin_base[r]], and the row-aligned tiling of S2 ---------
+// One block.  nf_tile_start[i], i = s * n_rows + r: first S2 tile of (sector s, row r); a tile is
+// kNfTile consecutive sorted clusters of ONE row; nf_tile_start[ns * n_rows] = total.
+constexpr int kNfTile = 256;
+
+__global__ void __launch_bounds__(1024)
+k_row_tables(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_start,
+             int32_t* __restrict__ row_start, int32_t* __restrict__ nf_tile_start) {
+  __shared__ int ws[33];
+  const int nr = T->n_rows, ns = T->n_sectors;
   const size_t stride = (size_t)T->bins_per_sector + 1;
-  for (int r = threadIdx.x; r <= nr; r += blockDim.x)
-    row_start[s * (nr + 1) + r] = (int32_t)bin_start[s * stride + T->bin_base[r]];
+  for (int i = threadIdx.x; i < ns * (nr + 1); i += blockDim.x) {
+    const int s = i / (nr + 1), r = i - s * (nr + 1);
+    row_start[i] = (int32_t)bin_start[s * stride + T->bin_base[r]];
+  }
+  __syncthreads();
+  int carry = 0;
+  const int n = ns * nr;
+  for (int base = 0; base < n; base += 1024) {
+    const int i = base + threadIdx.x;
+    int v = 0;
+    if (i < n) {
+      const int s = i / nr, r = i - s * nr;
+      const int cnt = row_start[s * (nr + 1) + r + 1] - row_start[s * (nr + 1) + r];
+      v = (cnt + kNfTile - 1) / kNfTile;
+    }
+    int total;
+    const int ex = block_exclusive_scan<int>(v, ws, total);
+    if (i < n) nf_tile_start[i] = carry + ex;
+    carry += total;
+  }
+  if (threadIdx.x == 0) nf_tile_start[n] = carry;
+}
+
+// ---- K1h: tile descriptors of S2: desc[t] = (s * n_rows + r, chunk inside the row) -------------
+__global__ void __launch_bounds__(64)
+k_nf_tile_desc(const DevTables* __restrict__ T, const int32_t* __restrict__ nf_tile_start, int2* __restrict__ desc) {
+  const int n = T->n_sectors * T->n_rows;
+  for (int i = blockIdx.x; i < n; i += gridDim.x) {
+    const int t0 = nf_tile_start[i], t1 = nf_tile_start[i + 1];
+    for (int t = t0 + threadIdx.x; t < t1; t += blockDim.x) desc[t] = make_int2(i, t - t0);
+  }
 }
 
 }  // namespace tpcca

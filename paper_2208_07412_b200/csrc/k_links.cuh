@@ -4,7 +4,8 @@
 
 namespace tpcca {
 
-constexpr int kNfKD = 8;   // down-candidates cached per thread in shared memory
+constexpr int kNfK = 6;        // window candidates cached per side and thread in shared memory
+constexpr int kNfThreads = 256;
 
 // row of sorted position p: rows are contiguous runs; start from the block's first row.
 __device__ __forceinline__ int row_of(const int32_t* __restrict__ rs, int r, int p) {
@@ -20,140 +21,155 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
   return lo;
 }
 
-// ---- K2: neighbour finder, one thread per cluster -----------------------------
+// Window candidates of one side (A, B, C = the side's NfConst groups): every cluster q of the
+// neighbour row with |y_q - y_c| <= hy and |z_q - z_c| <= hz.  The bin range is a superset of the
+// window; the z slices of the range are walked as ONE flattened loop so that the
+// lanes of a warp, whose slices hold different numbers of clusters, stay together.
+// Caches (dy * dxo, dz * dxo) and q of the first kNfK hits; returns the number of hits.
+// UP: the cached vector is (y_q - y_c) * dxo; down side: (y_c - y_q) * dxo (fl(a - b) = -fl(b - a),
+// so the negation is exact).
+template <bool UP>
+__device__ __forceinline__ int nf_gather(const float2 c, const float4 A, const float4 B, const int4 C, const float dxo,
+                                         const uint32_t* __restrict__ bs,
+                                         const float2* __restrict__ yz, float2 (*s_v)[kNfThreads],
+                                         int32_t (*s_i)[kNfThreads], const int tid) {
+  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
+  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
+  const uint32_t* bp = bs + C.w + bz0 * C.z;
+  const int nsl = bz1 - bz0 + 1;
+  uint32_t q = __ldg(&bp[by0]), e = __ldg(&bp[by1 + 1]);
+  uint32_t q1 = 0, e1 = 0;
+  if (nsl > 1) { q1 = __ldg(&bp[C.z + by0]); e1 = __ldg(&bp[C.z + by1 + 1]); }
+  int k = 0, n = 0;
+  for (;;) {
+    if (q >= e) {
+      if (++k >= nsl) break;
+      if (k == 1) { q = q1; e = e1; }
+      else { q = __ldg(&bp[k * C.z + by0]); e = __ldg(&bp[k * C.z + by1 + 1]); }
+      continue;
+    }
+    const float2 v = __ldg(&yz[q]);
+    const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
+    if (fabsf(dy) <= A.x && fabsf(dz) <= A.y) {
+      if (n < kNfK) {
+        s_v[n][tid] = make_float2(__fmul_rn(UP ? dy : -dy, dxo), __fmul_rn(UP ? dz : -dz, dxo));
+        s_i[n][tid] = (int32_t)q;
+      }
+      ++n;
+    }
+    ++q;
+  }
+  return n;
+}
+
+// visit every window candidate of one side (plain nested loops; slow path only)
+template <class F>
+__device__ __forceinline__ void nf_for_each(const float2 c, const float4 A, const float4 B, const int4 C,
+                                            const uint32_t* __restrict__ bs, const float2* __restrict__ yz, F fn) {
+  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
+  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
+  for (int bz = bz0; bz <= bz1; ++bz) {
+    const uint32_t* bp = bs + C.w + bz * C.z;
+    const uint32_t e = __ldg(&bp[by1 + 1]);
+    for (uint32_t q = __ldg(&bp[by0]); q < e; ++q) {
+      const float2 v = __ldg(&yz[q]);
+      const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
+      if (fabsf(dy) <= A.x && fabsf(dz) <= A.y) fn(q, dy, dz);
+    }
+  }
+}
+
+// Slow path of S2 for a cluster with more than kNfK window candidates on a side (dense noise):
+// the full U x D product by nested rescans of both windows.
+__device__ __noinline__ void nf_slow(const float2 c, const NfConst* __restrict__ kc, const uint32_t* __restrict__ bs,
+                                     const float2* __restrict__ yz, const int32_t* __restrict__ ord,
+                                     float& best, int32_t& bu, int32_t& bd) {
+  const float4 dA = kc->dA, dB = kc->dB, uA = kc->uA, uB = kc->uB, g = kc->g;
+  const int4 dC = kc->dC, uC = kc->uC;
+  bu = -1; bd = -1; best = 0.0f;
+  nf_for_each(c, uA, uB, uC, bs, yz, [&](uint32_t u, float dyu, float dzu) {
+    const float Ay = __fmul_rn(dyu, g.y), Az = __fmul_rn(dzu, g.y);
+    nf_for_each(c, dA, dB, dC, bs, yz, [&](uint32_t d, float dyd, float dzd) {
+      const float ay = __fsub_rn(Ay, __fmul_rn(-dyd, g.x));
+      const float az = __fsub_rn(Az, __fmul_rn(-dzd, g.x));
+      const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
+      bool better;
+      if (bu < 0) better = true;
+      else if (sc < best) better = true;
+      else if (sc == best) {
+        const int32_t ou = __ldg(&ord[u]), obu = __ldg(&ord[bu]);
+        better = (ou != obu) ? (ou < obu) : (__ldg(&ord[d]) < __ldg(&ord[bd]));
+      } else better = false;
+      if (better) { best = sc; bu = (int32_t)u; bd = (int32_t)d; }
+    });
+  });
+}
+
+// ---- K2: neighbour finder, one thread per cluster ------------------------
 // For cluster c of row r (1 <= r <= n_rows-2): over U x D (exact windows in rows r+1, r-1) the
 // pair minimising score = ay^2 + az^2, ay = (yu-yc)*dxd - (yc-yd)*dxu; ties -> smallest original
 // id of u, then of d; stored if score <= nf_cut[r].
-__global__ void __launch_bounds__(256)
+// A tile = kNfThreads consecutive sorted clusters of ONE row, so every per-row constant is block
+// uniform (seven 128-bit loads); blocks walk the tile list with a grid stride.  Three flattened,
+// warp-friendly loops per thread: gather D, gather U (window hits cached in shared memory), then
+// the nu * nd pair scores.
+__global__ void __launch_bounds__(kNfThreads)
 k_neighbours(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
              const float2* __restrict__ syz, const uint32_t* __restrict__ bin_start,
              const int32_t* __restrict__ row_start, const int32_t* __restrict__ order,
+             const int32_t* __restrict__ nf_tile_start, const int2* __restrict__ nf_desc,
              int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
-  __shared__ float s_by[kNfKD][256];
-  __shared__ float s_bz[kNfKD][256];
-  __shared__ int32_t s_id[kNfKD][256];
-  __shared__ int s_r0;
-  const int ns = __ldg(&T->n_sectors);
+  __shared__ float2 s_uv[kNfK][kNfThreads];
+  __shared__ float2 s_dv[kNfK][kNfThreads];
+  __shared__ int32_t s_ui[kNfK][kNfThreads];
+  __shared__ int32_t s_di[kNfK][kNfThreads];
   const int n_rows = __ldg(&T->n_rows);
-  const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
-  const int n = __ldg(&sec[s].n), off = __ldg(&sec[s].off);
-  const int p0 = (blockIdx.x - __ldg(&sec[s].tile256)) * 256;
-  const int32_t* rs = row_start + s * (n_rows + 1);
-  if (threadIdx.x == 0) s_r0 = row_search(rs, n_rows, p0);
-  __syncthreads();
-  const int p = p0 + threadIdx.x;
-  if (p >= n) return;
+  const int n_tiles = __ldg(&nf_tile_start[__ldg(&T->n_sectors) * n_rows]);
+  const size_t nbp1 = (size_t)__ldg(&T->bins_per_sector) + 1;
   const int tid = threadIdx.x;
-  const int r = row_of(rs, s_r0, p);
-  const float2* yz = syz + off;
-  const int32_t* ord = order + off;
-  const uint32_t* bs = bin_start + (size_t)s * (__ldg(&T->bins_per_sector) + 1);
-  int32_t bu = -1, bd = -1;
-  if (r >= 1 && r <= n_rows - 2) {
-    const float2 c = yz[p];
-    const float margin = __ldg(&T->margin);
-    const float dxu = __fsub_rn(__ldg(&T->row_x[r + 1]), __ldg(&T->row_x[r]));
-    const float dxd = __fsub_rn(__ldg(&T->row_x[r]), __ldg(&T->row_x[r - 1]));
-    // ---- pass 1: down window (row r-1): cache (By, Bz, id)
-    int nd = 0;
-    {
-      const int r2 = r - 1;
-      const float hy = __ldg(&T->hy_dn[r]), hz = __ldg(&T->hz_dn[r]);
-      const float my = __fadd_rn(hy, margin), mz = __fadd_rn(hz, margin);
-      const float ylo = __ldg(&T->y_lo[r2]), iby = __ldg(&T->inv_by[r2]), nyh = __ldg(&T->ny_hi[r2]);
-      const float zlo = __ldg(&T->grid_z_lo), ibz = __ldg(&T->inv_bz[r2]), nzh = __ldg(&T->nz_hi[r2]);
-      const int by0 = bin_coord(__fsub_rn(c.x, my), ylo, iby, nyh), by1 = bin_coord(__fadd_rn(c.x, my), ylo, iby, nyh);
-      const int bz0 = bin_coord(__fsub_rn(c.y, mz), zlo, ibz, nzh), bz1 = bin_coord(__fadd_rn(c.y, mz), zlo, ibz, nzh);
-      const int ny = __ldg(&T->ny[r2]);
-      const int base = __ldg(&T->bin_base[r2]);
-      for (int bz = bz0; bz <= bz1; ++bz) {
-        const int b0 = base + bz * ny;
-        const uint32_t e = __ldg(&bs[b0 + by1 + 1]);
-        for (uint32_t q = __ldg(&bs[b0 + by0]); q < e; ++q) {
-          const float2 d = __ldg(&yz[q]);
-          const float dy = __fsub_rn(d.x, c.x), dz = __fsub_rn(d.y, c.y);
-          if (fabsf(dy) <= hy && fabsf(dz) <= hz) {
-            if (nd < kNfKD) {
-              s_by[nd][tid] = __fmul_rn(__fsub_rn(c.x, d.x), dxu);
-              s_bz[nd][tid] = __fmul_rn(__fsub_rn(c.y, d.y), dxu);
-              s_id[nd][tid] = (int32_t)q;
-            }
-            ++nd;
-          }
-        }
-      }
-    }
-    if (nd > 0) {
-      // ---- pass 2: up window (row r+1); score against the cached (or re-scanned) D
-      const int r2 = r + 1;
-      const float hy = __ldg(&T->hy_up[r]), hz = __ldg(&T->hz_up[r]);
-      const float my = __fadd_rn(hy, margin), mz = __fadd_rn(hz, margin);
-      const float ylo = __ldg(&T->y_lo[r2]), iby = __ldg(&T->inv_by[r2]), nyh = __ldg(&T->ny_hi[r2]);
-      const float zlo = __ldg(&T->grid_z_lo), ibz = __ldg(&T->inv_bz[r2]), nzh = __ldg(&T->nz_hi[r2]);
-      const int by0 = bin_coord(__fsub_rn(c.x, my), ylo, iby, nyh), by1 = bin_coord(__fadd_rn(c.x, my), ylo, iby, nyh);
-      const int bz0 = bin_coord(__fsub_rn(c.y, mz), zlo, ibz, nzh), bz1 = bin_coord(__fadd_rn(c.y, mz), zlo, ibz, nzh);
-      const int ny = __ldg(&T->ny[r2]);
-      const int base = __ldg(&T->bin_base[r2]);
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int2 td = __ldg(&nf_desc[tile]);
+    const int s = td.x / n_rows, r = td.x - s * n_rows;
+    const int32_t* rs = row_start + s * (n_rows + 1) + r;
+    const int p = __ldg(&rs[0]) + td.y * kNfThreads + tid;
+    if (p >= __ldg(&rs[1])) continue;
+    const int off = __ldg(&sec[s].off);
+    int32_t bu = -1, bd = -1;
+    if (r >= 1 && r <= n_rows - 2) {
+      const float2* yz = syz + off;
+      const uint32_t* bs = bin_start + (size_t)s * nbp1;
+      const NfConst* kc = &T->nf[r];
+      const float2 c = yz[p];
+      const float4 g = __ldg(&kc->g);
+      const int nd = nf_gather<false>(c, __ldg(&kc->dA), __ldg(&kc->dB), __ldg(&kc->dC), g.x, bs, yz, s_dv, s_di, tid);
+      const int nu = nf_gather<true>(c, __ldg(&kc->uA), __ldg(&kc->uB), __ldg(&kc->uC), g.y, bs, yz, s_uv, s_ui, tid);
       float best = 0.0f;
-      bool have = false;
-      auto consider = [&](float s, int32_t u, int32_t d) {
-        bool better;
-        if (!have) better = true;
-        else if (s < best) better = true;
-        else if (s == best) {
-          const int32_t ou = __ldg(&ord[u]), obu = __ldg(&ord[bu]);
-          if (ou != obu) better = ou < obu;
-          else better = __ldg(&ord[d]) < __ldg(&ord[bd]);
-        } else better = false;
-        if (better) { have = true; best = s; bu = u; bd = d; }
-      };
-      for (int bz = bz0; bz <= bz1; ++bz) {
-        const int b0 = base + bz * ny;
-        const uint32_t e = __ldg(&bs[b0 + by1 + 1]);
-        for (uint32_t q = __ldg(&bs[b0 + by0]); q < e; ++q) {
-          const float2 u = __ldg(&yz[q]);
-          const float dy = __fsub_rn(u.x, c.x), dz = __fsub_rn(u.y, c.y);
-          if (!(fabsf(dy) <= hy && fabsf(dz) <= hz)) continue;
-          const float Ay = __fmul_rn(dy, dxd), Az = __fmul_rn(dz, dxd);
-          if (nd <= kNfKD) {
-            for (int k = 0; k < nd; ++k) {
-              const float ay = __fsub_rn(Ay, s_by[k][tid]);
-              const float az = __fsub_rn(Az, s_bz[k][tid]);
-              const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
-              consider(sc, (int32_t)q, s_id[k][tid]);
-            }
-          } else {
-            // overflow (dense noise): re-scan the down window for this u
-            const int rd = r - 1;
-            const float hyd = __ldg(&T->hy_dn[r]), hzd = __ldg(&T->hz_dn[r]);
-            const float myd = __fadd_rn(hyd, margin), mzd = __fadd_rn(hzd, margin);
-            const float ylod = __ldg(&T->y_lo[rd]), ibyd = __ldg(&T->inv_by[rd]), nyhd = __ldg(&T->ny_hi[rd]);
-            const float ibzd = __ldg(&T->inv_bz[rd]), nzhd = __ldg(&T->nz_hi[rd]);
-            const int dy0 = bin_coord(__fsub_rn(c.x, myd), ylod, ibyd, nyhd), dy1 = bin_coord(__fadd_rn(c.x, myd), ylod, ibyd, nyhd);
-            const int dz0 = bin_coord(__fsub_rn(c.y, mzd), zlo, ibzd, nzhd), dz1 = bin_coord(__fadd_rn(c.y, mzd), zlo, ibzd, nzhd);
-            const int nyd = __ldg(&T->ny[rd]);
-            const int based = __ldg(&T->bin_base[rd]);
-            for (int bzd = dz0; bzd <= dz1; ++bzd) {
-              const int bd0 = based + bzd * nyd;
-              const uint32_t ed = __ldg(&bs[bd0 + dy1 + 1]);
-              for (uint32_t qd = __ldg(&bs[bd0 + dy0]); qd < ed; ++qd) {
-                const float2 d = __ldg(&yz[qd]);
-                const float ddy = __fsub_rn(d.x, c.x), ddz = __fsub_rn(d.y, c.y);
-                if (!(fabsf(ddy) <= hyd && fabsf(ddz) <= hzd)) continue;
-                const float ay = __fsub_rn(Ay, __fmul_rn(__fsub_rn(c.x, d.x), dxu));
-                const float az = __fsub_rn(Az, __fmul_rn(__fsub_rn(c.y, d.y), dxu));
-                const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
-                consider(sc, (int32_t)q, (int32_t)qd);
-              }
-            }
+      if (nd <= kNfK && nu <= kNfK) {
+        const int np = nu * nd;
+        int iu = 0, id = 0, bi = -1, bj = 0;
+        for (int k = 0; k < np; ++k) {
+          const float2 a = s_uv[iu][tid], b = s_dv[id][tid];
+          const float ay = __fsub_rn(a.x, b.x), az = __fsub_rn(a.y, b.y);
+          const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
+          bool better = (bi < 0) || (sc < best);
+          if (!better && sc == best) {
+            const int32_t* ord = order + off;
+            const int32_t u = s_ui[iu][tid], ub = s_ui[bi][tid];
+            if (u != ub) better = __ldg(&ord[u]) < __ldg(&ord[ub]);
+            else better = __ldg(&ord[s_di[id][tid]]) < __ldg(&ord[s_di[bj][tid]]);
           }
+          if (better) { best = sc; bi = iu; bj = id; }
+          if (++id == nd) { id = 0; ++iu; }
         }
+        if (bi >= 0) { bu = s_ui[bi][tid]; bd = s_di[bj][tid]; }
+      } else {
+        nf_slow(c, kc, bs, yz, order + off, best, bu, bd);
       }
-      if (!(have && best <= __ldg(&T->nf_cut[r]))) { bu = -1; bd = -1; }
+      if (!(bu >= 0 && best <= g.z)) { bu = -1; bd = -1; }
     }
+    link_up[off + p] = bu;
+    link_dn[off + p] = bd;
   }
-  link_up[off + p] = bu;
-  link_dn[off + p] = bd;
 }
 
 // ---- K3: link cleaner + per-tile start-hit count -------------------------

@@ -136,8 +136,18 @@ constexpr int kTrkF = 24;   // x_ref, z_ref, p0..p4, c[15], chi2, (pad)
 constexpr int kTrkI = 4;    // n_hits (0 = rejected), n_fit, first_row, last_row
 
 constexpr int kS5Threads = 128;   // threads per block of k_tracklets
-constexpr int kS5BlocksPerSM = 6;  // resident blocks per SM the kernel is compiled for (persistent grid)
-constexpr int kS5Refill = 4;      // idle lanes of a warp that trigger a refill from the work counter
+#ifndef TPCCA_S5_BPS
+#define TPCCA_S5_BPS 6
+#endif
+constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
+#ifndef TPCCA_S5_REFILL
+#define TPCCA_S5_REFILL 4
+#endif
+constexpr int kS5Refill = TPCCA_S5_REFILL;      // idle lanes of a warp that trigger a refill from the work counter
+#ifndef TPCCA_S5_UNROLL
+#define TPCCA_S5_UNROLL 4
+#endif
+constexpr int kS5Unroll = TPCCA_S5_UNROLL;   // candidate loads in flight per lane in the S5 search
 constexpr int kSnapF = 22;        // floats of a saved Kalman state: x, p[5], c[15], chi2
 
 // scalars of S5, passed by value (constant bank: no registers)
@@ -147,6 +157,51 @@ struct S5Params {
   float win_y, win_z, gate, margin, grid_z_lo;
   int32_t n_rows, n_sectors, max_gap, min_hits, bins_per_sector;
 };
+
+// approximate reciprocal (one MUFU.RCP); used only to rank candidates and to pre-decide gates
+// that are nowhere near the threshold -- every decision that could flip is taken on the exact form
+__device__ __forceinline__ float rcp_fast(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// Gate of DESIGN.md 3.5: dist2 = ry^2 / wy + rz^2 / wz > gate, decided exactly.  The division-free
+// estimate is within ~1e-6 relative of dist2, so it decides whenever it is more than 1e-4 relative
+// away from the gate; otherwise (and for NaN / inf estimates) the defined expression is evaluated.
+__device__ __forceinline__ bool gate_exceeded(float ry, float rz, float wy, float wz, float iwy, float iwz, float gate) {
+  const float ry2 = ry * ry, rz2 = rz * rz;
+  const float est = ry2 * iwy + rz2 * iwz;
+  if (est > gate * 1.0001f + 1e-30f) return true;
+  if (est < gate * 0.9999f - 1e-30f) return false;
+  return (ry2 / wy + rz2 / wz) > gate;
+}
+
+// Exact search of S5: minimum d2 = ry^2 / wy + rz^2 / wz over the window, ties ->
+// smallest original id.  Out of line: the kernel's ranking loop calls it only when two candidates
+// are too close for its division-free ranking to separate.
+__device__ __noinline__ int search_exact(float p0, float p1, float z_ref, float wy, float wz, float win_y, float win_z,
+                                         const uint32_t* __restrict__ bp, int ny, int by0, int by1, int nsl,
+                                         const float2* __restrict__ yz, const int32_t* __restrict__ ord,
+                                         float& best_d2, float2& best_h, unsigned& n_cand) {
+  int best = -1;
+  best_d2 = 0.f;
+  for (int k = 0; k < nsl; ++k) {
+    const uint32_t e = __ldg(&bp[k * ny + by1 + 1]);
+    for (uint32_t c = __ldg(&bp[k * ny + by0]); c < e; ++c) {
+      const float2 h = __ldg(&yz[c]);
+      const float ry = h.x - p0;
+      const float rz = (h.y - z_ref) - p1;
+      if (!(fabsf(ry) <= win_y && fabsf(rz) <= win_z)) continue;
+      const float d2 = (ry * ry) / wy + (rz * rz) / wz;
+      ++n_cand;
+      if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
+        best = (int)c; best_d2 = d2; best_h = h;
+      }
+    }
+  }
+  return best;
+}
 
 // ---- K5a ---------------------------------------------------------------------------------------
 // One tracklet per thread.  The three phases (A follow links, B extrapolate up, C refit down) are
@@ -165,15 +220,15 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             const int32_t* __restrict__ start_hit, int32_t cap,
             int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
             int32_t* __restrict__ trk_i /*[kTrkI][cap]*/) {
-  __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_nyh[kMaxRows], t_ibz[kMaxRows], t_nzh[kMaxRows];
-  __shared__ int32_t t_ny[kMaxRows], t_base[kMaxRows];
+  __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];
+  __shared__ int32_t t_nyh[kMaxRows], t_nzh[kMaxRows], t_ny[kMaxRows], t_base[kMaxRows];
   __shared__ int s_start_off[kMaxSectors + 1];
   __shared__ int s_sec_off[kMaxSectors + 1];
   __shared__ float s_snap[kSnapF][kS5Threads];
   const int n_rows = P.n_rows, ns = P.n_sectors;
   for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
-    t_x[r] = T->row_x[r]; t_ylo[r] = T->y_lo[r]; t_iby[r] = T->inv_by[r]; t_nyh[r] = T->ny_hi[r];
-    t_ibz[r] = T->inv_bz[r]; t_nzh[r] = T->nz_hi[r]; t_ny[r] = T->ny[r]; t_base[r] = T->bin_base[r];
+    t_x[r] = T->row_x[r]; t_ylo[r] = T->y_lo[r]; t_iby[r] = T->inv_by[r]; t_nyh[r] = T->ny[r] - 1;
+    t_ibz[r] = T->inv_bz[r]; t_nzh[r] = T->nz[r] - 1; t_ny[r] = T->ny[r]; t_base[r] = T->bin_base[r];
   }
   for (int i = threadIdx.x; i <= ns; i += blockDim.x) { s_start_off[i] = st->start_off[i]; s_sec_off[i] = sec[i].off; }
   __syncthreads();
@@ -276,107 +331,147 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
         }
       }
     }
-    if (phase == PH_IDLE) continue;
-
-    // ---- one row step ---------------------------------------------------------------------------
+    // ---- one row step.  Every lane walks the same sequence of blocks (no early exits), with
+    // warp syncs in front of the heavy ones, so the warp executes propagate / search / update
+    // together whatever phases its lanes are in.  Phase changes are recorded in `ev` and applied
+    // once at the end of the step. ----------------------------------------------------------------
+    enum { EV_NONE = 0, EV_TO_C = 1, EV_FINISH = 2 };
+    const bool alive = phase != PH_IDLE;
+    int ev = EV_NONE;
     int32_t* hcol = hits + slot;
-    int cand = cur;                       // >= 0: cluster to use on this row; -1: none known
-    float2 h = make_float2(0.f, 0.f);
-    if (cand >= 0) h = __ldg(&yz[cand]);
+    int cand = -1;                        // >= 0: cluster to use on this row; -1: none known
     int nxt = -1;                         // candidate of the next row (loaded early)
-    if (phase == PH_A) nxt = __ldg(&lup[cand]);
-    else if (phase == PH_C && r - 1 >= r0) nxt = hcol[(size_t)(r - 1) * cap];
-    const float xr = t_x[r];
-    if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
-    w_prop += (xr != f.x) ? 1u : 0u;
-    if (!kf_propagate(f, xr, K)) {
-      if (phase == PH_C) finish(); else to_phase_c();
-      continue;
+    float2 h = make_float2(0.f, 0.f);
+    float xr = f.x;
+    if (alive) {
+      cand = cur;
+      if (cand >= 0) h = __ldg(&yz[cand]);
+      if (phase == PH_A) nxt = __ldg(&lup[cand]);
+      else if (phase == PH_C && r - 1 >= r0) nxt = hcol[(size_t)(r - 1) * cap];
+      xr = t_x[r];
+      if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
+      w_prop += (xr != f.x) ? 1u : 0u;
     }
-    bool took = false, is_new = false;
-    if (phase == PH_A) {
-      bool ok = true;
-      if (f.n >= 2) {
-        ++w_gate;
-        const float ry = h.x - f.p0, rz = (h.y - z_ref) - f.p1;
-        const float d2 = (ry * ry) / (f.c00 + K.err2_y) + (rz * rz) / (f.c11 + K.err2_z);
-        ok = !(d2 > P.gate);
+    __syncwarp();
+    bool go = false;                      // the lane carries on with this row
+    if (alive) {
+      go = kf_propagate(f, xr, K);
+      if (!go) ev = (phase == PH_C) ? EV_FINISH : EV_TO_C;
+    }
+    bool took = false, is_new = false, need_search = false;
+    const float wy = f.c00 + K.err2_y;
+    const float wz = f.c11 + K.err2_z;
+    const float iwy = rcp_fast(wy), iwz = rcp_fast(wz);   // ranking only, never a decision on its own
+    if (go) {
+      if (phase == PH_A) {
+        bool ok = true;
+        if (f.n >= 2) {
+          ++w_gate;
+          ok = !gate_exceeded(h.x - f.p0, (h.y - z_ref) - f.p1, wy, wz, iwy, iwz, P.gate);
+        }
+        if (ok) { took = true; is_new = true; }
+        else { phase = PH_B; gap = 0; cur = -1; go = false; }   // state already sits on row r (dx = 0 next)
+      } else if (cand >= 0) {
+        took = true;                      // phase C, row already holds a hit: no gate
+      } else {
+        need_search = (phase == PH_B) || (f.n >= 2);
       }
-      if (!ok) { phase = PH_B; gap = 0; cur = -1; continue; }   // state already sits on row r (dx = 0 next)
-      took = true; is_new = true;
-    } else if (cand >= 0) {
-      took = true;                        // phase C, row already holds a hit: no gate
-    } else if (phase == PH_B || f.n >= 2) {
+    }
+    __syncwarp();
+    if (need_search) {
       // search: best cluster of row r in the tc window around the prediction
       const float yc = f.p0;
       const float zc = z_ref + f.p1;
-      const float ylo = t_ylo[r], iby = t_iby[r], nyh = t_nyh[r], ibz = t_ibz[r], nzh = t_nzh[r];
-      const int by0 = bin_coord(yc - my, ylo, iby, nyh), by1 = bin_coord(yc + my, ylo, iby, nyh);
-      const int bz0 = bin_coord(zc - mz, P.grid_z_lo, ibz, nzh), bz1 = bin_coord(zc + mz, P.grid_z_lo, ibz, nzh);
-      const float wy = f.c00 + K.err2_y;
-      const float wz = f.c11 + K.err2_z;
+      const float ylo = t_ylo[r], iby = t_iby[r], ibz = t_ibz[r];
+      const int nyh = t_nyh[r], nzh = t_nzh[r];
+      const int by0 = bin_range(yc - my, ylo, iby, nyh), by1 = bin_range(yc + my, ylo, iby, nyh);
+      const int bz0 = bin_range(zc - mz, P.grid_z_lo, ibz, nzh), bz1 = bin_range(zc + mz, P.grid_z_lo, ibz, nzh);
       const int ny = t_ny[r];
       const uint32_t* bp = bs + t_base[r] + bz0 * ny;
-      int best = -1;
-      float best_d2 = 0.f;
-      float2 best_h = make_float2(0.f, 0.f);
-      ++w_search;
-      // bounds of the first three z slices are fetched together (a tc window spans <= 3 bins with
-      // the default tables); further slices, if any, are walked one by one
       const int nsl = bz1 - bz0 + 1;
-      uint32_t c = __ldg(&bp[by0]), e = __ldg(&bp[by1 + 1]);
+      ++w_search;
+      // The candidates of the (at most three) z slices are walked as ONE loop over a flat index,
+      // so the trip count of the warp is the largest candidate count of a lane, not the sum of the
+      // largest runs.  Ranking is done on d2~ = ry^2 * (1/wy)~ + rz^2 * (1/wz)~ (no division): d2~
+      // is within a few ulp of the defined d2, so the smallest d2~ is the smallest d2 unless the
+      // runner-up is within 2e-5 relative; then (ties, duplicates), and for windows of more than
+      // three slices, the exact loop decides.
+      uint32_t c0 = __ldg(&bp[by0]), e0 = __ldg(&bp[by1 + 1]);
       uint32_t c1 = 0, e1 = 0, c2 = 0, e2 = 0;
       if (nsl > 1) { c1 = __ldg(&bp[ny + by0]); e1 = __ldg(&bp[ny + by1 + 1]); }
       if (nsl > 2) { c2 = __ldg(&bp[2 * ny + by0]); e2 = __ldg(&bp[2 * ny + by1 + 1]); }
-      int k = 0;
-      for (;;) {
-        if (c >= e) {
-          ++k;
-          if (k >= nsl) break;
-          if (k == 1) { c = c1; e = e1; }
-          else if (k == 2) { c = c2; e = e2; }
-          else { c = __ldg(&bp[k * ny + by0]); e = __ldg(&bp[k * ny + by1 + 1]); }
-          continue;
+      const int n0 = (int)(e0 - c0), n01 = n0 + (int)(e1 - c1), total = nsl > 3 ? 0 : n01 + (int)(e2 - c2);
+      const uint32_t o1 = c1 - (uint32_t)n0, o2 = c2 - (uint32_t)n01;   // flat index i -> cluster o + i
+      float a1 = __int_as_float(0x7f800000), a2 = a1;
+      int best = -1;
+      // kS5Unroll candidate loads are issued together: the loop is bound by load latency
+      for (int i = 0; i < total; i += kS5Unroll) {
+        uint32_t cc[kS5Unroll];
+        float2 hh[kS5Unroll];
+#pragma unroll
+        for (int k = 0; k < kS5Unroll; ++k) {
+          const int j = min(i + k, total - 1);
+          cc[k] = (uint32_t)j + (j < n0 ? c0 : (j < n01 ? o1 : o2));
         }
-        const float2 hc = __ldg(&yz[c]);
-        const float ry = hc.x - f.p0;
-        const float rz = (hc.y - z_ref) - f.p1;
-        if (fabsf(ry) <= P.win_y && fabsf(rz) <= P.win_z) {
-          const float d2 = (ry * ry) / wy + (rz * rz) / wz;
-          ++w_cand;
-          if (best < 0 || d2 < best_d2 || (d2 == best_d2 && __ldg(&ord[c]) < __ldg(&ord[best]))) {
-            best = (int)c; best_d2 = d2; best_h = hc;
+#pragma unroll
+        for (int k = 0; k < kS5Unroll; ++k) hh[k] = __ldg(&yz[cc[k]]);
+#pragma unroll
+        for (int k = 0; k < kS5Unroll; ++k) {
+          const float ry = hh[k].x - f.p0;
+          const float rz = (hh[k].y - z_ref) - f.p1;
+          if (i + k < total && fabsf(ry) <= P.win_y && fabsf(rz) <= P.win_z) {
+            const float da = (ry * ry) * iwy + (rz * rz) * iwz;
+            ++w_cand;
+            if (da < a1) { a2 = a1; a1 = da; best = (int)cc[k]; }
+            else a2 = fminf(a2, da);
           }
         }
-        ++c;
       }
-      if (best >= 0 && best_d2 <= P.gate) { cand = best; h = best_h; took = true; is_new = true; }
+      if (best >= 0 || nsl > 3) {
+        bool pass;
+        if (nsl > 3 || !(a2 > a1 * 1.00002f + 1e-30f)) {
+          float best_d2;
+          unsigned n_cand = 0;
+          best = search_exact(f.p0, f.p1, z_ref, wy, wz, P.win_y, P.win_z, bp, ny, by0, by1, nsl, yz, ord, best_d2, h, n_cand);
+          if (nsl > 3) w_cand += n_cand;
+          pass = best >= 0 && best_d2 <= P.gate;
+        } else {
+          h = __ldg(&yz[best]);
+          pass = !gate_exceeded(h.x - f.p0, (h.y - z_ref) - f.p1, wy, wz, iwy, iwz, P.gate);
+        }
+        if (pass) { cand = best; took = true; is_new = true; }
+      }
     }
-    if (took) {
-      kf_update(f, h.x, h.y - z_ref, K);
-      ++w_upd;
-      if (is_new) { hcol[(size_t)r * cap] = cand; ++n_hits; }
-      if (phase == PH_C) {
-        fresh = true; saved = false;
-        if (is_new) { gap = 0; if (r < first) first = r; }
-      } else {
-        top = r; top_hit = cand; gap = 0;
-      }
-    } else {
-      if (phase == PH_B) {
+    __syncwarp();
+    if (go) {
+      if (took) {
+        kf_update(f, h.x, h.y - z_ref, K);
+        ++w_upd;
+        if (is_new) { hcol[(size_t)r * cap] = cand; ++n_hits; }
+        if (phase == PH_C) {
+          fresh = true; saved = false;
+          if (is_new) { gap = 0; if (r < first) first = r; }
+        } else {
+          top = r; top_hit = cand; gap = 0;
+        }
+      } else if (phase == PH_B) {
         hcol[(size_t)r * cap] = -1;
-        if (++gap > P.max_gap) { to_phase_c(); continue; }
+        if (++gap > P.max_gap) { ev = EV_TO_C; go = false; }
       } else if (r < r0) {                // phase C below the start hit
         hcol[(size_t)r * cap] = -1;
-        if (++gap > P.max_gap) { finish(); continue; }
+        if (++gap > P.max_gap) { ev = EV_FINISH; go = false; }
       }
     }
     // ---- advance to the next row -------------------------------------------------------------
-    if (phase == PH_A) { cur = nxt; ++r; if (cur == -1) { phase = PH_B; gap = 0; } }
-    else if (phase == PH_B) ++r;
-    else { cur = nxt; --r; }
-    if (phase == PH_B && r >= n_rows) to_phase_c();
-    if (phase == PH_C && r < 0) finish();
+    if (go) {
+      if (phase == PH_A) { cur = nxt; ++r; if (cur == -1) { phase = PH_B; gap = 0; } }
+      else if (phase == PH_B) ++r;
+      else { cur = nxt; --r; }
+      if (phase == PH_B && r >= n_rows) ev = EV_TO_C;
+      if (phase == PH_C && r < 0) ev = EV_FINISH;
+    }
+    if (ev == EV_TO_C) to_phase_c();
+    else if (ev == EV_FINISH) finish();
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};

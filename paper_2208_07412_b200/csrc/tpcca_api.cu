@@ -22,13 +22,13 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
   size_t tables, sec, status, tot;
   size_t in_y, in_z, in_row;
-  size_t syz, order, bin_start, row_start, multi_list, bin_tile_sum;
+  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, multi_list, bin_tile_sum;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
   size_t start_hit, hits, trk_f, trk_i;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t total;
-  int64_t n_bin_tiles, n_tiles_max, multi_cap;
+  int64_t n_bin_tiles, n_tiles_max, multi_cap, nf_tiles_max;
 };
 
 int64_t bins_per_sector(const tpcca_params* p) {
@@ -57,6 +57,9 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.order = take(4 * (size_t)N);
   L.bin_start = take(4 * (size_t)(ns * (nb + 1)));
   L.row_start = take(4 * (size_t)(ns * (nr + 1)));
+  L.nf_tiles_max = N / kNfTile + ns * nr + 1;
+  L.nf_tile_start = take(4 * (size_t)(ns * nr + 1));
+  L.nf_desc = take(sizeof(int2) * (size_t)L.nf_tiles_max);
   L.multi_list = take(4 * (size_t)L.multi_cap);
   L.bin_tile_sum = take(4 * (size_t)(L.n_bin_tiles + 1));
   L.up_raw = take(4 * (size_t)N);
@@ -117,6 +120,7 @@ int64_t default_cap(int64_t N, int64_t CS) {
 struct tpcca_ctx {
   int device = 0;
   int sm_count = 148;
+  int nf_blocks_per_sm = 4;
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   size_t ws_bytes = 0;
@@ -253,6 +257,18 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     t.hz_dn[r] = p->nf_hz_dn[r]; t.nf_cut[r] = p->nf_cut[r];
   }
   t.bin_base[p->n_rows] = base;
+  // S2 per-row constants; every float below is one fp32 operation on table values
+  for (int r = 1; r + 1 < p->n_rows; ++r) {
+    NfConst& k = t.nf[r];
+    const float m = p->grid_margin;
+    k.dA = make_float4(t.hy_dn[r], t.hz_dn[r], t.hy_dn[r] + m, t.hz_dn[r] + m);
+    k.dB = make_float4(t.y_lo[r - 1], t.inv_by[r - 1], t.inv_bz[r - 1], t.grid_z_lo);
+    k.dC = make_int4(t.ny[r - 1] - 1, t.nz[r - 1] - 1, t.ny[r - 1], t.bin_base[r - 1]);
+    k.uA = make_float4(t.hy_up[r], t.hz_up[r], t.hy_up[r] + m, t.hz_up[r] + m);
+    k.uB = make_float4(t.y_lo[r + 1], t.inv_by[r + 1], t.inv_bz[r + 1], t.grid_z_lo);
+    k.uC = make_int4(t.ny[r + 1] - 1, t.nz[r + 1] - 1, t.ny[r + 1], t.bin_base[r + 1]);
+    k.g = make_float4(t.row_x[r + 1] - t.row_x[r], t.row_x[r] - t.row_x[r - 1], t.nf_cut[r], 0.0f);
+  }
   cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
@@ -261,6 +277,11 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
     delete c;
     return TPCCA_E_CUDA;
+  }
+  {
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_neighbours, kNfThreads, 0) == cudaSuccess && occ > 0)
+      c->nf_blocks_per_sm = occ;
   }
   *out_ctx = c;
   return TPCCA_OK;
@@ -377,13 +398,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       k_grid_fixup<<<148 * 8, 256, 0, st>>>(T, sec, bin_start, multi, status, syz, order);
       c->launches += 2;
     }
-    k_row_start<<<c->ns, 256, 0, st>>>(T, bin_start, row_start);
-    ++c->launches;
+    k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start));
+    k_nf_tile_desc<<<std::min(c->ns * c->nr, 4096), 64, 0, st>>>(T, c->at<int32_t>(L.nf_tile_start), c->at<int2>(L.nf_desc));
+    c->launches += 2;
   }
   mark(1);
   if ((mask & TPCCA_STAGE_NEIGHBOURS) && c->n_tiles256 > 0) {
-    k_neighbours<<<c->n_tiles256, 256, 0, st>>>(T, sec, syz, bin_start, row_start, order, c->at<int32_t>(L.up_raw),
-                                               c->at<int32_t>(L.dn_raw));
+    const int64_t tiles_ub = c->n_total / kNfTile + (int64_t)c->ns * c->nr;
+    const int grid = (int)std::min<int64_t>(tiles_ub, (int64_t)c->sm_count * c->nf_blocks_per_sm);
+    k_neighbours<<<grid, kNfThreads, 0, st>>>(T, sec, syz, bin_start, row_start, order, c->at<int32_t>(L.nf_tile_start),
+                                              c->at<int2>(L.nf_desc), c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw));
     ++c->launches;
   }
   mark(2);

@@ -14,6 +14,18 @@ constexpr int kMaxSectors = TPCCA_MAX_SECTORS;
 // Per-row tables, copied verbatim from tpcca_params (DESIGN.md 3 "Derived tables").  Lives in
 // global memory; kernels read it through the read-only path (uniform per warp in S1-S4) or stage
 // the rows they need in shared memory (S5, where lanes sit on different rows).
+// S2 constants of one row r (1 <= r <= n_rows-2), 16-byte groups so that a thread fetches them
+// with seven 128-bit loads (block-uniform address).  d* = towards row r-1, u* = towards row r+1.
+struct NfConst {
+  float4 dA;   // hy_dn, hz_dn, hy_dn + margin, hz_dn + margin
+  float4 dB;   // y_lo[r-1], inv_by[r-1], inv_bz[r-1], grid_z_lo
+  int4 dC;     // ny[r-1] - 1, nz[r-1] - 1, ny[r-1], bin_base[r-1]
+  float4 uA;   // hy_up, hz_up, hy_up + margin, hz_up + margin
+  float4 uB;   // y_lo[r+1], inv_by[r+1], inv_bz[r+1], grid_z_lo
+  int4 uC;     // ny[r+1] - 1, nz[r+1] - 1, ny[r+1], bin_base[r+1]
+  float4 g;    // dxu = x[r+1] - x[r], dxd = x[r] - x[r-1], nf_cut[r], 0
+};
+
 struct DevTables {
   int32_t n_rows, n_sectors;
   int32_t bins_per_sector;              // nb = sum_r ny_r * nz_r
@@ -28,6 +40,7 @@ struct DevTables {
   int32_t ny[kMaxRows], nz[kMaxRows];
   int32_t bin_base[kMaxRows + 1];       // first bin of row r inside a sector
   float hy_up[kMaxRows], hz_up[kMaxRows], hy_dn[kMaxRows], hz_dn[kMaxRows], nf_cut[kMaxRows];
+  NfConst nf[kMaxRows];                 // S2 per-row constants (host-filled in tpcca_create)
 };
 
 // One sector's input arrays (device pointers; copies in the workspace or borrowed) and its place
@@ -65,6 +78,13 @@ __device__ __forceinline__ int bin_coord(float v, float lo, float inv, float hi)
   f = f < 0.0f ? 0.0f : f;
   f = f > hi ? hi : f;
   return (int)f;
+}
+
+// Same value as bin_coord for every input (floor + convert in one instruction, integer clamps);
+// used where the bin is only a search range (S2, S5), never for the S1 key itself.
+__device__ __forceinline__ int bin_range(float v, float lo, float inv, int hi) {
+  const int b = __float2int_rd(__fmul_rn(__fsub_rn(v, lo), inv));
+  return min(max(b, 0), hi);
 }
 
 // ---- block-wide exclusive scan over one int per thread (blockDim multiple of 32, <= 1024) ----
