@@ -137,7 +137,7 @@ constexpr int kTrkI = 4;    // n_hits (0 = rejected), n_fit, first_row, last_row
 
 constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 #ifndef TPCCA_S5_BPS
-#define TPCCA_S5_BPS 6
+#define TPCCA_S5_BPS 5
 #endif
 constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
 #ifndef TPCCA_S5_REFILL
@@ -239,7 +239,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   K.c24 = (float)(1.0 / 24.0); K.c640 = (float)(3.0 / 640.0); K.c12 = (float)(1.0 / 12.0);
   K.ic0 = P.ic0; K.ic1 = P.ic1; K.ic2 = P.ic2; K.ic3 = P.ic3; K.ic4 = P.ic4;
   const float my = P.win_y + P.margin, mz = P.win_z + P.margin;
-  const size_t nbp1 = (size_t)P.bins_per_sector + 1;
+  const uint32_t nbp1 = (uint32_t)P.bins_per_sector + 1u;
   const int lane = threadIdx.x & 31;
   const int tid = threadIdx.x;
   unsigned w_prop = 0, w_upd = 0, w_gate = 0, w_search = 0, w_cand = 0;   // work counters
@@ -252,10 +252,8 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   bool fresh = false;        // running state == snapshot (last operation was a phase-C update)
   bool saved = false;        // snapshot parked in shared memory
   float z_ref = 0.f;
-  const float2* yz = syz;
-  const int32_t* lup = link_up;
-  const int32_t* ord = order;
-  const uint32_t* bs = bin_start;
+  int off = 0;               // first sorted position of the lane's sector in the concatenated arrays
+  uint32_t bs_off = 0;       // first bin_start entry of the lane's sector (fits 32 bits: tpcca_create checks)
   KF f;
   f.x = 0.f; f.p0 = f.p1 = f.p2 = f.p3 = f.p4 = 0.f;
   kf_reset_cov(f, K);
@@ -310,14 +308,13 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (s_start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
             s = lo;
           }
-          const int off = s_sec_off[s];
-          yz = syz + off; ord = order + off; lup = link_up + off;
-          bs = bin_start + (size_t)s * nbp1;
+          off = s_sec_off[s];
+          bs_off = (uint32_t)s * nbp1;
           const int32_t* rs = row_start + s * (n_rows + 1);
           const int c0 = start_hit[slot];
           r0 = row_search(rs, n_rows, c0);
-          const int c1 = lup[c0];
-          const float2 h0 = yz[c0], h1 = yz[c1];
+          const int c1 = __ldg(&link_up[off + c0]);
+          const float2 h0 = __ldg(&syz[off + c0]), h1 = __ldg(&syz[off + c1]);
           z_ref = h0.y;
           const float dx = t_x[r0 + 1] - t_x[r0];
           const float dy = h1.x - h0.x;
@@ -345,8 +342,8 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     float xr = f.x;
     if (alive) {
       cand = cur;
-      if (cand >= 0) h = __ldg(&yz[cand]);
-      if (phase == PH_A) nxt = __ldg(&lup[cand]);
+      if (cand >= 0) h = __ldg(&syz[off + cand]);
+      if (phase == PH_A) nxt = __ldg(&link_up[off + cand]);
       else if (phase == PH_C && r - 1 >= r0) nxt = hcol[(size_t)(r - 1) * cap];
       xr = t_x[r];
       if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
@@ -387,7 +384,8 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       const int by0 = bin_range(yc - my, ylo, iby, nyh), by1 = bin_range(yc + my, ylo, iby, nyh);
       const int bz0 = bin_range(zc - mz, P.grid_z_lo, ibz, nzh), bz1 = bin_range(zc + mz, P.grid_z_lo, ibz, nzh);
       const int ny = t_ny[r];
-      const uint32_t* bp = bs + t_base[r] + bz0 * ny;
+      const uint32_t* bp = bin_start + (bs_off + (uint32_t)(t_base[r] + bz0 * ny));
+      const float2* yz = syz + off;
       const int nsl = bz1 - bz0 + 1;
       ++w_search;
       // The candidates of the (at most three) z slices are walked as ONE loop over a flat index,
@@ -432,7 +430,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
         if (nsl > 3 || !(a2 > a1 * 1.00002f + 1e-30f)) {
           float best_d2;
           unsigned n_cand = 0;
-          best = search_exact(f.p0, f.p1, z_ref, wy, wz, P.win_y, P.win_z, bp, ny, by0, by1, nsl, yz, ord, best_d2, h, n_cand);
+          best = search_exact(f.p0, f.p1, z_ref, wy, wz, P.win_y, P.win_z, bp, ny, by0, by1, nsl, yz, order + off, best_d2, h, n_cand);
           if (nsl > 3) w_cand += n_cand;
           pass = best >= 0 && best_d2 <= P.gate;
         } else {
