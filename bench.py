@@ -98,11 +98,36 @@ class ClockSampler:
         return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
 
 
+def rank_seed(config, seed, rank):
+    """Seed of the time frame rank `rank` tracks: the config's default seed on rank 0 (so the N = 1 workload is
+    exactly BASELINE.json's), a distinct one on every other rank (replicas process DIFFERENT time frames)."""
+    import tpcsynth
+    base = seed if seed is not None else tpcsynth.generator.BASE_SEED + config
+    return base + 1000 * rank
+
+
+def reduce_over_ranks(v, op, world, dev):
+    """max / sum of a host scalar over the ranks (identity for world == 1); NCCL on GPU, gloo in the CPU tests."""
+    if world == 1:
+        return v
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([v], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def whole_job_value(n_local, steps, ms_local, world, dev):
+    """Whole-job throughput: units all ranks processed / the slowest rank's device time."""
+    ms = reduce_over_ranks(ms_local, "max", world, dev)
+    n_all = reduce_over_ranks(float(n_local), "sum", world, dev)
+    return n_all * steps / (ms * 1e-3), ms, n_all
+
+
 def make_timeframe(args, rank):
     import tpcsynth
     t0 = time.time()
-    seed = None if rank == 0 and args.seed is None else (args.seed or (tpcsynth.generator.BASE_SEED + args.config)) + 1000 * rank
-    tf = tpcsynth.generate(args.config, seed=seed, mult_scale=args.mult_scale)
+    tf = tpcsynth.generate(args.config, seed=rank_seed(args.config, args.seed, rank), mult_scale=args.mult_scale)
     return tf, time.time() - t0
 
 
@@ -173,18 +198,10 @@ def run_tpcca(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(v, "max", world, dev)
 
     def sum_over_ranks(v):
-        if world == 1:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(v, "sum", world, dev)
 
     peaks = load_peaks()
     tf, gen_s = make_timeframe(args, rank)
@@ -223,11 +240,9 @@ def run_tpcca(args):
     torch.cuda.synchronize()
     t_wall1 = time.time()
     barrier()
-    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    value, ms_total, n_all = whole_job_value(N, args.steps, ev0.elapsed_time(ev1), world, dev)
     clocks = sampler.stop(t_wall0, t_wall1)
     trk.sync()
-    n_all = sum_over_ranks(float(N))
-    value = n_all * args.steps / (ms_total * 1e-3)
 
     # per-stage device times of the timed steps (events recorded inside tpcca_run on the same stream)
     k = min(args.steps, 16)
