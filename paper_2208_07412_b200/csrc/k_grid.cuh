@@ -209,14 +209,4 @@ k_row_tables(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_s
   if (threadIdx.x == 0) nf_tile_start[n] = carry;
 }
 
-// ---- K1h: tile descriptors of S2: desc[t] = (s * n_rows + r, chunk inside the row) -------------
-__global__ void __launch_bounds__(64)
-k_nf_tile_desc(const DevTables* __restrict__ T, const int32_t* __restrict__ nf_tile_start, int2* __restrict__ desc) {
-  const int n = T->n_sectors * T->n_rows;
-  for (int i = blockIdx.x; i < n; i += gridDim.x) {
-    const int t0 = nf_tile_start[i], t1 = nf_tile_start[i + 1];
-    for (int t = t0 + threadIdx.x; t < t1; t += blockDim.x) desc[t] = make_int2(i, t - t0);
-  }
-}
-
 }  // namespace tpcca

@@ -53,13 +53,13 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.in_y = take(4 * n_in);
   L.in_z = take(4 * n_in);
   L.in_row = take(2 * n_in);
-  L.syz = take(8 * (size_t)N);
+  L.syz = take(8 * (size_t)N + 64);                       // + pad: S2 stages 16-byte aligned runs
   L.order = take(4 * (size_t)N);
-  L.bin_start = take(4 * (size_t)(ns * (nb + 1)));
+  L.bin_start = take(4 * (size_t)(ns * (nb + 1)) + 64);   // + pad (same reason)
   L.row_start = take(4 * (size_t)(ns * (nr + 1)));
   L.nf_tiles_max = N / kNfTile + ns * nr + 1;
   L.nf_tile_start = take(4 * (size_t)(ns * nr + 1));
-  L.nf_desc = take(sizeof(int2) * (size_t)L.nf_tiles_max);
+  L.nf_desc = take(sizeof(NfTileDesc) * (size_t)L.nf_tiles_max);
   L.multi_list = take(4 * (size_t)L.multi_cap);
   L.bin_tile_sum = take(4 * (size_t)(L.n_bin_tiles + 1));
   L.up_raw = take(4 * (size_t)N);
@@ -120,7 +120,8 @@ int64_t default_cap(int64_t N, int64_t CS) {
 struct tpcca_ctx {
   int device = 0;
   int sm_count = 148;
-  int nf_blocks_per_sm = 4;
+  int nf_blocks_per_sm = 3;
+  NfTable nftab{};                    // S2 per-row constants, passed to k_neighbours by value (constant bank)
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   size_t ws_bytes = 0;
@@ -269,6 +270,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     k.uC = make_int4(t.ny[r + 1] - 1, t.nz[r + 1] - 1, t.ny[r + 1], t.bin_base[r + 1]);
     k.g = make_float4(t.row_x[r + 1] - t.row_x[r], t.row_x[r] - t.row_x[r - 1], t.nf_cut[r], 0.0f);
   }
+  for (int r = 0; r < kMaxRows; ++r) c->nftab.row[r] = t.nf[r];
   cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
@@ -280,7 +282,13 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   }
   {
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_neighbours, kNfThreads, 0) == cudaSuccess && occ > 0)
+    cudaError_t e2 = cudaFuncSetAttribute(k_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NfSmem));
+    if (e2 != cudaSuccess) {
+      set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: shared memory opt-in of k_neighbours failed: %s", cudaGetErrorString(e2));
+      delete c;
+      return TPCCA_E_CUDA;
+    }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_neighbours, kNfThreads, sizeof(NfSmem)) == cudaSuccess && occ > 0)
       c->nf_blocks_per_sm = occ;
   }
   *out_ctx = c;
@@ -399,16 +407,19 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       c->launches += 2;
     }
     k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start));
-    k_nf_tile_desc<<<std::min(c->ns * c->nr, 4096), 64, 0, st>>>(T, c->at<int32_t>(L.nf_tile_start), c->at<int2>(L.nf_desc));
-    c->launches += 2;
+    c->launches += 1;
   }
   mark(1);
   if ((mask & TPCCA_STAGE_NEIGHBOURS) && c->n_tiles256 > 0) {
     const int64_t tiles_ub = c->n_total / kNfTile + (int64_t)c->ns * c->nr;
     const int grid = (int)std::min<int64_t>(tiles_ub, (int64_t)c->sm_count * c->nf_blocks_per_sm);
-    k_neighbours<<<grid, kNfThreads, 0, st>>>(T, sec, syz, bin_start, row_start, order, c->at<int32_t>(L.nf_tile_start),
-                                              c->at<int2>(L.nf_desc), c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw));
-    ++c->launches;
+    NfTileDesc* nfd = c->at<NfTileDesc>(L.nf_desc);
+    const int32_t* nf_ts = c->at<int32_t>(L.nf_tile_start);
+    k_nf_plan<<<std::min(c->ns * c->nr, 148 * 64), 128, 0, st>>>(T, sec, syz, bin_start, row_start, nf_ts, nfd);
+    k_neighbours<<<grid, kNfThreads, sizeof(NfSmem), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
+                                                          nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
+                                                          c->at<int32_t>(L.dn_raw));
+    c->launches += 2;
   }
   mark(2);
   if ((mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
@@ -600,6 +611,15 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   CU(c, cudaStreamSynchronize(c->stream));
   return TPCCA_OK;
 }
+
+#ifdef TPCCA_NF_STATS
+int tpcca_debug_nf_hist(unsigned long long* out, int reset) {
+  cudaDeviceSynchronize();
+  if (out) cudaMemcpyFromSymbol(out, g_nf_hist, sizeof(unsigned long long) * 256);
+  if (reset) { static unsigned long long z[256]; cudaMemcpyToSymbol(g_nf_hist, z, sizeof z); }
+  return 0;
+}
+#endif
 
 void tpcca_destroy(tpcca_ctx* c) {
   if (!c) return;
