@@ -21,23 +21,22 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 // cluster runs and the two bin_start runs of the next tile in shared memory with 1-D bulk async
 // copies (TMA, mbarrier completion) while the current tile is searched entirely in shared memory.
 #ifndef TPCCA_NF_K
-#define TPCCA_NF_K 8
+#define TPCCA_NF_K 7
 #endif
-#ifndef TPCCA_NF_CAPC
-#define TPCCA_NF_CAPC 512
-#endif
-#ifndef TPCCA_NF_CAPB
-#define TPCCA_NF_CAPB 2048
+#ifndef TPCCA_NF_ARENA
+#define TPCCA_NF_ARENA 13056
 #endif
 constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory
 constexpr int kNfThreads = kNfTile;       // one thread per cluster of the tile
-constexpr int kNfCapC = TPCCA_NF_CAPC;    // staged clusters per side (8 B each)
-constexpr int kNfCapB = TPCCA_NF_CAPB;    // staged bin_start entries per side (4 B each)
+constexpr int kNfArena = TPCCA_NF_ARENA;  // bytes of one staging buffer: [up clusters | down clusters | up bins | down bins]
+constexpr int kNfMaxCn = 1022;            // staged clusters per side (staged indices are packed in 10 bits)
+constexpr int kNfMaxRun = 63;             // window candidates per side handled by the packed fast path
+constexpr int kNfMaxItems = kNfK * kNfThreads;   // up-side hits of a tile (pair work items)
 
 #ifdef TPCCA_NF_STATS
 __device__ unsigned long long g_nf_hist[4][64];   // tests per side, hits per side, pairs, pairs under cut
 #endif
-enum { NF_STAGED = 0, NF_NOLINK = 1, NF_GLOBAL = 2 };
+enum { NF_STAGED = 0, NF_NOLINK = 1, NF_GLOBAL = 2, NF_STAGED_C = 3 };   // STAGED_C: clusters staged, bins read from global memory
 
 struct NfSide {        // staging of one neighbour row for one tile
   int32_t c0;          // sector-local sorted position of staged cluster 0 ((sec_off + c0) is even; may be -1)
@@ -110,7 +109,7 @@ __device__ __forceinline__ void nf_plan_side(NfSide& o, int& flag, const DevTabl
   const int cn = (c_hi - c0 + 1) & ~1;
   o.c0 = c0; o.cn = cn; o.b0 = b0; o.bn = bn; o.s0 = s_lo;
   o.ds_shift = (s_hi - s_lo) | ((int)(gb_lo - b0) << 24);
-  if (cn > kNfCapC || bn > kNfCapB || (s_hi - s_lo) >= (1 << 24)) flag = NF_GLOBAL;
+  if (cn > kNfMaxCn || (s_hi - s_lo) >= (1 << 24)) flag = NF_GLOBAL;
 }
 
 __global__ void __launch_bounds__(128)
@@ -145,6 +144,8 @@ k_nf_plan(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, c
         const int b_last = bin_range(syz[d.p0 + d.n - 1].y, zlo, ibz, nz_r - 1);
         nf_plan_side(d.up, flag, T, r + 1, T->hz_up[r] + T->margin, b_first, b_last, nz_r, bin_r, bs_off, sec_off, bin_start);
         nf_plan_side(d.dn, flag, T, r - 1, T->hz_dn[r] + T->margin, b_first, b_last, nz_r, bin_r, bs_off, sec_off, bin_start);
+        if (flag == NF_STAGED && 8 * (d.up.cn + d.dn.cn) + 4 * (d.up.bn + d.dn.bn) > kNfArena)
+          flag = (8 * (d.up.cn + d.dn.cn) <= kNfArena) ? NF_STAGED_C : NF_GLOBAL;
       }
       d.rsf = r | (s << 8) | (flag << 16);
       desc[t] = d;
@@ -152,101 +153,8 @@ k_nf_plan(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, c
   }
 }
 
-// ---- candidate gathering ---------------------------------------------------------------------------
-// Window candidates of one side (A, B, C = the side's NfConst groups): every cluster q of the
-// neighbour row with |y_q - y_c| <= hy and |z_q - z_c| <= hz.  The bin range is a superset of the
-// window; the z slices of the range are walked as ONE flattened loop so that the
-// lanes of a warp, whose slices hold different numbers of clusters, stay together.
-// Caches (dy * dxo, dz * dxo) and the position of the first kNfK hits; returns the number of hits.
-// UP: the cached vector is (y_q - y_c) * dxo; down side: (y_c - y_q) * dxo (fl(a - b) = -fl(b - a),
-// so the negation is exact).
-struct NfCache {
-  float2 uv[kNfK][kNfThreads];
-  float2 dv[kNfK][kNfThreads];
-  int32_t ui[kNfK][kNfThreads];
-  int32_t di[kNfK][kNfThreads];
-};
-
-// global-memory version (tiles whose neighbour runs do not fit the staging buffers)
-template <bool UP>
-__device__ __forceinline__ int nf_gather(const float2 c, const float4 A, const float4 B, const int4 C, const float dxo,
-                                         const uint32_t* __restrict__ bs,
-                                         const float2* __restrict__ yz, float2 (*s_v)[kNfThreads],
-                                         int32_t (*s_i)[kNfThreads], const int tid) {
-  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
-  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
-  const uint32_t* bp = bs + C.w + bz0 * C.z;
-  const int nsl = bz1 - bz0 + 1;
-  uint32_t q = __ldg(&bp[by0]), e = __ldg(&bp[by1 + 1]);
-  uint32_t q1 = 0, e1 = 0;
-  if (nsl > 1) { q1 = __ldg(&bp[C.z + by0]); e1 = __ldg(&bp[C.z + by1 + 1]); }
-  int k = 0, n = 0;
-  for (;;) {
-    if (q >= e) {
-      if (++k >= nsl) break;
-      if (k == 1) { q = q1; e = e1; }
-      else { q = __ldg(&bp[k * C.z + by0]); e = __ldg(&bp[k * C.z + by1 + 1]); }
-      continue;
-    }
-    const float2 v = __ldg(&yz[q]);
-    const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
-    if (fabsf(dy) <= A.x && fabsf(dz) <= A.y) {
-      if (n < kNfK) {
-        s_v[n][tid] = make_float2(__fmul_rn(UP ? dy : -dy, dxo), __fmul_rn(UP ? dz : -dz, dxo));
-        s_i[n][tid] = (int32_t)q;
-      }
-      ++n;
-    }
-    ++q;
-  }
-  return n;
-}
-
-// shared-memory version: sC / sB are the staged cluster / bin_start runs of the side.  Returns the
-// number of hits, or -1 if the cluster's slices are not covered by the staged range (the caller then
-// takes the global-memory path for this cluster).
-template <bool UP>
-__device__ __forceinline__ int nf_gather_smem(const float2 c, const float4 A, const float4 B, const int4 C, const float dxo,
-                                              const NfSide& sd, const float2* __restrict__ sC,
-                                              const uint32_t* __restrict__ sB, float2 (*s_v)[kNfThreads],
-                                              int32_t (*s_i)[kNfThreads], const int tid) {
-  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
-  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
-  const int ds = sd.ds_shift & 0xffffff, shift = sd.ds_shift >> 24;
-  const int k0 = bz0 - sd.s0;
-  if (k0 < 0 || bz1 - sd.s0 > ds) return -1;
-  const uint32_t* bp = sB + shift + k0 * C.z;
-  int n = 0;
-  // two slices per pass (a window spans two slices, three when it straddles a bin edge by < margin)
-  for (int ks = bz1 - bz0; ks >= 0; ks -= 2, bp += 2 * C.z) {
-    const int q = (int)bp[by0] - sd.c0;
-    const int n0 = (int)bp[by1 + 1] - sd.c0 - q;
-    int total = n0, o1 = 0;
-    if (ks > 0) {
-      const int q1 = (int)bp[C.z + by0] - sd.c0;
-      total += (int)bp[C.z + by1 + 1] - sd.c0 - q1;
-      o1 = q1 - q - n0;                    // flat index j >= n0 -> staged index q + j + o1
-    }
-#ifdef TPCCA_NF_STATS
-    atomicAdd(&g_nf_hist[0][min(total, 63)], 1ull);
-#endif
-    for (int j = 0; j < total; ++j) {
-      const int idx = q + j + (j >= n0 ? o1 : 0);
-      const float2 v = sC[idx];
-      const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
-      if (fabsf(dy) <= A.x && fabsf(dz) <= A.y) {
-        if (n < kNfK) {
-          s_v[n][tid] = make_float2(__fmul_rn(UP ? dy : -dy, dxo), __fmul_rn(UP ? dz : -dz, dxo));
-          s_i[n][tid] = idx + sd.c0;
-        }
-        ++n;
-      }
-    }
-  }
-  return n;
-}
-
-// visit every window candidate of one side (plain nested loops; slow path only)
+// ---- exact slow path (global memory) ---------------------------------------------------------------
+// visit every window candidate of one side (A, B, C = the side's NfConst groups): plain nested loops
 template <class F>
 __device__ __forceinline__ void nf_for_each(const float2 c, const float4 A, const float4 B, const int4 C,
                                             const uint32_t* __restrict__ bs, const float2* __restrict__ yz, F fn) {
@@ -264,7 +172,9 @@ __device__ __forceinline__ void nf_for_each(const float2 c, const float4 A, cons
 }
 
 // Slow path of S2 (global memory, exact in every case: any number of candidates, ties by original
-// id): the full U x D product by nested rescans of both windows.
+// id): the full U x D product by nested rescans of both windows.  Taken by clusters whose windows
+// are not covered by the staged runs, hold more than kNfK hits or kNfMaxRun candidates on a side,
+// or whose best score is tied.
 __device__ __noinline__ void nf_slow(const float2 c, const NfConst& kc, const uint32_t* __restrict__ bs,
                                      const float2* __restrict__ yz, const int32_t* __restrict__ ord,
                                      float& best, int32_t& bu, int32_t& bd) {
@@ -289,49 +199,114 @@ __device__ __noinline__ void nf_slow(const float2 c, const NfConst& kc, const ui
   });
 }
 
-// best pair over the cached hits (nu, nd <= kNfK).  Returns false on an exact score tie (decided by
-// original ids in the slow path).
-__device__ __forceinline__ bool nf_best_pair(const NfCache& ch, int tid, int nu, int nd, float& best, int32_t& bu, int32_t& bd) {
-  const int np = nu * nd;
-  int iu = 0, id = 0, bi = 0, bj = 0;
-  bool tie = false;
-  best = __int_as_float(0x7f800000);
-  for (int k = 0; k < np; ++k) {
-    const float2 a = ch.uv[iu][tid], b = ch.dv[id][tid];
-    const float ay = __fsub_rn(a.x, b.x), az = __fsub_rn(a.y, b.y);
-    const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
-    tie |= (sc == best);
-    if (sc < best) { best = sc; bi = iu; bj = id; }
-    if (++id == nd) { id = 0; ++iu; }
-  }
-  bu = -1; bd = -1;
-  if (np > 0) { bu = ch.ui[bi][tid]; bd = ch.di[bj][tid]; }
-  return !tie;
+// ---- fast path, phase 0: the candidate runs of one side as a packed descriptor ----------------------
+// A window touches nsl = 2 (3 when it straddles a bin edge by less than the margin) z slices of the
+// neighbour row; in each slice its y range of bins is ONE run of sorted clusters.  The runs are
+// addressed by a flat candidate index j in [0, tot): staged index = q + j + (j >= n0 ? o1 : 0) +
+// (j >= n01 ? o2 : 0).  w0 = q | n0 << 10 | o1 << 16 | n01 << 26,  w1 = o2 | tot << 10.
+// Returns false if the window is not covered by the staged slices, spans more than 3 slices or holds
+// more than kNfMaxRun candidates.
+__device__ __forceinline__ bool nf_runs(const float2 c, const float4 A, const float4 B, const int4 C, const NfSide& sd,
+                                        const uint32_t* __restrict__ sB, uint32_t& w0, uint32_t& w1, int& tot) {
+  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
+  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
+  const int ds = sd.ds_shift & 0xffffff, shift = sd.ds_shift >> 24;
+  const int k0 = bz0 - sd.s0, nsl = bz1 - bz0;          // nsl = slices - 1
+  w0 = 0; w1 = 0; tot = 0;
+  if (k0 < 0 || bz1 - sd.s0 > ds || nsl > 2) return false;
+  const uint32_t* bp = sB + shift + k0 * C.z + by0;
+  const int w = by1 + 1 - by0;
+  const int qa = (int)bp[0], ea = (int)bp[w];
+  int qb = ea, eb = ea, qc, ec;
+  if (nsl >= 1) { qb = (int)bp[C.z]; eb = (int)bp[C.z + w]; }
+  qc = eb; ec = eb;
+  if (nsl >= 2) { qc = (int)bp[2 * C.z]; ec = (int)bp[2 * C.z + w]; }
+  const int n0 = ea - qa, n01 = n0 + (eb - qb);
+  tot = n01 + (ec - qc);
+  if (tot > kNfMaxRun) return false;
+  w0 = (uint32_t)(qa - sd.c0) | (uint32_t)n0 << 10 | (uint32_t)(qb - ea) << 16 | (uint32_t)n01 << 26;
+  w1 = (uint32_t)(qc - eb) | (uint32_t)tot << 10;
+  return true;
 }
 
-struct NfStage {
-  float2 uc[kNfCapC];
-  float2 dc[kNfCapC];
-  uint32_t ub[kNfCapB];
-  uint32_t db[kNfCapB];
-};
+// ---- shared-memory accessors on 32-bit shared addresses (no 64-bit pointer arithmetic in the loops) --
+__device__ __forceinline__ float2 lds_f2(uint32_t a) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts_f2(uint32_t a, float x, float y) {
+  asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(x), "f"(y) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t a) {
+  uint16_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) {
+  asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
+}
+
+constexpr uint32_t kVecRow = 8u * kNfThreads;   // bytes between consecutive rows of the hit-vector cache
+constexpr uint32_t kIdxRow = 2u * kNfThreads;   // ... of the hit-index cache
+
+// ---- fast path, phase A: window test of the tot candidates of one side ------------------------------
+// sC = shared address of the side's staged cluster run, (hy, hz) the exact window, scale = +dxd (up
+// side) or -dxu (down side: (y_c - y_d) * dxu = -((y_d - y_c) * dxu), exact).  Hits go to the thread's
+// cache column: vector (dy * scale, dz * scale) at pv + k * kVecRow, staged index at pi + k * kIdxRow.
+// Returns the number of hits (may exceed kNfK; only the first kNfK are cached).
+__device__ __forceinline__ int nf_test_runs(const float2 c, uint32_t w0, uint32_t w1, uint32_t sC, float hy, float hz,
+                                            float scale, uint32_t pv, uint32_t pi) {
+  const int n0 = (w0 >> 10) & 63, n01 = w0 >> 26, tot = w1 >> 10;
+  const uint32_t o1 = 8u * ((w0 >> 16) & 1023u), o2 = 8u * (w1 & 1023u);
+  uint32_t a = sC + 8u * (w0 & 1023u);
+  const uint32_t pv_end = pv + kNfK * kVecRow;
+  int n = 0;
+#pragma unroll 1
+  for (int j = 0; j < tot; ++j, a += 8u) {
+    if (j == n0) a += o1;
+    if (j == n01) a += o2;
+    const float2 v = lds_f2(a);
+    const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
+    if (fabsf(dy) <= hy && fabsf(dz) <= hz) {
+      if (pv != pv_end) {
+        sts_f2(pv, __fmul_rn(dy, scale), __fmul_rn(dz, scale));
+        sts_u16(pi, (a - sC) >> 3);
+        pv += kVecRow; pi += kIdxRow;
+      }
+      ++n;
+    }
+  }
+  return n;
+}
+
 struct NfSmem {
-  NfStage st[2];
-  NfCache ch;
+  alignas(128) unsigned char arena[kNfArena];   // staging buffer (TMA destination): [up clusters | down clusters | up bins | down bins]
+  float2 vec[2 * kNfK][kNfThreads];      // cached hits: rows [0, K) down side, [K, 2K) up side; column = cluster of the tile
+  uint16_t hidx[2 * kNfK][kNfThreads];   // staged indices of the cached hits
+  uint16_t items[kNfMaxItems];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 11
+  int hist[2][16], cnt[2][16];           // items per nd (work key) / emission cursors, two consecutive tiles
   NfTileDesc desc[4];
-  uint64_t full[2];
+  uint64_t full;
 };
 
-// ---- K2b: neighbour finder, one thread per cluster --------------------------
+// ---- K2b: neighbour finder --------------------------------------------------
 // For cluster c of row r (1 <= r <= n_rows-2): over U x D (exact windows in rows r+1, r-1) the
 // pair minimising score = ay^2 + az^2, ay = (yu-yc)*dxd - (yc-yd)*dxu; ties -> smallest original
 // id of u, then of d; stored if score <= nf_cut[r].
-// Persistent blocks walk the tile list with a grid stride (so the tiles in flight are neighbours in
-// memory and the three-fold reuse of a row stays in L2).  Iteration i: thread 0 issues the bulk
-// copies of tile i+1 into stage (i+1)&1, warp 0 fetches the descriptor of tile i+3, every thread
-// prefetches its own cluster of tile i+1, then the block waits for stage i&1 and searches tile i in
-// shared memory.  Per-row constants come from the constant bank (NfTable is a kernel parameter).
-__global__ void __launch_bounds__(kNfThreads)
+// Persistent blocks walk the tile list with a grid stride (tiles in flight are neighbours in memory,
+// so the three-fold reuse of a row stays in L2).  Per tile:
+//   phase A  thread t = cluster t: bin ranges of both windows, candidate runs from the staged
+//            bin_start entries, window tests of both sides; hits cached in the thread's column.
+//   phase B  the nu x nd pair scores are NOT looped per cluster (nu * nd has a long tail: mean 3.7,
+//            1 % above 24): every up-side hit becomes a work item (cluster, hit row, nd), the items
+//            are counting-sorted by nd in shared memory, and thread i scores item i against the nd
+//            down-side hits of its cluster, so the lanes of a warp run the same trip count (<= kNfK).
+//   phase C  thread t = cluster t: minimum over its nu item results, cut, coalesced link stores.
+// The staged runs of tile i+1 are fetched by bulk async copies (issued by thread 0 right after the
+// barrier that ends phase A of tile i, the only phase that reads the staging buffer); per-row
+// constants come from the constant bank (NfTable is a by-value kernel parameter).
+__global__ void __launch_bounds__(kNfThreads, 4)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
              const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ order, uint32_t nbp1,
              const int32_t* __restrict__ n_tiles_ptr, const NfTileDesc* __restrict__ desc,
@@ -343,85 +318,156 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
   const int stride = gridDim.x;
   const int first = blockIdx.x;
   if (first >= n_tiles) return;
-  if (tid == 0) { mbar_init(&S.full[0], 1); mbar_init(&S.full[1], 1); fence_mbar_init(); }
-  // descriptors of the block's first three tiles
-  if (tid < 48) {
+  if (tid == 0) { mbar_init(&S.full, 1); fence_mbar_init(); }
+  if (tid < 64) (&S.hist[0][0])[tid] = 0;            // hist[2][16] and cnt[2][16] are contiguous
+  if (tid < 48) {      // descriptors of the block's first three tiles
     const int k = tid >> 4, t = first + k * stride;
     if (t < n_tiles) reinterpret_cast<int32_t*>(&S.desc[k])[tid & 15] = __ldg(reinterpret_cast<const int32_t*>(&desc[t]) + (tid & 15));
   }
   __syncthreads();
-  auto issue = [&](const NfTileDesc& d, int stage) {      // thread 0 only
+  auto issue = [&](const NfTileDesc& d) {      // thread 0 only
+    const int flag = d.rsf >> 16;
     uint32_t bytes = 0;
-    const bool staged = (d.rsf >> 16) == NF_STAGED;
-    if (staged) bytes = 8u * (uint32_t)(d.up.cn + d.dn.cn) + 4u * (uint32_t)(d.up.bn + d.dn.bn);
-    mbar_arrive_expect_tx(&S.full[stage], bytes);
-    if (staged) {
-      NfStage& st = S.st[stage];
-      if (d.up.cn) bulk_g2s(st.uc, syz + (d.sec_off + d.up.c0), 8u * d.up.cn, &S.full[stage]);
-      if (d.dn.cn) bulk_g2s(st.dc, syz + (d.sec_off + d.dn.c0), 8u * d.dn.cn, &S.full[stage]);
-      if (d.up.bn) bulk_g2s(st.ub, bin_start + d.up.b0, 4u * d.up.bn, &S.full[stage]);
-      if (d.dn.bn) bulk_g2s(st.db, bin_start + d.dn.b0, 4u * d.dn.bn, &S.full[stage]);
+    if (flag == NF_STAGED) bytes = 8u * (uint32_t)(d.up.cn + d.dn.cn) + 4u * (uint32_t)(d.up.bn + d.dn.bn);
+    else if (flag == NF_STAGED_C) bytes = 8u * (uint32_t)(d.up.cn + d.dn.cn);
+    mbar_arrive_expect_tx(&S.full, bytes);
+    if (bytes) {
+      unsigned char* a = S.arena;
+      if (d.up.cn) bulk_g2s(a, syz + (d.sec_off + d.up.c0), 8u * d.up.cn, &S.full);
+      if (d.dn.cn) bulk_g2s(a + 8 * d.up.cn, syz + (d.sec_off + d.dn.c0), 8u * d.dn.cn, &S.full);
+      if (flag == NF_STAGED) {
+        unsigned char* b = a + 8 * (d.up.cn + d.dn.cn);
+        if (d.up.bn) bulk_g2s(b, bin_start + d.up.b0, 4u * d.up.bn, &S.full);
+        if (d.dn.bn) bulk_g2s(b + 4 * d.up.bn, bin_start + d.dn.b0, 4u * d.dn.bn, &S.full);
+      }
     }
   };
-  if (tid == 0) issue(S.desc[0], 0);
+  if (tid == 0) issue(S.desc[0]);
   float2 c_next = make_float2(0.f, 0.f);
   if (tid < S.desc[0].n) c_next = __ldg(&syz[S.desc[0].p0 + tid]);
+  const uint32_t sArena = smem_u32(S.arena);
+  const uint32_t sVecD = smem_u32(&S.vec[0][0]), sVecU = smem_u32(&S.vec[kNfK][0]);
+  const uint32_t sIdxD = smem_u32(&S.hidx[0][0]), sIdxU = smem_u32(&S.hidx[kNfK][0]);
   int it = 0;
   for (int tile = first; tile < n_tiles; tile += stride, ++it) {
-    const int stage = it & 1;
     const NfTileDesc& d = S.desc[it & 3];
     const bool have_next = tile + stride < n_tiles;
-    // descriptor of tile it+3 -> registers of warp 0 (stored at the end of the iteration)
-    int32_t dword = 0;
+    int32_t dword = 0;                       // descriptor of tile it+3 (stored at the end of the iteration)
     const bool fetch3 = tid < 16 && (long long)tile + 3ll * stride < n_tiles;
     if (fetch3) dword = __ldg(reinterpret_cast<const int32_t*>(&desc[tile + 3 * stride]) + tid);
-    if (tid == 0 && have_next) issue(S.desc[(it + 1) & 3], stage ^ 1);
     const float2 c = c_next;
     if (have_next) {
       const NfTileDesc& dn = S.desc[(it + 1) & 3];
       if (tid < dn.n) c_next = __ldg(&syz[dn.p0 + tid]);
     }
-    const int r = d.rsf & 0xff, flag = d.rsf >> 16;
-    const bool active = tid < d.n;
-    // wait for the staged runs of this tile (phase parity of the stage's barrier = (it >> 1) & 1)
-    while (!mbar_try_wait(&S.full[stage], (uint32_t)((it >> 1) & 1))) {}
-    int32_t bu = -1, bd = -1;
-    if (active && flag != NF_NOLINK) {
-      const NfConst& kc = tab.row[r];
-      const float4 g = kc.g;
-      float best = 0.0f;
-      int nd, nu;
+    const int r = d.rsf & 0xff, flag = d.rsf >> 16, n = d.n;
+    const NfConst& kc = tab.row[r];
+    const float4 g = kc.g;
+    int* hist = S.hist[it & 1];
+    int* cnt = S.cnt[it & 1];
+    // wait for the staged runs of this tile (one barrier phase per tile)
+    while (!mbar_try_wait(&S.full, (uint32_t)(it & 1))) {}
+    // ---- phase A -------------------------------------------------------------------------------
+    int nu = 0, nd = 0;
+    bool slow = false;
+    if (tid < n && flag != NF_NOLINK) {
+      uint32_t wd0, wd1, wu0, wu1;
+      int td, tu;
+      bool ok;
       if (flag == NF_STAGED) {
-        const NfStage& st = S.st[stage];
-        nd = nf_gather_smem<false>(c, kc.dA, kc.dB, kc.dC, g.x, d.dn, st.dc, st.db, S.ch.dv, S.ch.di, tid);
-        nu = nf_gather_smem<true>(c, kc.uA, kc.uB, kc.uC, g.y, d.up, st.uc, st.ub, S.ch.uv, S.ch.ui, tid);
+        const uint32_t* sUB = reinterpret_cast<const uint32_t*>(S.arena + 8 * (d.up.cn + d.dn.cn));
+        ok = nf_runs(c, kc.dA, kc.dB, kc.dC, d.dn, sUB + d.up.bn, wd0, wd1, td);
+        ok = nf_runs(c, kc.uA, kc.uB, kc.uC, d.up, sUB, wu0, wu1, tu) && ok;
+      } else if (flag == NF_STAGED_C) {
+        ok = nf_runs(c, kc.dA, kc.dB, kc.dC, d.dn, bin_start + d.dn.b0, wd0, wd1, td);
+        ok = nf_runs(c, kc.uA, kc.uB, kc.uC, d.up, bin_start + d.up.b0, wu0, wu1, tu) && ok;
       } else {
-        const int s = (d.rsf >> 8) & 0xff;
-        const uint32_t* bs = bin_start + (size_t)s * nbp1;
-        const float2* yz = syz + d.sec_off;
-        nd = nf_gather<false>(c, kc.dA, kc.dB, kc.dC, g.x, bs, yz, S.ch.dv, S.ch.di, tid);
-        nu = nf_gather<true>(c, kc.uA, kc.uB, kc.uC, g.y, bs, yz, S.ch.uv, S.ch.ui, tid);
+        ok = false; wd0 = wd1 = wu0 = wu1 = 0;
       }
-#ifdef TPCCA_NF_STATS
-      atomicAdd(&g_nf_hist[1][min(max(nd, 0), 63)], 1ull);
-      atomicAdd(&g_nf_hist[1][min(max(nu, 0), 63)], 1ull);
-      atomicAdd(&g_nf_hist[2][min(max(nu * nd, 0), 63)], 1ull);
-#endif
-      bool done = false;
-      if (nd >= 0 && nu >= 0 && nd <= kNfK && nu <= kNfK) done = nf_best_pair(S.ch, tid, nu, nd, best, bu, bd);
-      if (!done) {
+      if (ok) {
+        nd = nf_test_runs(c, wd0, wd1, sArena + 8u * (uint32_t)d.up.cn, kc.dA.x, kc.dA.y, -g.x, sVecD + 8u * tid, sIdxD + 2u * tid);
+        nu = nf_test_runs(c, wu0, wu1, sArena, kc.uA.x, kc.uA.y, g.y, sVecU + 8u * tid, sIdxU + 2u * tid);
+      }
+      slow = !ok || nd > kNfK || nu > kNfK;
+      if (slow) { nu = 0; nd = 0; }
+      if (nu > 0 && nd > 0) atomicAdd(&hist[nd], nu);
+    }
+    __syncthreads();                                          // (1) phase A done: staging buffer free, histogram complete
+    if (tid == 0 && have_next) issue(S.desc[(it + 1) & 3]);
+    // ---- phase B1: emit one work item per up-side hit, counting-sorted by nd (descending) -------------
+    int n_items = 0;
+    {
+      int above = 0;                                          // items with a larger nd than this thread's
+#pragma unroll
+      for (int k = kNfK; k >= 1; --k) {
+        const int h = hist[k];
+        if (k > nd) above += h;
+        n_items += h;
+      }
+      if (nu > 0 && nd > 0) {
+        const int slot = above + atomicAdd(&cnt[nd], nu);
+        const uint32_t code = (uint32_t)tid | (uint32_t)nd << 11;
+#pragma unroll 1
+        for (int k = 0; k < nu; ++k) S.items[slot + k] = (uint16_t)(code | (uint32_t)k << 8);
+      }
+    }
+    __syncthreads();                                          // (2) work items complete
+    if (tid < 16) { S.hist[(it + 1) & 1][tid] = 0; S.cnt[(it + 1) & 1][tid] = 0; }   // rows of the next tile
+    // ---- phase B2: thread i scores item i: one up-side hit against the nd down-side hits ---------------
+#pragma unroll 1
+    for (int i = tid; i < n_items; i += kNfThreads) {
+      const uint32_t item = S.items[i];
+      const uint32_t col = 8u * (item & 255u);
+      const uint32_t pa = sVecU + ((item >> 8) & 7u) * kVecRow + col;
+      const int ndd = (int)(item >> 11);
+      const float2 a = lds_f2(pa);
+      uint32_t pb = sVecD + col;
+      float best = __int_as_float(0x7f800000);
+      int bid = 0, tie = 0;
+#pragma unroll 1
+      for (int k = 0; k < ndd; ++k, pb += kVecRow) {
+        const float2 b = lds_f2(pb);
+        const float ay = __fsub_rn(a.x, b.x), az = __fsub_rn(a.y, b.y);
+        const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
+        if (sc == best) tie = 256;
+        if (sc < best) { best = sc; bid = k; }
+      }
+      sts_f2(pa, best, __int_as_float(bid | tie));           // the hit's vector is consumed: reuse its slot
+    }
+    __syncthreads();                                          // (3) item results complete
+    // ---- phase C: minimum over the cluster's items, cut, stores -----------------------------------------
+    if (tid < n) {
+      int32_t bu = -1, bd = -1;
+      float best = 0.0f;
+      if (nu > 0 && nd > 0) {
+        best = __int_as_float(0x7f800000);
+        int bk = 0, bcode = 0, tie = 0;
+        uint32_t pr = sVecU + 8u * tid;
+#pragma unroll 1
+        for (int k = 0; k < nu; ++k, pr += kVecRow) {
+          const float2 res = lds_f2(pr);
+          const int code = __float_as_int(res.y);
+          if (res.x == best) tie = 256;
+          if (res.x < best) { best = res.x; bk = k; bcode = code; }
+          tie |= code & 256;
+        }
+        if (tie) slow = true;
+        else {
+          bu = (int32_t)lds_u16(sIdxU + (uint32_t)bk * kIdxRow + 2u * tid) + d.up.c0;
+          bd = (int32_t)lds_u16(sIdxD + (uint32_t)(bcode & 255) * kIdxRow + 2u * tid) + d.dn.c0;
+        }
+      }
+      if (slow) {
         const int s = (d.rsf >> 8) & 0xff;
         nf_slow(c, kc, bin_start + (size_t)s * nbp1, syz + d.sec_off, order + d.sec_off, best, bu, bd);
       }
       if (!(bu >= 0 && best <= g.z)) { bu = -1; bd = -1; }
-    }
-    if (active) {
       link_up[d.p0 + tid] = bu;
       link_dn[d.p0 + tid] = bd;
     }
-    __syncthreads();           // stage and descriptor slot are free again
     if (fetch3) reinterpret_cast<int32_t*>(&S.desc[(it + 3) & 3])[tid] = dword;
-    // (visible to every thread after the next iteration's __syncthreads; it is first read two iterations later)
+    // no barrier here: phase A of the next tile writes only the thread's own cache column, the other
+    // histogram row and (after its mbarrier wait) reads the staging buffer refilled after barrier (1).
   }
 }
 
