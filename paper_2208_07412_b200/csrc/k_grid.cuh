@@ -178,7 +178,10 @@ k_grid_fixup(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
 // ---- K1g: row_start[s][r] = bin_start[s][bin_base[r]], and the row-aligned tiling of S2 ---------
 // One block.  nf_tile_start[i], i = s * n_rows + r: first S2 tile of (sector s, row r); a tile is
 // kNfTile consecutive sorted clusters of ONE row; nf_tile_start[ns * n_rows] = total.
-constexpr int kNfTile = 256;
+#ifndef TPCCA_NF_TILE
+#define TPCCA_NF_TILE 128
+#endif
+constexpr int kNfTile = TPCCA_NF_TILE;
 
 __global__ void __launch_bounds__(1024)
 k_row_tables(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_start,

@@ -24,7 +24,7 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 #define TPCCA_NF_K 7
 #endif
 #ifndef TPCCA_NF_ARENA
-#define TPCCA_NF_ARENA 13056
+#define TPCCA_NF_ARENA 7168
 #endif
 constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory
 constexpr int kNfThreads = kNfTile;       // one thread per cluster of the tile
@@ -306,7 +306,10 @@ struct NfSmem {
 // The staged runs of tile i+1 are fetched by bulk async copies (issued by thread 0 right after the
 // barrier that ends phase A of tile i, the only phase that reads the staging buffer); per-row
 // constants come from the constant bank (NfTable is a by-value kernel parameter).
-__global__ void __launch_bounds__(kNfThreads, 4)
+#ifndef TPCCA_NF_BPS
+#define TPCCA_NF_BPS 8
+#endif
+__global__ void __launch_bounds__(kNfThreads, TPCCA_NF_BPS)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
              const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ order, uint32_t nbp1,
              const int32_t* __restrict__ n_tiles_ptr, const NfTileDesc* __restrict__ desc,
