@@ -5,7 +5,15 @@
 
 namespace tpcca {
 
-constexpr int kScanTile = 2048;     // bins per scan tile (256 threads x 8)
+// S1 is a two-level sort.  Level 1 partitions the clusters of a sector into coarse
+// buckets (row, z slab of kSlab slices) with a counting sort on L2-resident counters; level 2 sorts
+// every bucket by (bin, original id) in shared memory and writes the sorted clusters and the
+// bucket's bin_start entries with coalesced stores.  Nothing touches the 1.5 GB bin_start array
+// with atomics and no pass runs over it except the one that writes it.
+constexpr int kSlabShift = 6;
+constexpr int kSlab = 1 << kSlabShift;        // z slices per coarse bucket
+constexpr int kSortCapR = 1024;               // clusters of a bucket sorted in shared memory
+constexpr int kSortCapB = 2048;               // fine bins of a bucket (kSlab * ny) handled in shared memory
 
 // sector of a tile: largest s with first_tile(s) <= tile (sectors with no tiles are skipped
 // because their first tile equals the next sector's).
@@ -19,119 +27,47 @@ __device__ __forceinline__ int find_sector(int ns, int tile, F first_tile) {
   return lo;
 }
 
-__device__ __forceinline__ int cluster_key(const DevTables* __restrict__ T, int r, float y, float z) {
-  int by = bin_coord(y, __ldg(&T->y_lo[r]), __ldg(&T->inv_by[r]), __ldg(&T->ny_hi[r]));
-  int bz = bin_coord(z, __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
-  return __ldg(&T->bin_base[r]) + bz * __ldg(&T->ny[r]) + by;
-}
+struct GridRec { float y, z; int32_t id; int32_t pad; };   // level-1 record (16 bytes, one 128-bit store)
 
-// ---- K1a: histogram.  cnt = bin_start + 1 (the cursor trick of DESIGN.md 5.1): cnt[s][key]++.
-// The thread that makes a bin's count 2 records the bin in the multi-bin list.
+// ---- K1a: level-1 histogram: cb_cnt[s][cb(row, bz >> kSlabShift)]++ ---------------------------------
 __global__ void __launch_bounds__(256)
-k_grid_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-             uint32_t* __restrict__ bin_start, uint32_t* __restrict__ multi_list, uint32_t multi_cap,
-             DevStatus* __restrict__ st) {
+k_cb_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, uint32_t* __restrict__ cb_cnt,
+           DevStatus* __restrict__ st) {
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
   const SectorDesc sd = sec[s];
   const int i = (blockIdx.x - sd.tile256) * 256 + threadIdx.x;
-  bool is_multi = false;
-  uint32_t slot = 0;
-  if (i < sd.n) {
-    const int r = sd.row[i];
-    if (r >= __ldg(&T->n_rows)) {
-      st->err_range = 1;
-    } else {
-      const int key = cluster_key(T, r, sd.y[i], sd.z[i]);
-      slot = (uint32_t)s * (uint32_t)(__ldg(&T->bins_per_sector) + 1) + 1u + (uint32_t)key;
-      const uint32_t old = atomicAdd(&bin_start[slot], 1u);
-      is_multi = (old == 1u);
-    }
-  }
-  // warp-aggregated append to the multi-bin list
-  const unsigned m = __ballot_sync(0xffffffffu, is_multi);
-  if (m) {
-    const int lane = threadIdx.x & 31;
-    uint32_t base = 0;
-    if (lane == (__ffs(m) - 1)) base = atomicAdd(&st->n_multi, (uint32_t)__popc(m));
-    base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
-    if (is_multi) {
-      const uint32_t k = base + (uint32_t)__popc(m & ((1u << lane) - 1u));
-      if (k < multi_cap) multi_list[k] = slot;
-    }
-  }
+  if (i >= sd.n) return;
+  const int r = sd.row[i];
+  if (r >= __ldg(&T->n_rows)) { st->err_range = 1; return; }
+  const int bz = bin_coord(sd.z[i], __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
+  const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
+  atomicAdd(&cb_cnt[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
 }
 
-// ---- K1b: per-tile sums of the bin counts (tiles never cross a sector) ------------------------
-__global__ void __launch_bounds__(256)
-k_scan_tile_sums(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-                 const uint32_t* __restrict__ bin_start, uint32_t* __restrict__ tile_sum) {
-  __shared__ uint32_t ws[33];
-  const int ns = __ldg(&T->n_sectors);
-  const int nb = __ldg(&T->bins_per_sector);
-  const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].bin_tile); });
-  const int t = blockIdx.x - __ldg(&sec[s].bin_tile);
-  const uint32_t* a = bin_start + (size_t)s * (nb + 1) + 1;   // cnt[0..nb)
-  const int b0 = t * kScanTile + threadIdx.x * 8;
-  uint32_t v = 0;
-  if (b0 + 8 <= nb && ((((size_t)s * (nb + 1) + 1 + b0) & 3) == 0)) {
-    const uint4 q0 = *reinterpret_cast<const uint4*>(a + b0);
-    const uint4 q1 = *reinterpret_cast<const uint4*>(a + b0 + 4);
-    v = q0.x + q0.y + q0.z + q0.w + q1.x + q1.y + q1.z + q1.w;
-  } else {
-    for (int k = 0; k < 8; ++k) if (b0 + k < nb) v += a[b0 + k];
-  }
-  uint32_t total;
-  block_exclusive_scan<uint32_t>(v, ws, total);
-  if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
-}
-
-// ---- K1c: one block per sector scans that sector's tile sums (exclusive, in place) ------------
+// ---- K1b: one block per sector: cb_start = exclusive scan of cb_cnt (sector-local), cursors = copy ---
 __global__ void __launch_bounds__(1024)
-k_scan_sector_tiles(const SectorDesc* __restrict__ sec, uint32_t* __restrict__ tile_sum) {
+k_cb_scan(const DevTables* __restrict__ T, const uint32_t* __restrict__ cb_cnt, uint32_t* __restrict__ cb_start,
+          uint32_t* __restrict__ cb_cur) {
   __shared__ uint32_t ws[33];
-  const int s = blockIdx.x;
-  const int t0 = sec[s].bin_tile, t1 = sec[s + 1].bin_tile;
+  const int ncb = T->n_cb;
+  const size_t base = (size_t)blockIdx.x * (ncb + 1);
   uint32_t carry = 0;
-  for (int base = t0; base < t1; base += 1024) {
-    const int t = base + threadIdx.x;
-    const uint32_t v = t < t1 ? tile_sum[t] : 0u;
+  for (int b0 = 0; b0 < ncb; b0 += 1024) {
+    const int b = b0 + threadIdx.x;
+    const uint32_t v = b < ncb ? cb_cnt[base + b] : 0u;
     uint32_t total;
     const uint32_t ex = block_exclusive_scan<uint32_t>(v, ws, total);
-    if (t < t1) tile_sum[t] = carry + ex;
+    if (b < ncb) { cb_start[base + b] = carry + ex; cb_cur[base + b] = carry + ex; }
     carry += total;
   }
+  if (threadIdx.x == 0) cb_start[base + ncb] = carry;
 }
 
-// ---- K1d: apply: bin_start[s][1 + b] = exclusive prefix of the counts (sector-local) ----------
+// ---- K1c: level-1 scatter: record (y, z, id) to the bucket's next free slot (arrival order) ---------
 __global__ void __launch_bounds__(256)
-k_scan_apply(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-             uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ tile_sum) {
-  __shared__ uint32_t ws[33];
-  const int ns = __ldg(&T->n_sectors);
-  const int nb = __ldg(&T->bins_per_sector);
-  const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].bin_tile); });
-  const int t = blockIdx.x - __ldg(&sec[s].bin_tile);
-  uint32_t* a = bin_start + (size_t)s * (nb + 1) + 1;
-  const int b0 = t * kScanTile + threadIdx.x * 8;
-  uint32_t c[8];
-  uint32_t v = 0;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) { c[k] = (b0 + k < nb) ? a[b0 + k] : 0u; v += c[k]; }
-  uint32_t total;
-  uint32_t run = block_exclusive_scan<uint32_t>(v, ws, total) + tile_sum[blockIdx.x];
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    if (b0 + k < nb) a[b0 + k] = run;
-    run += c[k];
-  }
-}
-
-// ---- K1e: scatter.  pos = cursor[key]++ (arrival order inside a bin; K1f restores id order).
-// Afterwards bin_start[s][j] = first position of bin j for every j in [0, nb] (cursor trick).
-__global__ void __launch_bounds__(256)
-k_grid_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-               uint32_t* __restrict__ bin_start, float2* __restrict__ syz, int32_t* __restrict__ order) {
+k_cb_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, uint32_t* __restrict__ cb_cur,
+             GridRec* __restrict__ rec) {
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
   const SectorDesc sd = sec[s];
@@ -140,38 +76,172 @@ k_grid_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ s
   const int r = sd.row[i];
   if (r >= __ldg(&T->n_rows)) return;
   const float y = sd.y[i], z = sd.z[i];
-  const int key = cluster_key(T, r, y, z);
-  uint32_t* cur = bin_start + (size_t)s * (__ldg(&T->bins_per_sector) + 1) + 1;
-  const uint32_t pos = atomicAdd(&cur[key], 1u);
-  const size_t g = (size_t)sd.off + pos;
-  syz[g] = make_float2(y, z);
-  order[g] = i;
+  const int bz = bin_coord(z, __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
+  const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
+  const uint32_t pos = atomicAdd(&cb_cur[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
+  GridRec o; o.y = y; o.z = z; o.id = i; o.pad = 0;
+  *reinterpret_cast<float4*>(&rec[(size_t)sd.off + pos]) = *reinterpret_cast<const float4*>(&o);
 }
 
-// ---- K1f: bins with >= 2 clusters: insertion sort by original index (canonical order) --------
+// row and slab of a coarse bucket: largest r with cb_base[r] <= cb
+__device__ __forceinline__ void cb_row_slab(const DevTables* __restrict__ T, int cb, int& r, int& k) {
+  int lo = 0, hi = __ldg(&T->n_rows) - 1;
+  while (lo < hi) {
+    int mid = (lo + hi + 1) >> 1;
+    if (__ldg(&T->cb_base[mid]) <= cb) lo = mid; else hi = mid - 1;
+  }
+  r = lo; k = cb - __ldg(&T->cb_base[lo]);
+}
+
+// ---- K1d: level 2, one block per (sector, coarse bucket) ------------------------------------------
+// Counting sort of the bucket's clusters by fine bin in shared memory (arrival rank from the
+// shared-memory histogram), then the canonical in-bin order (ascending original id) by counting the
+// smaller ids of the same bin; writes syz / order (sorted positions) and the bucket's bin_start
+// entries.  Buckets that do not fit the shared-memory buffers go to the big-bucket list.
 __global__ void __launch_bounds__(256)
-k_grid_fixup(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-             const uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ multi_list,
-             const DevStatus* __restrict__ st, float2* __restrict__ syz, int32_t* __restrict__ order) {
-  const uint32_t n_multi = st->n_multi;
-  const uint32_t stride = (uint32_t)(__ldg(&T->bins_per_sector) + 1);
-  for (uint32_t k = blockIdx.x * blockDim.x + threadIdx.x; k < n_multi; k += gridDim.x * blockDim.x) {
-    const uint32_t slot = multi_list[k];         // = s*stride + 1 + key
-    const uint32_t s = slot / stride;
-    const size_t off = (size_t)sec[s].off;
-    const uint32_t lo = bin_start[slot - 1], hi = bin_start[slot];
-    for (uint32_t a = lo + 1; a < hi; ++a) {
-      const int32_t oa = order[off + a];
-      const float2 va = syz[off + a];
-      uint32_t b = a;
-      while (b > lo && order[off + b - 1] > oa) {
-        order[off + b] = order[off + b - 1];
-        syz[off + b] = syz[off + b - 1];
-        --b;
-      }
-      order[off + b] = oa;
-      syz[off + b] = va;
+k_grid_sort(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const uint32_t* __restrict__ cb_start,
+            const GridRec* __restrict__ rec, float2* __restrict__ syz, int32_t* __restrict__ order,
+            uint32_t* __restrict__ bin_start, uint32_t* __restrict__ big_list, DevStatus* __restrict__ st) {
+  __shared__ float s_y[kSortCapR], s_z[kSortCapR];
+  __shared__ int32_t s_id[kSortCapR];
+  __shared__ uint16_t s_lb[kSortCapR], s_rank[kSortCapR], s_perm[kSortCapR];
+  __shared__ uint32_t s_hist[kSortCapB + 8];
+  __shared__ uint32_t ws[33];
+  const int ncb = __ldg(&T->n_cb);
+  const int s = blockIdx.x / ncb, cb = blockIdx.x - s * ncb;
+  int r, k;
+  cb_row_slab(T, cb, r, k);
+  const int ny = __ldg(&T->ny[r]), nz = __ldg(&T->nz[r]);
+  const int nsl = min(kSlab, nz - k * kSlab);
+  const int nbins = nsl * ny;
+  const uint32_t* cs = cb_start + (size_t)s * (ncb + 1) + cb;
+  const uint32_t bstart = __ldg(&cs[0]);
+  const int nb_ = (int)(__ldg(&cs[1]) - bstart);
+  if (nb_ > kSortCapR || nbins > kSortCapB) {
+    if (threadIdx.x == 0) big_list[atomicAdd(&st->n_big, 1u)] = blockIdx.x;
+    return;
+  }
+  const int off = __ldg(&sec[s].off);
+  const size_t gb0 = (size_t)s * (__ldg(&T->bins_per_sector) + 1) + __ldg(&T->bin_base[r]) + (size_t)k * kSlab * ny;
+  for (int j = threadIdx.x; j < nbins; j += 256) s_hist[j] = 0;
+  __syncthreads();
+  const float ylo = __ldg(&T->y_lo[r]), iby = __ldg(&T->inv_by[r]), nyh = __ldg(&T->ny_hi[r]);
+  const float zlo = __ldg(&T->grid_z_lo), ibz = __ldg(&T->inv_bz[r]), nzh = __ldg(&T->nz_hi[r]);
+  for (int i = threadIdx.x; i < nb_; i += 256) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(&rec[(size_t)off + bstart + i]));
+    const int by = bin_coord(q.x, ylo, iby, nyh), bz = bin_coord(q.y, zlo, ibz, nzh);
+    const int lb = (bz - k * kSlab) * ny + by;
+    s_y[i] = q.x; s_z[i] = q.y; s_id[i] = __float_as_int(q.z);
+    s_lb[i] = (uint16_t)lb;
+    s_rank[i] = (uint16_t)atomicAdd(&s_hist[lb], 1u);
+  }
+  __syncthreads();
+  // exclusive scan of the bin counts (8 consecutive bins per thread), in place; s_hist[nbins] = nb_
+  {
+    const int b0 = threadIdx.x * 8;
+    uint32_t cnt[8], v = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { cnt[j] = (b0 + j < nbins) ? s_hist[b0 + j] : 0u; v += cnt[j]; }
+    uint32_t total;
+    uint32_t run = block_exclusive_scan<uint32_t>(v, ws, total);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { if (b0 + j < nbins) s_hist[b0 + j] = run; run += cnt[j]; }
+    if (threadIdx.x == 0) s_hist[nbins] = (uint32_t)nb_;
+  }
+  __syncthreads();
+  // bin_start of the bucket's bins; entry nbins (= first bin of the next bucket, or the sector's
+  // closing entry) is written with the same value by its own bucket as well
+  for (int j = threadIdx.x; j <= nbins; j += 256) bin_start[gb0 + j] = bstart + s_hist[j];
+  for (int i = threadIdx.x; i < nb_; i += 256) s_perm[s_hist[s_lb[i]] + s_rank[i]] = (uint16_t)i;
+  __syncthreads();
+  for (int i = threadIdx.x; i < nb_; i += 256) {
+    const int lb = s_lb[i];
+    const uint32_t lo = s_hist[lb], hi = s_hist[lb + 1];
+    uint32_t pos = lo;
+    if (hi - lo > 1) {
+      const int32_t id = s_id[i];
+      for (uint32_t q = lo; q < hi; ++q) pos += (s_id[s_perm[q]] < id) ? 1u : 0u;
     }
+    const size_t g = (size_t)off + bstart + pos;
+    syz[g] = make_float2(s_y[i], s_z[i]);
+    order[g] = s_id[i];
+  }
+}
+
+// ---- K1e: buckets too large for shared memory: one block per listed bucket, global memory -----------
+// counts in bin_start[gb0 + 1 + lb], exclusive scan in place (entry j + 1 = start of bin j), scatter
+// with the cursor trick (afterwards entry j + 1 = end of bin j = start of bin j + 1), then insertion
+// sort by original id inside every bin with more than one cluster.
+__global__ void __launch_bounds__(256)
+k_grid_big(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const uint32_t* __restrict__ cb_start,
+           const GridRec* __restrict__ rec, float2* __restrict__ syz, int32_t* __restrict__ order,
+           uint32_t* __restrict__ bin_start, const uint32_t* __restrict__ big_list, const DevStatus* __restrict__ st) {
+  __shared__ uint32_t ws[33];
+  __shared__ uint32_t s_carry;
+  const int ncb = __ldg(&T->n_cb);
+  const uint32_t n_big = st->n_big;
+  for (uint32_t bi = blockIdx.x; bi < n_big; bi += gridDim.x) {
+    const int bid = (int)big_list[bi];
+    const int s = bid / ncb, cb = bid - s * ncb;
+    int r, k;
+    cb_row_slab(T, cb, r, k);
+    const int ny = __ldg(&T->ny[r]), nz = __ldg(&T->nz[r]);
+    const int nsl = min(kSlab, nz - k * kSlab);
+    const int nbins = nsl * ny;
+    const uint32_t* cs = cb_start + (size_t)s * (ncb + 1) + cb;
+    const uint32_t bstart = cs[0];
+    const int nb_ = (int)(cs[1] - bstart);
+    const int off = sec[s].off;
+    uint32_t* bs = bin_start + (size_t)s * (__ldg(&T->bins_per_sector) + 1) + __ldg(&T->bin_base[r]) + (size_t)k * kSlab * ny;
+    const float ylo = __ldg(&T->y_lo[r]), iby = __ldg(&T->inv_by[r]), nyh = __ldg(&T->ny_hi[r]);
+    const float zlo = __ldg(&T->grid_z_lo), ibz = __ldg(&T->inv_bz[r]), nzh = __ldg(&T->nz_hi[r]);
+    auto local_bin = [&](float y, float z) {
+      return (bin_coord(z, zlo, ibz, nzh) - k * kSlab) * ny + bin_coord(y, ylo, iby, nyh);
+    };
+    for (int j = 1 + threadIdx.x; j <= nbins; j += 256) bs[j] = 0;    // entry 0 belongs to the previous bucket
+    __syncthreads();
+    for (int i = threadIdx.x; i < nb_; i += 256) {
+      const GridRec q = rec[(size_t)off + bstart + i];
+      atomicAdd(&bs[1 + local_bin(q.y, q.z)], 1u);
+    }
+    if (threadIdx.x == 0) s_carry = bstart;
+    __syncthreads();
+    for (int b0 = 0; b0 < nbins; b0 += 256) {      // bs[1 + j] = bstart + (clusters in bins < j)
+      const int j = b0 + threadIdx.x;
+      const uint32_t v = j < nbins ? bs[1 + j] : 0u;
+      uint32_t total;
+      const uint32_t ex = block_exclusive_scan<uint32_t>(v, ws, total);
+      const uint32_t carry = s_carry;
+      if (j < nbins) bs[1 + j] = carry + ex;
+      __syncthreads();
+      if (threadIdx.x == 0) s_carry = carry + total;
+      __syncthreads();
+    }
+    if (threadIdx.x == 0 && cb == 0) bs[0] = bstart;
+    __syncthreads();
+    for (int i = threadIdx.x; i < nb_; i += 256) {
+      const GridRec q = rec[(size_t)off + bstart + i];
+      const uint32_t pos = atomicAdd(&bs[1 + local_bin(q.y, q.z)], 1u);
+      syz[(size_t)off + pos] = make_float2(q.y, q.z);
+      order[(size_t)off + pos] = q.id;
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < nbins; j += 256) {
+      const uint32_t lo = j == 0 ? bstart : bs[j], hi = bs[j + 1];
+      for (uint32_t a = lo + 1; a < hi; ++a) {
+        const int32_t oa = order[off + a];
+        const float2 va = syz[off + a];
+        uint32_t b = a;
+        while (b > lo && order[off + b - 1] > oa) {
+          order[off + b] = order[off + b - 1];
+          syz[off + b] = syz[off + b - 1];
+          --b;
+        }
+        order[off + b] = oa;
+        syz[off + b] = va;
+      }
+    }
+    __syncthreads();
   }
 }
 

@@ -22,13 +22,13 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
   size_t tables, sec, status, tot;
   size_t in_y, in_z, in_row;
-  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, multi_list, bin_tile_sum;
+  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
   size_t start_hit, hits, trk_f, trk_i;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t total;
-  int64_t n_bin_tiles, n_tiles_max, multi_cap, nf_tiles_max;
+  int64_t n_tiles_max, nf_tiles_max, n_cb;
 };
 
 int64_t bins_per_sector(const tpcca_params* p) {
@@ -42,9 +42,9 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   size_t cur = 0;
   auto take = [&](size_t bytes) { size_t o = cur; cur = align_up(cur + bytes); return o; };
   const int64_t ns = p->n_sectors, nr = p->n_rows, nb = bins_per_sector(p);
-  L.n_bin_tiles = ns * ((nb + kScanTile - 1) / kScanTile);
   L.n_tiles_max = std::max<int64_t>(N / 2048 + ns + 1, CS / 1024 + 2);
-  L.multi_cap = N / 2 + 1;
+  L.n_cb = 0;
+  for (int r = 0; r < p->n_rows; ++r) L.n_cb += (p->grid_nz[r] + kSlab - 1) / kSlab;
   L.tables = take(sizeof(DevTables));
   L.sec = take(sizeof(SectorDesc) * (kMaxSectors + 1));
   L.status = take(sizeof(DevStatus));
@@ -60,8 +60,11 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.nf_tiles_max = N / kNfTile + ns * nr + 1;
   L.nf_tile_start = take(4 * (size_t)(ns * nr + 1));
   L.nf_desc = take(sizeof(NfTileDesc) * (size_t)L.nf_tiles_max);
-  L.multi_list = take(4 * (size_t)L.multi_cap);
-  L.bin_tile_sum = take(4 * (size_t)(L.n_bin_tiles + 1));
+  L.cb_cnt = take(4 * (size_t)(ns * (L.n_cb + 1)));
+  L.cb_start = take(4 * (size_t)(ns * (L.n_cb + 1)));
+  L.cb_cur = take(4 * (size_t)(ns * (L.n_cb + 1)));
+  L.big_list = take(4 * (size_t)(ns * L.n_cb));
+  L.rec = take(16 * (size_t)N);
   L.up_raw = take(4 * (size_t)N);
   L.dn_raw = take(4 * (size_t)N);
   L.up = take(4 * (size_t)N);
@@ -179,7 +182,6 @@ int fetch_status(tpcca_ctx* c) {
   if (c->status.err_capacity)
     return set_err(c, TPCCA_E_WORKSPACE, "start-hit capacity exceeded: %d start hits > max_start_hits %lld",
                    c->status.n_start, (long long)c->CS);
-  if (c->status.n_multi > (uint32_t)c->L.multi_cap) return set_err(c, TPCCA_E_WORKSPACE, "internal: multi-bin list overflow");
   return TPCCA_OK;
 }
 
@@ -258,6 +260,12 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     t.hz_dn[r] = p->nf_hz_dn[r]; t.nf_cut[r] = p->nf_cut[r];
   }
   t.bin_base[p->n_rows] = base;
+  {
+    int32_t cb = 0;
+    for (int r = 0; r < p->n_rows; ++r) { t.cb_base[r] = cb; cb += (p->grid_nz[r] + kSlab - 1) / kSlab; }
+    t.cb_base[p->n_rows] = cb;
+    t.n_cb = cb;
+  }
   // S2 per-row constants; every float below is one fp32 operation on table values
   for (int r = 1; r + 1 < p->n_rows; ++r) {
     NfConst& k = t.nf[r];
@@ -359,7 +367,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   if (!c->desc_valid) {
     c->desc.assign(kMaxSectors + 1, SectorDesc{});
     int64_t off = 0, t256 = 0, t2048 = 0, bt = 0;
-    const int64_t bin_tiles = (c->nb + kScanTile - 1) / kScanTile;
+    const int64_t bin_tiles = 0;
     for (int s = 0; s <= c->ns; ++s) {
       SectorDesc& d = c->desc[s];
       const int64_t n = s < c->ns ? c->sec[s].n : 0;
@@ -390,22 +398,25 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
 
   if (mask & TPCCA_STAGE_GRID) {
     CU(c, cudaMemsetAsync(status, 0, sizeof(DevStatus), st));
-    CU(c, cudaMemsetAsync(bin_start, 0, 4 * (size_t)c->ns * (size_t)(c->nb + 1), st));
-    uint32_t* multi = c->at<uint32_t>(L.multi_list);
-    uint32_t* tsum = c->at<uint32_t>(L.bin_tile_sum);
+    uint32_t* cb_cnt = c->at<uint32_t>(L.cb_cnt);
+    uint32_t* cb_start = c->at<uint32_t>(L.cb_start);
+    uint32_t* cb_cur = c->at<uint32_t>(L.cb_cur);
+    uint32_t* big = c->at<uint32_t>(L.big_list);
+    GridRec* rec = c->at<GridRec>(L.rec);
+    CU(c, cudaMemsetAsync(cb_cnt, 0, 4 * (size_t)c->ns * (size_t)(L.n_cb + 1), st));
     if (c->n_tiles256 > 0) {
-      k_grid_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, bin_start, multi, (uint32_t)L.multi_cap, status);
+      k_cb_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cnt, status);
       ++c->launches;
     }
-    k_scan_tile_sums<<<(unsigned)L.n_bin_tiles, 256, 0, st>>>(T, sec, bin_start, tsum);
-    k_scan_sector_tiles<<<c->ns, 1024, 0, st>>>(sec, tsum);
-    k_scan_apply<<<(unsigned)L.n_bin_tiles, 256, 0, st>>>(T, sec, bin_start, tsum);
-    c->launches += 3;
+    k_cb_scan<<<c->ns, 1024, 0, st>>>(T, cb_cnt, cb_start, cb_cur);
+    ++c->launches;
     if (c->n_tiles256 > 0) {
-      k_grid_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, bin_start, syz, order);
-      k_grid_fixup<<<148 * 8, 256, 0, st>>>(T, sec, bin_start, multi, status, syz, order);
-      c->launches += 2;
+      k_cb_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cur, rec);
+      ++c->launches;
     }
+    k_grid_sort<<<(unsigned)(c->ns * L.n_cb), 256, 0, st>>>(T, sec, cb_start, rec, syz, order, bin_start, big, status);
+    k_grid_big<<<c->sm_count * 4, 256, 0, st>>>(T, sec, cb_start, rec, syz, order, bin_start, big, status);
+    c->launches += 2;
     k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start));
     c->launches += 1;
   }

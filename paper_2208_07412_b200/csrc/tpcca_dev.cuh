@@ -39,6 +39,8 @@ struct DevTables {
   float ny_hi[kMaxRows], nz_hi[kMaxRows];   // (float)(ny-1), (float)(nz-1): exact for < 2^24 bins
   int32_t ny[kMaxRows], nz[kMaxRows];
   int32_t bin_base[kMaxRows + 1];       // first bin of row r inside a sector
+  int32_t cb_base[kMaxRows + 1];        // S1 level 1: first coarse bucket (row, z slab) of row r
+  int32_t n_cb;                         // coarse buckets per sector
   float hy_up[kMaxRows], hz_up[kMaxRows], hy_dn[kMaxRows], hz_dn[kMaxRows], nf_cut[kMaxRows];
   NfConst nf[kMaxRows];                 // S2 per-row constants (host-filled in tpcca_create)
 };
@@ -61,7 +63,7 @@ struct SectorDesc {
 struct DevStatus {
   int32_t err_range;       // some cluster had row >= n_rows
   int32_t err_capacity;    // n_start exceeded max_start_hits
-  uint32_t n_multi;        // bins holding >= 2 clusters (S1 fix-up list)
+  uint32_t n_big;          // S1 coarse buckets too large for the shared-memory sort
   int32_t n_start;         // total start hits
   int32_t work_counter;    // S5 dynamic work distribution
   int32_t pad[3];

@@ -165,6 +165,21 @@ def test_dense_random_windows(pkg, seed, n, zmax):
     check(pkg, ArrTF(P, [(y, z, row)]))
 
 
+def test_oversized_buckets_and_tiles(pkg):
+    """Thousands of clusters in a few rows and a short z range: S1 coarse buckets beyond the shared-memory
+    sort (global-memory bucket path), S2 tiles whose neighbour runs exceed the staging buffer (global path),
+    bins holding many clusters with shuffled ids."""
+    P = tpcsynth.default_params(n_sectors=2)
+    rng = np.random.default_rng(11)
+    n = 9000
+    row = rng.integers(4, 8, n).astype(np.uint16)
+    y = (rng.random(n) * 30.0 - 15.0).astype(np.float32)
+    z = (rng.random(n) * 120.0).astype(np.float32)
+    e = (np.empty(0, np.float32), np.empty(0, np.float32), np.empty(0, np.uint16))
+    check(pkg, ArrTF(P, [(y, z, row), e]))
+    check(pkg, ArrTF(P, [e, (y[:3000], z[:3000] * 0.02, row[:3000])]))
+
+
 def test_grid_variants(pkg):
     """P3 on the GPU: other bin sizes / margins (bin ranges spanning more than 3 bins)."""
     tf = tpcsynth.generate(1, n_tracks=600)
