@@ -567,4 +567,46 @@ k_start_hits(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
     }
 }
 
+// ---- K4c-e: processing order of S5 ---------------------------------------------------
+// Tracks are emitted in start-hit order, but the ORDER IN WHICH S5 works through the start hits is
+// free.  Walking them sector by sector in ascending z (time) instead of row-major keeps the clusters
+// and bin_start entries touched by the tracklets in flight inside a z window of the sector, i.e. in
+// L2.  The unit of the ordering is the S1 coarse bucket (row, z slab): its start hits are one
+// contiguous range of slots; zorder[j] = j-th bucket of a sector by ascending z (host table).
+__global__ void __launch_bounds__(256)
+k_sh_bucket_counts(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, const int32_t* __restrict__ zorder,
+                   const uint32_t* __restrict__ cb_start, const int32_t* __restrict__ start_hit, int32_t cap,
+                   int32_t* __restrict__ sh_first, int2* __restrict__ cnt) {
+  const int ncb = T->n_cb, ns = T->n_sectors;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ns * ncb) return;
+  const int s = i / ncb, j = i - s * ncb;
+  int a = 0, n = 0;
+  if (!st->err_capacity) {
+    const int cb = zorder[j];
+    const uint32_t lo_pos = cb_start[(size_t)s * (ncb + 1) + cb], hi_pos = cb_start[(size_t)s * (ncb + 1) + cb + 1];
+    const int s0 = st->start_off[s], s1 = st->start_off[s + 1];
+    auto lower = [&](uint32_t pos) {             // first slot in [s0, s1) whose start hit is >= pos
+      int lo = s0, hi = s1;
+      while (lo < hi) { const int mid = (lo + hi) >> 1; if ((uint32_t)start_hit[mid] < pos) lo = mid + 1; else hi = mid; }
+      return lo;
+    };
+    a = lower(lo_pos);
+    n = lower(hi_pos) - a;
+  }
+  sh_first[i] = a;
+  cnt[i] = make_int2(n, 0);
+}
+
+__global__ void __launch_bounds__(256)
+k_sh_perm(const DevTables* __restrict__ T, const int32_t* __restrict__ sh_first, const int2* __restrict__ cnt,
+          const longlong2* __restrict__ pre, int32_t* __restrict__ perm) {
+  const int n = T->n_sectors * T->n_cb;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int a = sh_first[i], c = cnt[i].x;
+  int32_t* o = perm + pre[i].x;
+  for (int k = 0; k < c; ++k) o[k] = a + k;
+}
+
 }  // namespace tpcca

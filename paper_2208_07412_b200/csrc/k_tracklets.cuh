@@ -217,7 +217,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             DevStatus* __restrict__ st, const S5Params P, const float2* __restrict__ syz,
             const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
             const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
-            const int32_t* __restrict__ start_hit, int32_t cap,
+            const int32_t* __restrict__ start_hit, const int32_t* __restrict__ perm, int32_t cap,
             int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
             int32_t* __restrict__ trk_i /*[kTrkI][cap]*/) {
   __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];
@@ -301,7 +301,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       if (phase == PH_IDLE) {
         const int my_slot = base + __popc(idle & ((1u << lane) - 1u));
         if (my_slot < n_start) {
-          slot = my_slot;
+          slot = __ldg(&perm[my_slot]);
           int s = 0;
           {
             int lo = 0, hi = ns - 1;

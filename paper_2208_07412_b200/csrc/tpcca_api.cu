@@ -5,6 +5,8 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <algorithm>
+#include <utility>
 #include <vector>
 
 #include "k_tracklets.cuh"
@@ -22,7 +24,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
   size_t tables, sec, status, tot;
   size_t in_y, in_z, in_row;
-  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec;
+  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
   size_t start_hit, hits, trk_f, trk_i;
@@ -48,7 +50,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.tables = take(sizeof(DevTables));
   L.sec = take(sizeof(SectorDesc) * (kMaxSectors + 1));
   L.status = take(sizeof(DevStatus));
-  L.tot = take(sizeof(int64_t) * 4);
+  L.tot = take(sizeof(int64_t) * 8);
   const size_t n_in = (size_t)N + 8 * kMaxSectors;   // every sector's copy starts 8-element aligned
   L.in_y = take(4 * n_in);
   L.in_z = take(4 * n_in);
@@ -65,6 +67,11 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.cb_cur = take(4 * (size_t)(ns * (L.n_cb + 1)));
   L.big_list = take(4 * (size_t)(ns * L.n_cb));
   L.rec = take(16 * (size_t)N);
+  L.zorder = take(4 * (size_t)L.n_cb);
+  L.sh_first = take(4 * (size_t)(ns * L.n_cb));
+  L.sh_cnt = take(sizeof(int2) * (size_t)(ns * L.n_cb));
+  L.sh_pre = take(sizeof(longlong2) * (size_t)(ns * L.n_cb));
+  L.perm = take(4 * (size_t)CS);
   L.up_raw = take(4 * (size_t)N);
   L.dn_raw = take(4 * (size_t)N);
   L.up = take(4 * (size_t)N);
@@ -279,6 +286,23 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     k.g = make_float4(t.row_x[r + 1] - t.row_x[r], t.row_x[r] - t.row_x[r - 1], t.nf_cut[r], 0.0f);
   }
   for (int r = 0; r < kMaxRows; ++r) c->nftab.row[r] = t.nf[r];
+  {
+    // S5 processing order: coarse buckets of a sector by ascending lower z edge, then row
+    std::vector<std::pair<std::pair<float, int>, int>> zo;
+    for (int r = 0; r < p->n_rows; ++r)
+      for (int k = 0; k < t.cb_base[r + 1] - t.cb_base[r]; ++k)
+        zo.push_back({{(float)(k * kSlab) / p->grid_inv_bin_z[r], r}, t.cb_base[r] + k});
+    std::sort(zo.begin(), zo.end());
+    std::vector<int32_t> zl(zo.size());
+    for (size_t i = 0; i < zo.size(); ++i) zl[i] = zo[i].second;
+    cudaError_t ez = cudaMemcpyAsync(c->at<int32_t>(L.zorder), zl.data(), 4 * zl.size(), cudaMemcpyHostToDevice, c->stream);
+    if (ez == cudaSuccess) ez = cudaStreamSynchronize(c->stream);
+    if (ez != cudaSuccess) {
+      set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(ez));
+      delete c;
+      return TPCCA_E_CUDA;
+    }
+  }
   cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
@@ -454,6 +478,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       k_start_hits<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_off, cap, start_hit);
       ++c->launches;
     }
+    {   // processing order of S5: start-hit slots by (sector, z)
+      const int nbk = (int)(c->ns * L.n_cb);
+      int2* shc = c->at<int2>(L.sh_cnt);
+      longlong2* shp = c->at<longlong2>(L.sh_pre);
+      k_sh_bucket_counts<<<(nbk + 255) / 256, 256, 0, st>>>(T, status, c->at<int32_t>(L.zorder), c->at<uint32_t>(L.cb_start), start_hit, cap,
+                                                           c->at<int32_t>(L.sh_first), shc);
+      k_scan_pairs<<<1, 1024, 0, st>>>(shc, shp, nbk, tot + 4);
+      k_sh_perm<<<(nbk + 255) / 256, 256, 0, st>>>(T, c->at<int32_t>(L.sh_first), shc, shp, c->at<int32_t>(L.perm));
+      c->launches += 3;
+    }
   }
   mark(4);
   if (mask & TPCCA_STAGE_TRACKLETS) {
@@ -476,7 +510,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     sp.n_rows = t.n_rows; sp.n_sectors = t.n_sectors; sp.max_gap = t.tc_max_gap; sp.min_hits = t.tc_min_hits;
     sp.bins_per_sector = t.bins_per_sector;
     k_tracklets<<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order,
-                                                                     c->at<int32_t>(L.up), start_hit, cap, hits, trk_f, trk_i);
+                                                                     c->at<int32_t>(L.up), start_hit, c->at<int32_t>(L.perm), cap, hits, trk_f, trk_i);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
