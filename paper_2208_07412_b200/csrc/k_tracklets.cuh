@@ -139,6 +139,10 @@ constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 #ifndef TPCCA_S5_BPS
 #define TPCCA_S5_BPS 5
 #endif
+#ifndef TPCCA_S5_BPS_A
+#define TPCCA_S5_BPS_A 8
+#endif
+constexpr int kS5BlocksPerSMA = TPCCA_S5_BPS_A;   // ... of the phase-A kernel (no search code: fewer registers)
 constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
 #ifndef TPCCA_S5_REFILL
 #define TPCCA_S5_REFILL 4
@@ -212,14 +216,27 @@ __device__ __noinline__ int search_exact(float p0, float p1, float z_ref, float 
 // The phase-C snapshot ("state right after the last update") lives in registers while it equals
 // the running state and is parked in shared memory the moment the running state moves on without
 // an update, which keeps the register count at one Kalman state per lane.
-__global__ void __launch_bounds__(kS5Threads, kS5BlocksPerSM)
+// The kernel is compiled in three modes and launched three times: MODE_A runs phase A
+// for every start hit, MODE_B phase B, MODE_C phase C.  A lane whose tracklet leaves the kernel's phase
+// parks the tracklet (Kalman state + bookkeeping, kHsF floats and kHsI ints, indexed by the work
+// index so that the lanes refilled together store and load neighbouring words) and takes new work.
+// Per lane the sequence of operations is exactly that of the single loop; what changes is which
+// lanes share a warp: link followers (no search), extrapolators (a search every row) and refitters
+// no longer wait for each other's code.
+enum { MODE_A = 1, MODE_B = 2, MODE_C = 3 };
+constexpr int kHsF = 23;    // x, p0..p4, c[15], chi2, z_ref
+constexpr int kHsI = 10;    // n, r, cur, top, top_hit, gap, n_hits, first, r0, phase
+
+template <int MODE>
+__global__ void __launch_bounds__(kS5Threads, MODE == MODE_A ? kS5BlocksPerSMA : kS5BlocksPerSM)
 k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             DevStatus* __restrict__ st, const S5Params P, const float2* __restrict__ syz,
             const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
             const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
             const int32_t* __restrict__ start_hit, const int32_t* __restrict__ perm, int32_t cap,
             int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
-            int32_t* __restrict__ trk_i /*[kTrkI][cap]*/) {
+            int32_t* __restrict__ trk_i /*[kTrkI][cap]*/, float* __restrict__ hs_f /*[kHsF][cap]*/,
+            int32_t* __restrict__ hs_i /*[kHsI][cap]*/) {
   __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];
   __shared__ int32_t t_nyh[kMaxRows], t_nzh[kMaxRows], t_ny[kMaxRows], t_base[kMaxRows];
   __shared__ int s_start_off[kMaxSectors + 1];
@@ -248,6 +265,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   // ---- per-lane tracklet state ---------------------------------------------------------------
   int phase = PH_IDLE;
   bool drained = false;      // warp-uniform: the work counter ran out
+  int wi = 0;                // work index of the lane's tracklet (parking slot)
   int slot = 0, r = 0, cur = -1, top = 0, top_hit = -1, gap = 0, n_hits = 0, first = 0, r0 = 0;
   bool fresh = false;        // running state == snapshot (last operation was a phase-C update)
   bool saved = false;        // snapshot parked in shared memory
@@ -288,6 +306,20 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; cur = top_hit; fresh = false; saved = false;
   };
 
+  // park the tracklet for the next kernel and go idle
+  auto park = [&]() {
+    const size_t cs = (size_t)cap;
+    float* o = hs_f + wi;
+    o[0 * cs] = f.x; o[1 * cs] = f.p0; o[2 * cs] = f.p1; o[3 * cs] = f.p2; o[4 * cs] = f.p3; o[5 * cs] = f.p4;
+    o[6 * cs] = f.c00; o[7 * cs] = f.c10; o[8 * cs] = f.c11; o[9 * cs] = f.c20; o[10 * cs] = f.c21; o[11 * cs] = f.c22;
+    o[12 * cs] = f.c30; o[13 * cs] = f.c31; o[14 * cs] = f.c32; o[15 * cs] = f.c33; o[16 * cs] = f.c40; o[17 * cs] = f.c41;
+    o[18 * cs] = f.c42; o[19 * cs] = f.c43; o[20 * cs] = f.c44; o[21 * cs] = f.chi2; o[22 * cs] = z_ref;
+    int32_t* q = hs_i + wi;
+    q[0 * cs] = f.n; q[1 * cs] = r; q[2 * cs] = cur; q[3 * cs] = top; q[4 * cs] = top_hit; q[5 * cs] = gap;
+    q[6 * cs] = n_hits; q[7 * cs] = first; q[8 * cs] = r0; q[9 * cs] = phase;
+    phase = PH_IDLE;
+  };
+
   for (;;) {
     // ---- refill idle lanes from the work counter ---------------------------------------------
     const unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
@@ -295,13 +327,14 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     if (!drained && (__popc(idle) >= kS5Refill || idle == 0xffffffffu)) {
       const int n_idle = __popc(idle);
       int base = 0;
-      if (lane == 0) base = atomicAdd(&st->work_counter, n_idle);
+      if (lane == 0) base = atomicAdd(&st->work_counter[MODE], n_idle);
       base = __shfl_sync(0xffffffffu, base, 0);
       if (base + n_idle >= n_start) drained = true;
       if (phase == PH_IDLE) {
-        const int my_slot = base + __popc(idle & ((1u << lane) - 1u));
-        if (my_slot < n_start) {
-          slot = __ldg(&perm[my_slot]);
+        const int my_w = base + __popc(idle & ((1u << lane) - 1u));
+        if (my_w < n_start) {
+          wi = my_w;
+          slot = __ldg(&perm[my_w]);
           int s = 0;
           {
             int lo = 0, hi = ns - 1;
@@ -310,21 +343,37 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
           }
           off = s_sec_off[s];
           bs_off = (uint32_t)s * nbp1;
-          const int32_t* rs = row_start + s * (n_rows + 1);
-          const int c0 = start_hit[slot];
-          r0 = row_search(rs, n_rows, c0);
-          const int c1 = __ldg(&link_up[off + c0]);
-          const float2 h0 = __ldg(&syz[off + c0]), h1 = __ldg(&syz[off + c1]);
-          z_ref = h0.y;
-          const float dx = t_x[r0 + 1] - t_x[r0];
-          const float dy = h1.x - h0.x;
-          const float dz = h1.y - z_ref;
-          const float d = sqrtf(dx * dx + dy * dy);
-          f.x = t_x[r0];
-          f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
-          kf_reset_cov(f, K);
-          phase = PH_A; r = r0; cur = c0; top = r0; top_hit = c0; gap = 0; n_hits = 0; first = r0;
-          fresh = false; saved = false;
+          if (MODE == MODE_A) {
+            const int32_t* rs = row_start + s * (n_rows + 1);
+            const int c0 = start_hit[slot];
+            r0 = row_search(rs, n_rows, c0);
+            const int c1 = __ldg(&link_up[off + c0]);
+            const float2 h0 = __ldg(&syz[off + c0]), h1 = __ldg(&syz[off + c1]);
+            z_ref = h0.y;
+            const float dx = t_x[r0 + 1] - t_x[r0];
+            const float dy = h1.x - h0.x;
+            const float dz = h1.y - z_ref;
+            const float d = sqrtf(dx * dx + dy * dy);
+            f.x = t_x[r0];
+            f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
+            kf_reset_cov(f, K);
+            phase = PH_A; r = r0; cur = c0; top = r0; top_hit = c0; gap = 0; n_hits = 0; first = r0;
+            fresh = false; saved = false;
+          } else {
+            const size_t cs = (size_t)cap;
+            const int32_t* q = hs_i + wi;
+            const int ph = q[9 * cs];
+            if (ph == (MODE == MODE_B ? PH_B : PH_C)) {     // MODE_B skips the tracklets that went from A straight to C
+              const float* o = hs_f + wi;
+              f.x = o[0 * cs]; f.p0 = o[1 * cs]; f.p1 = o[2 * cs]; f.p2 = o[3 * cs]; f.p3 = o[4 * cs]; f.p4 = o[5 * cs];
+              f.c00 = o[6 * cs]; f.c10 = o[7 * cs]; f.c11 = o[8 * cs]; f.c20 = o[9 * cs]; f.c21 = o[10 * cs]; f.c22 = o[11 * cs];
+              f.c30 = o[12 * cs]; f.c31 = o[13 * cs]; f.c32 = o[14 * cs]; f.c33 = o[15 * cs]; f.c40 = o[16 * cs]; f.c41 = o[17 * cs];
+              f.c42 = o[18 * cs]; f.c43 = o[19 * cs]; f.c44 = o[20 * cs]; f.chi2 = o[21 * cs]; z_ref = o[22 * cs];
+              f.n = q[0 * cs]; r = q[1 * cs]; cur = q[2 * cs]; top = q[3 * cs]; top_hit = q[4 * cs]; gap = q[5 * cs];
+              n_hits = q[6 * cs]; first = q[7 * cs]; r0 = q[8 * cs]; phase = ph;
+              fresh = false; saved = false;
+            }
+          }
         }
       }
     }
@@ -375,7 +424,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       }
     }
     __syncwarp();
-    if (need_search) {
+    if (MODE != MODE_A && need_search) {
       // search: best cluster of row r in the tc window around the prediction
       const float yc = f.p0;
       const float zc = z_ref + f.p1;
@@ -470,6 +519,8 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     }
     if (ev == EV_TO_C) to_phase_c();
     else if (ev == EV_FINISH) finish();
+    if (MODE == MODE_A && (phase == PH_B || phase == PH_C)) park();
+    if (MODE == MODE_B && phase == PH_C) park();
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};

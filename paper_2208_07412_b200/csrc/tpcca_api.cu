@@ -27,7 +27,7 @@ struct Layout {
   size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
-  size_t start_hit, hits, trk_f, trk_i;
+  size_t start_hit, hits, trk_f, trk_i, hs_f, hs_i;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
@@ -82,6 +82,8 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.hits = take(4 * (size_t)(nr * CS));
   L.trk_f = take(4 * (size_t)(kTrkF * CS));
   L.trk_i = take(4 * (size_t)(kTrkI * CS));
+  L.hs_f = take(4 * (size_t)(kHsF * CS));
+  L.hs_i = take(4 * (size_t)(kHsI * CS));
   L.o_x_ref = take(4 * (size_t)CS);
   L.o_z_ref = take(4 * (size_t)CS);
   L.o_chi2 = take(4 * (size_t)CS);
@@ -500,7 +502,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     float* trk_f = c->at<float>(L.trk_f);
     int32_t* trk_i = c->at<int32_t>(L.trk_i);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
-    CU(c, cudaMemsetAsync(&status->work_counter, 0, sizeof(int32_t), st));
+    CU(c, cudaMemsetAsync(status->work_counter, 0, sizeof(status->work_counter), st));
     CU(c, cudaMemsetAsync(status->work, 0, sizeof(status->work), st));
     const DevTables& t = c->tab;
     S5Params sp;
@@ -509,14 +511,21 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     sp.win_y = t.win_y; sp.win_z = t.win_z; sp.gate = t.gate; sp.margin = t.margin; sp.grid_z_lo = t.grid_z_lo;
     sp.n_rows = t.n_rows; sp.n_sectors = t.n_sectors; sp.max_gap = t.tc_max_gap; sp.min_hits = t.tc_min_hits;
     sp.bins_per_sector = t.bins_per_sector;
-    k_tracklets<<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order,
-                                                                     c->at<int32_t>(L.up), start_hit, c->at<int32_t>(L.perm), cap, hits, trk_f, trk_i);
+    float* hs_f = c->at<float>(L.hs_f);
+    int32_t* hs_i = c->at<int32_t>(L.hs_i);
+    const int32_t* perm = c->at<int32_t>(L.perm);
+    k_tracklets<MODE_A><<<c->sm_count * kS5BlocksPerSMA, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
+                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+    k_tracklets<MODE_B><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+    k_tracklets<MODE_C><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
     k_track_gather<<<cap_tiles, 1024, 0, st>>>(T, status, start_hit, cap, hits, trk_f, trk_i, tile_off, o);
     k_track_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, o);
-    c->launches += 6;
+    c->launches += 8;
   }
   mark(5);
   CU(c, cudaGetLastError());
