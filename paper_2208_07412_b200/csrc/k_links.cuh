@@ -535,7 +535,7 @@ __global__ void k_start_offsets(const DevTables* __restrict__ T, const SectorDes
   if (s == 0) {
     st->n_start = (int32_t)tot[0];
     if (tot[0] > (int64_t)cap) st->err_capacity = 1;
-    for (int i = 0; i < 4; ++i) st->work_counter[i] = 0;
+    for (int i = 0; i < 8; ++i) st->work_counter[i] = 0;
   }
 }
 

@@ -217,13 +217,14 @@ __device__ __noinline__ int search_exact(float p0, float p1, float z_ref, float 
 // the running state and is parked in shared memory the moment the running state moves on without
 // an update, which keeps the register count at one Kalman state per lane.
 // The kernel is compiled in three modes and launched three times: MODE_A runs phase A
-// for every start hit, MODE_B phase B, MODE_C phase C.  A lane whose tracklet leaves the kernel's phase
+// for every start hit, MODE_B phase B, MODE_C1 phase C down to the start row (hits known: updates, a search
+// only on gap rows), MODE_C2 phase C below the start row (a search every row).  A lane whose tracklet leaves the kernel's phase
 // parks the tracklet (Kalman state + bookkeeping, kHsF floats and kHsI ints, indexed by the work
 // index so that the lanes refilled together store and load neighbouring words) and takes new work.
 // Per lane the sequence of operations is exactly that of the single loop; what changes is which
 // lanes share a warp: link followers (no search), extrapolators (a search every row) and refitters
 // no longer wait for each other's code.
-enum { MODE_A = 1, MODE_B = 2, MODE_C = 3 };
+enum { MODE_A = 1, MODE_B = 2, MODE_C1 = 3, MODE_C2 = 4 };
 constexpr int kHsF = 23;    // x, p0..p4, c[15], chi2, z_ref
 constexpr int kHsI = 10;    // n, r, cur, top, top_hit, gap, n_hits, first, r0, phase
 
@@ -261,7 +262,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   const int tid = threadIdx.x;
   unsigned w_prop = 0, w_upd = 0, w_gate = 0, w_search = 0, w_cand = 0;   // work counters
 
-  enum { PH_A = 0, PH_B = 1, PH_C = 2, PH_IDLE = 3 };
+  enum { PH_A = 0, PH_B = 1, PH_C = 2, PH_IDLE = 3, PH_C2 = 4 };   // PH_C2: parked marker only (phase C below the start row)
   // ---- per-lane tracklet state ---------------------------------------------------------------
   int phase = PH_IDLE;
   bool drained = false;      // warp-uniform: the work counter ran out
@@ -363,15 +364,16 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             const size_t cs = (size_t)cap;
             const int32_t* q = hs_i + wi;
             const int ph = q[9 * cs];
-            if (ph == (MODE == MODE_B ? PH_B : PH_C)) {     // MODE_B skips the tracklets that went from A straight to C
+            if (ph == (MODE == MODE_B ? PH_B : (MODE == MODE_C1 ? PH_C : PH_C2))) {   // others are not this kernel's
               const float* o = hs_f + wi;
               f.x = o[0 * cs]; f.p0 = o[1 * cs]; f.p1 = o[2 * cs]; f.p2 = o[3 * cs]; f.p3 = o[4 * cs]; f.p4 = o[5 * cs];
               f.c00 = o[6 * cs]; f.c10 = o[7 * cs]; f.c11 = o[8 * cs]; f.c20 = o[9 * cs]; f.c21 = o[10 * cs]; f.c22 = o[11 * cs];
               f.c30 = o[12 * cs]; f.c31 = o[13 * cs]; f.c32 = o[14 * cs]; f.c33 = o[15 * cs]; f.c40 = o[16 * cs]; f.c41 = o[17 * cs];
               f.c42 = o[18 * cs]; f.c43 = o[19 * cs]; f.c44 = o[20 * cs]; f.chi2 = o[21 * cs]; z_ref = o[22 * cs];
               f.n = q[0 * cs]; r = q[1 * cs]; cur = q[2 * cs]; top = q[3 * cs]; top_hit = q[4 * cs]; gap = q[5 * cs];
-              n_hits = q[6 * cs]; first = q[7 * cs]; r0 = q[8 * cs]; phase = ph;
-              fresh = false; saved = false;
+              n_hits = q[6 * cs]; first = q[7 * cs]; r0 = q[8 * cs]; phase = (MODE == MODE_C2) ? (int)PH_C : ph;
+              // C1 always hands over right after the update on the start row: running state == snapshot
+              fresh = (MODE == MODE_C2); saved = false;
             }
           }
         }
@@ -521,6 +523,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     else if (ev == EV_FINISH) finish();
     if (MODE == MODE_A && (phase == PH_B || phase == PH_C)) park();
     if (MODE == MODE_B && phase == PH_C) park();
+    if (MODE == MODE_C1 && phase == PH_C && r < r0) { phase = PH_C2; park(); }
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};

@@ -518,14 +518,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
                                                                               start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
     k_tracklets<MODE_B><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
-    k_tracklets<MODE_C><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
+    k_tracklets<MODE_C1><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+    k_tracklets<MODE_C2><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
     k_track_gather<<<cap_tiles, 1024, 0, st>>>(T, status, start_hit, cap, hits, trk_f, trk_i, tile_off, o);
     k_track_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, o);
-    c->launches += 8;
+    c->launches += 9;
   }
   mark(5);
   CU(c, cudaGetLastError());

@@ -65,7 +65,7 @@ struct DevStatus {
   int32_t err_capacity;    // n_start exceeded max_start_hits
   uint32_t n_big;          // S1 coarse buckets too large for the shared-memory sort
   int32_t n_start;         // total start hits
-  int32_t work_counter[4]; // S5 dynamic work distribution: one counter per kernel mode (index 1..3)
+  int32_t work_counter[8]; // S5 dynamic work distribution: one counter per kernel mode (index 1..4)
   int32_t start_off[kMaxSectors + 1];   // first start-hit slot of each sector
   int32_t trk_off[kMaxSectors + 1];     // first track of each sector
   int64_t hit_off[kMaxSectors + 1];     // first hit of each sector (global CSR base)
