@@ -145,13 +145,17 @@ constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 constexpr int kS5BlocksPerSMA = TPCCA_S5_BPS_A;   // ... of the phase-A kernel (no search code: fewer registers)
 constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
 #ifndef TPCCA_S5_REFILL
-#define TPCCA_S5_REFILL 4
+#define TPCCA_S5_REFILL 8
 #endif
 constexpr int kS5Refill = TPCCA_S5_REFILL;      // idle lanes of a warp that trigger a refill from the work counter
 #ifndef TPCCA_S5_UNROLL
 #define TPCCA_S5_UNROLL 4
 #endif
 constexpr int kS5Unroll = TPCCA_S5_UNROLL;   // candidate loads in flight per lane in the S5 search
+#ifndef TPCCA_S5_PREFETCH
+#define TPCCA_S5_PREFETCH 0
+#endif
+constexpr int kS5Prefetch = TPCCA_S5_PREFETCH;   // 0 off, 1 L1, 2 L2
 constexpr int kSnapF = 22;        // floats of a saved Kalman state: x, p[5], c[15], chi2
 
 // scalars of S5, passed by value (constant bank: no registers)
@@ -161,6 +165,11 @@ struct S5Params {
   float win_y, win_z, gate, margin, grid_z_lo;
   int32_t n_rows, n_sectors, max_gap, min_hits, bins_per_sector;
 };
+
+__device__ __forceinline__ void prefetch_l1(const void* p) {
+  if (kS5Prefetch == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+  else asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
 
 // approximate reciprocal (one MUFU.RCP); used only to rank candidates and to pre-decide gates
 // that are nowhere near the threshold -- every decision that could flip is taken on the exact form
@@ -235,7 +244,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
             const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
             const int32_t* __restrict__ start_hit, const int32_t* __restrict__ perm, int32_t cap,
-            int32_t* __restrict__ hits /*[n_rows][cap]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
+            int32_t* __restrict__ hits /*[cap][n_rows]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
             int32_t* __restrict__ trk_i /*[kTrkI][cap]*/, float* __restrict__ hs_f /*[kHsF][cap]*/,
             int32_t* __restrict__ hs_i /*[kHsI][cap]*/) {
   __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];
@@ -386,7 +395,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     enum { EV_NONE = 0, EV_TO_C = 1, EV_FINISH = 2 };
     const bool alive = phase != PH_IDLE;
     int ev = EV_NONE;
-    int32_t* hcol = hits + slot;
+    int32_t* hcol = hits + (size_t)slot * n_rows;   // the tracklet's hit per row: one contiguous line per tracklet
     int cand = -1;                        // >= 0: cluster to use on this row; -1: none known
     int nxt = -1;                         // candidate of the next row (loaded early)
     float2 h = make_float2(0.f, 0.f);
@@ -395,7 +404,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       cand = cur;
       if (cand >= 0) h = __ldg(&syz[off + cand]);
       if (phase == PH_A) nxt = __ldg(&link_up[off + cand]);
-      else if (phase == PH_C && r - 1 >= r0) nxt = hcol[(size_t)(r - 1) * cap];
+      else if (phase == PH_C && r - 1 >= r0) nxt = hcol[r - 1];
       xr = t_x[r];
       if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
       w_prop += (xr != f.x) ? 1u : 0u;
@@ -496,7 +505,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       if (took) {
         kf_update(f, h.x, h.y - z_ref, K);
         ++w_upd;
-        if (is_new) { hcol[(size_t)r * cap] = cand; ++n_hits; }
+        if (is_new) { hcol[r] = cand; ++n_hits; }
         if (phase == PH_C) {
           fresh = true; saved = false;
           if (is_new) { gap = 0; if (r < first) first = r; }
@@ -504,10 +513,10 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
           top = r; top_hit = cand; gap = 0;
         }
       } else if (phase == PH_B) {
-        hcol[(size_t)r * cap] = -1;
+        hcol[r] = -1;
         if (++gap > P.max_gap) { ev = EV_TO_C; go = false; }
       } else if (r < r0) {                // phase C below the start hit
-        hcol[(size_t)r * cap] = -1;
+        hcol[r] = -1;
         if (++gap > P.max_gap) { ev = EV_FINISH; go = false; }
       }
     }
@@ -524,6 +533,22 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     if (MODE == MODE_A && (phase == PH_B || phase == PH_C)) park();
     if (MODE == MODE_B && phase == PH_C) park();
     if (MODE == MODE_C1 && phase == PH_C && r < r0) { phase = PH_C2; park(); }
+    // ---- prefetch hint for the next row's search (kernels that search every row) ---------------------
+    // Straight-line guess of the next prediction; only the cache lines of the bin_start entries around
+    // it are touched (no value is used), so the hint cannot change any result.
+    if ((MODE == MODE_B || MODE == MODE_C2) && kS5Prefetch && phase != PH_IDLE && r >= 0 && r < n_rows) {
+      const float dxn = t_x[r] - f.x;
+      const float sec = rsqrtf(fmaxf(1.0f - f.p2 * f.p2, 0.05f));
+      const float yn = f.p0 + dxn * (f.p2 * sec);
+      const float zn = z_ref + f.p1 + dxn * (f.p3 * sec);
+      const int nyh = t_nyh[r], nzh = t_nzh[r], ny = t_ny[r];
+      const int by = bin_range(yn - my, t_ylo[r], t_iby[r], nyh);
+      const int bz = bin_range(zn - mz, P.grid_z_lo, t_ibz[r], nzh);
+      const uint32_t* bp = bin_start + (bs_off + (uint32_t)(t_base[r] + bz * ny + by));
+      const int up = (bz < nzh) ? ny : 0;
+      prefetch_l1(bp); prefetch_l1(bp + 2);
+      prefetch_l1(bp + up); prefetch_l1(bp + up + 2);
+    }
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};
@@ -578,7 +603,7 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
                const float* __restrict__ trk_f, const int32_t* __restrict__ trk_i,
                const longlong2* __restrict__ tile_off, TrackOut o) {
   __shared__ int ws[33];
-  const int ns = T->n_sectors;
+  const int ns = T->n_sectors, n_rows_g = T->n_rows;
   const int n_start = st->err_capacity ? 0 : st->n_start;
   const int slot = blockIdx.x * 1024 + threadIdx.x;
   const int nh = slot < n_start ? trk_i[slot] : 0;
@@ -615,7 +640,7 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
     o.start_hit[t] = start_hit[slot];
     long long w = h;
     for (int r = first; r <= last; ++r) {
-      const int c = hits[(size_t)r * cs + slot];
+      const int c = hits[(size_t)slot * n_rows_g + r];
       if (c != -1) o.hit_idx[w++] = c;
     }
   }
