@@ -576,13 +576,13 @@ k_start_hits(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
 __global__ void __launch_bounds__(256)
 k_sh_bucket_counts(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, const int32_t* __restrict__ zorder,
                    const uint32_t* __restrict__ cb_start, const int32_t* __restrict__ start_hit, int32_t cap,
-                   int32_t* __restrict__ sh_first, int2* __restrict__ cnt) {
+                   int32_t* __restrict__ sh_first, int32_t* __restrict__ cnt, int2* __restrict__ blk_cnt) {
+  __shared__ int ws[33];
   const int ncb = T->n_cb, ns = T->n_sectors;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= ns * ncb) return;
-  const int s = i / ncb, j = i - s * ncb;
   int a = 0, n = 0;
-  if (!st->err_capacity) {
+  if (i < ns * ncb && !st->err_capacity) {
+    const int s = i / ncb, j = i - s * ncb;
     const int cb = zorder[j];
     const uint32_t lo_pos = cb_start[(size_t)s * (ncb + 1) + cb], hi_pos = cb_start[(size_t)s * (ncb + 1) + cb + 1];
     const int s0 = st->start_off[s], s1 = st->start_off[s + 1];
@@ -594,18 +594,24 @@ k_sh_bucket_counts(const DevTables* __restrict__ T, const DevStatus* __restrict_
     a = lower(lo_pos);
     n = lower(hi_pos) - a;
   }
-  sh_first[i] = a;
-  cnt[i] = make_int2(n, 0);
+  if (i < ns * ncb) { sh_first[i] = a; cnt[i] = n; }
+  int total;
+  block_exclusive_scan<int>(n, ws, total);
+  if (threadIdx.x == 0) blk_cnt[blockIdx.x] = make_int2(total, 0);
 }
 
 __global__ void __launch_bounds__(256)
-k_sh_perm(const DevTables* __restrict__ T, const int32_t* __restrict__ sh_first, const int2* __restrict__ cnt,
-          const longlong2* __restrict__ pre, int32_t* __restrict__ perm) {
+k_sh_perm(const DevTables* __restrict__ T, const int32_t* __restrict__ sh_first, const int32_t* __restrict__ cnt,
+          const longlong2* __restrict__ blk_pre, int32_t* __restrict__ perm) {
+  __shared__ int ws[33];
   const int n = T->n_sectors * T->n_cb;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int c = i < n ? cnt[i] : 0;
+  int total;
+  const int ex = block_exclusive_scan<int>(c, ws, total);
   if (i >= n) return;
-  const int a = sh_first[i], c = cnt[i].x;
-  int32_t* o = perm + pre[i].x;
+  const int a = sh_first[i];
+  int32_t* o = perm + blk_pre[blockIdx.x].x + ex;
   for (int k = 0; k < c; ++k) o[k] = a + k;
 }
 

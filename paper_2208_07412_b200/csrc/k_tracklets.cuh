@@ -610,46 +610,61 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
   int ta, tb;
   const int ea = block_exclusive_scan<int>(nh > 0 ? 1 : 0, ws, ta);
   const int eb = block_exclusive_scan<int>(nh, ws, tb);
-  if (slot >= n_start) return;
+  const bool valid = slot < n_start;
   // sector of the slot
   int s = 0;
-  {
+  if (valid) {
     int lo = 0, hi = ns - 1;
     while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (st->start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
     s = lo;
   }
   const long long t = tile_off[blockIdx.x].x + ea;       // global track index
   const long long h = tile_off[blockIdx.x].y + eb;       // global hit index
-  const long long hloc = h - st->hit_off[s];
-  // hit_offset of sector s lives at [trk_off[s] + s, trk_off[s+1] + s + 1)
-  if (nh > 0) {
-    const size_t cs = (size_t)cap;
-    o.hit_offset[t + s] = (int32_t)hloc;
-    o.x_ref[t] = trk_f[0 * cs + slot];
-    o.z_ref[t] = trk_f[1 * cs + slot];
+  int first = 0, last = -1;
+  if (valid) {
+    const long long hloc = h - st->hit_off[s];
+    // hit_offset of sector s lives at [trk_off[s] + s, trk_off[s+1] + s + 1)
+    if (nh > 0) {
+      const size_t cs = (size_t)cap;
+      o.hit_offset[t + s] = (int32_t)hloc;
+      o.x_ref[t] = trk_f[0 * cs + slot];
+      o.z_ref[t] = trk_f[1 * cs + slot];
 #pragma unroll
-    for (int i = 0; i < 5; ++i) o.par[i * cs + t] = trk_f[(2 + i) * cs + slot];
+      for (int i = 0; i < 5; ++i) o.par[i * cs + t] = trk_f[(2 + i) * cs + slot];
 #pragma unroll
-    for (int i = 0; i < 15; ++i) o.cov[i * cs + t] = trk_f[(7 + i) * cs + slot];
-    o.chi2[t] = trk_f[22 * cs + slot];
-    o.n_hits[t] = nh;
-    o.n_fit[t] = trk_i[1 * cs + slot];
-    const int first = trk_i[2 * cs + slot], last = trk_i[3 * cs + slot];
-    o.first_row[t] = first;
-    o.last_row[t] = last;
-    o.start_hit[t] = start_hit[slot];
-    long long w = h;
-    for (int r = first; r <= last; ++r) {
-      const int c = hits[(size_t)slot * n_rows_g + r];
-      if (c != -1) o.hit_idx[w++] = c;
+      for (int i = 0; i < 15; ++i) o.cov[i * cs + t] = trk_f[(7 + i) * cs + slot];
+      o.chi2[t] = trk_f[22 * cs + slot];
+      o.n_hits[t] = nh;
+      o.n_fit[t] = trk_i[1 * cs + slot];
+      first = trk_i[2 * cs + slot]; last = trk_i[3 * cs + slot];
+      o.first_row[t] = first;
+      o.last_row[t] = last;
+      o.start_hit[t] = start_hit[slot];
+    }
+    // closing entry of each sector's hit_offset: written by the last slot of the sector (empty
+    // sectors are closed by k_track_close_empty)
+    if (slot + 1 == st->start_off[s + 1] || slot + 1 == n_start) {
+      const long long tend = t + (nh > 0 ? 1 : 0);
+      o.hit_offset[tend + s] = (int32_t)(hloc + nh);
     }
   }
-  // closing entry of each sector's hit_offset: written by the last slot of the sector
-  if (slot + 1 == st->start_off[s + 1] || slot + 1 == n_start) {
-    // all later sectors that are empty share the same closing value pattern: handle each sector
-    // whose slot range ends here (this one) -- empty sectors are closed by k_track_close_empty.
-    const long long tend = t + (nh > 0 ? 1 : 0);
-    o.hit_offset[tend + s] = (int32_t)(hloc + nh);
+  // hit CSR: the warp copies the hit line of each of its accepted tracklets together (coalesced
+  // 128-byte reads of the tracklet's line, ballot compaction of the rows that hold a hit)
+  const int lane = threadIdx.x & 31;
+  unsigned todo = __ballot_sync(0xffffffffu, valid && nh > 0);
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int sl = __shfl_sync(0xffffffffu, slot, src);
+    const int f0 = __shfl_sync(0xffffffffu, first, src), l0 = __shfl_sync(0xffffffffu, last, src);
+    long long w = __shfl_sync(0xffffffffu, h, src);
+    const int32_t* line = hits + (size_t)sl * n_rows_g;
+    for (int r = f0 + lane; r - lane <= l0; r += 32) {
+      const int c = r <= l0 ? line[r] : -1;
+      const unsigned m = __ballot_sync(0xffffffffu, c != -1);
+      if (c != -1) o.hit_idx[w + __popc(m & ((1u << lane) - 1u))] = c;
+      w += __popc(m);
+    }
   }
 }
 

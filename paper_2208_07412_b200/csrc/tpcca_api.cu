@@ -24,7 +24,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
   size_t tables, sec, status, tot;
   size_t in_y, in_z, in_row;
-  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_pre, perm;
+  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_blk, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
   size_t start_hit, hits, trk_f, trk_i, hs_f, hs_i;
@@ -69,8 +69,9 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.rec = take(16 * (size_t)N);
   L.zorder = take(4 * (size_t)L.n_cb);
   L.sh_first = take(4 * (size_t)(ns * L.n_cb));
-  L.sh_cnt = take(sizeof(int2) * (size_t)(ns * L.n_cb));
-  L.sh_pre = take(sizeof(longlong2) * (size_t)(ns * L.n_cb));
+  L.sh_cnt = take(4 * (size_t)(ns * L.n_cb));
+  L.sh_blk = take(sizeof(int2) * (size_t)(ns * L.n_cb / 256 + 2));
+  L.sh_pre = take(sizeof(longlong2) * (size_t)(ns * L.n_cb / 256 + 2));
   L.perm = take(4 * (size_t)CS);
   L.up_raw = take(4 * (size_t)N);
   L.dn_raw = take(4 * (size_t)N);
@@ -481,13 +482,14 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       ++c->launches;
     }
     {   // processing order of S5: start-hit slots by (sector, z)
-      const int nbk = (int)(c->ns * L.n_cb);
-      int2* shc = c->at<int2>(L.sh_cnt);
+      const int nbk = (int)(c->ns * L.n_cb), nblk = (nbk + 255) / 256;
+      int32_t* shc = c->at<int32_t>(L.sh_cnt);
+      int2* blc = c->at<int2>(L.sh_blk);
       longlong2* shp = c->at<longlong2>(L.sh_pre);
-      k_sh_bucket_counts<<<(nbk + 255) / 256, 256, 0, st>>>(T, status, c->at<int32_t>(L.zorder), c->at<uint32_t>(L.cb_start), start_hit, cap,
-                                                           c->at<int32_t>(L.sh_first), shc);
-      k_scan_pairs<<<1, 1024, 0, st>>>(shc, shp, nbk, tot + 4);
-      k_sh_perm<<<(nbk + 255) / 256, 256, 0, st>>>(T, c->at<int32_t>(L.sh_first), shc, shp, c->at<int32_t>(L.perm));
+      k_sh_bucket_counts<<<nblk, 256, 0, st>>>(T, status, c->at<int32_t>(L.zorder), c->at<uint32_t>(L.cb_start), start_hit, cap,
+                                               c->at<int32_t>(L.sh_first), shc, blc);
+      k_scan_pairs<<<1, 1024, 0, st>>>(blc, shp, nblk, tot + 4);
+      k_sh_perm<<<nblk, 256, 0, st>>>(T, c->at<int32_t>(L.sh_first), shc, shp, c->at<int32_t>(L.perm));
       c->launches += 3;
     }
   }
