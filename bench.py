@@ -49,6 +49,18 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def ncu_traffic(args, n_clusters):
+    """dram bytes read + written per launch of the S2 kernels from the committed ncu capture of this workload
+    (profiles/r1_traffic.json), or None when the workload differs from the captured one."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    if not os.path.exists(p):
+        return None
+    d = json.load(open(p))
+    if d.get("config") != args.config or d.get("n_clusters") != n_clusters:
+        return None
+    return float(d["s2_dram_bytes_per_launch"])
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -319,10 +331,11 @@ def run_tpcca(args):
                         l2="inputs larger than L2 (no flush needed)", inputs="device-resident, borrowed"),
             stage_ms=dict(zip(("S1_grid", "S2_neighbours", "S3_clean", "S4_start", "S5_tracklets", "total"),
                               (round(float(v), 4) for v in stage_ms))),
-            roofline=dict(kernel="k_neighbours (S2)", bound="hbm", achieved=s2_gbs, peak=peaks["hbm_gbs"], unit="GB/s",
-                          frac=s2_gbs / peaks["hbm_gbs"], frac_of_nominal_8000=s2_gbs / 8000.0, traffic=None,
+            roofline=dict(kernel="S2 neighbour finder: k_nf_plan + k_neighbours", bound="hbm", achieved=s2_gbs,
+                          peak=peaks["hbm_gbs"], unit="GB/s", frac=s2_gbs / peaks["hbm_gbs"],
+                          frac_of_nominal_8000=s2_gbs / 8000.0, traffic=ncu_traffic(args, N),
                           algorithmic_bytes=s2_bytes, peak_source=peaks["source"]),
-            roofline_dominant=dict(kernel="k_tracklets (S5)", bound="alu", achieved=s5_tops, peak=alu_peak,
+            roofline_dominant=dict(kernel="S5 tracklets: k_tracklets<A,B,C1,C2> + k_track_gather", bound="alu", achieved=s5_tops, peak=alu_peak,
                                    unit="Tfp32op/s (no FMA)", frac=s5_tops / alu_peak, traffic=None, flops=flops,
                                    work=work),
             e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
