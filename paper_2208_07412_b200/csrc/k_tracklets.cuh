@@ -31,9 +31,15 @@ __device__ __forceinline__ void kf_reset_cov(KF& s, const KFConst& k) {
   s.chi2 = 0.f; s.n = 0;
 }
 
-// DESIGN.md 3.5 "Propagate to x2".  false (state untouched) if |sin phi| would exceed the limit.
-__device__ __forceinline__ bool kf_propagate(KF& s, float x2, const KFConst& K) {
+// DESIGN.md 3.5 "Propagate to x2", in two parts so that a kernel can issue the loads of the search
+// between them (the search window depends only on the transported mean): kf_prop_mean transports x,
+// p0, p1, p2 and returns the Jacobian terms; kf_prop_cov transports the covariance.  Every operation
+// and its order are those of the definition.  false (state untouched) if |sin phi| would exceed the limit.
+struct KFJac { float n02, n04, n12, n13, n14, n24; bool moved; };
+
+__device__ __forceinline__ bool kf_prop_mean(KF& s, float x2, const KFConst& K, KFJac& J) {
   const float dx = x2 - s.x;
+  J.moved = false;
   if (dx == 0.0f) return true;
   const float k = s.p4 * K.Bc;
   const float ey = s.p2;
@@ -51,17 +57,24 @@ __device__ __forceinline__ bool kf_propagate(KF& s, float x2, const KFConst& K) 
   const float tt = (k * k) * d2;
   const float dS = d * (1.0f + tt * (K.c24 + tt * K.c640));
   const float cc = 1.0f + (ex * ex2 + ey * ey2);
-  const float n02 = (dx * cc) / ((sx * ex) * ex2);
+  J.n02 = (dx * cc) / ((sx * ex) * ex2);
   const float j4 = ((dx * dx) * cc) / (ex2 * (sx * sx));
-  const float n04 = K.Bc * j4;
-  const float n12 = s.p3 * ((dx * tg) / (ex * ex2));
-  const float n13 = dS;
-  const float n14 = (s.p3 * K.Bc) * ((dy / d) * j4 + ((k * d) * d2) * K.c12);
-  const float n24 = K.Bc * dx;
+  J.n04 = K.Bc * j4;
+  J.n12 = s.p3 * ((dx * tg) / (ex * ex2));
+  J.n13 = dS;
+  J.n14 = (s.p3 * K.Bc) * ((dy / d) * j4 + ((k * d) * d2) * K.c12);
+  J.n24 = K.Bc * dx;
+  J.moved = true;
   s.p0 = s.p0 + dy;
   s.p1 = s.p1 + s.p3 * dS;
   s.p2 = ey2;
   s.x = x2;
+  return true;
+}
+
+__device__ __forceinline__ void kf_prop_cov(KF& s, const KFJac& J) {
+  if (!J.moved) return;
+  const float n02 = J.n02, n04 = J.n04, n12 = J.n12, n13 = J.n13, n14 = J.n14, n24 = J.n24;
   // A = J*C (rows 0..2 differ from C), C' = A*J^T (lower triangle); terms left to right.
   const float A00 = s.c00 + n02 * s.c20 + n04 * s.c40;
   const float A02 = s.c20 + n02 * s.c22 + n04 * s.c42;
@@ -93,6 +106,12 @@ __device__ __forceinline__ bool kf_propagate(KF& s, float x2, const KFConst& K) 
   s.c33 = A33;
   s.c43 = A43;
   s.c44 = A44;
+}
+
+__device__ __forceinline__ bool kf_propagate(KF& s, float x2, const KFConst& K) {
+  KFJac J;
+  if (!kf_prop_mean(s, x2, K, J)) return false;
+  kf_prop_cov(s, J);
   return true;
 }
 
@@ -411,9 +430,29 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     }
     __syncwarp();
     bool go = false;                      // the lane carries on with this row
+    // kernels that search every row: the bin_start loads of the search are issued between the two
+    // halves of the propagation (the window depends only on the transported mean), so their latency
+    // overlaps the covariance transport
+    constexpr bool kEarly = (MODE == MODE_B || MODE == MODE_C2);
+    uint32_t c0 = 0, e0 = 0, c1 = 0, e1 = 0, c2 = 0, e2 = 0;
+    int nsl = 0;
     if (alive) {
-      go = kf_propagate(f, xr, K);
+      KFJac J;
+      go = kf_prop_mean(f, xr, K, J);
       if (!go) ev = (phase == PH_C) ? EV_FINISH : EV_TO_C;
+      if (kEarly && go && cand < 0 && (phase == PH_B || f.n >= 2)) {
+        const float ylo = t_ylo[r], iby = t_iby[r], ibz = t_ibz[r];
+        const int nyh = t_nyh[r], nzh = t_nzh[r], ny = t_ny[r];
+        const float zc = z_ref + f.p1;
+        const int by0 = bin_range(f.p0 - my, ylo, iby, nyh), by1 = bin_range(f.p0 + my, ylo, iby, nyh);
+        const int bz0 = bin_range(zc - mz, P.grid_z_lo, ibz, nzh), bz1 = bin_range(zc + mz, P.grid_z_lo, ibz, nzh);
+        const uint32_t* bp = bin_start + (bs_off + (uint32_t)(t_base[r] + bz0 * ny));
+        nsl = bz1 - bz0 + 1;
+        c0 = __ldg(&bp[by0]); e0 = __ldg(&bp[by1 + 1]);
+        if (nsl > 1) { c1 = __ldg(&bp[ny + by0]); e1 = __ldg(&bp[ny + by1 + 1]); }
+        if (nsl > 2) { c2 = __ldg(&bp[2 * ny + by0]); e2 = __ldg(&bp[2 * ny + by1 + 1]); }
+      }
+      if (go) kf_prop_cov(f, J);
     }
     bool took = false, is_new = false, need_search = false;
     const float wy = f.c00 + K.err2_y;
@@ -446,7 +485,6 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       const int ny = t_ny[r];
       const uint32_t* bp = bin_start + (bs_off + (uint32_t)(t_base[r] + bz0 * ny));
       const float2* yz = syz + off;
-      const int nsl = bz1 - bz0 + 1;
       ++w_search;
       // The candidates of the (at most three) z slices are walked as ONE loop over a flat index,
       // so the trip count of the warp is the largest candidate count of a lane, not the sum of the
@@ -454,10 +492,12 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       // is within a few ulp of the defined d2, so the smallest d2~ is the smallest d2 unless the
       // runner-up is within 2e-5 relative; then (ties, duplicates), and for windows of more than
       // three slices, the exact loop decides.
-      uint32_t c0 = __ldg(&bp[by0]), e0 = __ldg(&bp[by1 + 1]);
-      uint32_t c1 = 0, e1 = 0, c2 = 0, e2 = 0;
-      if (nsl > 1) { c1 = __ldg(&bp[ny + by0]); e1 = __ldg(&bp[ny + by1 + 1]); }
-      if (nsl > 2) { c2 = __ldg(&bp[2 * ny + by0]); e2 = __ldg(&bp[2 * ny + by1 + 1]); }
+      if (!kEarly) {
+        nsl = bz1 - bz0 + 1;
+        c0 = __ldg(&bp[by0]); e0 = __ldg(&bp[by1 + 1]);
+        if (nsl > 1) { c1 = __ldg(&bp[ny + by0]); e1 = __ldg(&bp[ny + by1 + 1]); }
+        if (nsl > 2) { c2 = __ldg(&bp[2 * ny + by0]); e2 = __ldg(&bp[2 * ny + by1 + 1]); }
+      }
       const int n0 = (int)(e0 - c0), n01 = n0 + (int)(e1 - c1), total = nsl > 3 ? 0 : n01 + (int)(e2 - c2);
       const uint32_t o1 = c1 - (uint32_t)n0, o2 = c2 - (uint32_t)n01;   // flat index i -> cluster o + i
       float a1 = __int_as_float(0x7f800000), a2 = a1;
