@@ -21,12 +21,13 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 // cluster runs and the two bin_start runs of the next tile in shared memory with 1-D bulk async
 // copies (TMA, mbarrier completion) while the current tile is searched entirely in shared memory.
 #ifndef TPCCA_NF_K
-#define TPCCA_NF_K 7
+#define TPCCA_NF_K 10
 #endif
 #ifndef TPCCA_NF_ARENA
-#define TPCCA_NF_ARENA 7168
+#define TPCCA_NF_ARENA 8448
 #endif
-constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory
+constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory (<= 15)
+static_assert(TPCCA_NF_K <= 15 && TPCCA_NF_TILE <= 256, "work-item encoding: 8 bits cluster, 4 bits hit row, 4 bits nd");
 constexpr int kNfThreads = kNfTile;       // one thread per cluster of the tile
 constexpr int kNfArena = TPCCA_NF_ARENA;  // bytes of one staging buffer: [up clusters | down clusters | up bins | down bins]
 constexpr int kNfMaxCn = 1022;            // staged clusters per side (staged indices are packed in 10 bits)
@@ -280,11 +281,51 @@ __device__ __forceinline__ int nf_test_runs(const float2 c, uint32_t w0, uint32_
   return n;
 }
 
+// ---- medium path: more than kNfK hits on a side (dense regions) -------------------------------------
+// Nested loops over the staged candidate runs of both sides (no hit cache): the U x D product in the
+// order and arithmetic of nf_slow, in shared memory.  Returns false on an exact score tie (decided by
+// original ids in nf_slow).  iu / id are staged indices.
+__device__ __noinline__ bool nf_medium(const float2 c, uint32_t wu0, uint32_t wu1, uint32_t wd0, uint32_t wd1, uint32_t sUC,
+                                       uint32_t sDC, const float4 uA, const float4 dA, const float4 g, float& best,
+                                       int& iu, int& id) {
+  const int un0 = (wu0 >> 10) & 63, un01 = wu0 >> 26, utot = wu1 >> 10;
+  const uint32_t uo1 = 8u * ((wu0 >> 16) & 1023u), uo2 = 8u * (wu1 & 1023u);
+  const int dn0 = (wd0 >> 10) & 63, dn01 = wd0 >> 26, dtot = wd1 >> 10;
+  const uint32_t do1 = 8u * ((wd0 >> 16) & 1023u), do2 = 8u * (wd1 & 1023u);
+  bool have = false, tie = false;
+  best = 0.0f; iu = -1; id = -1;
+  uint32_t au = sUC + 8u * (wu0 & 1023u);
+#pragma unroll 1
+  for (int ju = 0; ju < utot; ++ju, au += 8u) {
+    if (ju == un0) au += uo1;
+    if (ju == un01) au += uo2;
+    const float2 u = lds_f2(au);
+    const float dyu = __fsub_rn(u.x, c.x), dzu = __fsub_rn(u.y, c.y);
+    if (!(fabsf(dyu) <= uA.x && fabsf(dzu) <= uA.y)) continue;
+    const float Ay = __fmul_rn(dyu, g.y), Az = __fmul_rn(dzu, g.y);
+    uint32_t ad = sDC + 8u * (wd0 & 1023u);
+#pragma unroll 1
+    for (int jd = 0; jd < dtot; ++jd, ad += 8u) {
+      if (jd == dn0) ad += do1;
+      if (jd == dn01) ad += do2;
+      const float2 d = lds_f2(ad);
+      const float dyd = __fsub_rn(d.x, c.x), dzd = __fsub_rn(d.y, c.y);
+      if (!(fabsf(dyd) <= dA.x && fabsf(dzd) <= dA.y)) continue;
+      const float ay = __fsub_rn(Ay, __fmul_rn(-dyd, g.x));
+      const float az = __fsub_rn(Az, __fmul_rn(-dzd, g.x));
+      const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
+      if (have && sc == best) tie = true;
+      if (!have || sc < best) { have = true; best = sc; iu = (int)((au - sUC) >> 3); id = (int)((ad - sDC) >> 3); }
+    }
+  }
+  return !tie;
+}
+
 struct NfSmem {
   alignas(128) unsigned char arena[kNfArena];   // staging buffer (TMA destination): [up clusters | down clusters | up bins | down bins]
   float2 vec[2 * kNfK][kNfThreads];      // cached hits: rows [0, K) down side, [K, 2K) up side; column = cluster of the tile
   uint16_t hidx[2 * kNfK][kNfThreads];   // staged indices of the cached hits
-  uint16_t items[kNfMaxItems];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 11
+  uint16_t items[kNfMaxItems];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 12
   int hist[2][16], cnt[2][16];           // items per nd (work key) / emission cursors, two consecutive tiles
   NfTileDesc desc[4];
   uint64_t full;
@@ -307,7 +348,7 @@ struct NfSmem {
 // barrier that ends phase A of tile i, the only phase that reads the staging buffer); per-row
 // constants come from the constant bank (NfTable is a by-value kernel parameter).
 #ifndef TPCCA_NF_BPS
-#define TPCCA_NF_BPS 8
+#define TPCCA_NF_BPS 6
 #endif
 __global__ void __launch_bounds__(kNfThreads, TPCCA_NF_BPS)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
@@ -372,7 +413,9 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     while (!mbar_try_wait(&S.full, (uint32_t)(it & 1))) {}
     // ---- phase A -------------------------------------------------------------------------------
     int nu = 0, nd = 0;
-    bool slow = false;
+    bool slow = false, m_done = false;       // m_*: result of the medium path (more than kNfK hits on a side)
+    int32_t m_bu = -1, m_bd = -1;
+    float m_best = 0.0f;
     if (tid < n && flag != NF_NOLINK) {
       uint32_t wd0, wd1, wu0, wu1;
       int td, tu;
@@ -391,7 +434,17 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
         nd = nf_test_runs(c, wd0, wd1, sArena + 8u * (uint32_t)d.up.cn, kc.dA.x, kc.dA.y, -g.x, sVecD + 8u * tid, sIdxD + 2u * tid);
         nu = nf_test_runs(c, wu0, wu1, sArena, kc.uA.x, kc.uA.y, g.y, sVecU + 8u * tid, sIdxU + 2u * tid);
       }
-      slow = !ok || nd > kNfK || nu > kNfK;
+      if (ok && (nd > kNfK || nu > kNfK)) {               // dense region: decide now, while the staged runs are here
+        int iu, id;
+        if (nf_medium(c, wu0, wu1, wd0, wd1, sArena, sArena + 8u * (uint32_t)d.up.cn, kc.uA, kc.dA, g, m_best, iu, id)) {
+          m_done = true;
+          if (iu >= 0) { m_bu = iu + d.up.c0; m_bd = id + d.dn.c0; }
+        } else {
+          ok = false;                                       // exact tie: global slow path
+        }
+        nu = 0; nd = 0;
+      }
+      slow = !ok;
       if (slow) { nu = 0; nd = 0; }
       if (nu > 0 && nd > 0) atomicAdd(&hist[nd], nu);
     }
@@ -409,7 +462,7 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
       }
       if (nu > 0 && nd > 0) {
         const int slot = above + atomicAdd(&cnt[nd], nu);
-        const uint32_t code = (uint32_t)tid | (uint32_t)nd << 11;
+        const uint32_t code = (uint32_t)tid | (uint32_t)nd << 12;
 #pragma unroll 1
         for (int k = 0; k < nu; ++k) S.items[slot + k] = (uint16_t)(code | (uint32_t)k << 8);
       }
@@ -421,8 +474,8 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     for (int i = tid; i < n_items; i += kNfThreads) {
       const uint32_t item = S.items[i];
       const uint32_t col = 8u * (item & 255u);
-      const uint32_t pa = sVecU + ((item >> 8) & 7u) * kVecRow + col;
-      const int ndd = (int)(item >> 11);
+      const uint32_t pa = sVecU + ((item >> 8) & 15u) * kVecRow + col;
+      const int ndd = (int)(item >> 12);
       const float2 a = lds_f2(pa);
       uint32_t pb = sVecD + col;
       float best = __int_as_float(0x7f800000);
@@ -440,8 +493,8 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     __syncthreads();                                          // (3) item results complete
     // ---- phase C: minimum over the cluster's items, cut, stores -----------------------------------------
     if (tid < n) {
-      int32_t bu = -1, bd = -1;
-      float best = 0.0f;
+      int32_t bu = m_bu, bd = m_bd;
+      float best = m_best;
       if (nu > 0 && nd > 0) {
         best = __int_as_float(0x7f800000);
         int bk = 0, bcode = 0, tie = 0;
