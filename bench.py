@@ -280,9 +280,13 @@ def run_tpcca(args):
             trk.load_clusters(s, a, b, c)
         trk.run()
         out = 0
+        early = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START          # ready after S4: copied while S5 runs
         for s in range(tf.n_sectors):
-            v = trk.get_tracks_view(s, B.MEM_HOST, what)
-            out += 12 * v.n_clusters + 4 * v.n_start + 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
+            v = trk.get_tracks_view(s, B.MEM_HOST, early)
+            out += 12 * v.n_clusters + 4 * v.n_start
+        for s in range(tf.n_sectors):
+            v = trk.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS)
+            out += 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
         d2h = int(out)
 
     e2e_steps = max(1, min(args.steps, args.e2e_steps))

@@ -179,11 +179,14 @@ int tpcca_run(tpcca_ctx *ctx, uint32_t stage_mask);
  * TPCCA_E_WORKSPACE) or TPCCA_E_CUDA. */
 int tpcca_sync(tpcca_ctx *ctx);
 
-/* Outputs of one sector (BASELINE.json:5 "links and fitted tracks out").  Synchronises the
- * stream.  mem_space: TPCCA_MEM_DEVICE (pointers into the workspace, no copy) or TPCCA_MEM_HOST
- * (asynchronous D2H copies on the context's stream into a context-owned PINNED host arena, then
- * one synchronise; par/cov are packed with trk_stride = n_tracks).  `what` selects the output
- * groups (TPCCA_OUT_*); groups not selected, or whose stage was not run, are NULL.  Counts are
+/* Outputs of one sector (BASELINE.json:5 "links and fitted tracks out").
+ * mem_space: TPCCA_MEM_DEVICE (pointers into the workspace, no copy; synchronises the stream) or
+ * TPCCA_MEM_HOST (asynchronous D2H copies on a copy stream owned by the context into a context-owned
+ * PINNED host arena, then one synchronise of that copy stream; par/cov are packed with trk_stride =
+ * n_tracks).  `what` selects the output groups (TPCCA_OUT_*); groups not selected, or whose stage was not
+ * run, are NULL.  A HOST call waits only for the last stage whose outputs it asks for: asking for
+ * ORDER | LINKS | START while S5 of the same tpcca_run is still running copies them concurrently with S5
+ * (n_tracks / n_hits are then reported as 0; ask for TPCCA_OUT_TRACKS afterwards).  The other counts are
  * always filled.  Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
 int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, uint32_t what, tpcca_tracks_view *out);
 

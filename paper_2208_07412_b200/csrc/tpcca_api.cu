@@ -136,6 +136,7 @@ struct tpcca_ctx {
   int nf_blocks_per_sm = 3;
   NfTable nftab{};                    // S2 per-row constants, passed to k_neighbours by value (constant bank)
   cudaStream_t stream = nullptr;
+  cudaStream_t copy_stream = nullptr;  // D2H copies of tpcca_get_tracks(HOST): they wait only for the stage that made the data
   char* ws = nullptr;
   size_t ws_bytes = 0;
   int64_t N = 0, CS = 0;
@@ -183,6 +184,28 @@ int set_err(tpcca_ctx* c, int code, const char* fmt, ...) {
     cudaError_t e_ = (call);                                                                    \
     if (e_ != cudaSuccess) return set_err((c), TPCCA_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
+
+int fetch_status(tpcca_ctx* c);
+
+int status_errors(tpcca_ctx* c) {
+  if (c->status.err_range) return set_err(c, TPCCA_E_RANGE, "a cluster has row >= n_rows (%d)", c->nr);
+  if (c->status.err_capacity)
+    return set_err(c, TPCCA_E_WORKSPACE, "start-hit capacity exceeded: %d start hits > max_start_hits %lld",
+                   c->status.n_start, (long long)c->CS);
+  return TPCCA_OK;
+}
+
+// Device status as of the end of stage `stage` (1..5) of the last run, without waiting for later stages:
+// the copy stream waits for that stage's event only.  The start-hit fields are final after S4, the track
+// fields after S5.
+int fetch_status_after(tpcca_ctx* c, int stage) {
+  if (c->run_count == 0) return fetch_status(c);
+  const int k = (int)((c->run_count - 1) % tpcca_ctx::kRing);
+  CU(c, cudaStreamWaitEvent(c->copy_stream, c->ev[k][stage], 0));
+  CU(c, cudaMemcpyAsync(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost, c->copy_stream));
+  CU(c, cudaStreamSynchronize(c->copy_stream));
+  return status_errors(c);
+}
 
 int fetch_status(tpcca_ctx* c) {
   CU(c, cudaStreamSynchronize(c->stream));
@@ -308,6 +331,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   }
   cudaError_t e1 = cudaMemcpyAsync(c->at<DevTables>(L.tables), &t, sizeof t, cudaMemcpyHostToDevice, c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
+  if (e1 == cudaSuccess) e1 = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
     for (int i = 0; i < 6 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
@@ -588,14 +612,23 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
   if (mem_space != TPCCA_MEM_HOST && mem_space != TPCCA_MEM_DEVICE) return set_err(c, TPCCA_E_ARG, "bad mem_space");
   if (!c->done_mask || !c->desc_valid) return set_err(c, TPCCA_E_STATE, "nothing was run");
-  int rc = fetch_status(c);
+  const bool host = mem_space == TPCCA_MEM_HOST;
+  // HOST copies wait only for the last stage whose outputs are asked for (so that the links of a time
+  // frame can travel while S5 still runs); the track counts are filled once S5 is covered.
+  int need_stage = 1;
+  if (what & TPCCA_OUT_LINKS_RAW) need_stage = 2;
+  if (what & TPCCA_OUT_LINKS) need_stage = 3;
+  if (what & TPCCA_OUT_START) need_stage = 4;
+  if (what & TPCCA_OUT_TRACKS) need_stage = 5;
+  while (need_stage > 1 && !(c->done_mask & (1u << (need_stage - 1)))) --need_stage;     // stages that were never run deliver nothing
+  const bool partial = host && need_stage < 5 && (c->done_mask & TPCCA_STAGE_TRACKLETS) && c->run_count > 0;
+  int rc = partial ? fetch_status_after(c, std::max(need_stage, (c->done_mask & TPCCA_STAGE_START) ? 4 : need_stage)) : fetch_status(c);
   if (rc) return rc;
   memset(v, 0, sizeof *v);
   const Layout& L = c->L;
   const DevStatus& S = c->status;
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
-  const uint32_t done = c->done_mask;
-  const bool host = mem_space == TPCCA_MEM_HOST;
+  const uint32_t done = partial ? (c->done_mask & ~TPCCA_STAGE_TRACKLETS) : c->done_mask;
   v->n_clusters = n;
   v->n_bins = c->nb;
   int64_t s0 = 0, s1 = 0, t0 = 0, nt = 0, h0 = 0, h1 = 0;
@@ -656,28 +689,22 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
     if (e != cudaSuccess) return set_err(c, TPCCA_E_CUDA, "cudaMallocHost(%zu) failed: %s", want, cudaGetErrorString(e));
     c->arena_bytes = want;
   }
+  // the copies run on the context's copy stream: it has already waited for the stage that made the
+  // data (partial) or the whole run is complete (fetch_status synchronised the main stream)
+  cudaStream_t cs = c->copy_stream;
   size_t cur = 0;
   for (auto& it : items) {
     char* dst = c->arena + cur;
     if (it.bytes) {
-      if (it.planes == 1) CU(c, cudaMemcpyAsync(dst, it.src, it.bytes, cudaMemcpyDeviceToHost, c->stream));
-      else CU(c, cudaMemcpy2DAsync(dst, it.bytes, it.src, 4 * (size_t)c->CS, it.bytes, it.planes, cudaMemcpyDeviceToHost, c->stream));
+      if (it.planes == 1) CU(c, cudaMemcpyAsync(dst, it.src, it.bytes, cudaMemcpyDeviceToHost, cs));
+      else CU(c, cudaMemcpy2DAsync(dst, it.bytes, it.src, 4 * (size_t)c->CS, it.bytes, it.planes, cudaMemcpyDeviceToHost, cs));
     }
     *it.dst = dst;
     cur += align_up(it.bytes * it.planes + 4);
   }
-  CU(c, cudaStreamSynchronize(c->stream));
+  CU(c, cudaStreamSynchronize(cs));
   return TPCCA_OK;
 }
-
-#ifdef TPCCA_NF_STATS
-int tpcca_debug_nf_hist(unsigned long long* out, int reset) {
-  cudaDeviceSynchronize();
-  if (out) cudaMemcpyFromSymbol(out, g_nf_hist, sizeof(unsigned long long) * 256);
-  if (reset) { static unsigned long long z[256]; cudaMemcpyToSymbol(g_nf_hist, z, sizeof z); }
-  return 0;
-}
-#endif
 
 void tpcca_destroy(tpcca_ctx* c) {
   if (!c) return;
@@ -685,6 +712,7 @@ void tpcca_destroy(tpcca_ctx* c) {
   for (int k = 0; k < tpcca_ctx::kRing; ++k)
     for (int i = 0; i < 6; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
   if (c->arena) cudaFreeHost(c->arena);
+  if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
   delete c;
 }
 

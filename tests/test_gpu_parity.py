@@ -290,6 +290,24 @@ def test_device_inputs_and_borrow(pkg, cfg0):
         trk.close()
 
 
+def test_early_fetch_while_s5_runs(pkg, cfg1_small):
+    """HOST fetch of the S1-S4 outputs right after tpcca_run (it waits for S4 only and overlaps S5) delivers
+    the same arrays as the fetch after the whole run."""
+    from paper_2208_07412_b200 import binding as B
+    tf = cfg1_small
+    trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+    trk.load_timeframe(tf)
+    trk.run()
+    early = [trk.get_tracks(s, B.OUT_ORDER | B.OUT_LINKS | B.OUT_START) for s in (0, 7, 35)]
+    full = [trk.get_tracks(s) for s in (0, 7, 35)]
+    for a, b in zip(early, full):
+        assert a.x_ref is None and a.n_tracks == 0 and b.n_tracks > 0
+        for f in ("order", "link_up", "link_dn", "start_hit"):
+            assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    compare_timeframe(trk, tf, Oracle(tf.params), sectors=(0, 7, 35))
+    trk.close()
+
+
 def test_config1_full_size(pkg):
     """BASELINE.json config 1 at full size (10k tracks, ~1.5M clusters): every sector, every output."""
     tf = tpcsynth.generate(1)
