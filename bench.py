@@ -269,37 +269,71 @@ def run_tpcca(args):
     s5_tops = flops / (stage_ms[4] * 1e-3) / 1e12
 
     # ---- end to end: host buffers in, host buffers out, through the public API ---------------------
-    what = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START | B.OUT_TRACKS
     h2d = int(10 * N)
-    d2h = 0
 
-    def e2e_step():
-        nonlocal d2h
-        trk.reset()
+    def e2e_step(t):
+        """One whole step through the public API: pinned HOST inputs in, HOST outputs out."""
+        t.reset()
         for s, (a, b, c) in enumerate(host):
-            trk.load_clusters(s, a, b, c)
-        trk.run()
+            t.load_clusters(s, a, b, c)
+        t.run()
         out = 0
         early = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START          # ready after S4: copied while S5 runs
         for s in range(tf.n_sectors):
-            v = trk.get_tracks_view(s, B.MEM_HOST, early)
+            v = t.get_tracks_view(s, B.MEM_HOST, early)
             out += 12 * v.n_clusters + 4 * v.n_start
         for s in range(tf.n_sectors):
-            v = trk.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS)
+            v = t.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS)
             out += 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
-        d2h = int(out)
+        return int(out)
 
+    # (a) serial: one context, step after step
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    e2e_step()   # warm-up: grows the pinned arena
+    d2h = e2e_step(trk)   # warm-up: grows the pinned arena
     barrier()
     ev0.record()
     for _ in range(e2e_steps):
-        e2e_step()
+        e2e_step(trk)
     ev1.record()
     torch.cuda.synchronize()
     barrier()
-    e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
-    e2e_value = n_all * e2e_steps / (e2e_ms * 1e-3)
+    e2e_serial_ms = max_over_ranks(ev0.elapsed_time(ev1))
+
+    # (b) streaming (the EPN operating mode, PAPER.md:21/29: time frames follow each other): two contexts on two
+    # streams, each step still does its own H2D, S1-S5 and D2H, but the copies of one time frame overlap the
+    # kernels of the other (PCIe is full duplex).  One host thread per context (ctypes releases the GIL).
+    e2e_ms, e2e_n = e2e_serial_ms, e2e_steps
+    e2e_mode = "serial, 1 context"
+    if not args.no_streaming:
+        side = torch.cuda.Stream(device=dev)
+        trk2 = pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local, stream=side)
+        e2e_step(trk2)
+        torch.cuda.synchronize()
+        per = e2e_steps
+
+        def worker(t, delay):
+            time.sleep(delay)              # the second context starts half a step later: its copies meet the other's kernels
+            for _ in range(per):
+                e2e_step(t)
+
+        barrier()
+        ev0.record()
+        th = [threading.Thread(target=worker, args=(t, dl)) for t, dl in ((trk, 0.0), (trk2, 0.5e-3 * e2e_serial_ms / e2e_steps))]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        torch.cuda.current_stream().wait_stream(side)
+        ev1.record()
+        torch.cuda.synchronize()
+        barrier()
+        e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
+        e2e_n = 2 * per
+        e2e_mode = "streaming, 2 contexts on 2 streams"
+        trk2.close()
+    e2e_value = n_all * e2e_n / (e2e_ms * 1e-3)
+    e2e_steps_serial = e2e_steps
+    e2e_steps = e2e_n
 
     # ---- CPU baseline = the oracle on one core over sector 0 (rank 0, N = 1 only); parity check ----
     cpu = None
@@ -343,7 +377,9 @@ def run_tpcca(args):
                                    unit="Tfp32op/s (no FMA)", frac=s5_tops / alu_peak, traffic=None, flops=flops,
                                    work=work),
             e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
-                     ms_per_step=e2e_ms / e2e_steps),
+                     ms_per_step=e2e_ms / e2e_steps, mode=e2e_mode,
+                     serial_value=n_all * e2e_steps_serial / (e2e_serial_ms * 1e-3),
+                     serial_ms_per_step=e2e_serial_ms / e2e_steps_serial),
             gpu_launches=int(launches_per_step * args.steps),
             clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1),
         )
@@ -366,6 +402,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-z-frac", type=float, default=0.25)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "tpcca":
         args.warmup = 3        # timing rule: W >= 3

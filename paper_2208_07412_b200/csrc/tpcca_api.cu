@@ -208,8 +208,9 @@ int fetch_status_after(tpcca_ctx* c, int stage) {
 }
 
 int fetch_status(tpcca_ctx* c) {
+  // (never the legacy default stream: a synchronous cudaMemcpy would wait for every other context's work)
+  CU(c, cudaMemcpyAsync(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
-  CU(c, cudaMemcpy(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost));
   c->status_valid = true;
   if (c->status.err_range) return set_err(c, TPCCA_E_RANGE, "a cluster has row >= n_rows (%d)", c->nr);
   if (c->status.err_capacity)
