@@ -653,19 +653,27 @@ k_sh_bucket_counts(const DevTables* __restrict__ T, const DevStatus* __restrict_
   if (threadIdx.x == 0) blk_cnt[blockIdx.x] = make_int2(total, 0);
 }
 
+// perm[j] = work record of the j-th tracklet in processing order: (slot, start row | sector << 16, start hit, 0).
+// One 16-byte load gives the S5 kernels everything a refill needs (no row / sector search, no second
+// dependent load of start_hit): the row of a bucket's start hits is the bucket's row.
 __global__ void __launch_bounds__(256)
-k_sh_perm(const DevTables* __restrict__ T, const int32_t* __restrict__ sh_first, const int32_t* __restrict__ cnt,
-          const longlong2* __restrict__ blk_pre, int32_t* __restrict__ perm) {
+k_sh_perm(const DevTables* __restrict__ T, const int32_t* __restrict__ zorder, const int32_t* __restrict__ start_hit,
+          const int32_t* __restrict__ sh_first, const int32_t* __restrict__ cnt,
+          const longlong2* __restrict__ blk_pre, int4* __restrict__ perm) {
   __shared__ int ws[33];
-  const int n = T->n_sectors * T->n_cb;
+  const int ncb = T->n_cb;
+  const int n = T->n_sectors * ncb;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int c = i < n ? cnt[i] : 0;
   int total;
   const int ex = block_exclusive_scan<int>(c, ws, total);
-  if (i >= n) return;
+  if (i >= n || c == 0) return;
+  const int s = i / ncb, j = i - s * ncb;
+  int r, k;
+  cb_row_slab(T, zorder[j], r, k);
   const int a = sh_first[i];
-  int32_t* o = perm + blk_pre[blockIdx.x].x + ex;
-  for (int k = 0; k < c; ++k) o[k] = a + k;
+  int4* o = perm + blk_pre[blockIdx.x].x + ex;
+  for (int q = 0; q < c; ++q) o[q] = make_int4(a + q, r | (s << 16), start_hit[a + q], 0);
 }
 
 }  // namespace tpcca

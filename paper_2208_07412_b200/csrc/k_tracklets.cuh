@@ -151,8 +151,9 @@ __device__ __forceinline__ void kf_update(KF& s, float ym, float zm, const KFCon
 }
 
 // slot-space scratch of S5 (SoA with stride cap): 24 float planes + 4 int planes
-constexpr int kTrkF = 24;   // x_ref, z_ref, p0..p4, c[15], chi2, (pad)
-constexpr int kTrkI = 4;    // n_hits (0 = rejected), n_fit, first_row, last_row
+// slot-space scratch of S5: one record of kTrkV 16-byte vectors per slot (written by the lane that completes the
+// tracklet with 128-bit stores, read by k_track_gather) + the n_hits plane (0 = rejected) the scans read
+constexpr int kTrkV = 7;    // (n_fit, first_row, last_row, -) (x_ref, z_ref, p0, p1) (p2, p3, p4, c00) ... (c43, c44, chi2, -)
 
 constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 #ifndef TPCCA_S5_BPS
@@ -253,8 +254,10 @@ __device__ __noinline__ int search_exact(float p0, float p1, float z_ref, float 
 // lanes share a warp: link followers (no search), extrapolators (a search every row) and refitters
 // no longer wait for each other's code.
 enum { MODE_A = 1, MODE_B = 2, MODE_C1 = 3, MODE_C2 = 4 };
-constexpr int kHsF = 23;    // x, p0..p4, c[15], chi2, z_ref
-constexpr int kHsI = 10;    // n, r, cur, top, top_hit, gap, n_hits, first, r0, phase
+// parked tracklet: one record of kHsV 16-byte vectors, indexed by the work index; a tracklet bound for phase C
+// only fills the first four: (x, p0, p1, p2) (p3, p4, z_ref, phase) (top, top_hit, n_hits, first) (r0, n, r, cur)
+// (gap, c00, c10, c11) (c20, c21, c22, c30) (c31, c32, c33, c40) (c41, c42, c43, c44) (chi2, -, -, -)
+constexpr int kHsV = 9;
 
 template <int MODE>
 __global__ void __launch_bounds__(kS5Threads, MODE == MODE_A ? kS5BlocksPerSMA : kS5BlocksPerSM)
@@ -262,13 +265,11 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             DevStatus* __restrict__ st, const S5Params P, const float2* __restrict__ syz,
             const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
             const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
-            const int32_t* __restrict__ start_hit, const int32_t* __restrict__ perm, int32_t cap,
-            int32_t* __restrict__ hits /*[cap][n_rows]*/, float* __restrict__ trk_f /*[kTrkF][cap]*/,
-            int32_t* __restrict__ trk_i /*[kTrkI][cap]*/, float* __restrict__ hs_f /*[kHsF][cap]*/,
-            int32_t* __restrict__ hs_i /*[kHsI][cap]*/) {
+            const int32_t* __restrict__ start_hit, const int4* __restrict__ perm, int32_t cap,
+            int32_t* __restrict__ hits /*[cap][n_rows]*/, float4* __restrict__ trk_v /*[cap][kTrkV]*/,
+            int32_t* __restrict__ trk_n /*[cap]*/, float4* __restrict__ hs /*[cap][kHsV]*/) {
   __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];
   __shared__ int32_t t_nyh[kMaxRows], t_nzh[kMaxRows], t_ny[kMaxRows], t_base[kMaxRows];
-  __shared__ int s_start_off[kMaxSectors + 1];
   __shared__ int s_sec_off[kMaxSectors + 1];
   __shared__ float s_snap[kSnapF][kS5Threads];
   const int n_rows = P.n_rows, ns = P.n_sectors;
@@ -276,7 +277,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     t_x[r] = T->row_x[r]; t_ylo[r] = T->y_lo[r]; t_iby[r] = T->inv_by[r]; t_nyh[r] = T->ny[r] - 1;
     t_ibz[r] = T->inv_bz[r]; t_nzh[r] = T->nz[r] - 1; t_ny[r] = T->ny[r]; t_base[r] = T->bin_base[r];
   }
-  for (int i = threadIdx.x; i <= ns; i += blockDim.x) { s_start_off[i] = st->start_off[i]; s_sec_off[i] = sec[i].off; }
+  for (int i = threadIdx.x; i <= ns; i += blockDim.x) s_sec_off[i] = sec[i].off;
   __syncthreads();
   if (st->err_capacity) return;
   const int n_start = st->n_start;
@@ -318,34 +319,39 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   auto finish = [&]() {
     if (fresh) { save_snap(); snap_n = f.n; saved = true; }
     const bool accept = (n_hits >= P.min_hits) && saved;
-    trk_i[0 * (size_t)cap + slot] = accept ? n_hits : 0;
+    trk_n[slot] = accept ? n_hits : 0;
     if (accept) {
-      trk_i[1 * (size_t)cap + slot] = snap_n;
-      trk_i[2 * (size_t)cap + slot] = first;
-      trk_i[3 * (size_t)cap + slot] = top;
-      float* o = trk_f + slot;
-      const size_t cs = (size_t)cap;
-      o[0 * cs] = s_snap[0][tid]; o[1 * cs] = z_ref;
-#pragma unroll
-      for (int k = 1; k < kSnapF; ++k) o[(k + 1) * cs] = s_snap[k][tid];
+      float4* o = trk_v + (size_t)slot * kTrkV;
+      const float* sn = &s_snap[0][tid];
+      auto S = [&](int k) { return sn[k * kS5Threads]; };
+      o[0] = make_float4(__int_as_float(snap_n), __int_as_float(first), __int_as_float(top), 0.f);
+      o[1] = make_float4(S(0), z_ref, S(1), S(2));
+      o[2] = make_float4(S(3), S(4), S(5), S(6));
+      o[3] = make_float4(S(7), S(8), S(9), S(10));
+      o[4] = make_float4(S(11), S(12), S(13), S(14));
+      o[5] = make_float4(S(15), S(16), S(17), S(18));
+      o[6] = make_float4(S(19), S(20), S(21), 0.f);
     }
     phase = PH_IDLE;
   };
-  auto to_phase_c = [&]() {
-    phase = PH_C; kf_reset_cov(f, K); gap = 0; r = top; cur = top_hit; fresh = false; saved = false;
-  };
 
-  // park the tracklet for the next kernel and go idle
+  // park the tracklet for the next kernel and go idle.  A tracklet bound for phase C carries only x, p
+  // and z_ref: the covariance reset, r = top, cur = top_hit and gap = 0 of the phase change are applied by
+  // the phase-C1 kernel when it loads the tracklet.
   auto park = [&]() {
-    const size_t cs = (size_t)cap;
-    float* o = hs_f + wi;
-    o[0 * cs] = f.x; o[1 * cs] = f.p0; o[2 * cs] = f.p1; o[3 * cs] = f.p2; o[4 * cs] = f.p3; o[5 * cs] = f.p4;
-    o[6 * cs] = f.c00; o[7 * cs] = f.c10; o[8 * cs] = f.c11; o[9 * cs] = f.c20; o[10 * cs] = f.c21; o[11 * cs] = f.c22;
-    o[12 * cs] = f.c30; o[13 * cs] = f.c31; o[14 * cs] = f.c32; o[15 * cs] = f.c33; o[16 * cs] = f.c40; o[17 * cs] = f.c41;
-    o[18 * cs] = f.c42; o[19 * cs] = f.c43; o[20 * cs] = f.c44; o[21 * cs] = f.chi2; o[22 * cs] = z_ref;
-    int32_t* q = hs_i + wi;
-    q[0 * cs] = f.n; q[1 * cs] = r; q[2 * cs] = cur; q[3 * cs] = top; q[4 * cs] = top_hit; q[5 * cs] = gap;
-    q[6 * cs] = n_hits; q[7 * cs] = first; q[8 * cs] = r0; q[9 * cs] = phase;
+    float4* o = hs + (size_t)wi * kHsV;
+    auto I = [](int v) { return __int_as_float(v); };
+    o[0] = make_float4(f.x, f.p0, f.p1, f.p2);
+    o[1] = make_float4(f.p3, f.p4, z_ref, I(phase));
+    o[2] = make_float4(I(top), I(top_hit), I(n_hits), I(first));
+    o[3] = make_float4(I(r0), I(f.n), I(r), I(cur));
+    if (phase != PH_C) {
+      o[4] = make_float4(I(gap), f.c00, f.c10, f.c11);
+      o[5] = make_float4(f.c20, f.c21, f.c22, f.c30);
+      o[6] = make_float4(f.c31, f.c32, f.c33, f.c40);
+      o[7] = make_float4(f.c41, f.c42, f.c43, f.c44);
+      o[8] = make_float4(f.chi2, 0.f, 0.f, 0.f);
+    }
     phase = PH_IDLE;
   };
 
@@ -363,19 +369,14 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
         const int my_w = base + __popc(idle & ((1u << lane) - 1u));
         if (my_w < n_start) {
           wi = my_w;
-          slot = __ldg(&perm[my_w]);
-          int s = 0;
-          {
-            int lo = 0, hi = ns - 1;
-            while (lo < hi) { int mid = (lo + hi + 1) >> 1; if (s_start_off[mid] <= slot) lo = mid; else hi = mid - 1; }
-            s = lo;
-          }
+          const int4 pr = __ldg(&perm[my_w]);   // slot, start row | sector << 16, start hit
+          slot = pr.x;
+          const int s = pr.y >> 16;
           off = s_sec_off[s];
           bs_off = (uint32_t)s * nbp1;
           if (MODE == MODE_A) {
-            const int32_t* rs = row_start + s * (n_rows + 1);
-            const int c0 = start_hit[slot];
-            r0 = row_search(rs, n_rows, c0);
+            const int c0 = pr.z;
+            r0 = pr.y & 0xffff;
             const int c1 = __ldg(&link_up[off + c0]);
             const float2 h0 = __ldg(&syz[off + c0]), h1 = __ldg(&syz[off + c1]);
             z_ref = h0.y;
@@ -389,17 +390,24 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             phase = PH_A; r = r0; cur = c0; top = r0; top_hit = c0; gap = 0; n_hits = 0; first = r0;
             fresh = false; saved = false;
           } else {
-            const size_t cs = (size_t)cap;
-            const int32_t* q = hs_i + wi;
-            const int ph = q[9 * cs];
+            const float4* o = hs + (size_t)wi * kHsV;
+            auto I = [](float v) { return __float_as_int(v); };
+            const float4 v0 = o[0], v1 = o[1], v2 = o[2], v3 = o[3];
+            float4 v4, v5, v6, v7, v8;
+            if (MODE != MODE_C1) { v4 = o[4]; v5 = o[5]; v6 = o[6]; v7 = o[7]; v8 = o[8]; }   // issued before the phase test
+            const int ph = I(v1.w);
             if (ph == (MODE == MODE_B ? PH_B : (MODE == MODE_C1 ? PH_C : PH_C2))) {   // others are not this kernel's
-              const float* o = hs_f + wi;
-              f.x = o[0 * cs]; f.p0 = o[1 * cs]; f.p1 = o[2 * cs]; f.p2 = o[3 * cs]; f.p3 = o[4 * cs]; f.p4 = o[5 * cs];
-              f.c00 = o[6 * cs]; f.c10 = o[7 * cs]; f.c11 = o[8 * cs]; f.c20 = o[9 * cs]; f.c21 = o[10 * cs]; f.c22 = o[11 * cs];
-              f.c30 = o[12 * cs]; f.c31 = o[13 * cs]; f.c32 = o[14 * cs]; f.c33 = o[15 * cs]; f.c40 = o[16 * cs]; f.c41 = o[17 * cs];
-              f.c42 = o[18 * cs]; f.c43 = o[19 * cs]; f.c44 = o[20 * cs]; f.chi2 = o[21 * cs]; z_ref = o[22 * cs];
-              f.n = q[0 * cs]; r = q[1 * cs]; cur = q[2 * cs]; top = q[3 * cs]; top_hit = q[4 * cs]; gap = q[5 * cs];
-              n_hits = q[6 * cs]; first = q[7 * cs]; r0 = q[8 * cs]; phase = (MODE == MODE_C2) ? (int)PH_C : ph;
+              f.x = v0.x; f.p0 = v0.y; f.p1 = v0.z; f.p2 = v0.w; f.p3 = v1.x; f.p4 = v1.y; z_ref = v1.z;
+              top = I(v2.x); top_hit = I(v2.y); n_hits = I(v2.z); first = I(v2.w); r0 = I(v3.x);
+              if (MODE == MODE_C1) {          // the phase change A/B -> C is completed here
+                kf_reset_cov(f, K); gap = 0; r = top; cur = top_hit;
+              } else {
+                f.n = I(v3.y); r = I(v3.z); cur = I(v3.w); gap = I(v4.x);
+                f.c00 = v4.y; f.c10 = v4.z; f.c11 = v4.w; f.c20 = v5.x; f.c21 = v5.y; f.c22 = v5.z; f.c30 = v5.w;
+                f.c31 = v6.x; f.c32 = v6.y; f.c33 = v6.z; f.c40 = v6.w; f.c41 = v7.x; f.c42 = v7.y; f.c43 = v7.z; f.c44 = v7.w;
+                f.chi2 = v8.x;
+              }
+              phase = (MODE == MODE_C2) ? (int)PH_C : ph;
               // C1 always hands over right after the update on the start row: running state == snapshot
               fresh = (MODE == MODE_C2); saved = false;
             }
@@ -568,10 +576,14 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       if (phase == PH_B && r >= n_rows) ev = EV_TO_C;
       if (phase == PH_C && r < 0) ev = EV_FINISH;
     }
-    if (ev == EV_TO_C) to_phase_c();
-    else if (ev == EV_FINISH) finish();
-    if (MODE == MODE_A && (phase == PH_B || phase == PH_C)) park();
-    if (MODE == MODE_B && phase == PH_C) park();
+    // A tracklet that leaves the kernel's phase is parked (the record is a few 128-bit stores), a complete one
+    // is emitted; either way the lane goes idle.
+    if (ev == EV_TO_C) {                  // phases A / B only, i.e. MODE_A / MODE_B: the tracklet leaves the kernel
+      phase = PH_C; park();               // (covariance reset, r, cur, gap: applied by MODE_C1 on load)
+    } else if (ev == EV_FINISH) {
+      finish();
+    }
+    if (MODE == MODE_A && phase == PH_B) park();
     if (MODE == MODE_C1 && phase == PH_C && r < r0) { phase = PH_C2; park(); }
     // ---- prefetch hint for the next row's search (kernels that search every row) ---------------------
     // Straight-line guess of the next prediction; only the cache lines of the bin_start entries around
@@ -603,11 +615,11 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
 
 // ---- K5b: per-tile (1024 slots) sums of (accepted, n_hits) ------------------------------------
 __global__ void __launch_bounds__(1024)
-k_track_tile_sums(const DevStatus* __restrict__ st, const int32_t* __restrict__ trk_i, int2* __restrict__ tile_cnt) {
+k_track_tile_sums(const DevStatus* __restrict__ st, const int32_t* __restrict__ trk_n, int2* __restrict__ tile_cnt) {
   __shared__ int ws[33];
   const int n_start = st->err_capacity ? 0 : st->n_start;
   const int slot = blockIdx.x * 1024 + threadIdx.x;
-  const int nh = slot < n_start ? trk_i[slot] : 0;
+  const int nh = slot < n_start ? trk_n[slot] : 0;
   int ta, tb;
   block_exclusive_scan<int>(nh > 0 ? 1 : 0, ws, ta);
   block_exclusive_scan<int>(nh, ws, tb);
@@ -616,7 +628,7 @@ k_track_tile_sums(const DevStatus* __restrict__ st, const int32_t* __restrict__ 
 
 // ---- K5c': sector bases of the track table and of the hit CSR ---------------------------------
 __global__ void k_track_sector_bases(const DevTables* __restrict__ T, DevStatus* __restrict__ st,
-                                     const int32_t* __restrict__ trk_i, const longlong2* __restrict__ tile_off,
+                                     const int32_t* __restrict__ trk_n, const longlong2* __restrict__ tile_off,
                                      const int64_t* __restrict__ tot) {
   const int ns = T->n_sectors;
   const int s = threadIdx.x;
@@ -626,7 +638,7 @@ __global__ void k_track_sector_bases(const DevTables* __restrict__ T, DevStatus*
   if (slot >= n_start) { st->trk_off[s] = (int32_t)tot[0]; st->hit_off[s] = tot[1]; return; }
   const int t = slot >> 10;
   long long a = tile_off[t].x, b = tile_off[t].y;
-  for (int q = t << 10; q < slot; ++q) { const int nh = trk_i[q]; a += nh > 0; b += nh; }
+  for (int q = t << 10; q < slot; ++q) { const int nh = trk_n[q]; a += nh > 0; b += nh; }
   st->trk_off[s] = (int32_t)a;
   st->hit_off[s] = b;
 }
@@ -640,13 +652,13 @@ struct TrackOut {
 __global__ void __launch_bounds__(1024)
 k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st,
                const int32_t* __restrict__ start_hit, int32_t cap, const int32_t* __restrict__ hits,
-               const float* __restrict__ trk_f, const int32_t* __restrict__ trk_i,
+               const float4* __restrict__ trk_v, const int32_t* __restrict__ trk_n,
                const longlong2* __restrict__ tile_off, TrackOut o) {
   __shared__ int ws[33];
   const int ns = T->n_sectors, n_rows_g = T->n_rows;
   const int n_start = st->err_capacity ? 0 : st->n_start;
   const int slot = blockIdx.x * 1024 + threadIdx.x;
-  const int nh = slot < n_start ? trk_i[slot] : 0;
+  const int nh = slot < n_start ? trk_n[slot] : 0;
   int ta, tb;
   const int ea = block_exclusive_scan<int>(nh > 0 ? 1 : 0, ws, ta);
   const int eb = block_exclusive_scan<int>(nh, ws, tb);
@@ -667,16 +679,20 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
     if (nh > 0) {
       const size_t cs = (size_t)cap;
       o.hit_offset[t + s] = (int32_t)hloc;
-      o.x_ref[t] = trk_f[0 * cs + slot];
-      o.z_ref[t] = trk_f[1 * cs + slot];
+      const float4* v = trk_v + (size_t)slot * kTrkV;
+      const float4 v0 = v[0], v1 = v[1], v2 = v[2], v3 = v[3], v4 = v[4], v5 = v[5], v6 = v[6];
+      o.x_ref[t] = v1.x;
+      o.z_ref[t] = v1.y;
+      const float par[5] = {v1.z, v1.w, v2.x, v2.y, v2.z};
+      const float cov[15] = {v2.w, v3.x, v3.y, v3.z, v3.w, v4.x, v4.y, v4.z, v4.w, v5.x, v5.y, v5.z, v5.w, v6.x, v6.y};
 #pragma unroll
-      for (int i = 0; i < 5; ++i) o.par[i * cs + t] = trk_f[(2 + i) * cs + slot];
+      for (int i = 0; i < 5; ++i) o.par[i * cs + t] = par[i];
 #pragma unroll
-      for (int i = 0; i < 15; ++i) o.cov[i * cs + t] = trk_f[(7 + i) * cs + slot];
-      o.chi2[t] = trk_f[22 * cs + slot];
+      for (int i = 0; i < 15; ++i) o.cov[i * cs + t] = cov[i];
+      o.chi2[t] = v6.z;
       o.n_hits[t] = nh;
-      o.n_fit[t] = trk_i[1 * cs + slot];
-      first = trk_i[2 * cs + slot]; last = trk_i[3 * cs + slot];
+      o.n_fit[t] = __float_as_int(v0.x);
+      first = __float_as_int(v0.y); last = __float_as_int(v0.z);
       o.first_row[t] = first;
       o.last_row[t] = last;
       o.start_hit[t] = start_hit[slot];

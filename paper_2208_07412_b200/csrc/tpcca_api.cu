@@ -72,7 +72,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.sh_cnt = take(4 * (size_t)(ns * L.n_cb));
   L.sh_blk = take(sizeof(int2) * (size_t)(ns * L.n_cb / 256 + 2));
   L.sh_pre = take(sizeof(longlong2) * (size_t)(ns * L.n_cb / 256 + 2));
-  L.perm = take(4 * (size_t)CS);
+  L.perm = take(16 * (size_t)CS);      // int4 work records of S5
   L.up_raw = take(4 * (size_t)N);
   L.dn_raw = take(4 * (size_t)N);
   L.up = take(4 * (size_t)N);
@@ -81,10 +81,10 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.tile_off = take(sizeof(longlong2) * (size_t)L.n_tiles_max);
   L.start_hit = take(4 * (size_t)CS);
   L.hits = take(4 * (size_t)(nr * CS));
-  L.trk_f = take(4 * (size_t)(kTrkF * CS));
-  L.trk_i = take(4 * (size_t)(kTrkI * CS));
-  L.hs_f = take(4 * (size_t)(kHsF * CS));
-  L.hs_i = take(4 * (size_t)(kHsI * CS));
+  L.trk_f = take(16 * (size_t)(kTrkV * CS));
+  L.trk_i = take(4 * (size_t)CS);
+  L.hs_f = take(16 * (size_t)(kHsV * CS));
+  L.hs_i = take(16);
   L.o_x_ref = take(4 * (size_t)CS);
   L.o_z_ref = take(4 * (size_t)CS);
   L.o_chi2 = take(4 * (size_t)CS);
@@ -514,7 +514,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       k_sh_bucket_counts<<<nblk, 256, 0, st>>>(T, status, c->at<int32_t>(L.zorder), c->at<uint32_t>(L.cb_start), start_hit, cap,
                                                c->at<int32_t>(L.sh_first), shc, blc);
       k_scan_pairs<<<1, 1024, 0, st>>>(blc, shp, nblk, tot + 4);
-      k_sh_perm<<<nblk, 256, 0, st>>>(T, c->at<int32_t>(L.sh_first), shc, shp, c->at<int32_t>(L.perm));
+      k_sh_perm<<<nblk, 256, 0, st>>>(T, c->at<int32_t>(L.zorder), start_hit, c->at<int32_t>(L.sh_first), shc, shp, c->at<int4>(L.perm));
       c->launches += 3;
     }
   }
@@ -526,7 +526,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     o.n_fit = c->at<int32_t>(L.o_n_fit); o.first_row = c->at<int32_t>(L.o_first); o.last_row = c->at<int32_t>(L.o_last);
     o.start_hit = c->at<int32_t>(L.o_start); o.hit_offset = c->at<int32_t>(L.o_hit_offset); o.hit_idx = c->at<int32_t>(L.o_hit_idx);
     int32_t* hits = c->at<int32_t>(L.hits);
-    float* trk_f = c->at<float>(L.trk_f);
+    float4* trk_f = c->at<float4>(L.trk_f);
     int32_t* trk_i = c->at<int32_t>(L.trk_i);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
     CU(c, cudaMemsetAsync(status->work_counter, 0, sizeof(status->work_counter), st));
@@ -538,17 +538,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     sp.win_y = t.win_y; sp.win_z = t.win_z; sp.gate = t.gate; sp.margin = t.margin; sp.grid_z_lo = t.grid_z_lo;
     sp.n_rows = t.n_rows; sp.n_sectors = t.n_sectors; sp.max_gap = t.tc_max_gap; sp.min_hits = t.tc_min_hits;
     sp.bins_per_sector = t.bins_per_sector;
-    float* hs_f = c->at<float>(L.hs_f);
-    int32_t* hs_i = c->at<int32_t>(L.hs_i);
-    const int32_t* perm = c->at<int32_t>(L.perm);
+    float4* hs_f = c->at<float4>(L.hs_f);
+    const int4* perm = c->at<int4>(L.perm);
     k_tracklets<MODE_A><<<c->sm_count * kS5BlocksPerSMA, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
     k_tracklets<MODE_B><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
     k_tracklets<MODE_C1><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
     k_tracklets<MODE_C2><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f, hs_i);
+                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
