@@ -20,6 +20,9 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 // contiguous run as well.  k_nf_plan writes one descriptor per tile; k_neighbours stages the two
 // cluster runs and the two bin_start runs of the next tile in shared memory with 1-D bulk async
 // copies (TMA, mbarrier completion) while the current tile is searched entirely in shared memory.
+#ifndef TPCCA_NF_T2
+#define TPCCA_NF_T2 2      // window-test candidates per loop trip
+#endif
 #ifndef TPCCA_NF_K
 #define TPCCA_NF_K 10
 #endif
@@ -263,19 +266,32 @@ __device__ __forceinline__ int nf_test_runs(const float2 c, uint32_t w0, uint32_
   uint32_t a = sC + 8u * (w0 & 1023u);
   const uint32_t pv_end = pv + kNfK * kVecRow;
   int n = 0;
+  // kT candidates per trip: their shared-memory loads are issued before the first test (independent chains)
+  constexpr int kT = TPCCA_NF_T2;
 #pragma unroll 1
-  for (int j = 0; j < tot; ++j, a += 8u) {
-    if (j == n0) a += o1;
-    if (j == n01) a += o2;
-    const float2 v = lds_f2(a);
-    const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
-    if (fabsf(dy) <= hy && fabsf(dz) <= hz) {
-      if (pv != pv_end) {
-        sts_f2(pv, __fmul_rn(dy, scale), __fmul_rn(dz, scale));
-        sts_u16(pi, (a - sC) >> 3);
-        pv += kVecRow; pi += kIdxRow;
+  for (int j = 0; j < tot; j += kT) {
+    uint32_t aa[kT];
+    float2 v[kT];
+#pragma unroll
+    for (int k = 0; k < kT; ++k) {
+      if (j + k == n0) a += o1;
+      if (j + k == n01) a += o2;
+      aa[k] = (k == 0 || j + k < tot) ? a : aa[0];
+      a += 8u;
+    }
+#pragma unroll
+    for (int k = 0; k < kT; ++k) v[k] = lds_f2(aa[k]);
+#pragma unroll
+    for (int k = 0; k < kT; ++k) {
+      const float dy = __fsub_rn(v[k].x, c.x), dz = __fsub_rn(v[k].y, c.y);
+      if ((k == 0 || j + k < tot) && fabsf(dy) <= hy && fabsf(dz) <= hz) {
+        if (pv != pv_end) {
+          sts_f2(pv, __fmul_rn(dy, scale), __fmul_rn(dz, scale));
+          sts_u16(pi, (aa[k] - sC) >> 3);
+          pv += kVecRow; pi += kIdxRow;
+        }
+        ++n;
       }
-      ++n;
     }
   }
   return n;
@@ -348,7 +364,7 @@ struct NfSmem {
 // barrier that ends phase A of tile i, the only phase that reads the staging buffer); per-row
 // constants come from the constant bank (NfTable is a by-value kernel parameter).
 #ifndef TPCCA_NF_BPS
-#define TPCCA_NF_BPS 6
+#define TPCCA_NF_BPS 5
 #endif
 __global__ void __launch_bounds__(kNfThreads, TPCCA_NF_BPS)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
