@@ -305,32 +305,48 @@ def run_tpcca(args):
     e2e_ms, e2e_n = e2e_serial_ms, e2e_steps
     e2e_mode = "serial, 1 context"
     if not args.no_streaming:
-        side = torch.cuda.Stream(device=dev)
-        trk2 = pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local, stream=side)
-        e2e_step(trk2)
-        torch.cuda.synchronize()
-        per = e2e_steps
-
-        def worker(t, delay):
-            time.sleep(delay)              # the second context starts half a step later: its copies meet the other's kernels
-            for _ in range(per):
+        n_ctx = max(2, args.e2e_contexts)
+        sides = [torch.cuda.Stream(device=dev) for _ in range(n_ctx - 1)]
+        extra = []
+        try:
+            for sd in sides:
+                extra.append(pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local, stream=sd))
+        except torch.OutOfMemoryError:      # the workspace of another time frame does not fit beside the first
+            for t in extra:
+                t.close()
+            extra = None
+            torch.cuda.empty_cache()
+        if extra:
+            for t in extra:
                 e2e_step(t)
+            torch.cuda.synchronize()
+            per = e2e_steps
 
-        barrier()
-        ev0.record()
-        th = [threading.Thread(target=worker, args=(t, dl)) for t, dl in ((trk, 0.0), (trk2, 0.5e-3 * e2e_serial_ms / e2e_steps))]
-        for t in th:
-            t.start()
-        for t in th:
-            t.join()
-        torch.cuda.current_stream().wait_stream(side)
-        ev1.record()
-        torch.cuda.synchronize()
-        barrier()
-        e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
-        e2e_n = 2 * per
-        e2e_mode = "streaming, 2 contexts on 2 streams"
-        trk2.close()
+            def worker(t, delay):
+                time.sleep(delay)              # the contexts start a fraction of a step apart: the copies of one meet the kernels of another
+                for _ in range(per):
+                    e2e_step(t)
+
+            barrier()
+            ev0.record()
+            step_s = 1e-3 * e2e_serial_ms / e2e_steps
+            th = [threading.Thread(target=worker, args=(t, i * step_s / n_ctx)) for i, t in enumerate([trk] + extra)]
+            for t in th:
+                t.start()
+            for t in th:
+                t.join()
+            for sd in sides:
+                torch.cuda.current_stream().wait_stream(sd)
+            ev1.record()
+            torch.cuda.synchronize()
+            barrier()
+            e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
+            e2e_n = n_ctx * per
+            e2e_mode = "streaming, %d contexts on %d streams" % (n_ctx, n_ctx)
+            for t in extra:
+                t.close()
+        else:
+            e2e_mode = "serial, 1 context (no device memory for a second time frame)"
     e2e_value = n_all * e2e_n / (e2e_ms * 1e-3)
     e2e_steps_serial = e2e_steps
     e2e_steps = e2e_n
@@ -403,6 +419,7 @@ def main():
     ap.add_argument("--ref-z-frac", type=float, default=0.25)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
+    ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "tpcca":
         args.warmup = 3        # timing rule: W >= 3
