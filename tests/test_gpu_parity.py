@@ -86,6 +86,15 @@ def test_timeframe_slice_small(pkg):
     assert rep["n_tracks"] > 300 and rep["links_differing"] == 0
 
 
+def test_timeframe_slice_dense(pkg):
+    """One orbit of the time-frame recipe at 2.75x multiplicity: the occupancy of the ~4e8-cluster footprint
+    BASELINE.json:10 names (dense windows: S2 medium / slow paths, long candidate lists in the S5 search)."""
+    tf = tpcsynth.generate(2, n_orbits=1, mult_scale=2.75, seed=220807499)
+    assert tf.n_clusters > 200_000
+    rep = check(pkg, tf)
+    assert rep["n_tracks"] > 2000 and rep["links_differing"] == 0
+
+
 def test_stage_by_stage_equals_all_at_once(pkg, cfg0):
     tf = cfg0
     a = run_gpu(pkg, tf, 0x1F)
