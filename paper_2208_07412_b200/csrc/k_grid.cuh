@@ -27,6 +27,11 @@ __device__ __forceinline__ int find_sector(int ns, int tile, F first_tile) {
   return lo;
 }
 
+// ---- zero n 32-bit words (grid-stride) ---------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_zero_words(uint32_t* __restrict__ p, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) p[i] = 0u;
+}
+
 struct GridRec { float y, z; int32_t id; int32_t pad; };   // level-1 record (16 bytes, one 128-bit store)
 
 // ---- K1a: level-1 histogram: cb_cnt[s][cb(row, bz >> kSlabShift)]++ ---------------------------------

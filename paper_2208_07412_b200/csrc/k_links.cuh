@@ -429,7 +429,7 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     while (!mbar_try_wait(&S.full, (uint32_t)(it & 1))) {}
     // ---- phase A -------------------------------------------------------------------------------
     int nu = 0, nd = 0;
-    bool slow = false, m_done = false;       // m_*: result of the medium path (more than kNfK hits on a side)
+    bool slow = false;                         // m_*: result of the medium path (more than kNfK hits on a side)
     int32_t m_bu = -1, m_bd = -1;
     float m_best = 0.0f;
     if (tid < n && flag != NF_NOLINK) {
@@ -453,7 +453,6 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
       if (ok && (nd > kNfK || nu > kNfK)) {               // dense region: decide now, while the staged runs are here
         int iu, id;
         if (nf_medium(c, wu0, wu1, wd0, wd1, sArena, sArena + 8u * (uint32_t)d.up.cn, kc.uA, kc.dA, g, m_best, iu, id)) {
-          m_done = true;
           if (iu >= 0) { m_bu = iu + d.up.c0; m_bd = id + d.dn.c0; }
         } else {
           ok = false;                                       // exact tie: global slow path

@@ -201,7 +201,9 @@ int status_errors(tpcca_ctx* c) {
 int fetch_status_after(tpcca_ctx* c, int stage) {
   if (c->run_count == 0) return fetch_status(c);
   const int k = (int)((c->run_count - 1) % tpcca_ctx::kRing);
-  CU(c, cudaStreamWaitEvent(c->copy_stream, c->ev[k][stage], 0));
+  // The wait is taken on the HOST: a copy-stream entry that waits for the event would sit in a copy-engine queue
+  // until the stage is done and hold up every copy another context has queued behind it on the same engine.
+  CU(c, cudaEventSynchronize(c->ev[k][stage]));
   CU(c, cudaMemcpyAsync(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost, c->copy_stream));
   CU(c, cudaStreamSynchronize(c->copy_stream));
   return status_errors(c);
@@ -449,13 +451,19 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   mark(0);
 
   if (mask & TPCCA_STAGE_GRID) {
-    CU(c, cudaMemsetAsync(status, 0, sizeof(DevStatus), st));
+    // (zeroing is done by kernels, not cudaMemsetAsync: a memset may be queued on a copy engine, where it waits
+    // for the kernels before it and blocks the copies of other contexts queued behind it)
+    k_zero_words<<<1, 256, 0, st>>>(reinterpret_cast<uint32_t*>(status), sizeof(DevStatus) / 4);
     uint32_t* cb_cnt = c->at<uint32_t>(L.cb_cnt);
     uint32_t* cb_start = c->at<uint32_t>(L.cb_start);
     uint32_t* cb_cur = c->at<uint32_t>(L.cb_cur);
     uint32_t* big = c->at<uint32_t>(L.big_list);
     GridRec* rec = c->at<GridRec>(L.rec);
-    CU(c, cudaMemsetAsync(cb_cnt, 0, 4 * (size_t)c->ns * (size_t)(L.n_cb + 1), st));
+    {
+      const size_t nw = (size_t)c->ns * (size_t)(L.n_cb + 1);
+      k_zero_words<<<(unsigned)std::min<size_t>((nw + 1023) / 1024, 1024), 256, 0, st>>>(cb_cnt, nw);
+      c->launches += 2;
+    }
     if (c->n_tiles256 > 0) {
       k_cb_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cnt, status);
       ++c->launches;
@@ -529,8 +537,10 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     float4* trk_f = c->at<float4>(L.trk_f);
     int32_t* trk_i = c->at<int32_t>(L.trk_i);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
-    CU(c, cudaMemsetAsync(status->work_counter, 0, sizeof(status->work_counter), st));
-    CU(c, cudaMemsetAsync(status->work, 0, sizeof(status->work), st));
+    static_assert(sizeof(status->work_counter) % 4 == 0 && sizeof(status->work) % 4 == 0, "word-sized counters");
+    k_zero_words<<<1, 32, 0, st>>>(reinterpret_cast<uint32_t*>(status->work_counter), sizeof(status->work_counter) / 4);
+    k_zero_words<<<1, 32, 0, st>>>(reinterpret_cast<uint32_t*>(status->work), sizeof(status->work) / 4);
+    c->launches += 2;
     const DevTables& t = c->tab;
     S5Params sp;
     sp.Bc = t.Bc; sp.err2_y = t.err2_y; sp.err2_z = t.err2_z; sp.max_sinphi = t.max_sinphi;
