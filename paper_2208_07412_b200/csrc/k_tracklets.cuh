@@ -263,9 +263,8 @@ template <int MODE>
 __global__ void __launch_bounds__(kS5Threads, MODE == MODE_A ? kS5BlocksPerSMA : kS5BlocksPerSM)
 k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             DevStatus* __restrict__ st, const S5Params P, const float2* __restrict__ syz,
-            const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ row_start,
-            const int32_t* __restrict__ order, const int32_t* __restrict__ link_up,
-            const int32_t* __restrict__ start_hit, const int4* __restrict__ perm, int32_t cap,
+            const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ order,
+            const int32_t* __restrict__ link_up, const int4* __restrict__ perm, int32_t cap,
             int32_t* __restrict__ hits /*[cap][n_rows]*/, float4* __restrict__ trk_v /*[cap][kTrkV]*/,
             int32_t* __restrict__ trk_n /*[cap]*/, float4* __restrict__ hs /*[cap][kHsV]*/) {
   __shared__ float t_x[kMaxRows], t_ylo[kMaxRows], t_iby[kMaxRows], t_ibz[kMaxRows];

@@ -27,7 +27,7 @@ struct Layout {
   size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_blk, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
-  size_t start_hit, hits, trk_f, trk_i, hs_f, hs_i;
+  size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
@@ -81,10 +81,9 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.tile_off = take(sizeof(longlong2) * (size_t)L.n_tiles_max);
   L.start_hit = take(4 * (size_t)CS);
   L.hits = take(4 * (size_t)(nr * CS));
-  L.trk_f = take(16 * (size_t)(kTrkV * CS));
-  L.trk_i = take(4 * (size_t)CS);
-  L.hs_f = take(16 * (size_t)(kHsV * CS));
-  L.hs_i = take(16);
+  L.trk_v = take(16 * (size_t)(kTrkV * CS));   // finished tracks: records of kTrkV 16-byte vectors
+  L.trk_n = take(4 * (size_t)CS);             // n_hits per slot (0 = rejected)
+  L.hs = take(16 * (size_t)(kHsV * CS));      // parked tracklets: records of kHsV 16-byte vectors
   L.o_x_ref = take(4 * (size_t)CS);
   L.o_z_ref = take(4 * (size_t)CS);
   L.o_chi2 = take(4 * (size_t)CS);
@@ -534,8 +533,8 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     o.n_fit = c->at<int32_t>(L.o_n_fit); o.first_row = c->at<int32_t>(L.o_first); o.last_row = c->at<int32_t>(L.o_last);
     o.start_hit = c->at<int32_t>(L.o_start); o.hit_offset = c->at<int32_t>(L.o_hit_offset); o.hit_idx = c->at<int32_t>(L.o_hit_idx);
     int32_t* hits = c->at<int32_t>(L.hits);
-    float4* trk_f = c->at<float4>(L.trk_f);
-    int32_t* trk_i = c->at<int32_t>(L.trk_i);
+    float4* trk_f = c->at<float4>(L.trk_v);
+    int32_t* trk_i = c->at<int32_t>(L.trk_n);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
     static_assert(sizeof(status->work_counter) % 4 == 0 && sizeof(status->work) % 4 == 0, "word-sized counters");
     k_zero_words<<<1, 32, 0, st>>>(reinterpret_cast<uint32_t*>(status->work_counter), sizeof(status->work_counter) / 4);
@@ -548,16 +547,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     sp.win_y = t.win_y; sp.win_z = t.win_z; sp.gate = t.gate; sp.margin = t.margin; sp.grid_z_lo = t.grid_z_lo;
     sp.n_rows = t.n_rows; sp.n_sectors = t.n_sectors; sp.max_gap = t.tc_max_gap; sp.min_hits = t.tc_min_hits;
     sp.bins_per_sector = t.bins_per_sector;
-    float4* hs_f = c->at<float4>(L.hs_f);
+    float4* hs_f = c->at<float4>(L.hs);
     const int4* perm = c->at<int4>(L.perm);
-    k_tracklets<MODE_A><<<c->sm_count * kS5BlocksPerSMA, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                              start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
-    k_tracklets<MODE_B><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
-    k_tracklets<MODE_C1><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
-    k_tracklets<MODE_C2><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, row_start, order, c->at<int32_t>(L.up),
-                                                                             start_hit, perm, cap, hits, trk_f, trk_i, hs_f);
+    k_tracklets<MODE_A><<<c->sm_count * kS5BlocksPerSMA, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, order, c->at<int32_t>(L.up),
+                                                                              perm, cap, hits, trk_f, trk_i, hs_f);
+    k_tracklets<MODE_B><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, order, c->at<int32_t>(L.up),
+                                                                              perm, cap, hits, trk_f, trk_i, hs_f);
+    k_tracklets<MODE_C1><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, order, c->at<int32_t>(L.up),
+                                                                              perm, cap, hits, trk_f, trk_i, hs_f);
+    k_tracklets<MODE_C2><<<c->sm_count * kS5BlocksPerSM, kS5Threads, 0, st>>>(T, sec, status, sp, syz, bin_start, order, c->at<int32_t>(L.up),
+                                                                              perm, cap, hits, trk_f, trk_i, hs_f);
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
