@@ -104,7 +104,8 @@ __device__ __forceinline__ void cb_row_slab(const DevTables* __restrict__ T, int
 // smaller ids of the same bin; writes syz / order (sorted positions) and the bucket's bin_start
 // entries.  Buckets that do not fit the shared-memory buffers go to the big-bucket list.
 __global__ void __launch_bounds__(256)
-k_grid_sort(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const uint32_t* __restrict__ cb_start,
+k_grid_sort(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const int32_t* __restrict__ cb_rs,
+            const uint32_t* __restrict__ cb_start,
             const GridRec* __restrict__ rec, float2* __restrict__ syz, int32_t* __restrict__ order,
             uint32_t* __restrict__ bin_start, uint32_t* __restrict__ big_list, DevStatus* __restrict__ st) {
   __shared__ float s_y[kSortCapR], s_z[kSortCapR];
@@ -114,8 +115,8 @@ k_grid_sort(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   __shared__ uint32_t ws[33];
   const int ncb = __ldg(&T->n_cb);
   const int s = blockIdx.x / ncb, cb = blockIdx.x - s * ncb;
-  int r, k;
-  cb_row_slab(T, cb, r, k);
+  const int rs = __ldg(&cb_rs[cb]);             // host table: row | slab << 8 (no search per block)
+  const int r = rs & 0xff, k = rs >> 8;
   const int ny = __ldg(&T->ny[r]), nz = __ldg(&T->nz[r]);
   const int nsl = min(kSlab, nz - k * kSlab);
   const int nbins = nsl * ny;

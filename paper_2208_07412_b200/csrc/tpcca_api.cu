@@ -67,7 +67,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.cb_cur = take(4 * (size_t)(ns * (L.n_cb + 1)));
   L.big_list = take(4 * (size_t)(ns * L.n_cb));
   L.rec = take(16 * (size_t)N);
-  L.zorder = take(4 * (size_t)L.n_cb);
+  L.zorder = take(4 * (size_t)(2 * L.n_cb));   // [n_cb] buckets by ascending z, then [n_cb] bucket -> row | slab << 8
   L.sh_first = take(4 * (size_t)(ns * L.n_cb));
   L.sh_cnt = take(4 * (size_t)(ns * L.n_cb));
   L.sh_blk = take(sizeof(int2) * (size_t)(ns * L.n_cb / 256 + 2));
@@ -321,8 +321,10 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
       for (int k = 0; k < t.cb_base[r + 1] - t.cb_base[r]; ++k)
         zo.push_back({{(float)(k * kSlab) / p->grid_inv_bin_z[r], r}, t.cb_base[r] + k});
     std::sort(zo.begin(), zo.end());
-    std::vector<int32_t> zl(zo.size());
+    std::vector<int32_t> zl(2 * zo.size());
     for (size_t i = 0; i < zo.size(); ++i) zl[i] = zo[i].second;
+    for (int r = 0; r < p->n_rows; ++r)      // second half: coarse bucket -> (row, slab), read by k_grid_sort
+      for (int k = 0; k < t.cb_base[r + 1] - t.cb_base[r]; ++k) zl[zo.size() + (size_t)(t.cb_base[r] + k)] = r | (k << 8);
     cudaError_t ez = cudaMemcpyAsync(c->at<int32_t>(L.zorder), zl.data(), 4 * zl.size(), cudaMemcpyHostToDevice, c->stream);
     if (ez == cudaSuccess) ez = cudaStreamSynchronize(c->stream);
     if (ez != cudaSuccess) {
@@ -473,7 +475,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       k_cb_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cur, rec);
       ++c->launches;
     }
-    k_grid_sort<<<(unsigned)(c->ns * L.n_cb), 256, 0, st>>>(T, sec, cb_start, rec, syz, order, bin_start, big, status);
+    k_grid_sort<<<(unsigned)(c->ns * L.n_cb), 256, 0, st>>>(T, sec, c->at<int32_t>(L.zorder) + L.n_cb, cb_start, rec, syz, order, bin_start, big, status);
     k_grid_big<<<c->sm_count * 4, 256, 0, st>>>(T, sec, cb_start, rec, syz, order, bin_start, big, status);
     c->launches += 2;
     k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start));
