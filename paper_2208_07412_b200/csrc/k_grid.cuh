@@ -37,7 +37,7 @@ struct GridRec { float y, z; int32_t id; int32_t pad; };   // level-1 record (16
 // ---- K1a: level-1 histogram: cb_cnt[s][cb(row, bz >> kSlabShift)]++ ---------------------------------
 __global__ void __launch_bounds__(256)
 k_cb_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, uint32_t* __restrict__ cb_cnt,
-           DevStatus* __restrict__ st) {
+           uint32_t* __restrict__ rank, DevStatus* __restrict__ st) {
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
   const SectorDesc sd = sec[s];
@@ -47,13 +47,13 @@ k_cb_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, 
   if (r >= __ldg(&T->n_rows)) { st->err_range = 1; return; }
   const int bz = bin_coord(sd.z[i], __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
   const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
-  atomicAdd(&cb_cnt[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
+  // the arrival rank inside the bucket is kept: the scatter pass needs no second atomic
+  rank[(size_t)sd.off + i] = atomicAdd(&cb_cnt[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
 }
 
-// ---- K1b: one block per sector: cb_start = exclusive scan of cb_cnt (sector-local), cursors = copy ---
+// ---- K1b: one block per sector: cb_start = exclusive scan of cb_cnt (sector-local) -----------------
 __global__ void __launch_bounds__(1024)
-k_cb_scan(const DevTables* __restrict__ T, const uint32_t* __restrict__ cb_cnt, uint32_t* __restrict__ cb_start,
-          uint32_t* __restrict__ cb_cur) {
+k_cb_scan(const DevTables* __restrict__ T, const uint32_t* __restrict__ cb_cnt, uint32_t* __restrict__ cb_start) {
   __shared__ uint32_t ws[33];
   const int ncb = T->n_cb;
   const size_t base = (size_t)blockIdx.x * (ncb + 1);
@@ -63,16 +63,16 @@ k_cb_scan(const DevTables* __restrict__ T, const uint32_t* __restrict__ cb_cnt, 
     const uint32_t v = b < ncb ? cb_cnt[base + b] : 0u;
     uint32_t total;
     const uint32_t ex = block_exclusive_scan<uint32_t>(v, ws, total);
-    if (b < ncb) { cb_start[base + b] = carry + ex; cb_cur[base + b] = carry + ex; }
+    if (b < ncb) cb_start[base + b] = carry + ex;
     carry += total;
   }
   if (threadIdx.x == 0) cb_start[base + ncb] = carry;
 }
 
-// ---- K1c: level-1 scatter: record (y, z, id) to the bucket's next free slot (arrival order) ---------
+// ---- K1c: level-1 scatter: record (y, z, id) to slot cb_start + arrival rank of its bucket ----------
 __global__ void __launch_bounds__(256)
-k_cb_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, uint32_t* __restrict__ cb_cur,
-             GridRec* __restrict__ rec) {
+k_cb_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const uint32_t* __restrict__ cb_start,
+             const uint32_t* __restrict__ rank, GridRec* __restrict__ rec) {
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
   const SectorDesc sd = sec[s];
@@ -83,7 +83,7 @@ k_cb_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
   const float y = sd.y[i], z = sd.z[i];
   const int bz = bin_coord(z, __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
   const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
-  const uint32_t pos = atomicAdd(&cb_cur[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
+  const uint32_t pos = __ldg(&cb_start[(size_t)s * (__ldg(&T->n_cb) + 1) + cb]) + rank[(size_t)sd.off + i];
   GridRec o; o.y = y; o.z = z; o.id = i; o.pad = 0;
   *reinterpret_cast<float4*>(&rec[(size_t)sd.off + pos]) = *reinterpret_cast<const float4*>(&o);
 }

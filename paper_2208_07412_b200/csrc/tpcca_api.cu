@@ -24,7 +24,7 @@ inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 struct Layout {
   size_t tables, sec, status, tot;
   size_t in_y, in_z, in_row;
-  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, cb_cur, big_list, rec, zorder, sh_first, sh_cnt, sh_blk, sh_pre, perm;
+  size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, big_list, rec, zorder, sh_first, sh_cnt, sh_blk, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
   size_t tile_cnt, tile_off;
   size_t start_hit, hits, trk_v, trk_n, hs;
@@ -64,7 +64,6 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.nf_desc = take(sizeof(NfTileDesc) * (size_t)L.nf_tiles_max);
   L.cb_cnt = take(4 * (size_t)(ns * (L.n_cb + 1)));
   L.cb_start = take(4 * (size_t)(ns * (L.n_cb + 1)));
-  L.cb_cur = take(4 * (size_t)(ns * (L.n_cb + 1)));
   L.big_list = take(4 * (size_t)(ns * L.n_cb));
   L.rec = take(16 * (size_t)N);
   L.zorder = take(4 * (size_t)(2 * L.n_cb));   // [n_cb] buckets by ascending z, then [n_cb] bucket -> row | slab << 8
@@ -457,7 +456,6 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     k_zero_words<<<1, 256, 0, st>>>(reinterpret_cast<uint32_t*>(status), sizeof(DevStatus) / 4);
     uint32_t* cb_cnt = c->at<uint32_t>(L.cb_cnt);
     uint32_t* cb_start = c->at<uint32_t>(L.cb_start);
-    uint32_t* cb_cur = c->at<uint32_t>(L.cb_cur);
     uint32_t* big = c->at<uint32_t>(L.big_list);
     GridRec* rec = c->at<GridRec>(L.rec);
     {
@@ -466,13 +464,13 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       c->launches += 2;
     }
     if (c->n_tiles256 > 0) {
-      k_cb_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cnt, status);
+      k_cb_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cnt, reinterpret_cast<uint32_t*>(order), status);   // `order` is free until level 2
       ++c->launches;
     }
-    k_cb_scan<<<c->ns, 1024, 0, st>>>(T, cb_cnt, cb_start, cb_cur);
+    k_cb_scan<<<c->ns, 1024, 0, st>>>(T, cb_cnt, cb_start);
     ++c->launches;
     if (c->n_tiles256 > 0) {
-      k_cb_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cur, rec);
+      k_cb_scatter<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_start, reinterpret_cast<const uint32_t*>(order), rec);
       ++c->launches;
     }
     k_grid_sort<<<(unsigned)(c->ns * L.n_cb), 256, 0, st>>>(T, sec, c->at<int32_t>(L.zorder) + L.n_cb, cb_start, rec, syz, order, bin_start, big, status);
