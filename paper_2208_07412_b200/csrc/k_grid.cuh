@@ -38,10 +38,12 @@ struct GridRec { float y, z; int32_t id; int32_t pad; };   // level-1 record (16
 __global__ void __launch_bounds__(256)
 k_cb_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, uint32_t* __restrict__ cb_cnt,
            uint32_t* __restrict__ rank, DevStatus* __restrict__ st) {
+  // consecutive blocks work on different sectors: the atomics of the blocks in flight are spread over the
+  // counters of all sectors (36 x 58 KB) instead of hammering the few hundred cache lines of one
   const int ns = __ldg(&T->n_sectors);
-  const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile256); });
+  const int s = blockIdx.x % ns;
   const SectorDesc sd = sec[s];
-  const int i = (blockIdx.x - sd.tile256) * 256 + threadIdx.x;
+  const int i = (blockIdx.x / ns) * 256 + threadIdx.x;
   if (i >= sd.n) return;
   const int r = sd.row[i];
   if (r >= __ldg(&T->n_rows)) { st->err_range = 1; return; }

@@ -148,7 +148,7 @@ struct tpcca_ctx {
   int64_t in_used = 0;
   std::vector<SectorDesc> desc;       // as uploaded by the last run
   int64_t n_total = 0;
-  int n_tiles256 = 0, n_tiles2048 = 0;
+  int n_tiles256 = 0, n_tiles2048 = 0, max_tiles256 = 0;
   uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
   bool desc_valid = false;
   static constexpr int kRing = 16;
@@ -430,6 +430,9 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       off += n; t256 += (n + 255) / 256; t2048 += (n + 2047) / 2048; bt += bin_tiles;
     }
     c->n_total = off; c->n_tiles256 = (int)t256; c->n_tiles2048 = (int)t2048;
+    int64_t mx = 0;
+    for (int s = 0; s < c->ns; ++s) mx = std::max<int64_t>(mx, (c->sec[s].n + 255) / 256);
+    c->max_tiles256 = (int)mx;
     CU(c, cudaMemcpyAsync(c->at<SectorDesc>(L.sec), c->desc.data(), sizeof(SectorDesc) * (kMaxSectors + 1), cudaMemcpyHostToDevice, st));
     c->desc_valid = true;
   }
@@ -464,7 +467,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       c->launches += 2;
     }
     if (c->n_tiles256 > 0) {
-      k_cb_count<<<c->n_tiles256, 256, 0, st>>>(T, sec, cb_cnt, reinterpret_cast<uint32_t*>(order), status);   // `order` is free until level 2
+      k_cb_count<<<(unsigned)(c->ns * c->max_tiles256), 256, 0, st>>>(T, sec, cb_cnt, reinterpret_cast<uint32_t*>(order), status);   // `order` is free until level 2
       ++c->launches;
     }
     k_cb_scan<<<c->ns, 1024, 0, st>>>(T, cb_cnt, cb_start);
