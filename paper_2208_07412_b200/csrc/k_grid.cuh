@@ -10,10 +10,11 @@ namespace tpcca {
 // every bucket by (bin, original id) in shared memory and writes the sorted clusters and the
 // bucket's bin_start entries with coalesced stores.  Nothing touches the 1.5 GB bin_start array
 // with atomics and no pass runs over it except the one that writes it.
-constexpr int kSlabShift = 6;
-constexpr int kSlab = 1 << kSlabShift;        // z slices per coarse bucket
+// z slices per coarse bucket = 1 << DevTables::slab_shift, chosen per context (slab_shift_for in tpcca_api.cu)
+// so that a bucket holds a few hundred clusters at the context's capacity
+constexpr int kSlabShiftMin = 5, kSlabShiftMax = 7;
 constexpr int kSortCapR = 1024;               // clusters of a bucket sorted in shared memory
-constexpr int kSortCapB = 2048;               // fine bins of a bucket (kSlab * ny) handled in shared memory
+constexpr int kSortCapB = 2048;               // fine bins of a bucket (slab * ny) handled in shared memory
 
 // sector of a tile: largest s with first_tile(s) <= tile (sectors with no tiles are skipped
 // because their first tile equals the next sector's).
@@ -48,7 +49,7 @@ k_cb_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, 
   const int r = sd.row[i];
   if (r >= __ldg(&T->n_rows)) { st->err_range = 1; return; }
   const int bz = bin_coord(sd.z[i], __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
-  const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
+  const int cb = __ldg(&T->cb_base[r]) + (bz >> __ldg(&T->slab_shift));
   // the arrival rank inside the bucket is kept: the scatter pass needs no second atomic
   rank[(size_t)sd.off + i] = atomicAdd(&cb_cnt[(size_t)s * (__ldg(&T->n_cb) + 1) + cb], 1u);
 }
@@ -84,7 +85,7 @@ k_cb_scatter(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec
   if (r >= __ldg(&T->n_rows)) return;
   const float y = sd.y[i], z = sd.z[i];
   const int bz = bin_coord(z, __ldg(&T->grid_z_lo), __ldg(&T->inv_bz[r]), __ldg(&T->nz_hi[r]));
-  const int cb = __ldg(&T->cb_base[r]) + (bz >> kSlabShift);
+  const int cb = __ldg(&T->cb_base[r]) + (bz >> __ldg(&T->slab_shift));
   const uint32_t pos = __ldg(&cb_start[(size_t)s * (__ldg(&T->n_cb) + 1) + cb]) + rank[(size_t)sd.off + i];
   GridRec o; o.y = y; o.z = z; o.id = i; o.pad = 0;
   *reinterpret_cast<float4*>(&rec[(size_t)sd.off + pos]) = *reinterpret_cast<const float4*>(&o);
@@ -120,6 +121,7 @@ k_grid_sort(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   const int rs = __ldg(&cb_rs[cb]);             // host table: row | slab << 8 (no search per block)
   const int r = rs & 0xff, k = rs >> 8;
   const int ny = __ldg(&T->ny[r]), nz = __ldg(&T->nz[r]);
+  const int kSlab = 1 << __ldg(&T->slab_shift);
   const int nsl = min(kSlab, nz - k * kSlab);
   const int nbins = nsl * ny;
   const uint32_t* cs = cb_start + (size_t)s * (ncb + 1) + cb;
@@ -194,6 +196,7 @@ k_grid_big(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, 
     int r, k;
     cb_row_slab(T, cb, r, k);
     const int ny = __ldg(&T->ny[r]), nz = __ldg(&T->nz[r]);
+    const int kSlab = 1 << __ldg(&T->slab_shift);
     const int nsl = min(kSlab, nz - k * kSlab);
     const int nbins = nsl * ny;
     const uint32_t* cs = cb_start + (size_t)s * (ncb + 1) + cb;

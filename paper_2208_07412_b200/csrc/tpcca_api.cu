@@ -39,8 +39,24 @@ int64_t bins_per_sector(const tpcca_params* p) {
   return nb;
 }
 
+// S1 level 1: z slices per coarse bucket (log2).  Larger buckets amortise the per-block work of the level-2
+// sort, but a bucket must fit its shared-memory buffers (kSortCapR clusters, kSortCapB bins): the largest shift
+// that keeps the mean bucket at the context's capacity below ~700 clusters and every bucket within kSortCapB bins.
+int slab_shift_for(const tpcca_params* p, int64_t N) {
+  int ny_max = 1;
+  for (int r = 0; r < p->n_rows; ++r) ny_max = std::max(ny_max, (int)p->grid_ny[r]);
+  for (int sh = kSlabShiftMax; sh > kSlabShiftMin; --sh) {
+    int64_t ncb = 0;
+    for (int r = 0; r < p->n_rows; ++r) ncb += (p->grid_nz[r] + (1 << sh) - 1) >> sh;
+    const double mean = (double)N / ((double)p->n_sectors * (double)std::max<int64_t>(ncb, 1));
+    if (mean <= 700.0 && (int64_t)ny_max << sh <= kSortCapB) return sh;
+  }
+  return kSlabShiftMin;
+}
+
 Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   Layout L{};
+  const int kSlab = 1 << slab_shift_for(p, N);
   size_t cur = 0;
   auto take = [&](size_t bytes) { size_t o = cur; cur = align_up(cur + bytes); return o; };
   const int64_t ns = p->n_sectors, nr = p->n_rows, nb = bins_per_sector(p);
@@ -296,6 +312,8 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   t.bin_base[p->n_rows] = base;
   {
     int32_t cb = 0;
+    const int kSlab = 1 << slab_shift_for(p, c->N);
+    t.slab_shift = slab_shift_for(p, c->N);
     for (int r = 0; r < p->n_rows; ++r) { t.cb_base[r] = cb; cb += (p->grid_nz[r] + kSlab - 1) / kSlab; }
     t.cb_base[p->n_rows] = cb;
     t.n_cb = cb;
@@ -318,7 +336,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     std::vector<std::pair<std::pair<float, int>, int>> zo;
     for (int r = 0; r < p->n_rows; ++r)
       for (int k = 0; k < t.cb_base[r + 1] - t.cb_base[r]; ++k)
-        zo.push_back({{(float)(k * kSlab) / p->grid_inv_bin_z[r], r}, t.cb_base[r] + k});
+        zo.push_back({{(float)(k << t.slab_shift) / p->grid_inv_bin_z[r], r}, t.cb_base[r] + k});
     std::sort(zo.begin(), zo.end());
     std::vector<int32_t> zl(2 * zo.size());
     for (size_t i = 0; i < zo.size(); ++i) zl[i] = zo[i].second;

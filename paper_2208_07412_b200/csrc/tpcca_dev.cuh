@@ -41,6 +41,7 @@ struct DevTables {
   int32_t bin_base[kMaxRows + 1];       // first bin of row r inside a sector
   int32_t cb_base[kMaxRows + 1];        // S1 level 1: first coarse bucket (row, z slab) of row r
   int32_t n_cb;                         // coarse buckets per sector
+  int32_t slab_shift;                   // S1 level 1: log2 of the z slices per coarse bucket
   float hy_up[kMaxRows], hz_up[kMaxRows], hy_dn[kMaxRows], hz_dn[kMaxRows], nf_cut[kMaxRows];
   NfConst nf[kMaxRows];                 // S2 per-row constants (host-filled in tpcca_create)
 };
