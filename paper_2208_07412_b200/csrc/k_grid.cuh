@@ -13,7 +13,10 @@ namespace tpcca {
 // z slices per coarse bucket = 1 << DevTables::slab_shift, chosen per context (slab_shift_for in tpcca_api.cu)
 // so that a bucket holds a few hundred clusters at the context's capacity
 constexpr int kSlabShiftMin = 5, kSlabShiftMax = 7;
-constexpr int kSortCapR = 1024;               // clusters of a bucket sorted in shared memory
+#ifndef TPCCA_SORT_CAPR
+#define TPCCA_SORT_CAPR 1536
+#endif
+constexpr int kSortCapR = TPCCA_SORT_CAPR;               // clusters of a bucket sorted in shared memory
 constexpr int kSortCapB = 2048;               // fine bins of a bucket (slab * ny) handled in shared memory
 
 // sector of a tile: largest s with first_tile(s) <= tile (sectors with no tiles are skipped
