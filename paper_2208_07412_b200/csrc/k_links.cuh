@@ -29,13 +29,13 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 #ifndef TPCCA_NF_ARENA
 #define TPCCA_NF_ARENA 8448
 #endif
-constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory (<= 15)
+constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory (<= 15): normal occupancy
+constexpr int kNfKDense = 15;             // ... of the kernel instance used for dense time frames (tpcca_create chooses)
 static_assert(TPCCA_NF_K <= 15 && TPCCA_NF_TILE <= 256, "work-item encoding: 8 bits cluster, 4 bits hit row, 4 bits nd");
 constexpr int kNfThreads = kNfTile;       // one thread per cluster of the tile
 constexpr int kNfArena = TPCCA_NF_ARENA;  // bytes of one staging buffer: [up clusters | down clusters | up bins | down bins]
 constexpr int kNfMaxCn = 1022;            // staged clusters per side (staged indices are packed in 10 bits)
 constexpr int kNfMaxRun = 63;             // window candidates per side handled by the packed fast path
-constexpr int kNfMaxItems = kNfK * kNfThreads;   // up-side hits of a tile (pair work items)
 
 #ifdef TPCCA_NF_STATS
 __device__ unsigned long long g_nf_hist[4][64];   // tests per side, hits per side, pairs, pairs under cut
@@ -259,12 +259,13 @@ constexpr uint32_t kIdxRow = 2u * kNfThreads;   // ... of the hit-index cache
 // side) or -dxu (down side: (y_c - y_d) * dxu = -((y_d - y_c) * dxu), exact).  Hits go to the thread's
 // cache column: vector (dy * scale, dz * scale) at pv + k * kVecRow, staged index at pi + k * kIdxRow.
 // Returns the number of hits (may exceed kNfK; only the first kNfK are cached).
+template <int K>
 __device__ __forceinline__ int nf_test_runs(const float2 c, uint32_t w0, uint32_t w1, uint32_t sC, float hy, float hz,
                                             float scale, uint32_t pv, uint32_t pi) {
   const int n0 = (w0 >> 10) & 63, n01 = w0 >> 26, tot = w1 >> 10;
   const uint32_t o1 = 8u * ((w0 >> 16) & 1023u), o2 = 8u * (w1 & 1023u);
   uint32_t a = sC + 8u * (w0 & 1023u);
-  const uint32_t pv_end = pv + kNfK * kVecRow;
+  const uint32_t pv_end = pv + K * kVecRow;
   int n = 0;
   // kT candidates per trip: their shared-memory loads are issued before the first test (independent chains)
   constexpr int kT = TPCCA_NF_T2;
@@ -337,11 +338,12 @@ __device__ __noinline__ bool nf_medium(const float2 c, uint32_t wu0, uint32_t wu
   return !tie;
 }
 
+template <int K>
 struct NfSmem {
   alignas(128) unsigned char arena[kNfArena];   // staging buffer (TMA destination): [up clusters | down clusters | up bins | down bins]
-  float2 vec[2 * kNfK][kNfThreads];      // cached hits: rows [0, K) down side, [K, 2K) up side; column = cluster of the tile
-  uint16_t hidx[2 * kNfK][kNfThreads];   // staged indices of the cached hits
-  uint16_t items[kNfMaxItems];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 12
+  float2 vec[2 * K][kNfThreads];      // cached hits: rows [0, K) down side, [K, 2K) up side; column = cluster of the tile
+  uint16_t hidx[2 * K][kNfThreads];   // staged indices of the cached hits
+  uint16_t items[K * kNfThreads];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 12
   int hist[2][16], cnt[2][16];           // items per nd (work key) / emission cursors, two consecutive tiles
   NfTileDesc desc[4];
   uint64_t full;
@@ -366,13 +368,14 @@ struct NfSmem {
 #ifndef TPCCA_NF_BPS
 #define TPCCA_NF_BPS 5
 #endif
-__global__ void __launch_bounds__(kNfThreads, TPCCA_NF_BPS)
+template <int K>
+__global__ void __launch_bounds__(kNfThreads, K == kNfK ? TPCCA_NF_BPS : 4)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
              const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ order, uint32_t nbp1,
              const int32_t* __restrict__ n_tiles_ptr, const NfTileDesc* __restrict__ desc,
              int32_t* __restrict__ link_up, int32_t* __restrict__ link_dn) {
   extern __shared__ __align__(128) unsigned char nf_smem_raw[];
-  NfSmem& S = *reinterpret_cast<NfSmem*>(nf_smem_raw);
+  NfSmem<K>& S = *reinterpret_cast<NfSmem<K>*>(nf_smem_raw);
   const int tid = threadIdx.x;
   const int n_tiles = __ldg(n_tiles_ptr);
   const int stride = gridDim.x;
@@ -406,8 +409,8 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
   float2 c_next = make_float2(0.f, 0.f);
   if (tid < S.desc[0].n) c_next = __ldg(&syz[S.desc[0].p0 + tid]);
   const uint32_t sArena = smem_u32(S.arena);
-  const uint32_t sVecD = smem_u32(&S.vec[0][0]), sVecU = smem_u32(&S.vec[kNfK][0]);
-  const uint32_t sIdxD = smem_u32(&S.hidx[0][0]), sIdxU = smem_u32(&S.hidx[kNfK][0]);
+  const uint32_t sVecD = smem_u32(&S.vec[0][0]), sVecU = smem_u32(&S.vec[K][0]);
+  const uint32_t sIdxD = smem_u32(&S.hidx[0][0]), sIdxU = smem_u32(&S.hidx[K][0]);
   int it = 0;
   for (int tile = first; tile < n_tiles; tile += stride, ++it) {
     const NfTileDesc& d = S.desc[it & 3];
@@ -447,10 +450,10 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
         ok = false; wd0 = wd1 = wu0 = wu1 = 0;
       }
       if (ok) {
-        nd = nf_test_runs(c, wd0, wd1, sArena + 8u * (uint32_t)d.up.cn, kc.dA.x, kc.dA.y, -g.x, sVecD + 8u * tid, sIdxD + 2u * tid);
-        nu = nf_test_runs(c, wu0, wu1, sArena, kc.uA.x, kc.uA.y, g.y, sVecU + 8u * tid, sIdxU + 2u * tid);
+        nd = nf_test_runs<K>(c, wd0, wd1, sArena + 8u * (uint32_t)d.up.cn, kc.dA.x, kc.dA.y, -g.x, sVecD + 8u * tid, sIdxD + 2u * tid);
+        nu = nf_test_runs<K>(c, wu0, wu1, sArena, kc.uA.x, kc.uA.y, g.y, sVecU + 8u * tid, sIdxU + 2u * tid);
       }
-      if (ok && (nd > kNfK || nu > kNfK)) {               // dense region: decide now, while the staged runs are here
+      if (ok && (nd > K || nu > K)) {               // dense region: decide now, while the staged runs are here
         int iu, id;
         if (nf_medium(c, wu0, wu1, wd0, wd1, sArena, sArena + 8u * (uint32_t)d.up.cn, kc.uA, kc.dA, g, m_best, iu, id)) {
           if (iu >= 0) { m_bu = iu + d.up.c0; m_bd = id + d.dn.c0; }
@@ -470,7 +473,7 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     {
       int above = 0;                                          // items with a larger nd than this thread's
 #pragma unroll
-      for (int k = kNfK; k >= 1; --k) {
+      for (int k = K; k >= 1; --k) {
         const int h = hist[k];
         if (k > nd) above += h;
         n_items += h;

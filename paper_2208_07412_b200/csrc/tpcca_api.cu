@@ -148,6 +148,7 @@ struct tpcca_ctx {
   int device = 0;
   int sm_count = 148;
   int nf_blocks_per_sm = 3;
+  bool nf_dense = false;               // S2 kernel instance with the deeper hit cache (tpcca_create)
   NfTable nftab{};                    // S2 per-row constants, passed to k_neighbours by value (constant bank)
   cudaStream_t stream = nullptr;
   cudaStream_t copy_stream = nullptr;  // D2H copies of tpcca_get_tracks(HOST): they wait only for the stage that made the data
@@ -362,13 +363,19 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   }
   {
     int occ = 0;
-    cudaError_t e2 = cudaFuncSetAttribute(k_neighbours, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(NfSmem));
+    // S2 kernel instance: the hit cache holds kNfK hits per side (5 blocks per SM) or, for dense time frames (more
+    // than ~0.7 clusters per grid bin at the context's capacity: windows with more than kNfK hits are common there
+    // and each one stalls its warp in the uncached path), kNfKDense hits (4 blocks per SM)
+    c->nf_dense = (double)c->N > 0.7 * (double)c->ns * (double)c->nb;
+    const void* nf_fn = c->nf_dense ? (const void*)k_neighbours<kNfKDense> : (const void*)k_neighbours<kNfK>;
+    const size_t nf_smem = c->nf_dense ? sizeof(NfSmem<kNfKDense>) : sizeof(NfSmem<kNfK>);
+    cudaError_t e2 = cudaFuncSetAttribute(nf_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_smem);
     if (e2 != cudaSuccess) {
       set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: shared memory opt-in of k_neighbours failed: %s", cudaGetErrorString(e2));
       delete c;
       return TPCCA_E_CUDA;
     }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_neighbours, kNfThreads, sizeof(NfSmem)) == cudaSuccess && occ > 0)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, nf_fn, kNfThreads, nf_smem) == cudaSuccess && occ > 0)
       c->nf_blocks_per_sm = occ;
   }
   *out_ctx = c;
@@ -507,9 +514,14 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     NfTileDesc* nfd = c->at<NfTileDesc>(L.nf_desc);
     const int32_t* nf_ts = c->at<int32_t>(L.nf_tile_start);
     k_nf_plan<<<std::min(c->ns * c->nr, 148 * 64), 128, 0, st>>>(T, sec, syz, bin_start, row_start, nf_ts, nfd);
-    k_neighbours<<<grid, kNfThreads, sizeof(NfSmem), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
-                                                          nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
-                                                          c->at<int32_t>(L.dn_raw));
+    if (c->nf_dense)
+      k_neighbours<kNfKDense><<<grid, kNfThreads, sizeof(NfSmem<kNfKDense>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
+                                                                                   nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
+                                                                                   c->at<int32_t>(L.dn_raw));
+    else
+      k_neighbours<kNfK><<<grid, kNfThreads, sizeof(NfSmem<kNfK>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
+                                                                         nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
+                                                                         c->at<int32_t>(L.dn_raw));
     c->launches += 2;
   }
   mark(2);
