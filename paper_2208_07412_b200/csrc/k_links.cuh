@@ -551,7 +551,8 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
 __global__ void __launch_bounds__(256)
 k_clean_links(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
               const int32_t* __restrict__ up_raw, const int32_t* __restrict__ dn_raw,
-              int32_t* __restrict__ up, int32_t* __restrict__ dn, int2* __restrict__ tile_cnt) {
+              int32_t* __restrict__ up, int32_t* __restrict__ dn, int2* __restrict__ tile_cnt,
+              uint32_t* __restrict__ start_bits /*[tile][64]: bit p of the tile = start hit (read by S4)*/) {
   __shared__ int ws[33];
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile2048); });
@@ -561,14 +562,19 @@ k_clean_links(const DevTables* __restrict__ T, const SectorDesc* __restrict__ se
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
     const int p = p0 + k * 256 + threadIdx.x;
+    bool is_start = false;
     if (p < n) {
       const int32_t u = up_raw[off + p], d = dn_raw[off + p];
       const int32_t uc = (u >= 0 && __ldg(&dn_raw[off + u]) == p) ? u : -1;
       const int32_t dc = (d >= 0 && __ldg(&up_raw[off + d]) == p) ? d : -1;
       up[off + p] = uc;
       dn[off + p] = dc;
-      cnt += (dc == -1 && uc >= 0) ? 1 : 0;
+      is_start = (dc == -1 && uc >= 0);
+      cnt += is_start ? 1 : 0;
     }
+    // the 32 positions of a warp are consecutive: one ballot = one word of the tile's start-hit bitmap
+    const unsigned m = __ballot_sync(0xffffffffu, is_start);
+    if ((threadIdx.x & 31) == 0) start_bits[(size_t)blockIdx.x * 64 + k * 8 + (threadIdx.x >> 5)] = m;
   }
   int total;
   block_exclusive_scan<int>(cnt, ws, total);
@@ -614,19 +620,14 @@ __global__ void k_start_offsets(const DevTables* __restrict__ T, const SectorDes
 // Each thread owns 8 CONSECUTIVE positions so that ranks are ascending in sorted position.
 __global__ void __launch_bounds__(256)
 k_start_hits(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
-             const int32_t* __restrict__ up, const int32_t* __restrict__ dn,
+             const uint32_t* __restrict__ start_bits,
              const longlong2* __restrict__ tile_off, int32_t cap, int32_t* __restrict__ start_hit) {
   __shared__ int ws[33];
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile2048); });
-  const int n = __ldg(&sec[s].n), off = __ldg(&sec[s].off);
   const int p0 = (blockIdx.x - __ldg(&sec[s].tile2048)) * 2048 + threadIdx.x * 8;
-  unsigned flags = 0;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    const int p = p0 + k;
-    if (p < n && dn[off + p] == -1 && up[off + p] >= 0) flags |= 1u << k;
-  }
+  // the thread's 8 consecutive positions are one byte of the bitmap S3 wrote (positions >= n hold 0 bits)
+  const unsigned flags = (__ldg(&start_bits[(size_t)blockIdx.x * 64 + (threadIdx.x >> 2)]) >> ((threadIdx.x & 3) * 8)) & 0xffu;
   int total;
   int rank = block_exclusive_scan<int>(__popc(flags), ws, total);
   long long o = tile_off[blockIdx.x].x + rank;

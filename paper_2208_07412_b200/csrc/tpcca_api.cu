@@ -26,7 +26,7 @@ struct Layout {
   size_t in_y, in_z, in_row;
   size_t syz, order, bin_start, row_start, nf_tile_start, nf_desc, cb_cnt, cb_start, big_list, rec, zorder, sh_first, sh_cnt, sh_blk, sh_pre, perm;
   size_t up_raw, dn_raw, up, dn;
-  size_t tile_cnt, tile_off;
+  size_t tile_cnt, tile_off, start_bits;
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t total;
@@ -94,6 +94,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.dn = take(4 * (size_t)N);
   L.tile_cnt = take(sizeof(int2) * (size_t)L.n_tiles_max);
   L.tile_off = take(sizeof(longlong2) * (size_t)L.n_tiles_max);
+  L.start_bits = take(4 * 64 * (size_t)(N / 2048 + ns + 1));   // S3 -> S4: start-hit bitmap, 64 words per 2048-cluster tile
   L.start_hit = take(4 * (size_t)CS);
   L.hits = take(4 * (size_t)(nr * CS));
   L.trk_v = take(16 * (size_t)(kTrkV * CS));   // finished tracks: records of kTrkV 16-byte vectors
@@ -527,7 +528,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   mark(2);
   if ((mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
     k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
-                                                 c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt);
+                                                 c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits));
     ++c->launches;
   }
   mark(3);
@@ -536,14 +537,14 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     // buffer, so S4 on its own recounts through S3's kernel (cheap, idempotent).
     if (!(mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
       k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
-                                                   c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt);
+                                                   c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits));
       ++c->launches;
     }
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, c->n_tiles2048, tot);
     k_start_offsets<<<1, kMaxSectors + 1, 0, st>>>(T, sec, tile_off, tot, c->n_tiles2048, cap, status);
     c->launches += 2;
     if (c->n_tiles2048 > 0) {
-      k_start_hits<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_off, cap, start_hit);
+      k_start_hits<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<uint32_t>(L.start_bits), tile_off, cap, start_hit);
       ++c->launches;
     }
     {   // processing order of S5: start-hit slots by (sector, z)
