@@ -714,11 +714,22 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
     const int f0 = __shfl_sync(0xffffffffu, first, src), l0 = __shfl_sync(0xffffffffu, last, src);
     long long w = __shfl_sync(0xffffffffu, h, src);
     const int32_t* line = hits + (size_t)sl * n_rows_g;
-    for (int r = f0 + lane; r - lane <= l0; r += 32) {
-      const int c = r <= l0 ? line[r] : -1;
-      const unsigned m = __ballot_sync(0xffffffffu, c != -1);
-      if (c != -1) o.hit_idx[w + __popc(m & ((1u << lane) - 1u))] = c;
-      w += __popc(m);
+    // the loads of up to kG x 32 rows are issued together (one memory latency per tracklet, not one per 32 rows)
+    constexpr int kG = 5;
+    for (int r0 = f0; r0 <= l0; r0 += 32 * kG) {
+      int cc[kG];
+#pragma unroll
+      for (int q = 0; q < kG; ++q) {
+        const int r = r0 + 32 * q + lane;
+        cc[q] = r <= l0 ? __ldcs(&line[r]) : -1;
+      }
+#pragma unroll
+      for (int q = 0; q < kG; ++q) {
+        if (r0 + 32 * q > l0) break;             // warp-uniform
+        const unsigned m = __ballot_sync(0xffffffffu, cc[q] != -1);
+        if (cc[q] != -1) o.hit_idx[w + __popc(m & ((1u << lane) - 1u))] = cc[q];
+        w += __popc(m);
+      }
     }
   }
 }
