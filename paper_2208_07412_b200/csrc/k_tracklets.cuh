@@ -296,6 +296,8 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   bool drained = false;      // warp-uniform: the work counter ran out
   int wi = 0;                // work index of the lane's tracklet (parking slot)
   int slot = 0, r = 0, cur = -1, top = 0, top_hit = -1, gap = 0, n_hits = 0, first = 0, r0 = 0;
+  int nxt_pre = -1;          // MODE_C1: hit of row r - 1 (read one step ahead) ...
+  float2 h_pre = make_float2(0.f, 0.f);   // ... and the cluster of row r (loaded one step ahead)
   bool fresh = false;        // running state == snapshot (last operation was a phase-C update)
   bool saved = false;        // snapshot parked in shared memory
   float z_ref = 0.f;
@@ -400,6 +402,11 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
               top = I(v2.x); top_hit = I(v2.y); n_hits = I(v2.z); first = I(v2.w); r0 = I(v3.x);
               if (MODE == MODE_C1) {          // the phase change A/B -> C is completed here
                 kf_reset_cov(f, K); gap = 0; r = top; cur = top_hit;
+                {
+                  const int32_t* line = hits + (size_t)slot * n_rows;
+                  nxt_pre = (r - 1 >= r0) ? line[r - 1] : -1;
+                  h_pre = cur >= 0 ? __ldg(&syz[off + cur]) : make_float2(0.f, 0.f);
+                }
               } else {
                 f.n = I(v3.y); r = I(v3.z); cur = I(v3.w); gap = I(v4.x);
                 f.c00 = v4.y; f.c10 = v4.z; f.c11 = v4.w; f.c20 = v5.x; f.c21 = v5.y; f.c22 = v5.z; f.c30 = v5.w;
@@ -424,13 +431,23 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     int32_t* hcol = hits + (size_t)slot * n_rows;   // the tracklet's hit per row: one contiguous line per tracklet
     int cand = -1;                        // >= 0: cluster to use on this row; -1: none known
     int nxt = -1;                         // candidate of the next row (loaded early)
+    int nn = -1;                          // MODE_C1: candidate of the row after the next
+    float2 hn = make_float2(0.f, 0.f);    // MODE_C1: cluster of the next row
     float2 h = make_float2(0.f, 0.f);
     float xr = f.x;
     if (alive) {
       cand = cur;
-      if (cand >= 0) h = __ldg(&syz[off + cand]);
-      if (phase == PH_A) nxt = __ldg(&link_up[off + cand]);
-      else if (phase == PH_C && r - 1 >= r0) nxt = hcol[r - 1];
+      if (MODE == MODE_C1) {
+        // refit over known hits: the hit of the next row and the cluster of this row were read one step
+        // ahead, the loads issued here are consumed at the end of the step (their latency is off the path)
+        h = h_pre; nxt = nxt_pre;
+        if (r - 2 >= r0) nn = hcol[r - 2];
+        if (nxt >= 0) hn = __ldg(&syz[off + nxt]);
+      } else {
+        if (cand >= 0) h = __ldg(&syz[off + cand]);
+        if (phase == PH_A) nxt = __ldg(&link_up[off + cand]);
+        else if (phase == PH_C && r - 1 >= r0) nxt = hcol[r - 1];
+      }
       xr = t_x[r];
       if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
       w_prop += (xr != f.x) ? 1u : 0u;
@@ -571,7 +588,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     if (go) {
       if (phase == PH_A) { cur = nxt; ++r; if (cur == -1) { phase = PH_B; gap = 0; } }
       else if (phase == PH_B) ++r;
-      else { cur = nxt; --r; }
+      else { cur = nxt; --r; if (MODE == MODE_C1) { nxt_pre = nn; h_pre = hn; } }
       if (phase == PH_B && r >= n_rows) ev = EV_TO_C;
       if (phase == PH_C && r < 0) ev = EV_FINISH;
     }
