@@ -160,7 +160,7 @@ constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 #define TPCCA_S5_BPS 5
 #endif
 #ifndef TPCCA_S5_BPS_A
-#define TPCCA_S5_BPS_A 8
+#define TPCCA_S5_BPS_A 5
 #endif
 constexpr int kS5BlocksPerSMA = TPCCA_S5_BPS_A;   // ... of the phase-A kernel (no search code: fewer registers)
 constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
@@ -296,7 +296,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   bool drained = false;      // warp-uniform: the work counter ran out
   int wi = 0;                // work index of the lane's tracklet (parking slot)
   int slot = 0, r = 0, cur = -1, top = 0, top_hit = -1, gap = 0, n_hits = 0, first = 0, r0 = 0;
-  int nxt_pre = -1;          // MODE_C1: hit of row r - 1 (read one step ahead) ...
+  int nxt_pre = -1;          // MODE_A / MODE_C1: hit of the next row (read one step ahead) ...
   float2 h_pre = make_float2(0.f, 0.f);   // ... and the cluster of row r (loaded one step ahead)
   bool fresh = false;        // running state == snapshot (last operation was a phase-C update)
   bool saved = false;        // snapshot parked in shared memory
@@ -389,6 +389,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
             f.p0 = h0.x; f.p1 = 0.f; f.p2 = dy / d; f.p3 = dz / d; f.p4 = 0.f;
             kf_reset_cov(f, K);
             phase = PH_A; r = r0; cur = c0; top = r0; top_hit = c0; gap = 0; n_hits = 0; first = r0;
+            h_pre = h0; nxt_pre = c1;
             fresh = false; saved = false;
           } else {
             const float4* o = hs + (size_t)wi * kHsV;
@@ -443,10 +444,13 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
         h = h_pre; nxt = nxt_pre;
         if (r - 2 >= r0) nn = hcol[r - 2];
         if (nxt >= 0) hn = __ldg(&syz[off + nxt]);
+      } else if (MODE == MODE_A) {
+        // link following: the chain is walked one link ahead of the fit (same reason)
+        h = h_pre; nxt = nxt_pre;
+        if (nxt >= 0) { nn = __ldg(&link_up[off + nxt]); hn = __ldg(&syz[off + nxt]); }
       } else {
         if (cand >= 0) h = __ldg(&syz[off + cand]);
-        if (phase == PH_A) nxt = __ldg(&link_up[off + cand]);
-        else if (phase == PH_C && r - 1 >= r0) nxt = hcol[r - 1];
+        if (phase == PH_C && r - 1 >= r0) nxt = hcol[r - 1];
       }
       xr = t_x[r];
       if (phase == PH_C && fresh && cand < 0) { save_snap(); snap_n = f.n; saved = true; fresh = false; }
@@ -586,7 +590,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     }
     // ---- advance to the next row -------------------------------------------------------------
     if (go) {
-      if (phase == PH_A) { cur = nxt; ++r; if (cur == -1) { phase = PH_B; gap = 0; } }
+      if (phase == PH_A) { cur = nxt; ++r; if (MODE == MODE_A) { nxt_pre = nn; h_pre = hn; } if (cur == -1) { phase = PH_B; gap = 0; } }
       else if (phase == PH_B) ++r;
       else { cur = nxt; --r; if (MODE == MODE_C1) { nxt_pre = nn; h_pre = hn; } }
       if (phase == PH_B && r >= n_rows) ev = EV_TO_C;
