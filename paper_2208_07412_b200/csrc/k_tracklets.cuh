@@ -165,11 +165,11 @@ constexpr int kS5Threads = 128;   // threads per block of k_tracklets
 constexpr int kS5BlocksPerSMA = TPCCA_S5_BPS_A;   // ... of the phase-A kernel (no search code: fewer registers)
 constexpr int kS5BlocksPerSM = TPCCA_S5_BPS;  // resident blocks per SM the kernel is compiled for (persistent grid)
 #ifndef TPCCA_S5_REFILL
-#define TPCCA_S5_REFILL 4
+#define TPCCA_S5_REFILL 6
 #endif
 constexpr int kS5Refill = TPCCA_S5_REFILL;      // idle lanes of a warp that trigger a refill from the work counter
 #ifndef TPCCA_S5_UNROLL
-#define TPCCA_S5_UNROLL 6
+#define TPCCA_S5_UNROLL 5
 #endif
 constexpr int kS5Unroll = TPCCA_S5_UNROLL;   // candidate loads in flight per lane in the S5 search
 #ifndef TPCCA_S5_PREFETCH
