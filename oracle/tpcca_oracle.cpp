@@ -23,9 +23,12 @@
 // geometry, score == 0), P5 link invariants, P6 noise-free helix recovery 1e-5 (double),
 // P7 textbook weighted-least-squares reduction, P8 pulls / chi2, P9 covariance sanity,
 // P10 generator truth (efficiency / fake), P11 determinism, P12 z-translation, plus a
-// finite-difference pin of the transport Jacobian.  Nothing can be pinned to values the
-// paper prints (it prints none): S5's heuristic choices (gate, gap, passes) are pinned
-// only by P4/P6/P7/P8/P10 -- "parity unpinned to the paper" in that sense.
+// finite-difference pin of the transport Jacobian; the S5 DECISIONS (gap counting, phase-A
+// gate, tc_min_hits, search window / tie-break, chi2 gate, readings R2 / R3) by the
+// hand-worked toy tests/golden/toy_tracklets.txt and by the one-bin-per-row (brute-force
+// search) metamorphic pin; tests/mutation_check.py re-checks that one-line mutations of
+// those decisions fail a pin.  Nothing can be pinned to values the paper prints (it prints
+// none) -- "parity unpinned to the paper" in that sense only.
 // =========================================================================================
 #include <algorithm>
 #include <cmath>
@@ -390,7 +393,7 @@ class Oracle {
         }
       }
     }
-    // ---- phase C: start at the highest row holding a hit (reading R2)
+    // ---- phase C: start at the highest row holding a hit (DESIGN.md 3.8 reading R2)
     reset_cov(s);
     int gap = 0;
     bool have_snap = false;

@@ -231,6 +231,20 @@ def test_toy_worked_example(pkg):
     trk.close()
 
 
+@pytest.mark.parametrize("reverse_ids", [False, True])
+def test_toy_tracklet_decisions(pkg, reverse_ids):
+    """The hand-worked S5 decision toy (tests/golden/toy_tracklets.txt) through the CUDA path: expected
+    membership written by hand (gaps, phase-A gate, min hits, window edges, tie-breaks, chi2 gate, R2 / R3)."""
+    import toy_tracklets
+    for sc in toy_tracklets.load():
+        y, z, row = sc.arrays(reverse_ids)
+        tf = ArrTF(sc.params(), [(y, z, row)])
+        trk = run_gpu(pkg, tf)
+        toy_tracklets.check_result(sc, trk.get_tracks(0), reverse_ids)
+        compare_timeframe(trk, tf, Oracle(tf.params))
+        trk.close()
+
+
 def test_straight_tracks_dyadic(pkg):
     """P4 on the GPU: exact recovery, 152-hit tracks, rows 0 and 151 attached by the search."""
     row_x = 64.0 + 0.75 * np.arange(152)

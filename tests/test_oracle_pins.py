@@ -681,3 +681,106 @@ def test_p12_z_translation_is_exact():
     for u, v in zip(_all_arrays(a), _all_arrays(b)):
         assert np.array_equal(u, v)
     assert np.array_equal(a.z_ref + shift, b.z_ref)
+
+
+# ----------------------------------------------------------------------------------------
+# S5 decisions: hand-worked toy (tests/golden/toy_tracklets.txt)
+# ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", ["f32", "f64"])
+@pytest.mark.parametrize("reverse_ids", [False, True])
+def test_toy_tracklet_decisions(precision, reverse_ids):
+    """Gap counting (phase B, phase C below the start row only), the phase-A gate from the third
+    hit, tc_min_hits, window edges, search tie-breaks, the chi2 gate just inside / outside (threshold
+    from the textbook prediction variance of a straight-line fit) and readings R2 / R3: expected
+    membership written by hand in the golden file, never by an implementation."""
+    import toy_tracklets
+    scen = toy_tracklets.load()
+    assert [s.name for s in scen] == ["A", "B", "C"] and sum(len(s.tracks) for s in scen) >= 20
+    for sc in scen:
+        y, z, row = sc.arrays(reverse_ids)
+        res = Oracle(sc.params(), precision).run(y, z, row)
+        toy_tracklets.check_result(sc, res, reverse_ids)
+
+
+# ----------------------------------------------------------------------------------------
+# full pipeline: tracks do not depend on the grid (bin size -> one bin per row = brute force)
+# ----------------------------------------------------------------------------------------
+def tracks_in_original_ids(res):
+    """{original id of the start hit: (hit original ids, x_ref, z_ref, par, cov, chi2, n_fit)}"""
+    o = res.order.astype(np.int64)
+    out = {}
+    for t in range(res.n_tracks):
+        hits = o[res.hit_idx[res.hit_offset[t]:res.hit_offset[t + 1]]]
+        out[int(o[res.trk_start_hit[t]])] = (tuple(hits.tolist()), res.x_ref[t], res.z_ref[t], tuple(res.par[t]),
+                                             tuple(res.cov[t]), res.chi2[t], int(res.n_fit[t]))
+    return out
+
+
+@pytest.mark.parametrize("config,n_tracks,sector", [(1, 600, 3), (4, 1500, 0)])
+def test_tracks_independent_of_grid_and_brute_force_search(config, n_tracks, sector):
+    """P3 extended to S5: hit lists, parameters, covariances and chi2 in original-id space are
+    bit-identical under other bin sizes / margins.  With bin_scale = 1000 every row is ONE bin, so
+    the S2 windows and every S5 Search walk the whole row: the grid search equals brute force."""
+    tf = tpcsynth.generate(config, n_tracks=n_tracks)
+    y, z, row = tf.y[sector], tf.z[sector], tf.row[sector]
+    assert y.shape[0] <= 8000
+    sigma = tf.params.sigma
+    base = tracks_in_original_ids(Oracle(tf.params).run(y, z, row))
+    assert len(base) > 60
+    for bs, gm in ((0.5, 0.01), (1.7, 0.01), (3.0, 0.5), (1000.0, 0.0)):
+        P2 = tpcsynth.default_params(n_sectors=36, sigma=sigma, bin_scale=bs, grid_margin=gm)
+        if bs == 1000.0:
+            assert np.all(P2.grid_ny == 1) and np.all(P2.grid_nz == 1)
+        got = tracks_in_original_ids(Oracle(P2).run(y, z, row))
+        assert got == base, (bs, gm)
+
+
+def test_search_on_dense_rows_equals_whole_row_scan():
+    """Dense uniform clusters (several candidates in every search window, S5 decisions dominated by
+    Search): one bin per row (whole-row scan) and the default grid give bit-identical tracks."""
+    P = tpcsynth.default_params(n_sectors=1)
+    rng = np.random.default_rng(8)
+    n = 1800
+    row = rng.integers(0, 40, n).astype(np.uint16)
+    y = (rng.random(n) * 10.0 - 5.0).astype(np.float32)
+    z = (rng.random(n) * 24.0).astype(np.float32)
+    # thread a few straight tracks through the noise so that searches have something to extend
+    rx = P.row_x.astype(np.float64)
+    r2, y2, z2, _ = tpcsynth.straight_tracks(rx[:40], [-3.0, 0.0, 2.5], [0.05, -0.02, 0.0], [4.0, 12.0, 20.0], [0.1, 0.0, -0.1])
+    row = np.concatenate([row, r2]); y = np.concatenate([y, y2.astype(np.float32)]); z = np.concatenate([z, z2.astype(np.float32)])
+    P1 = tpcsynth.default_params(n_sectors=1, bin_scale=1000.0, grid_margin=0.0)
+    a = tracks_in_original_ids(Oracle(P).run(y, z, row))
+    b = tracks_in_original_ids(Oracle(P1).run(y, z, row))
+    assert len(a) >= 3 and a == b
+
+
+# ----------------------------------------------------------------------------------------
+# n14 (d z / d q/pT) where its second term, (k d) d^2 / 12, dominates
+# ----------------------------------------------------------------------------------------
+def test_jacobian_n14_arc_term():
+    """A long symmetric step (sin phi: -a -> +a, so dy = 0 and the chord term (dy/d) j4 of n14
+    vanishes) leaves n14 = p3 Bc (k d) d^2 c12.  Compared with central differences of the z
+    transport in q/pT: pins c12 = 1/12 (1/6 would be off by a factor 2)."""
+    P = tpcsynth.default_params(n_sectors=1)
+    orc = Oracle(P, "f64")
+    Bc = float(P.kappa_per_qpt)
+    x1, x2 = 100.0, 130.0
+    p4 = 5.0
+    a = 0.5 * p4 * Bc * (x2 - x1)
+    p = np.array([1.0, 2.0, -a, 0.8, p4])
+    tri = lambda i, j: i * (i + 1) // 2 + j
+
+    def z_at(q4):
+        q = p.copy(); q[4] = q4
+        ok, s = orc.kf_propagate(_state(x1, q), x2)
+        assert ok
+        return s[2], s[1]
+    z0, y_end = z_at(p4)
+    assert abs(y_end - 1.0) < 1e-12                                   # symmetric step: dy == 0
+    h = 1e-4
+    fd = (z_at(p4 + h)[0] - z_at(p4 - h)[0]) / (2 * h)
+    C = np.zeros(15); C[tri(4, 4)] = 1.0
+    ok, s = orc.kf_propagate(_state(x1, p, C), x2)
+    n14 = s[6 + tri(4, 1)]                                            # C'_41 = J_14 * J_44
+    want = p[3] * Bc * (p4 * Bc * 30.0) * 900.0 / 12.0                # p3 Bc (k d) d^2 / 12 with d = dx
+    assert abs(fd - want) < 0.02 * want and abs(n14 - fd) < 0.02 * abs(fd), (n14, fd, want)
