@@ -46,7 +46,7 @@ def load_peaks():
     if os.path.exists(p):
         d = json.load(open(p))
         return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
-    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+    return dict(hbm_gbs=7700.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md nominal)")
 
 
 def ncu_traffic(args, n_clusters):
@@ -265,7 +265,8 @@ def run_tpcca(args):
     s2_gbs = s2_bytes / (stage_ms[1] * 1e-3) / 1e9
     flops = (work["propagations"] * FLOPS_PROPAGATE + work["updates"] * FLOPS_UPDATE + work["gates"] * FLOPS_GATE
              + work["searches"] * FLOPS_SEARCH + work["candidates"] * FLOPS_CANDIDATE)
-    alu_peak = 148 * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12       # T fp32 op/s without FMA
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    alu_peak = n_sm * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12      # T fp32 op/s without FMA
     s5_tops = flops / (stage_ms[4] * 1e-3) / 1e12
 
     # ---- end to end: host buffers in, host buffers out, through the public API ---------------------

@@ -209,6 +209,12 @@ int tpcca_get_work_counters(tpcca_ctx *ctx, int64_t out[5]);
 /* Number of kernels the last tpcca_run launched (for bench.py's "gpu_launches"). */
 int tpcca_get_launch_count(const tpcca_ctx *ctx, int64_t *out);
 
+/* How the context was configured by tpcca_create from its capacities (for tests and logs): out[0] = log2 of the
+ * z slices per S1 coarse bucket, out[1] = S1 coarse buckets per sector, out[2] = S2 kernel variant (hit-list
+ * depth per side), out[3] = SMs of the device, out[4] = resident S2 blocks per SM, out[5] = max_clusters_total,
+ * out[6] = max_start_hits, out[7] = workspace bytes in use.  No device work.  Errors: TPCCA_E_ARG. */
+int tpcca_get_info(const tpcca_ctx *ctx, int64_t out[8]);
+
 /* Message of the last failing call on this context ("" if none).  Never NULL.  With ctx == NULL:
  * the message of the last failing tpcca_create / tpcca_workspace_bytes of this thread. */
 const char *tpcca_last_error(const tpcca_ctx *ctx);

@@ -24,7 +24,7 @@ _up = C.POINTER(C.c_uint32)
 #: every symbol include/tpcca.h declares
 ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "tpcca_reset", "tpcca_run",
                "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
-               "tpcca_get_launch_count", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
+               "tpcca_get_launch_count", "tpcca_get_info", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
 
 
@@ -89,6 +89,7 @@ def load_library():
     lib.tpcca_get_timings.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_float)]
     lib.tpcca_get_work_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+    lib.tpcca_get_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_last_error.argtypes = [C.c_void_p]
     lib.tpcca_last_error.restype = C.c_char_p
     lib.tpcca_destroy.argtypes = [C.c_void_p]
@@ -185,7 +186,8 @@ def _np(ptr, n, dtype):
 class Tracker:
     """One tpcca context: tables + a torch-owned device workspace + the current torch stream."""
 
-    def __init__(self, params, max_clusters: int, max_start_hits: int = 0, device: int = 0, stream=None):
+    def __init__(self, params, max_clusters: int, max_start_hits: int = 0, device: int = 0, stream=None,
+                 workspace_fill: int | None = None):
         import torch  # device memory and streams only
         self._lib = load_library()
         if not torch.cuda.is_available():
@@ -202,6 +204,9 @@ class Tracker:
         self.workspace_bytes = int(nbytes.value)
         with torch.cuda.device(self.device):
             self._ws = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8, device=f"cuda:{self.device}")
+            if workspace_fill is not None:      # tests: the library must not depend on what the workspace held
+                self._ws.fill_(int(workspace_fill))
+                torch.cuda.synchronize(self.device)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         base = self._ws.data_ptr()
         aligned = (base + 255) // 256 * 256
@@ -297,6 +302,13 @@ class Tracker:
         out = (C.c_int64 * 5)()
         self._check(self._lib.tpcca_get_work_counters(self._h, out))
         return dict(zip(("propagations", "updates", "gates", "searches", "candidates"), (int(v) for v in out)))
+
+    def info(self) -> dict:
+        """tpcca_get_info: how tpcca_create configured the context."""
+        out = (C.c_int64 * 8)()
+        self._check(self._lib.tpcca_get_info(self._h, out))
+        return dict(zip(("slab_shift", "n_coarse_buckets", "s2_variant", "sm_count", "s2_blocks_per_sm", "max_clusters",
+                         "max_start_hits", "workspace_bytes"), (int(v) for v in out)))
 
     def launch_count(self) -> int:
         out = C.c_int64(0)

@@ -43,7 +43,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     cmd = [_nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include")]
-    cmd += os.environ.get("TPCCA_NVCC_EXTRA", "").split()   # tuning experiments, e.g. -DTPCCA_S5_BPS=6
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]

@@ -269,7 +269,7 @@ constexpr int kNfTile = TPCCA_NF_TILE;
 
 __global__ void __launch_bounds__(1024)
 k_row_tables(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_start,
-             int32_t* __restrict__ row_start, int32_t* __restrict__ nf_tile_start) {
+             int32_t* __restrict__ row_start, int32_t* __restrict__ nf_tile_start, const DevStatus* __restrict__ st) {
   __shared__ int ws[33];
   const int nr = T->n_rows, ns = T->n_sectors;
   const size_t stride = (size_t)T->bins_per_sector + 1;
@@ -286,7 +286,7 @@ k_row_tables(const DevTables* __restrict__ T, const uint32_t* __restrict__ bin_s
     if (i < n) {
       const int s = i / nr, r = i - s * nr;
       const int cnt = row_start[s * (nr + 1) + r + 1] - row_start[s * (nr + 1) + r];
-      v = (cnt + kNfTile - 1) / kNfTile;
+      v = st->err_range ? 0 : (cnt + kNfTile - 1) / kNfTile;     // a failed S1 (TPCCA_E_RANGE) leaves S2 nothing to do
     }
     int total;
     const int ex = block_exclusive_scan<int>(v, ws, total);

@@ -37,9 +37,6 @@ constexpr int kNfArena = TPCCA_NF_ARENA;  // bytes of one staging buffer: [up cl
 constexpr int kNfMaxCn = 1022;            // staged clusters per side (staged indices are packed in 10 bits)
 constexpr int kNfMaxRun = 63;             // window candidates per side handled by the packed fast path
 
-#ifdef TPCCA_NF_STATS
-__device__ unsigned long long g_nf_hist[4][64];   // tests per side, hits per side, pairs, pairs under cut
-#endif
 enum { NF_STAGED = 0, NF_NOLINK = 1, NF_GLOBAL = 2, NF_STAGED_C = 3 };   // STAGED_C: clusters staged, bins read from global memory
 
 struct NfSide {        // staging of one neighbour row for one tile
@@ -552,8 +549,15 @@ __global__ void __launch_bounds__(256)
 k_clean_links(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
               const int32_t* __restrict__ up_raw, const int32_t* __restrict__ dn_raw,
               int32_t* __restrict__ up, int32_t* __restrict__ dn, int2* __restrict__ tile_cnt,
-              uint32_t* __restrict__ start_bits /*[tile][64]: bit p of the tile = start hit (read by S4)*/) {
+              uint32_t* __restrict__ start_bits /*[tile][64]: bit p of the tile = start hit (read by S4)*/,
+              const DevStatus* __restrict__ st) {
   __shared__ int ws[33];
+  if (st->err_range) {     // S1 dropped clusters (row >= n_rows): positions >= n - dropped were never written by S1 / S2.
+    // The run is reported as TPCCA_E_RANGE; S3-S5 produce nothing (no start hit) instead of following stale links.
+    if (threadIdx.x < 64) start_bits[(size_t)blockIdx.x * 64 + threadIdx.x] = 0u;
+    if (threadIdx.x == 0) tile_cnt[blockIdx.x] = make_int2(0, 0);
+    return;
+  }
   const int ns = __ldg(&T->n_sectors);
   const int s = find_sector(ns, blockIdx.x, [&](int i) { return __ldg(&sec[i].tile2048); });
   const int n = __ldg(&sec[s].n), off = __ldg(&sec[s].off);
@@ -565,8 +569,9 @@ k_clean_links(const DevTables* __restrict__ T, const SectorDesc* __restrict__ se
     bool is_start = false;
     if (p < n) {
       const int32_t u = up_raw[off + p], d = dn_raw[off + p];
-      const int32_t uc = (u >= 0 && __ldg(&dn_raw[off + u]) == p) ? u : -1;
-      const int32_t dc = (d >= 0 && __ldg(&up_raw[off + d]) == p) ? d : -1;
+      // (u, d < n always holds for links written by S2; the bound is a safety net against stale workspace bytes)
+      const int32_t uc = (u >= 0 && u < n && __ldg(&dn_raw[off + u]) == p) ? u : -1;
+      const int32_t dc = (d >= 0 && d < n && __ldg(&up_raw[off + d]) == p) ? d : -1;
       up[off + p] = uc;
       dn[off + p] = dc;
       is_start = (dc == -1 && uc >= 0);

@@ -150,7 +150,6 @@ __device__ __forceinline__ void kf_update(KF& s, float ym, float zm, const KFCon
   s.n++;
 }
 
-// slot-space scratch of S5 (SoA with stride cap): 24 float planes + 4 int planes
 // slot-space scratch of S5: one record of kTrkV 16-byte vectors per slot (written by the lane that completes the
 // tracklet with 128-bit stores, read by k_track_gather) + the n_hits plane (0 = rejected) the scans read
 constexpr int kTrkV = 7;    // (n_fit, first_row, last_row, -) (x_ref, z_ref, p0, p1) (p2, p3, p4, c00) ... (c43, c44, chi2, -)
@@ -172,10 +171,6 @@ constexpr int kS5Refill = TPCCA_S5_REFILL;      // idle lanes of a warp that tri
 #define TPCCA_S5_UNROLL 5
 #endif
 constexpr int kS5Unroll = TPCCA_S5_UNROLL;   // candidate loads in flight per lane in the S5 search
-#ifndef TPCCA_S5_PREFETCH
-#define TPCCA_S5_PREFETCH 0
-#endif
-constexpr int kS5Prefetch = TPCCA_S5_PREFETCH;   // 0 off, 1 L1, 2 L2
 constexpr int kSnapF = 22;        // floats of a saved Kalman state: x, p[5], c[15], chi2
 
 // scalars of S5, passed by value (constant bank: no registers)
@@ -185,11 +180,6 @@ struct S5Params {
   float win_y, win_z, gate, margin, grid_z_lo;
   int32_t n_rows, n_sectors, max_gap, min_hits, bins_per_sector;
 };
-
-__device__ __forceinline__ void prefetch_l1(const void* p) {
-  if (kS5Prefetch == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-  else asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-}
 
 // approximate reciprocal (one MUFU.RCP); used only to rank candidates and to pre-decide gates
 // that are nowhere near the threshold -- every decision that could flip is taken on the exact form
@@ -245,7 +235,7 @@ __device__ __noinline__ int search_exact(float p0, float p1, float z_ref, float 
 // The phase-C snapshot ("state right after the last update") lives in registers while it equals
 // the running state and is parked in shared memory the moment the running state moves on without
 // an update, which keeps the register count at one Kalman state per lane.
-// The kernel is compiled in three modes and launched three times: MODE_A runs phase A
+// The kernel is compiled in four modes and launched four times: MODE_A runs phase A
 // for every start hit, MODE_B phase B, MODE_C1 phase C down to the start row (hits known: updates, a search
 // only on gap rows), MODE_C2 phase C below the start row (a search every row).  A lane whose tracklet leaves the kernel's phase
 // parks the tracklet (Kalman state + bookkeeping, kHsF floats and kHsI ints, indexed by the work
@@ -278,7 +268,7 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   }
   for (int i = threadIdx.x; i <= ns; i += blockDim.x) s_sec_off[i] = sec[i].off;
   __syncthreads();
-  if (st->err_capacity) return;
+  if (st->err_capacity || st->err_range) return;
   const int n_start = st->n_start;
   KFConst K;
   K.Bc = P.Bc; K.err2_y = P.err2_y; K.err2_z = P.err2_z; K.max_sinphi = P.max_sinphi;
@@ -605,22 +595,6 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     }
     if (MODE == MODE_A && phase == PH_B) park();
     if (MODE == MODE_C1 && phase == PH_C && r < r0) { phase = PH_C2; park(); }
-    // ---- prefetch hint for the next row's search (kernels that search every row) ---------------------
-    // Straight-line guess of the next prediction; only the cache lines of the bin_start entries around
-    // it are touched (no value is used), so the hint cannot change any result.
-    if ((MODE == MODE_B || MODE == MODE_C2) && kS5Prefetch && phase != PH_IDLE && r >= 0 && r < n_rows) {
-      const float dxn = t_x[r] - f.x;
-      const float sec = rsqrtf(fmaxf(1.0f - f.p2 * f.p2, 0.05f));
-      const float yn = f.p0 + dxn * (f.p2 * sec);
-      const float zn = z_ref + f.p1 + dxn * (f.p3 * sec);
-      const int nyh = t_nyh[r], nzh = t_nzh[r], ny = t_ny[r];
-      const int by = bin_range(yn - my, t_ylo[r], t_iby[r], nyh);
-      const int bz = bin_range(zn - mz, P.grid_z_lo, t_ibz[r], nzh);
-      const uint32_t* bp = bin_start + (bs_off + (uint32_t)(t_base[r] + bz * ny + by));
-      const int up = (bz < nzh) ? ny : 0;
-      prefetch_l1(bp); prefetch_l1(bp + 2);
-      prefetch_l1(bp + up); prefetch_l1(bp + up + 2);
-    }
   }
   // work counters: one atomic per warp and counter
   unsigned long long w[5] = {w_prop, w_upd, w_gate, w_search, w_cand};

@@ -201,6 +201,22 @@ int set_err(tpcca_ctx* c, int code, const char* fmt, ...) {
     if (e_ != cudaSuccess) return set_err((c), TPCCA_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 
+// Every entry point that issues CUDA calls runs on the context's device and leaves the caller's current device
+// as it found it (a host thread that serves several GPUs must not have its device switched under it).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int dev) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) { err = cudaSetDevice(dev); switched = (err == cudaSuccess); }
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define GUARD(c)                                                                                        \
+  DeviceGuard guard_((c)->device);                                                                      \
+  if (guard_.err != cudaSuccess) return set_err((c), TPCCA_E_CUDA, "cudaSetDevice(%d) failed: %s", (c)->device, cudaGetErrorString(guard_.err))
+
 int fetch_status(tpcca_ctx* c);
 
 int status_errors(tpcca_ctx* c) {
@@ -272,7 +288,8 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     return set_err(nullptr, TPCCA_E_CUDA, "no usable CUDA device (%s); tpcca has no CPU path",
                    ce != cudaSuccess ? cudaGetErrorString(ce) : "device count 0");
   if (cuda_device < 0 || cuda_device >= n_dev) return set_err(nullptr, TPCCA_E_ARG, "cuda_device out of range");
-  CU(nullptr, cudaSetDevice(cuda_device));
+  DeviceGuard guard(cuda_device);
+  if (guard.err != cudaSuccess) return set_err(nullptr, TPCCA_E_CUDA, "cudaSetDevice(%d) failed: %s", cuda_device, cudaGetErrorString(guard.err));
   cudaDeviceProp prop;
   CU(nullptr, cudaGetDeviceProperties(&prop, cuda_device));
   if (prop.major != 10)
@@ -348,7 +365,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     if (ez == cudaSuccess) ez = cudaStreamSynchronize(c->stream);
     if (ez != cudaSuccess) {
       set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(ez));
-      delete c;
+      tpcca_destroy(c);      // one cleanup path: releases whatever the partially built context owns
       return TPCCA_E_CUDA;
     }
   }
@@ -359,7 +376,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     for (int i = 0; i < 6 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
-    delete c;
+    tpcca_destroy(c);
     return TPCCA_E_CUDA;
   }
   {
@@ -373,7 +390,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
     cudaError_t e2 = cudaFuncSetAttribute(nf_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_smem);
     if (e2 != cudaSuccess) {
       set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: shared memory opt-in of k_neighbours failed: %s", cudaGetErrorString(e2));
-      delete c;
+      tpcca_destroy(c);
       return TPCCA_E_CUDA;
     }
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, nf_fn, kNfThreads, nf_smem) == cudaSuccess && occ > 0)
@@ -404,6 +421,7 @@ int tpcca_load_clusters(tpcca_ctx* c, int sector, int64_t n, const float* x, con
   int64_t tot = n;
   for (auto& s : c->sec) if (s.loaded) tot += s.n;
   if (tot > c->N) return set_err(c, TPCCA_E_WORKSPACE, "%lld clusters exceed max_clusters_total %lld", (long long)tot, (long long)c->N);
+  GUARD(c);
   auto& S = c->sec[sector];
   if (mem_space == TPCCA_MEM_DEVICE_BORROW || n == 0) {
     S.y = y; S.z = z; S.row = row;
@@ -438,7 +456,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
       if ((need & ~(c->done_mask | mask)) != 0)
         return set_err(c, TPCCA_E_STATE, "stage %d needs the outputs of earlier stages (done 0x%x, asked 0x%x)", i + 1, c->done_mask, mask);
     }
-  CU(c, cudaSetDevice(c->device));
+  GUARD(c);
   const Layout& L = c->L;
   cudaStream_t st = c->stream;
   c->launches = 0;
@@ -446,14 +464,13 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   // ---- sector descriptors
   if (!c->desc_valid) {
     c->desc.assign(kMaxSectors + 1, SectorDesc{});
-    int64_t off = 0, t256 = 0, t2048 = 0, bt = 0;
-    const int64_t bin_tiles = 0;
+    int64_t off = 0, t256 = 0, t2048 = 0;
     for (int s = 0; s <= c->ns; ++s) {
       SectorDesc& d = c->desc[s];
       const int64_t n = s < c->ns ? c->sec[s].n : 0;
       if (s < c->ns) { d.y = c->sec[s].y; d.z = c->sec[s].z; d.row = c->sec[s].row; }
-      d.n = (int32_t)n; d.off = (int32_t)off; d.tile256 = (int32_t)t256; d.tile2048 = (int32_t)t2048; d.bin_tile = (int32_t)bt;
-      off += n; t256 += (n + 255) / 256; t2048 += (n + 2047) / 2048; bt += bin_tiles;
+      d.n = (int32_t)n; d.off = (int32_t)off; d.tile256 = (int32_t)t256; d.tile2048 = (int32_t)t2048;
+      off += n; t256 += (n + 255) / 256; t2048 += (n + 2047) / 2048;
     }
     c->n_total = off; c->n_tiles256 = (int)t256; c->n_tiles2048 = (int)t2048;
     int64_t mx = 0;
@@ -476,7 +493,15 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   const int32_t cap = (int32_t)c->CS;
   const int slot_ev = (int)(c->run_count % tpcca_ctx::kRing);
   c->ev_mask[slot_ev] = 0;
-  auto mark = [&](int i) { cudaEventRecord(c->ev[slot_ev][i], st); };
+  // end of a stage: its event, and the launch errors of ITS kernels (so a failed launch names its stage)
+  static const char* const kStageName[6] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets"};
+  cudaError_t stage_err = cudaSuccess;
+  int stage_bad = -1;
+  auto mark = [&](int i) {
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev[slot_ev][i], st);
+    if (e != cudaSuccess && stage_err == cudaSuccess) { stage_err = e; stage_bad = i; }
+  };
   mark(0);
 
   if (mask & TPCCA_STAGE_GRID) {
@@ -505,7 +530,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     k_grid_sort<<<(unsigned)(c->ns * L.n_cb), 256, 0, st>>>(T, sec, c->at<int32_t>(L.zorder) + L.n_cb, cb_start, rec, syz, order, bin_start, big, status);
     k_grid_big<<<c->sm_count * 4, 256, 0, st>>>(T, sec, cb_start, rec, syz, order, bin_start, big, status);
     c->launches += 2;
-    k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start));
+    k_row_tables<<<1, 1024, 0, st>>>(T, bin_start, row_start, c->at<int32_t>(L.nf_tile_start), status);
     c->launches += 1;
   }
   mark(1);
@@ -514,7 +539,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     const int grid = (int)std::min<int64_t>(tiles_ub, (int64_t)c->sm_count * c->nf_blocks_per_sm);
     NfTileDesc* nfd = c->at<NfTileDesc>(L.nf_desc);
     const int32_t* nf_ts = c->at<int32_t>(L.nf_tile_start);
-    k_nf_plan<<<std::min(c->ns * c->nr, 148 * 64), 128, 0, st>>>(T, sec, syz, bin_start, row_start, nf_ts, nfd);
+    k_nf_plan<<<std::min(c->ns * c->nr, c->sm_count * 64), 128, 0, st>>>(T, sec, syz, bin_start, row_start, nf_ts, nfd);
     if (c->nf_dense)
       k_neighbours<kNfKDense><<<grid, kNfThreads, sizeof(NfSmem<kNfKDense>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
                                                                                    nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
@@ -528,7 +553,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   mark(2);
   if ((mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
     k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
-                                                 c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits));
+                                                 c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits), status);
     ++c->launches;
   }
   mark(3);
@@ -537,7 +562,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     // buffer, so S4 on its own recounts through S3's kernel (cheap, idempotent).
     if (!(mask & TPCCA_STAGE_CLEAN) && c->n_tiles2048 > 0) {
       k_clean_links<<<c->n_tiles2048, 256, 0, st>>>(T, sec, c->at<int32_t>(L.up_raw), c->at<int32_t>(L.dn_raw),
-                                                   c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits));
+                                                   c->at<int32_t>(L.up), c->at<int32_t>(L.dn), tile_cnt, c->at<uint32_t>(L.start_bits), status);
       ++c->launches;
     }
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, c->n_tiles2048, tot);
@@ -599,7 +624,8 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     c->launches += 9;
   }
   mark(5);
-  CU(c, cudaGetLastError());
+  if (stage_err != cudaSuccess)
+    return set_err(c, TPCCA_E_CUDA, "tpcca_run: stage %s failed: %s", kStageName[stage_bad], cudaGetErrorString(stage_err));
   c->ev_mask[slot_ev] = mask;
   ++c->run_count;
   c->done_mask |= mask;
@@ -608,11 +634,13 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
 
 int tpcca_sync(tpcca_ctx* c) {
   if (!c) return TPCCA_E_ARG;
+  GUARD(c);
   return fetch_status(c);
 }
 
 int tpcca_get_counts(tpcca_ctx* c, int64_t out[5]) {
   if (!c || !out) return TPCCA_E_ARG;
+  GUARD(c);
   int rc = fetch_status(c);
   if (rc) return rc;
   out[0] = c->n_total;
@@ -630,6 +658,7 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[6]) {
   if (runs_back >= c->run_count) return set_err(c, TPCCA_E_STATE, "no such run");
   const int k = (int)((c->run_count - 1 - runs_back) % tpcca_ctx::kRing);
   if (!c->ev_mask[k]) return set_err(c, TPCCA_E_STATE, "no such run");
+  GUARD(c);
   CU(c, cudaStreamSynchronize(c->stream));
   for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[k][i], c->ev[k][i + 1]));
   CU(c, cudaEventElapsedTime(&ms[5], c->ev[k][0], c->ev[k][5]));
@@ -638,9 +667,17 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[6]) {
 
 int tpcca_get_work_counters(tpcca_ctx* c, int64_t out[5]) {
   if (!c || !out) return TPCCA_E_ARG;
+  GUARD(c);
   int rc = fetch_status(c);
   if (rc) return rc;
   for (int i = 0; i < 5; ++i) out[i] = (int64_t)c->status.work[i];
+  return TPCCA_OK;
+}
+
+int tpcca_get_info(const tpcca_ctx* c, int64_t out[8]) {
+  if (!c || !out) return TPCCA_E_ARG;
+  out[0] = c->tab.slab_shift; out[1] = c->tab.n_cb; out[2] = c->nf_dense ? kNfKDense : kNfK; out[3] = c->sm_count;
+  out[4] = c->nf_blocks_per_sm; out[5] = c->N; out[6] = c->CS; out[7] = (int64_t)c->L.total;
   return TPCCA_OK;
 }
 
@@ -655,6 +692,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
   if (mem_space != TPCCA_MEM_HOST && mem_space != TPCCA_MEM_DEVICE) return set_err(c, TPCCA_E_ARG, "bad mem_space");
   if (!c->done_mask || !c->desc_valid) return set_err(c, TPCCA_E_STATE, "nothing was run");
+  GUARD(c);
   const bool host = mem_space == TPCCA_MEM_HOST;
   // HOST copies wait only for the last stage whose outputs are asked for (so that the links of a time
   // frame can travel while S5 still runs); the track counts are filled once S5 is covered.
@@ -739,8 +777,11 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   for (auto& it : items) {
     char* dst = c->arena + cur;
     if (it.bytes) {
-      if (it.planes == 1) CU(c, cudaMemcpyAsync(dst, it.src, it.bytes, cudaMemcpyDeviceToHost, cs));
-      else CU(c, cudaMemcpy2DAsync(dst, it.bytes, it.src, 4 * (size_t)c->CS, it.bytes, it.planes, cudaMemcpyDeviceToHost, cs));
+      // par / cov planes are CS elements apart on the device and packed (n_tracks apart) on the host: one copy per
+      // plane (a 2-D copy would be bound by the device's maximum pitch, about 2 GiB, i.e. CS < 2^29)
+      for (int pl = 0; pl < it.planes; ++pl)
+        CU(c, cudaMemcpyAsync(dst + (size_t)pl * it.bytes, (const char*)it.src + (size_t)pl * 4 * (size_t)c->CS, it.bytes,
+                              cudaMemcpyDeviceToHost, cs));
     }
     *it.dst = dst;
     cur += align_up(it.bytes * it.planes + 4);
@@ -751,6 +792,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
 
 void tpcca_destroy(tpcca_ctx* c) {
   if (!c) return;
+  DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing; ++k)
     for (int i = 0; i < 6; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);

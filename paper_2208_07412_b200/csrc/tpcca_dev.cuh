@@ -56,8 +56,7 @@ struct SectorDesc {
   int32_t off;        // first global position of the sector in the concatenated arrays
   int32_t tile256;    // first 256-cluster tile of the sector
   int32_t tile2048;   // first 2048-cluster tile of the sector
-  int32_t bin_tile;   // first 2048-bin scan tile of the sector
-  int32_t pad;
+  int32_t pad[2];
 };
 
 // Device counters / status, mirrored to pinned host memory at the end of a run.

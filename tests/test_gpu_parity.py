@@ -271,6 +271,23 @@ def test_error_paths(pkg, cfg0):
     with pytest.raises(pkg.TpccaError) as e:
         trk.sync()
     assert e.value.code == -5
+    trk.close()
+    # the same with a workspace full of 0x7f bytes and good clusters around the bad one: the positions S1 / S2 never
+    # wrote hold garbage "links"; S3-S5 must not follow them (illegal-address fault instead of E_RANGE)
+    row = tf.row[0].copy(); row[len(row) // 2] = 400
+    for fill in (0x7f, 0xff, 0x00):
+        trk = pkg.Tracker(P, max_clusters=tf.n_clusters, workspace_fill=fill)
+        trk.load_clusters(0, tf.y[0], tf.z[0], row)
+        trk.run()
+        with pytest.raises(pkg.TpccaError) as e:
+            trk.sync()
+        assert e.value.code == -5
+        # the context (and the CUDA context of the process) is still usable
+        trk.load_timeframe(tf)
+        trk.run()
+        compare_timeframe(trk, tf, Oracle(P))
+        trk.close()
+    trk = pkg.Tracker(P, max_clusters=16)
     # loading a sector twice -> E_STATE; too many clusters -> E_WORKSPACE
     trk.reset()
     trk.load_clusters(0, np.zeros(3, np.float32), np.ones(3, np.float32), np.array([1, 2, 3], np.uint16))
@@ -337,3 +354,70 @@ def test_config1_full_size(pkg):
     assert tf.n_clusters > 1_000_000
     rep = check(pkg, tf)
     assert rep["n_tracks"] > 20000 and rep["links_differing"] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# kernel instances / capacities / sizes the small cases above never select
+# ------------------------------------------------------------------------------------------------
+def test_large_capacity_selects_dense_instances(pkg, cfg0):
+    """A context whose CAPACITY exceeds 0.7 clusters per grid bin takes the S2 variant for dense time frames
+    and, above ~700 clusters per coarse bucket, the smallest S1 slab (slab_shift 5): both must give the oracle's
+    outputs.  Asserted through tpcca_get_info."""
+    tf = cfg0
+    small = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+    big = pkg.Tracker(tf.params, max_clusters=120_000)
+    a, b = small.info(), big.info()
+    small.close()
+    assert b["slab_shift"] == 5 and a["slab_shift"] > 5
+    assert b["s2_variant"] > a["s2_variant"]
+    big.load_timeframe(tf)
+    big.run()
+    rep = compare_timeframe(big, tf, Oracle(tf.params))
+    big.close()
+    assert rep["n_tracks"] > 100 and rep["links_differing"] == 0
+
+
+def test_dense_uniform_sector(pkg):
+    """A genuinely dense input: 72k uniform clusters on 12 rows of one sector (about 1.3 clusters per bin on those
+    rows; S2 windows with tens of candidates, hit lists overflowing, S5 searches over long candidate lists), in a
+    context sized for it (dense S2 variant)."""
+    P = tpcsynth.default_params(n_sectors=1)
+    rng = np.random.default_rng(17)
+    n = 72_000
+    row = rng.integers(20, 32, n).astype(np.uint16)
+    y = ((rng.random(n) * 2.0 - 1.0) * 17.0).astype(np.float32)
+    z = (rng.random(n) * 250.0).astype(np.float32)
+    tf = ArrTF(P, [(y, z, row)])
+    trk = run_gpu(pkg, tf, max_start_hits=n // 2)
+    assert trk.info()["s2_variant"] >= 15
+    rep = compare_timeframe(trk, tf, Oracle(P))
+    trk.close()
+    assert rep["links_differing"] == 0
+
+
+def test_full_time_frame_axis_128_orbits(pkg):
+    """The 29 617 cm z axis of BASELINE.json configs[3] with its full grid tables (10.3 M bins per sector):
+    collisions at t = 0, T/2 and T (fp32 ulp of z is 2e-3 cm at the far end: K-rule Z and the bin keys are the
+    parts that depend on it).  All 36 sectors, every output."""
+    T = 128 * tpcsynth.ORBIT_US
+    tf = tpcsynth.generate(3, coll_times=[0.0, 0.013, 0.5 * T, 0.5 * T + 31.0, T - 0.02, T], coll_mult=700)
+    assert max(float(z.max()) for z in tf.z) > 29_500.0 and tf.params.bins_per_sector() > 10_000_000
+    rep = check(pkg, tf)
+    assert rep["sectors"] == 36 and rep["n_tracks"] > 4000 and rep["links_differing"] == 0
+
+
+def test_config4_full_size(pkg):
+    """BASELINE.json configs[4] at full size (15k tracks, ~2.1 M clusters, 20 % noise, loopers): all sectors."""
+    tf = tpcsynth.generate(4)
+    assert tf.n_clusters > 1_800_000
+    rep = check(pkg, tf)
+    assert rep["sectors"] == 36 and rep["n_tracks"] > 20000 and rep["links_differing"] == 0
+
+
+def test_config2_full_size_six_sectors(pkg):
+    """BASELINE.json configs[2] at full size (32 orbits, ~3.6e7 clusters) on the GPU; six sectors spread over
+    both sides are compared element by element with the oracle."""
+    tf = tpcsynth.generate(2)
+    assert tf.n_clusters > 25_000_000
+    rep = check(pkg, tf, sectors=(0, 7, 13, 18, 26, 35))
+    assert rep["sectors"] == 6 and rep["n_clusters"] > 4_000_000 and rep["links_differing"] == 0

@@ -7,9 +7,9 @@ both implementations, and (b) the seeded generators of BASELINE.json configs
 0-4 together with their generator-truth bookkeeping.
 """
 from .params import TrackerParams, default_params, BC_PER_QPT, V_DRIFT, ORBIT_US
-from .generator import (CONFIGS, Timeframe, generate, generate_config,
+from .generator import (CONFIGS, Timeframe, generate,
                         truth_state, straight_tracks, helix_hits)
 
 __all__ = ["TrackerParams", "default_params", "BC_PER_QPT", "V_DRIFT", "ORBIT_US",
-           "CONFIGS", "Timeframe", "generate", "generate_config", "truth_state",
+           "CONFIGS", "Timeframe", "generate", "truth_state",
            "straight_tracks", "helix_hits"]

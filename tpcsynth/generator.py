@@ -153,12 +153,15 @@ def _collision_clusters(row_x, h, pt, phi0, eta, zv, t_us, sigma, drop, rng, sin
 def generate(config: int, seed: int | None = None, mult_scale: float = 1.0,
              n_tracks: int | None = None, n_orbits: int | None = None,
              threads: int | None = None, noise: float | None = None,
-             drop: float | None = None, sigma: float | None = None) -> Timeframe:
+             drop: float | None = None, sigma: float | None = None,
+             coll_times=None, coll_mult=None) -> Timeframe:
     """Generate the clusters of BASELINE.json config `config` (0..4).
 
     `mult_scale` scales the per-collision multiplicity (config 3 at 2.75
     reaches the ~4e8 clusters BASELINE.json:10 names); `n_tracks` / `n_orbits` / `noise` /
-    `drop` / `sigma` override the config for reduced-size test variants.
+    `drop` / `sigma` override the config for reduced-size test variants; `coll_times` [us] (with
+    `coll_mult` tracks each, default n_tracks or 500) replaces the Poisson / impact-parameter draw of a
+    time-frame config by a hand-placed list of collisions (the z axis keeps the config's full length).
     """
     cfg = dict(CONFIGS[config])
     if seed is None:
@@ -186,6 +189,13 @@ def generate(config: int, seed: int | None = None, mult_scale: float = 1.0,
         coll_t = rng0.random(n_coll) * T
         b = 15.0 * np.sqrt(rng0.random(n_coll))
         mult = np.rint(10000.0 * (1.0 - b / 15.0) ** 2 * mult_scale).astype(np.int64)
+        if coll_times is not None:
+            coll_t = np.asarray(coll_times, dtype=np.float64)
+            assert coll_t.ndim == 1 and np.all(coll_t >= 0.0) and np.all(coll_t <= T)
+            n_coll = int(coll_t.shape[0])
+            if coll_mult is None:
+                coll_mult = cfg["n_tracks"] or 500
+            mult = np.broadcast_to(np.asarray(coll_mult, dtype=np.int64), (n_coll,)).copy()
     else:
         T = 0.0
         n_coll = 1
@@ -280,10 +290,6 @@ def generate(config: int, seed: int | None = None, mult_scale: float = 1.0,
     return Timeframe(config=config, seed=seed, params=params, x=X, y=Y, z=Z, q=Q, row=ROW, label=LAB,
                      trk_coll=trk_coll, trk_h=trk_h, trk_pt=trk_pt, trk_phi0=trk_phi0,
                      trk_eta=trk_eta, trk_zv=trk_zv, coll_t=coll_t)
-
-
-def generate_config(config: int, **kw) -> Timeframe:
-    return generate(config, **kw)
 
 
 def truth_state(tf: Timeframe, track: int, sector: int, x: float):
