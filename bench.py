@@ -12,8 +12,8 @@ tpcsynth recipe of DESIGN.md 6).  N>1: one time frame per GPU (the paper's own s
               order + cleaned links + start hits + track table + hit CSR inside the timed region
   roofline  : neighbour finder (S2; the stage BASELINE.json's metric names) vs the measured HBM peak;
   roofline_dominant : the stage that takes the most time (S5 tracklets), plain-ALU bound
-  cpu_baseline : the oracle as it stands on one host core over sector 0 of the same time frame
-                 (also used as a full-size parity check of that sector)
+  cpu_baseline : the oracle as it stands, one single-threaded oracle per host core, over 4 sectors of the same
+                 time frame spread over both sides (also the full-size parity check of those sectors)
 """
 from __future__ import annotations
 
@@ -188,26 +188,140 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------------
-def run_tpcca(args):
-    import torch
+def _oracle_sector_job(job):
+    """Worker of the CPU-baseline pool (a spawned process: no CUDA in here): the oracle as it stands on one
+    sector; returns (seconds of the S1-S5 run without output copies, full OracleResult)."""
+    params, y, z, row = job
+    from oracle import Oracle
+    orc = Oracle(params)
+    t0 = time.time()
+    orc.run(y, z, row, want=())
+    dt = time.time() - t0
+    return dt, orc.run(y, z, row)
+
+
+def cpu_baseline_and_parity(args, tf, trk):
+    """The oracle on `--cpu-sectors` sectors spread over both sides, one single-threaded oracle per host core,
+    timed; its outputs are then compared element by element with the CUDA path's outputs of the same sectors."""
+    import multiprocessing as mp
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from oracle import Oracle
+    from parity import compare_sector
+    ns = tf.n_sectors
+    k = max(1, min(args.cpu_sectors, ns))
+    sectors = sorted({(i * ns) // k for i in range(k)})
+    cores = min(len(sectors), len(os.sched_getaffinity(0)))
+    jobs = [(tf.params, tf.y[s], tf.z[s], tf.row[s]) for s in sectors]
+    t0 = time.time()
+    if cores > 1:
+        with mp.get_context("spawn").Pool(cores) as pool:
+            pool.map(int, range(cores))                  # workers up (interpreter + numpy imported) before the clock starts
+            t0 = time.time()
+            out = pool.map(_oracle_sector_job, jobs, chunksize=1)
+    else:
+        out = [_oracle_sector_job(j) for j in jobs]
+    wall = time.time() - t0
+    n_s = int(sum(tf.y[s].shape[0] for s in sectors))
+    busy = sum(dt for dt, _ in out)
+    waves = -(-len(sectors) // cores)
+    # throughput of `cores` concurrent single-threaded oracles: clusters of the sample / (time of the timed runs)
+    t_timed = max(dt for dt, _ in out) * waves
+    cpu = dict(value=float(n_s / t_timed), unit=UNIT, cores=cores, kind="oracle",
+               sample=f"sectors {sectors} of {ns}: {n_s} of {tf.n_clusters} clusters, S1-S5, one sector per core, "
+                      f"{t_timed:.1f} s timed ({busy:.1f} core-s; {wall:.1f} s with the output pass)",
+               one_core_value=float(n_s / busy))
+    orc = Oracle(tf.params)
+    parity = dict(sectors=sectors, n_clusters=0, n_tracks=0, links_differing=0, membership="bit-exact",
+                  par_bit_exact=True, status="pass")
+    for s, (_, o) in zip(sectors, out):
+        g = trk.get_tracks(s)
+        try:
+            rep = compare_sector(g, o, orc, tf.row[s][o.order])
+        except AssertionError as e:
+            parity.update(status="FAIL", error=f"sector {s}: {str(e)[:300]}")
+            break
+        parity["n_clusters"] += int(o.n); parity["n_tracks"] += int(o.n_tracks)
+        parity["links_differing"] += rep["links_differing"]
+        parity["par_bit_exact"] = bool(parity["par_bit_exact"] and rep.get("par_bit_exact", True))
+    return cpu, parity
+
+
+# --------------------------------------------------------------------------------------------------
+class CudaEnv:
+    """Everything run_tpcca needs from the device side: the tpcca Tracker (the product), torch.cuda for device
+    memory / streams / events, NCCL for the barrier and the reductions.  tests/test_multirank.py swaps it for a
+    CPU stand-in (gloo, a stub Tracker) to drive the N > 1 host logic of run_tpcca without a GPU."""
+    backend = "nccl"
+
+    def __init__(self, rank, world, local):
+        import torch
+        import paper_2208_07412_b200 as pkg
+        from paper_2208_07412_b200 import binding as B
+        if not torch.cuda.is_available():
+            raise RuntimeError(f"bench.py rank {rank}/{world}: needs a CUDA device: tpcca has no CPU path")
+        torch.cuda.set_device(local)
+        self.torch, self.pkg, self.B = torch, pkg, B
+        self.local = local
+        self.device = torch.device(f"cuda:{local}")
+        self.oom_error = torch.OutOfMemoryError
+
+    def init_process_group(self):
+        import torch.distributed as dist
+        dist.init_process_group(self.backend, device_id=self.device)
+
+    def tracker(self, params, max_clusters, max_start_hits, stream=None):
+        return self.pkg.Tracker(params, max_clusters=max_clusters, max_start_hits=max_start_hits, device=self.local, stream=stream)
+
+    def pin(self, a):
+        return self.torch.from_numpy(a).pin_memory()
+
+    def pin_u16(self, a):
+        return self.torch.from_numpy(a.view(np.int16)).pin_memory().view(self.torch.uint16)
+
+    def to_device(self, t):
+        return t.to(self.device)
+
+    def event(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def synchronize(self):
+        self.torch.cuda.synchronize()
+
+    def set_thread_device(self):
+        self.torch.cuda.set_device(self.local)       # a new host thread starts on device 0
+
+    def stream(self):
+        return self.torch.cuda.Stream(device=self.device)
+
+    def wait_stream(self, sd):
+        self.torch.cuda.current_stream().wait_stream(sd)
+
+    def empty_cache(self):
+        self.torch.cuda.empty_cache()
+
+    def sm_count(self):
+        return self.torch.cuda.get_device_properties(self.local).multi_processor_count
+
+    def clock_sampler(self):
+        return ClockSampler(self.local)
+
+
+def run_tpcca(args, env_cls=CudaEnv):
     import torch.distributed as dist
-    import paper_2208_07412_b200 as pkg
-    from paper_2208_07412_b200 import binding as B
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device: tpcca has no CPU path")
-    torch.cuda.set_device(local)
+    env = env_cls(rank, world, local)
+    B = env.B
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
-    dev = torch.device(f"cuda:{local}")
+        env.init_process_group()
+    dev = env.device
 
     def barrier():
         if world > 1:
             dist.barrier()
-        torch.cuda.synchronize()
+        env.synchronize()
 
     def max_over_ranks(v):
         return reduce_over_ranks(v, "max", world, dev)
@@ -219,16 +333,13 @@ def run_tpcca(args):
     tf, gen_s = make_timeframe(args, rank)
     N = tf.n_clusters
     cap = args.max_start_hits or (N // 8 + 1024)
-    trk = pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local)
+    trk = env.tracker(tf.params, N, cap)
 
     # ---- device-resident inputs (borrowed: no copy inside the timed region) ------------------------
     host = []
     for s in range(tf.n_sectors):
-        hy = torch.from_numpy(tf.y[s]).pin_memory()
-        hz = torch.from_numpy(tf.z[s]).pin_memory()
-        hr = torch.from_numpy(tf.row[s].view(np.int16)).pin_memory().view(torch.uint16)
-        host.append((hy, hz, hr))
-    devin = [(a.to(dev), b.to(dev), c.to(dev)) for a, b, c in host]
+        host.append((env.pin(tf.y[s]), env.pin(tf.z[s]), env.pin_u16(tf.row[s])))
+    devin = [(env.to_device(a), env.to_device(b), env.to_device(c)) for a, b, c in host]
     trk.reset()
     for s, (a, b, c) in enumerate(devin):
         trk.load_clusters(s, a, b, c, borrow=True)
@@ -239,17 +350,17 @@ def run_tpcca(args):
     launches_per_step = trk.launch_count()
     counts = trk.counts()
 
-    sampler = ClockSampler(local)
+    sampler = env.clock_sampler()
     sampler.start()
     time.sleep(0.3)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0, ev1 = env.event(), env.event()
     barrier()
     t_wall0 = time.time()
     ev0.record()
     for _ in range(args.steps):
         trk.run()
     ev1.record()
-    torch.cuda.synchronize()
+    env.synchronize()
     t_wall1 = time.time()
     barrier()
     value, ms_total, n_all = whole_job_value(N, args.steps, ev0.elapsed_time(ev1), world, dev)
@@ -265,7 +376,7 @@ def run_tpcca(args):
     s2_gbs = s2_bytes / (stage_ms[1] * 1e-3) / 1e9
     flops = (work["propagations"] * FLOPS_PROPAGATE + work["updates"] * FLOPS_UPDATE + work["gates"] * FLOPS_GATE
              + work["searches"] * FLOPS_SEARCH + work["candidates"] * FLOPS_CANDIDATE)
-    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    n_sm = env.sm_count()
     alu_peak = n_sm * 128 * peaks["sm_max_mhz"] * 1e6 / 1e12      # T fp32 op/s without FMA
     s5_tops = flops / (stage_ms[4] * 1e-3) / 1e12
 
@@ -296,7 +407,7 @@ def run_tpcca(args):
     for _ in range(e2e_steps):
         e2e_step(trk)
     ev1.record()
-    torch.cuda.synchronize()
+    env.synchronize()
     barrier()
     e2e_serial_ms = max_over_ranks(ev0.elapsed_time(ev1))
 
@@ -307,23 +418,24 @@ def run_tpcca(args):
     e2e_mode = "serial, 1 context"
     if not args.no_streaming:
         n_ctx = max(2, args.e2e_contexts)
-        sides = [torch.cuda.Stream(device=dev) for _ in range(n_ctx - 1)]
+        sides = [env.stream() for _ in range(n_ctx - 1)]
         extra = []
         try:
             for sd in sides:
-                extra.append(pkg.Tracker(tf.params, max_clusters=N, max_start_hits=cap, device=local, stream=sd))
-        except torch.OutOfMemoryError:      # the workspace of another time frame does not fit beside the first
+                extra.append(env.tracker(tf.params, N, cap, stream=sd))
+        except env.oom_error:      # the workspace of another time frame does not fit beside the first
             for t in extra:
                 t.close()
             extra = None
-            torch.cuda.empty_cache()
+            env.empty_cache()
         if extra:
             for t in extra:
                 e2e_step(t)
-            torch.cuda.synchronize()
+            env.synchronize()
             per = e2e_steps
 
             def worker(t, delay):
+                env.set_thread_device()
                 time.sleep(delay)              # the contexts start a fraction of a step apart: the copies of one meet the kernels of another
                 for _ in range(per):
                     e2e_step(t)
@@ -337,9 +449,9 @@ def run_tpcca(args):
             for t in th:
                 t.join()
             for sd in sides:
-                torch.cuda.current_stream().wait_stream(sd)
+                env.wait_stream(sd)
             ev1.record()
-            torch.cuda.synchronize()
+            env.synchronize()
             barrier()
             e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
             e2e_n = n_ctx * per
@@ -352,28 +464,12 @@ def run_tpcca(args):
     e2e_steps_serial = e2e_steps
     e2e_steps = e2e_n
 
-    # ---- CPU baseline = the oracle on one core over sector 0 (rank 0, N = 1 only); parity check ----
+    # ---- CPU baseline = the oracle, one sector per host core, on a bounded sample of the sectors (rank 0,
+    # N = 1 only); the same results are a full-size parity check of those sectors ----------------------------
     cpu = None
     parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sys.path.insert(0, os.path.join(ROOT, "tests"))
-        from oracle import Oracle
-        from parity import compare_sector
-        y, z, row = sample_sector(tf, 0, 1.0)
-        orc = Oracle(tf.params)
-        t0 = time.time()
-        orc.run(y, z, row, want=())
-        dt = time.time() - t0
-        cpu = dict(value=float(y.shape[0] / dt), unit=UNIT, cores=1, kind="oracle",
-                   sample=f"sector 0 of {tf.n_sectors}: {int(y.shape[0])} of {N} clusters, S1-S5, {dt:.1f} s")
-        o = orc.run(y, z, row)
-        g = trk.get_tracks(0)
-        try:
-            rep = compare_sector(g, o, orc, row[o.order])
-            parity = dict(sector=0, n_clusters=int(o.n), n_tracks=int(o.n_tracks), links_differing=rep["links_differing"],
-                          membership="bit-exact", par_bit_exact=rep.get("par_bit_exact"), status="pass")
-        except AssertionError as e:
-            parity = dict(sector=0, status="FAIL", error=str(e)[:300])
+        cpu, parity = cpu_baseline_and_parity(args, tf, trk)
 
     if rank == 0:
         line = dict(
@@ -406,7 +502,23 @@ def run_tpcca(args):
         dist.destroy_process_group()
 
 
-def main():
+def launch_ranks(n):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this same command line, one per GPU, under
+    torch.distributed.run on 127.0.0.1 (what the driver does itself for its scaling runs) and pass on the exit code.
+    NCCL's communicator log stays on (NCCL_DEBUG=INFO, INIT subsystem, stderr) so the ranks can be counted."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.run(cmd, env=env).returncode
+
+
+def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
@@ -419,13 +531,21 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-z-frac", type=float, default=0.25)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sectors", type=int, default=4, help="sectors of the CPU-baseline / full-size parity sample")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "tpcca":
         args.warmup = 3        # timing rule: W >= 3
+    return args
+
+
+def main():
+    args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(launch_ranks(args.gpus))
     else:
         run_tpcca(args)
 
