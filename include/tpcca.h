@@ -11,6 +11,8 @@
  *   S3 mutual-link confirmation ("link cleaner")
  *   S4 start-hit selection, ordered compaction
  *   S5 tracklet construction + fp32 Kalman helix fit   (Bz = 0.5 T)
+ * and, beyond the five (SURVEY.md 8(f) "next" rows):
+ *   S6 tracklet selector: per-cluster ownership, clone removal
  * "clusters per sector and pad row in, links and fitted tracks out" (BASELINE.json:5).
  *
  * Every stage runs in hand-written CUDA kernels for sm_100a; there is NO CPU fallback: every
@@ -59,7 +61,8 @@ extern "C" {
 #define TPCCA_STAGE_CLEAN      0x04u
 #define TPCCA_STAGE_START      0x08u
 #define TPCCA_STAGE_TRACKLETS  0x10u
-#define TPCCA_STAGE_ALL        0x1Fu
+#define TPCCA_STAGE_ALL        0x1Fu   /* the five stages of the hot path (BASELINE.json:5)             */
+#define TPCCA_STAGE_SELECT     0x20u   /* S6 tracklet selector; needs S1-S5           */
 
 /* which output groups tpcca_get_tracks delivers (HOST: copies) */
 #define TPCCA_OUT_ORDER      0x01u  /* order                                      (S1)            */
@@ -69,6 +72,10 @@ extern "C" {
 #define TPCCA_OUT_START      0x10u  /* start_hit                                  (S4)            */
 #define TPCCA_OUT_TRACKS     0x20u  /* track table + hit CSR                      (S5)            */
 #define TPCCA_OUT_ALL        0x3Fu
+#define TPCCA_OUT_SELECTION  0x40u  /* owner, n_own, sel_track                    (S6)            */
+#define TPCCA_OUT_TRACKS_SEL 0x80u  /* the track table + hit CSR of the SELECTED tracks only (S6): fills the S5    */
+                                    /* fields of the view from the compact table (array lengths: n_selected and    */
+                                    /* n_sel_hits instead of n_tracks and n_hits); not together with OUT_TRACKS   */
 
 typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
 
@@ -97,6 +104,7 @@ typedef struct {
   float grid_margin;               /* S2/S5: safety margin when turning a window into a bin range */
   int32_t tc_max_gap;              /* S5: consecutive rows without a hit before stopping          */
   int32_t tc_min_hits;             /* S5: minimum hits of an emitted track                        */
+  int32_t sel_max_shared_permille; /* S6: a tracklet is selected iff (n_hits - n_own) * 1000 <= this * n_hits     */
 } tpcca_params;
 
 /* Outputs of ONE sector.  With mem_space == TPCCA_MEM_DEVICE the pointers are DEVICE pointers
@@ -133,6 +141,12 @@ typedef struct {
   const int32_t  *first_row, *last_row, *trk_start_hit;   /* [n_tracks]                          */
   const int32_t  *hit_offset; /* [n_tracks + 1] CSR offsets into hit_idx, hit_offset[0] = 0      */
   const int32_t  *hit_idx;    /* [n_hits] sorted positions, ascending row inside a track         */
+  /* S6: tracklet selector */
+  int64_t n_selected;         /* selected tracks of the sector                                   */
+  int64_t n_sel_hits;         /* total hits of the selected tracks                               */
+  const int32_t  *owner;      /* [n_clusters] track (sector-local number) owning the cluster; -1 */
+  const int32_t  *n_own;      /* [n_tracks] hits of each S5 track that the track owns            */
+  const int32_t  *sel_track;  /* [n_selected] ascending sector-local numbers of the selected     */
 } tpcca_tracks_view;
 
 /* Bytes of DEVICE workspace that tpcca_create needs for at most `max_clusters_total` clusters
@@ -168,7 +182,7 @@ int tpcca_load_clusters(tpcca_ctx *ctx, int sector, int64_t n, const float *x, c
 /* Start a new time frame: forget all loaded sectors and all outputs (no device work). */
 int tpcca_reset(tpcca_ctx *ctx);
 
-/* Run the stages in `stage_mask` (bit i = stage i+1) over all sectors, asynchronously on the
+/* Run the stages in `stage_mask` (bit i = stage i+1; TPCCA_STAGE_SELECT = S6) over all sectors, asynchronously on the
  * context's stream.  A stage needs the outputs of the stages before it from this or an earlier
  * run on the same clusters (TPCCA_E_STATE otherwise).  Device-side failures (row out of range,
  * start-hit capacity overflow) are reported by the next tpcca_get_* / tpcca_sync call.
@@ -190,15 +204,17 @@ int tpcca_sync(tpcca_ctx *ctx);
  * always filled.  Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
 int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, uint32_t what, tpcca_tracks_view *out);
 
-/* Totals over all sectors after a run: out[0..4] = n_clusters, n_start, n_tracks, n_hits,
- * n_bins (per sector).  Synchronises the stream.  Errors as tpcca_sync. */
-int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[5]);
+/* Totals over all sectors after a run: out[0..6] = n_clusters, n_start, n_tracks, n_hits,
+ * n_bins (per sector), n_selected, n_sel_hits (S6; 0 if not run).  Synchronises the stream.
+ * Errors as tpcca_sync. */
+int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[7]);
 
 /* Device time of each stage [ms] of the run `runs_back` runs ago (0 = the last tpcca_run; the
  * context keeps the events of its last 16 runs), from CUDA events recorded on the context's
- * stream around the stages; ms[5] = whole run.  Synchronises the stream.
+ * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6 (0 if not run).
+ * Synchronises the stream.
  * Errors: TPCCA_E_ARG (runs_back outside 0..15), TPCCA_E_STATE (no such run). */
-int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[6]);
+int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[7]);
 
 /* Work counters of the last run's S5 kernel, for the ALU roofline:
  * out[0] = Kalman propagations that moved the state, out[1] = Kalman updates,

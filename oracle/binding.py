@@ -23,6 +23,7 @@ class _Params(C.Structure):
         ("tc_win_y", C.c_double), ("tc_win_z", C.c_double), ("tc_gate", C.c_double),
         ("max_sinphi", C.c_double), ("grid_margin", C.c_double),
         ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32),
+        ("sel_max_shared_permille", C.c_int32),
     ]
 
 
@@ -49,6 +50,11 @@ def _load():
         lib.oracle_kf_dist2.restype = C.c_double
         lib.oracle_score.argtypes = [C.c_void_p, C.c_int] + [C.c_double] * 6
         lib.oracle_score.restype = C.c_double
+        lib.oracle_n_selected.argtypes = [C.c_void_p]
+        lib.oracle_n_selected.restype = C.c_int64
+        lib.oracle_get_selection.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+        lib.oracle_select.argtypes = [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 3
+        lib.oracle_select.restype = C.c_int64
         _lib = lib
     return _lib
 
@@ -79,6 +85,9 @@ class OracleResult:
     trk_start_hit: np.ndarray = None
     hit_offset: np.ndarray = None
     hit_idx: np.ndarray = None
+    owner: np.ndarray = None        # S6: [n] track owning each cluster (-1 none)
+    n_own: np.ndarray = None        # S6: [n_tracks]
+    selected: np.ndarray = None     # S6: [n_selected] ascending track numbers
 
     @property
     def n_tracks(self) -> int:
@@ -122,6 +131,7 @@ class Oracle:
         p.tc_gate = float(params.tc_gate); p.max_sinphi = float(params.max_sinphi)
         p.grid_margin = float(params.grid_margin)
         p.tc_max_gap = int(params.tc_max_gap); p.tc_min_hits = int(params.tc_min_hits)
+        p.sel_max_shared_permille = int(getattr(params, "sel_max_shared_permille", 500))
         self._h = lib.oracle_create(C.byref(p), self.precision)
         if not self._h:
             raise RuntimeError("oracle_create failed")
@@ -173,6 +183,10 @@ class Oracle:
                                         res.hit_offset.ctypes.data, res.hit_idx.ctypes.data)
             res.n_hits, res.n_fit, res.first_row, res.last_row, res.trk_start_hit = (
                 np.ascontiguousarray(ints[:, i]) for i in range(5))
+        if "tracks" in want and (stage_mask & 32):
+            res.owner = np.empty(n, np.int32); res.n_own = np.empty(n_trk, np.int32)
+            res.selected = np.empty(int(self._lib.oracle_n_selected(self._h)), np.int32)
+            self._lib.oracle_get_selection(self._h, res.owner.ctypes.data, res.n_own.ctypes.data, res.selected.ctypes.data)
         return res
 
     # ---- unit entry points (pins) ---------------------------------------------------
@@ -192,6 +206,18 @@ class Oracle:
 
     def score(self, r, yc, zc, yu, zu, yd, zd):
         return float(self._lib.oracle_score(self._h, int(r), yc, zc, yu, zu, yd, zd))
+
+
+def select_tracks(n_clusters, hit_offset, hit_idx, max_shared_permille=500):
+    """The S6 selector of the oracle on caller-given hit lists -> (owner, n_own, selected)."""
+    lib = _load()
+    ho = np.ascontiguousarray(hit_offset, dtype=np.int32)
+    hi = np.ascontiguousarray(hit_idx, dtype=np.int32)
+    nt = int(ho.shape[0]) - 1
+    owner = np.empty(int(n_clusters), np.int32); n_own = np.empty(nt, np.int32); sel = np.empty(nt, np.int32)
+    k = lib.oracle_select(int(n_clusters), nt, ho.ctypes.data, hi.ctypes.data, int(max_shared_permille),
+                          owner.ctypes.data, n_own.ctypes.data, sel.ctypes.data)
+    return owner, n_own, sel[:int(k)].copy()
 
 
 def run_timeframe(tf, sectors=None, precision="f32", stage_mask=0x1F, brute=False):

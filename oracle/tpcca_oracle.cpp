@@ -55,6 +55,7 @@ struct oracle_params {      // all tables are double arrays holding the (fp32-re
   double init_cov[5];
   double tc_win_y, tc_win_z, tc_gate, max_sinphi, grid_margin;
   int32_t tc_max_gap, tc_min_hits;
+  int32_t sel_max_shared_permille;   // S6: a tracklet survives iff shared hits * 1000 <= this * n_hits
 };
 }
 
@@ -81,6 +82,39 @@ struct Track {
   int32_t n_hits, n_fit, first_row, last_row, start_hit;
 };
 
+// ----------------------------------------------------------------------------- S6: tracklet selector
+// SURVEY.md 8(f)-1 / DESIGN.md 3.7: "per-cluster ownership by (nHits, -trackId) ..., drop tracklets sharing
+// more than X % of hits".  Integers only.  Tracks are numbered in output (start-hit) order.
+//   owner[c]  = the track holding cluster c with the most hits; ties -> the smallest track number; -1 if none
+//   n_own[t]  = hits of t that t owns;  shared(t) = n_hits(t) - n_own[t]
+//   t is selected iff shared(t) * 1000 <= max_shared_permille * n_hits(t)
+// (with four near-identical clones per long track -- reading N3 -- the longest clone owns everything
+// the clones share and the others are dropped).
+inline void select_tracks_plain(int64_t n_clusters, int64_t n_tracks, const int32_t* hit_offset, const int32_t* hit_idx,
+                                int32_t max_shared_permille, std::vector<int32_t>& owner, std::vector<int32_t>& n_own,
+                                std::vector<int32_t>& selected) {
+  owner.assign(n_clusters, -1);
+  n_own.assign(n_tracks, 0);
+  selected.clear();
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    const int32_t nh = hit_offset[t + 1] - hit_offset[t];
+    for (int32_t k = hit_offset[t]; k < hit_offset[t + 1]; ++k) {
+      const int32_t c = hit_idx[k];
+      const int32_t o = owner[c];
+      // t ascends, so on equal hit counts the earlier (smaller) track keeps the cluster
+      if (o < 0 || nh > hit_offset[o + 1] - hit_offset[o]) owner[c] = (int32_t)t;
+    }
+  }
+  for (int64_t t = 0; t < n_tracks; ++t)
+    for (int32_t k = hit_offset[t]; k < hit_offset[t + 1]; ++k)
+      if (owner[hit_idx[k]] == (int32_t)t) n_own[t]++;
+  for (int64_t t = 0; t < n_tracks; ++t) {
+    const int64_t nh = hit_offset[t + 1] - hit_offset[t];
+    const int64_t shared = nh - n_own[t];
+    if (shared * 1000 <= (int64_t)max_shared_permille * nh) selected.push_back((int32_t)t);
+  }
+}
+
 template <class R>
 class Oracle {
  public:
@@ -101,6 +135,7 @@ class Oracle {
     win_y = (R)q.tc_win_y; win_z = (R)q.tc_win_z; gate = (R)q.tc_gate;
     max_sinphi = (R)q.max_sinphi; margin = (R)q.grid_margin;
     max_gap = q.tc_max_gap; min_hits = q.tc_min_hits;
+    sel_permille = q.sel_max_shared_permille;
     row_bin_base.resize(n_rows + 1);
     row_bin_base[0] = 0;
     for (int r = 0; r < n_rows; ++r) row_bin_base[r + 1] = row_bin_base[r] + (int64_t)ny[r] * nz[r];
@@ -450,6 +485,8 @@ class Oracle {
     if (stage_mask & 4u) clean_links();
     if (stage_mask & 8u) select_start_hits();
     if (stage_mask & 16u) construct_tracklets();
+    if (stage_mask & 32u)
+      select_tracks_plain(n, (int64_t)tracks.size(), hit_offset.data(), hit_idx.data(), sel_permille, owner, n_own, selected);
   }
 
   // tables
@@ -459,7 +496,7 @@ class Oracle {
   std::vector<int64_t> row_bin_base;
   R grid_z_lo, Bc, err2_y, err2_z, init_cov[5], win_y, win_z, gate, max_sinphi, margin;
   R c24, c640, c12;
-  int max_gap, min_hits;
+  int max_gap, min_hits, sel_permille;
   // data
   int64_t n = 0;
   std::vector<R> y, z, sy, sz;
@@ -469,6 +506,7 @@ class Oracle {
   std::vector<int32_t> link_up, link_dn, link_up_c, link_dn_c, start_hit;
   std::vector<Track<R>> tracks;
   std::vector<int32_t> hit_offset, hit_idx;
+  std::vector<int32_t> owner, n_own, selected;   // S6
 };
 
 struct Handle {
@@ -574,6 +612,31 @@ void oracle_get_tracks(void* hv, double* x_ref, double* z_ref, double* par, doub
     std::copy((o)->hit_idx.begin(), (o)->hit_idx.end(), hit_idx); } while (0)
   if (h->precision == 0) GT(h->f); else GT(h->d);
 #undef GT
+}
+
+// S6 outputs of the last run with stage bit 32: owner [n_clusters], n_own [n_tracks], selected [n_selected]
+int64_t oracle_n_selected(void* hv) {
+  Handle* h = (Handle*)hv;
+  return h->precision == 0 ? (int64_t)h->f->selected.size() : (int64_t)h->d->selected.size();
+}
+void oracle_get_selection(void* hv, int32_t* owner, int32_t* n_own, int32_t* selected) {
+  Handle* h = (Handle*)hv;
+#define GS(o) do { \
+    std::copy((o)->owner.begin(), (o)->owner.end(), owner); \
+    std::copy((o)->n_own.begin(), (o)->n_own.end(), n_own); \
+    std::copy((o)->selected.begin(), (o)->selected.end(), selected); } while (0)
+  if (h->precision == 0) GS(h->f); else GS(h->d);
+#undef GS
+}
+// the selector on its own, on hit lists given by the caller (pins): returns the number of selected tracks
+int64_t oracle_select(int64_t n_clusters, int64_t n_tracks, const int32_t* hit_offset, const int32_t* hit_idx,
+                      int32_t max_shared_permille, int32_t* owner, int32_t* n_own, int32_t* selected) {
+  std::vector<int32_t> o, w, s;
+  select_tracks_plain(n_clusters, n_tracks, hit_offset, hit_idx, max_shared_permille, o, w, s);
+  std::copy(o.begin(), o.end(), owner);
+  std::copy(w.begin(), w.end(), n_own);
+  std::copy(s.begin(), s.end(), selected);
+  return (int64_t)s.size();
 }
 
 // ---- unit entry points for the pins ---------------------------------------------------

@@ -15,6 +15,7 @@ import numpy as np
 from . import build as _build
 
 STAGE_GRID, STAGE_NEIGHBOURS, STAGE_CLEAN, STAGE_START, STAGE_TRACKLETS, STAGE_ALL = 1, 2, 4, 8, 16, 31
+STAGE_SELECT = 32
 MEM_HOST, MEM_DEVICE, MEM_DEVICE_BORROW = 0, 1, 2
 
 _fp = C.POINTER(C.c_float)
@@ -26,6 +27,7 @@ ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "
                "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
                "tpcca_get_launch_count", "tpcca_get_info", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
+OUT_SELECTION, OUT_TRACKS_SEL = 64, 128
 
 
 class TpccaError(RuntimeError):
@@ -44,7 +46,7 @@ class _Params(C.Structure):
         ("init_cov", C.c_float * 5),
         ("tc_win_y", C.c_float), ("tc_win_z", C.c_float), ("tc_gate", C.c_float),
         ("max_sinphi", C.c_float), ("grid_margin", C.c_float),
-        ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32),
+        ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32), ("sel_max_shared_permille", C.c_int32),
     ]
 
 
@@ -58,6 +60,7 @@ class _View(C.Structure):
         ("x_ref", _fp), ("z_ref", _fp), ("par", _fp), ("cov", _fp), ("chi2", _fp),
         ("n_hits_trk", _ip), ("n_fit", _ip), ("first_row", _ip), ("last_row", _ip), ("trk_start_hit", _ip),
         ("hit_offset", _ip), ("hit_idx", _ip),
+        ("n_selected", C.c_int64), ("n_sel_hits", C.c_int64), ("owner", _ip), ("n_own", _ip), ("sel_track", _ip),
     ]
 
 
@@ -130,6 +133,7 @@ def _make_params(P):
     p.tc_win_y = float(P.tc_win_y); p.tc_win_z = float(P.tc_win_z); p.tc_gate = float(P.tc_gate)
     p.max_sinphi = float(P.max_sinphi); p.grid_margin = float(P.grid_margin)
     p.tc_max_gap = int(P.tc_max_gap); p.tc_min_hits = int(P.tc_min_hits)
+    p.sel_max_shared_permille = int(getattr(P, "sel_max_shared_permille", 500))
     return p, keep
 
 
@@ -171,6 +175,9 @@ class SectorOutput:
     trk_start_hit: np.ndarray = None
     hit_offset: np.ndarray = None
     hit_idx: np.ndarray = None
+    owner: np.ndarray = None       # S6
+    n_own: np.ndarray = None
+    selected: np.ndarray = None
 
     @property
     def n_tracks(self) -> int:
@@ -286,14 +293,14 @@ class Tracker:
         self._check(self._lib.tpcca_sync(self._h))
 
     def counts(self) -> dict:
-        out = (C.c_int64 * 5)()
+        out = (C.c_int64 * 7)()
         self._check(self._lib.tpcca_get_counts(self._h, out))
         return dict(n_clusters=int(out[0]), n_start=int(out[1]), n_tracks=int(out[2]), n_hits=int(out[3]),
-                    n_bins=int(out[4]))
+                    n_bins=int(out[4]), n_selected=int(out[5]), n_sel_hits=int(out[6]))
 
     def timings(self, runs_back: int = 0):
-        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, total]."""
-        out = (C.c_float * 6)()
+        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, S1..S5, S6]."""
+        out = (C.c_float * 7)()
         self._check(self._lib.tpcca_get_timings(self._h, int(runs_back), out))
         return [float(v) for v in out]
 
@@ -336,6 +343,12 @@ class Tracker:
         o.link_up_raw = _np(v.link_up_raw, n, np.int32); o.link_dn_raw = _np(v.link_dn_raw, n, np.int32)
         o.link_up = _np(v.link_up, n, np.int32); o.link_dn = _np(v.link_dn, n, np.int32)
         o.start_hit = _np(v.start_hit, int(v.n_start), np.int32)
+        if what & OUT_TRACKS_SEL:          # the S5 fields hold the selected tracks only
+            nt = int(v.n_selected)
+        n_hits_total = int(v.n_sel_hits) if what & OUT_TRACKS_SEL else int(v.n_hits)
+        if v.owner:
+            o.owner = _np(v.owner, n, np.int32); o.n_own = _np(v.n_own, int(v.n_tracks), np.int32)
+            o.selected = _np(v.sel_track, int(v.n_selected), np.int32)
         if v.x_ref:
             o.x_ref = _np(v.x_ref, nt, np.float32); o.z_ref = _np(v.z_ref, nt, np.float32)
             o.chi2 = _np(v.chi2, nt, np.float32)
@@ -348,5 +361,5 @@ class Tracker:
             o.first_row = _np(v.first_row, nt, np.int32); o.last_row = _np(v.last_row, nt, np.int32)
             o.trk_start_hit = _np(v.trk_start_hit, nt, np.int32)
             o.hit_offset = _np(v.hit_offset, nt + 1, np.int32)
-            o.hit_idx = _np(v.hit_idx, int(v.n_hits), np.int32)
+            o.hit_idx = _np(v.hit_idx, n_hits_total, np.int32)
         return o

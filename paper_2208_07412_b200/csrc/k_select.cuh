@@ -1,0 +1,178 @@
+// S6 tracklet selector: per-cluster ownership by (n_hits, -track),
+// tracklets that share too many of their hits are dropped, the survivors are gathered into a compact
+// track table + hit CSR (the table a consumer downloads instead of the 4x larger clone-laden one).
+#pragma once
+#include "k_tracklets.cuh"
+
+namespace tpcca {
+
+// sector of global track t: largest s with trk_off[s] <= t (sectors without tracks are skipped)
+__device__ __forceinline__ int sector_of_track(const DevStatus* __restrict__ st, int ns, int t) {
+  int lo = 0, hi = ns - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (st->trk_off[mid] <= t) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+// ownership key of track t_local with nh hits: larger = better; ties in nh -> the smaller track number wins
+__device__ __forceinline__ unsigned long long sel_key(int nh, int t_local) {
+  return ((unsigned long long)(uint32_t)nh << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)t_local);
+}
+
+// ---- K6a: claim.  One warp per track: own_key[cluster] = max over the tracks holding it ---------------
+__global__ void __launch_bounds__(256)
+k_sel_claim(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
+            const int32_t* __restrict__ n_hits, const int32_t* __restrict__ hit_offset, const int32_t* __restrict__ hit_idx,
+            unsigned long long* __restrict__ own_key) {
+  const int ns = T->n_sectors;
+  const int n_trk = st->trk_off[ns];
+  const int lane = threadIdx.x & 31;
+  for (int t = blockIdx.x * 8 + (threadIdx.x >> 5); t < n_trk; t += gridDim.x * 8) {
+    const int s = sector_of_track(st, ns, t);
+    const int nh = n_hits[t];
+    const long long h0 = st->hit_off[s] + hit_offset[t + s];
+    const unsigned long long key = sel_key(nh, t - st->trk_off[s]);
+    unsigned long long* ok = own_key + sec[s].off;
+    for (int k = lane; k < nh; k += 32) {
+      const int c = hit_idx[h0 + k];
+      // (plain read first: most clusters are claimed by three or four clones and only the first few raise the key)
+      if (ok[c] < key) atomicMax(&ok[c], key);
+    }
+  }
+}
+
+// ---- K6b: count.  One warp per track: n_own[t] = hits whose key is the track's own ----------------------
+__global__ void __launch_bounds__(256)
+k_sel_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
+            const int32_t* __restrict__ n_hits, const int32_t* __restrict__ hit_offset, const int32_t* __restrict__ hit_idx,
+            const unsigned long long* __restrict__ own_key, int32_t* __restrict__ n_own) {
+  const int ns = T->n_sectors;
+  const int n_trk = st->trk_off[ns];
+  const int lane = threadIdx.x & 31;
+  for (int t = blockIdx.x * 8 + (threadIdx.x >> 5); t < n_trk; t += gridDim.x * 8) {
+    const int s = sector_of_track(st, ns, t);
+    const int nh = n_hits[t];
+    const long long h0 = st->hit_off[s] + hit_offset[t + s];
+    const unsigned long long key = sel_key(nh, t - st->trk_off[s]);
+    const unsigned long long* ok = own_key + sec[s].off;
+    int cnt = 0;
+    for (int k = lane; k < nh; k += 32) cnt += (ok[hit_idx[h0 + k]] == key) ? 1 : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+    if (lane == 0) n_own[t] = cnt;
+  }
+}
+
+// selection rule (integers): shared * 1000 <= max_shared_permille * n_hits
+__device__ __forceinline__ bool sel_keep(int nh, int own, int permille) {
+  return (long long)(nh - own) * 1000ll <= (long long)permille * (long long)nh;
+}
+
+// ---- K6c: per-tile (1024 tracks) sums of (selected, hits of selected) --------------------------------
+__global__ void __launch_bounds__(1024)
+k_sel_tile_sums(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, const int32_t* __restrict__ n_hits,
+                const int32_t* __restrict__ n_own, int2* __restrict__ tile_cnt) {
+  __shared__ int ws[33];
+  const int n_trk = st->trk_off[T->n_sectors];
+  const int t = blockIdx.x * 1024 + threadIdx.x;
+  const int nh = t < n_trk ? n_hits[t] : 0;
+  const bool keep = t < n_trk && sel_keep(nh, n_own[t], T->sel_permille);
+  int ta, tb;
+  block_exclusive_scan<int>(keep ? 1 : 0, ws, ta);
+  block_exclusive_scan<int>(keep ? nh : 0, ws, tb);
+  if (threadIdx.x == 0) tile_cnt[blockIdx.x] = make_int2(ta, tb);
+}
+
+// ---- K6d: sector bases of the selected table and of its hit CSR --------------------------------------
+__global__ void k_sel_sector_bases(const DevTables* __restrict__ T, DevStatus* __restrict__ st, const int32_t* __restrict__ n_hits,
+                                   const int32_t* __restrict__ n_own, const longlong2* __restrict__ tile_off,
+                                   const int64_t* __restrict__ tot) {
+  const int ns = T->n_sectors;
+  const int s = threadIdx.x;
+  if (s > ns) return;
+  const int n_trk = st->trk_off[ns];
+  const int t0 = st->trk_off[s];
+  if (t0 >= n_trk) { st->sel_off[s] = (int32_t)tot[0]; st->sel_hit_off[s] = tot[1]; return; }
+  const int tile = t0 >> 10;
+  long long a = tile_off[tile].x, b = tile_off[tile].y;
+  const int permille = T->sel_permille;
+  for (int q = tile << 10; q < t0; ++q) {
+    const int nh = n_hits[q];
+    if (sel_keep(nh, n_own[q], permille)) { a += 1; b += nh; }
+  }
+  st->sel_off[s] = (int32_t)a;
+  st->sel_hit_off[s] = b;
+}
+
+// ---- K6e: gather the selected tracks (ascending track number) into the compact table + hit CSR ----------
+struct SelOut {
+  int32_t* sel_track;        // [n_selected] sector-local track numbers
+  TrackOut o;                // compact table: same planes as the S5 table, plane stride = cap
+};
+
+__global__ void __launch_bounds__(1024)
+k_sel_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, int32_t cap, const int32_t* __restrict__ n_own,
+             const longlong2* __restrict__ tile_off, TrackOut in, SelOut out) {
+  __shared__ int ws[33];
+  const int ns = T->n_sectors;
+  const int n_trk = st->trk_off[ns];
+  const int t = blockIdx.x * 1024 + threadIdx.x;
+  const bool valid = t < n_trk;
+  const int nh = valid ? in.n_hits[t] : 0;
+  const bool keep = valid && sel_keep(nh, n_own[t], T->sel_permille);
+  int ta, tb;
+  const int ea = block_exclusive_scan<int>(keep ? 1 : 0, ws, ta);
+  const int eb = block_exclusive_scan<int>(keep ? nh : 0, ws, tb);
+  const long long k = tile_off[blockIdx.x].x + ea;       // global index in the selected table
+  const long long h = tile_off[blockIdx.x].y + eb;       // global index in the selected hit CSR
+  long long src_h = 0;
+  if (valid) {
+    const int s = sector_of_track(st, ns, t);
+    const long long hloc = h - st->sel_hit_off[s];
+    src_h = st->hit_off[s] + in.hit_offset[t + s];
+    if (keep) {
+      const size_t cs = (size_t)cap;
+      out.sel_track[k] = t - st->trk_off[s];
+      out.o.hit_offset[k + s] = (int32_t)hloc;
+      out.o.x_ref[k] = in.x_ref[t]; out.o.z_ref[k] = in.z_ref[t]; out.o.chi2[k] = in.chi2[t];
+#pragma unroll
+      for (int i = 0; i < 5; ++i) out.o.par[i * cs + k] = in.par[i * cs + t];
+#pragma unroll
+      for (int i = 0; i < 15; ++i) out.o.cov[i * cs + k] = in.cov[i * cs + t];
+      out.o.n_hits[k] = nh; out.o.n_fit[k] = in.n_fit[t]; out.o.first_row[k] = in.first_row[t];
+      out.o.last_row[k] = in.last_row[t]; out.o.start_hit[k] = in.start_hit[t];
+    }
+    // closing entry of the sector's hit_offset: written by the sector's last track
+    if (t + 1 == st->trk_off[s + 1]) out.o.hit_offset[k + (keep ? 1 : 0) + s] = (int32_t)(hloc + (keep ? nh : 0));
+  }
+  // hit lists: the warp copies the list of each of its selected tracks together
+  const int lane = threadIdx.x & 31;
+  unsigned todo = __ballot_sync(0xffffffffu, keep);
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int n = __shfl_sync(0xffffffffu, nh, src);
+    const long long from = __shfl_sync(0xffffffffu, src_h, src), to = __shfl_sync(0xffffffffu, h, src);
+    for (int q = lane; q < n; q += 32) out.o.hit_idx[to + q] = in.hit_idx[from + q];
+  }
+}
+
+// sectors without tracks still own a one-entry hit_offset = {0} in the selected table
+__global__ void k_sel_close_empty(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, SelOut out) {
+  const int s = threadIdx.x;
+  if (s >= T->n_sectors) return;
+  if (st->trk_off[s] == st->trk_off[s + 1]) out.o.hit_offset[st->sel_off[s] + s] = 0;
+}
+
+// ---- K6f: owner[c] = track number decoded from the key (-1: the cluster is in no track) ----------------
+__global__ void __launch_bounds__(256)
+k_sel_owner(const unsigned long long* __restrict__ own_key, int32_t* __restrict__ owner, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const unsigned long long k = own_key[i];
+    owner[i] = k ? (int32_t)(0xFFFFFFFFu - (uint32_t)k) : -1;
+  }
+}
+
+}  // namespace tpcca

@@ -9,7 +9,7 @@
 #include <utility>
 #include <vector>
 
-#include "k_tracklets.cuh"
+#include "k_select.cuh"
 
 using namespace tpcca;
 
@@ -29,6 +29,7 @@ struct Layout {
   size_t tile_cnt, tile_off, start_bits;
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
+  size_t sel_n_own, sel_track;   // S6 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
 };
@@ -99,7 +100,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.hits = take(4 * (size_t)(nr * CS));
   L.trk_v = take(16 * (size_t)(kTrkV * CS));   // finished tracks: records of kTrkV 16-byte vectors
   L.trk_n = take(4 * (size_t)CS);             // n_hits per slot (0 = rejected)
-  L.hs = take(16 * (size_t)(kHsV * CS));      // parked tracklets: records of kHsV 16-byte vectors
+  L.hs = take(16 * (size_t)(kHsV * CS) + 4 * (size_t)(ns + 1));   // parked tracklets: records of kHsV 16-byte vectors (S6: sel hit_offset)
   L.o_x_ref = take(4 * (size_t)CS);
   L.o_z_ref = take(4 * (size_t)CS);
   L.o_chi2 = take(4 * (size_t)CS);
@@ -112,6 +113,8 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.o_start = take(4 * (size_t)CS);
   L.o_hit_offset = take(4 * (size_t)(CS + ns + 1));
   L.o_hit_idx = take(4 * (size_t)(nr * CS));
+  L.sel_n_own = take(4 * (size_t)CS);
+  L.sel_track = take(4 * (size_t)CS);
   L.total = cur;
   return L;
 }
@@ -133,6 +136,7 @@ int check_params(const tpcca_params* p, std::string& err) {
   }
   if ((nb + 1) * (int64_t)p->n_sectors >= (int64_t)0xFFFFFFF0u) return fail("too many grid bins (n_sectors * (bins + 1) must fit 32 bits)");
   if (nb >= 0x7FFFFFF0) return fail("too many grid bins per sector");
+  if (p->sel_max_shared_permille < 0 || p->sel_max_shared_permille > 1000) return fail("sel_max_shared_permille must be in 0..1000");
   return TPCCA_OK;
 }
 
@@ -170,7 +174,7 @@ struct tpcca_ctx {
   uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
   bool desc_valid = false;
   static constexpr int kRing = 16;
-  cudaEvent_t ev[kRing][6]{};
+  cudaEvent_t ev[kRing][7]{};
   uint32_t ev_mask[kRing]{};          // stage mask of the run that used the slot (0 = unused)
   int64_t run_count = 0;
   char* arena = nullptr;              // pinned host arena of tpcca_get_tracks(HOST)
@@ -253,11 +257,29 @@ int fetch_status(tpcca_ctx* c) {
   return TPCCA_OK;
 }
 
+// S6 compact table of the selected tracks: 28 planes of CS words in the S5 slot-record buffer (trk_v: exactly
+// 28 * 4 * CS bytes), its hit_offset in the parked-tracklet buffer (hs), its hit CSR in the per-tracklet hit lines
+SelOut sel_out(const tpcca_ctx* c) {
+  static_assert(kTrkV * 16 == 28 * 4, "the selected table's 28 planes fill the slot-record buffer exactly");
+  const Layout& L = c->L;
+  const size_t cs = (size_t)c->CS;
+  float* f = c->at<float>(L.trk_v);
+  int32_t* i32 = reinterpret_cast<int32_t*>(f);
+  SelOut so;
+  so.sel_track = c->at<int32_t>(L.sel_track);
+  so.o.x_ref = f; so.o.z_ref = f + cs; so.o.chi2 = f + 2 * cs; so.o.par = f + 3 * cs; so.o.cov = f + 8 * cs;
+  so.o.n_hits = i32 + 23 * cs; so.o.n_fit = i32 + 24 * cs; so.o.first_row = i32 + 25 * cs; so.o.last_row = i32 + 26 * cs;
+  so.o.start_hit = i32 + 27 * cs;
+  so.o.hit_offset = c->at<int32_t>(L.hs);
+  so.o.hit_idx = c->at<int32_t>(L.hits);
+  return so;
+}
+
 }  // namespace
 
 extern "C" {
 
-const char* tpcca_version(void) { return "tpcca 0.1 (sm_100a)"; }
+const char* tpcca_version(void) { return "tpcca 0.2 (sm_100a)"; }
 
 const char* tpcca_last_error(const tpcca_ctx* ctx) { return ctx ? ctx->err.c_str() : g_last_error.c_str(); }
 
@@ -314,7 +336,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   DevTables& t = c->tab;
   memset(&t, 0, sizeof t);
   t.n_rows = p->n_rows; t.n_sectors = p->n_sectors; t.bins_per_sector = (int32_t)c->nb;
-  t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits;
+  t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits; t.sel_permille = p->sel_max_shared_permille;
   t.grid_z_lo = p->grid_z_lo; t.Bc = p->kappa_per_qpt; t.err2_y = p->err2_y; t.err2_z = p->err2_z;
   for (int i = 0; i < 5; ++i) t.init_cov[i] = p->init_cov[i];
   t.win_y = p->tc_win_y; t.win_z = p->tc_win_z; t.gate = p->tc_gate; t.max_sinphi = p->max_sinphi;
@@ -373,7 +395,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
-    for (int i = 0; i < 6 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
+    for (int i = 0; i < 7 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
     tpcca_destroy(c);
@@ -447,10 +469,10 @@ int tpcca_load_clusters(tpcca_ctx* c, int sector, int64_t n, const float* x, con
 
 int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   if (!c) return TPCCA_E_ARG;
-  mask &= TPCCA_STAGE_ALL;
+  mask &= (TPCCA_STAGE_ALL | TPCCA_STAGE_SELECT);
   if (!mask) return set_err(c, TPCCA_E_ARG, "empty stage mask");
   // a stage needs everything before it
-  for (int i = 0; i < 5; ++i)
+  for (int i = 0; i < 6; ++i)
     if (mask & (1u << i)) {
       const uint32_t need = (1u << i) - 1u;
       if ((need & ~(c->done_mask | mask)) != 0)
@@ -482,7 +504,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   const DevTables* T = c->at<DevTables>(L.tables);
   const SectorDesc* sec = c->at<SectorDesc>(L.sec);
   DevStatus* status = c->at<DevStatus>(L.status);
-  int64_t* tot = c->at<int64_t>(L.tot);
+  int64_t* tot = c->at<int64_t>(L.tot);     // [8]: pairs of scan totals (S4: 0,1; S5: 2,3; S4 order: 4,5; S6: 6,7)
   float2* syz = c->at<float2>(L.syz);
   int32_t* order = c->at<int32_t>(L.order);
   uint32_t* bin_start = c->at<uint32_t>(L.bin_start);
@@ -494,7 +516,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   const int slot_ev = (int)(c->run_count % tpcca_ctx::kRing);
   c->ev_mask[slot_ev] = 0;
   // end of a stage: its event, and the launch errors of ITS kernels (so a failed launch names its stage)
-  static const char* const kStageName[6] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets"};
+  static const char* const kStageName[7] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets", "S6 selector"};
   cudaError_t stage_err = cudaSuccess;
   int stage_bad = -1;
   auto mark = [&](int i) {
@@ -624,10 +646,39 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     c->launches += 9;
   }
   mark(5);
+  if (mask & TPCCA_STAGE_SELECT) {
+    // S6 buffers: own_key / owner live in the S1 level-1 record buffer (free after S1), the compact table of the
+    // selected tracks in the S5 scratch (slot records, parked tracklets, per-tracklet hit lines: free after S5)
+    TrackOut in;
+    in.x_ref = c->at<float>(L.o_x_ref); in.z_ref = c->at<float>(L.o_z_ref); in.par = c->at<float>(L.o_par);
+    in.cov = c->at<float>(L.o_cov); in.chi2 = c->at<float>(L.o_chi2); in.n_hits = c->at<int32_t>(L.o_n_hits);
+    in.n_fit = c->at<int32_t>(L.o_n_fit); in.first_row = c->at<int32_t>(L.o_first); in.last_row = c->at<int32_t>(L.o_last);
+    in.start_hit = c->at<int32_t>(L.o_start); in.hit_offset = c->at<int32_t>(L.o_hit_offset); in.hit_idx = c->at<int32_t>(L.o_hit_idx);
+    SelOut so = sel_out(c);
+    unsigned long long* own_key = c->at<unsigned long long>(L.rec);
+    int32_t* owner = reinterpret_cast<int32_t*>(c->ws + L.rec + 8 * (size_t)c->N);
+    int32_t* n_own = c->at<int32_t>(L.sel_n_own);
+    const int cap_tiles = (int)((c->CS + 1023) / 1024);
+    const size_t nk = (size_t)std::max<int64_t>(c->n_total, 1);
+    k_zero_words<<<(unsigned)std::min<size_t>((2 * nk + 1023) / 1024, (size_t)c->sm_count * 32), 256, 0, st>>>(reinterpret_cast<uint32_t*>(own_key), 2 * nk);
+    const int warp_grid = (int)std::min<int64_t>((c->CS + 7) / 8, (int64_t)c->sm_count * 64);
+    k_sel_claim<<<warp_grid, 256, 0, st>>>(T, sec, status, in.n_hits, in.hit_offset, in.hit_idx, own_key);
+    k_sel_count<<<warp_grid, 256, 0, st>>>(T, sec, status, in.n_hits, in.hit_offset, in.hit_idx, own_key, n_own);
+    k_sel_tile_sums<<<cap_tiles, 1024, 0, st>>>(T, status, in.n_hits, n_own, tile_cnt);
+    k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 6);
+    k_sel_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, in.n_hits, n_own, tile_off, tot + 6);
+    k_sel_gather<<<cap_tiles, 1024, 0, st>>>(T, status, cap, n_own, tile_off, in, so);
+    k_sel_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, so);
+    k_sel_owner<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(own_key, owner, nk);
+    c->launches += 9;
+  }
+  mark(6);
   if (stage_err != cudaSuccess)
     return set_err(c, TPCCA_E_CUDA, "tpcca_run: stage %s failed: %s", kStageName[stage_bad], cudaGetErrorString(stage_err));
   c->ev_mask[slot_ev] = mask;
   ++c->run_count;
+  // S6's outputs alias S1 / S5 scratch: re-running either without S6 leaves no valid selection
+  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS)) && !(mask & TPCCA_STAGE_SELECT)) c->done_mask &= ~TPCCA_STAGE_SELECT;
   c->done_mask |= mask;
   return TPCCA_OK;
 }
@@ -638,7 +689,7 @@ int tpcca_sync(tpcca_ctx* c) {
   return fetch_status(c);
 }
 
-int tpcca_get_counts(tpcca_ctx* c, int64_t out[5]) {
+int tpcca_get_counts(tpcca_ctx* c, int64_t out[7]) {
   if (!c || !out) return TPCCA_E_ARG;
   GUARD(c);
   int rc = fetch_status(c);
@@ -648,13 +699,15 @@ int tpcca_get_counts(tpcca_ctx* c, int64_t out[5]) {
   out[2] = (c->done_mask & TPCCA_STAGE_TRACKLETS) ? c->status.trk_off[c->ns] : 0;
   out[3] = (c->done_mask & TPCCA_STAGE_TRACKLETS) ? c->status.hit_off[c->ns] : 0;
   out[4] = c->nb;
+  out[5] = (c->done_mask & TPCCA_STAGE_SELECT) ? c->status.sel_off[c->ns] : 0;
+  out[6] = (c->done_mask & TPCCA_STAGE_SELECT) ? c->status.sel_hit_off[c->ns] : 0;
   return TPCCA_OK;
 }
 
-int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[6]) {
+int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[7]) {
   if (!c || !ms) return TPCCA_E_ARG;
   if (runs_back < 0 || runs_back >= tpcca_ctx::kRing) return set_err(c, TPCCA_E_ARG, "runs_back must be in 0..15");
-  for (int i = 0; i < 6; ++i) ms[i] = 0.f;
+  for (int i = 0; i < 7; ++i) ms[i] = 0.f;
   if (runs_back >= c->run_count) return set_err(c, TPCCA_E_STATE, "no such run");
   const int k = (int)((c->run_count - 1 - runs_back) % tpcca_ctx::kRing);
   if (!c->ev_mask[k]) return set_err(c, TPCCA_E_STATE, "no such run");
@@ -662,6 +715,7 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[6]) {
   CU(c, cudaStreamSynchronize(c->stream));
   for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[k][i], c->ev[k][i + 1]));
   CU(c, cudaEventElapsedTime(&ms[5], c->ev[k][0], c->ev[k][5]));
+  CU(c, cudaEventElapsedTime(&ms[6], c->ev[k][5], c->ev[k][6]));
   return TPCCA_OK;
 }
 
@@ -701,7 +755,10 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   if (what & TPCCA_OUT_LINKS) need_stage = 3;
   if (what & TPCCA_OUT_START) need_stage = 4;
   if (what & TPCCA_OUT_TRACKS) need_stage = 5;
-  while (need_stage > 1 && !(c->done_mask & (1u << (need_stage - 1)))) --need_stage;     // stages that were never run deliver nothing
+  if ((what & (TPCCA_OUT_SELECTION | TPCCA_OUT_TRACKS_SEL)) && (c->done_mask & TPCCA_STAGE_SELECT)) need_stage = 6;
+  if ((what & TPCCA_OUT_TRACKS) && (what & TPCCA_OUT_TRACKS_SEL))
+    return set_err(c, TPCCA_E_ARG, "TPCCA_OUT_TRACKS and TPCCA_OUT_TRACKS_SEL fill the same fields: ask for one");
+  while (need_stage > 1 && need_stage <= 5 && !(c->done_mask & (1u << (need_stage - 1)))) --need_stage;     // stages that were never run deliver nothing
   const bool partial = host && need_stage < 5 && (c->done_mask & TPCCA_STAGE_TRACKLETS) && c->run_count > 0;
   int rc = partial ? fetch_status_after(c, std::max(need_stage, (c->done_mask & TPCCA_STAGE_START) ? 4 : need_stage)) : fetch_status(c);
   if (rc) return rc;
@@ -709,7 +766,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   const Layout& L = c->L;
   const DevStatus& S = c->status;
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
-  const uint32_t done = partial ? (c->done_mask & ~TPCCA_STAGE_TRACKLETS) : c->done_mask;
+  const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT)) : c->done_mask;
   v->n_clusters = n;
   v->n_bins = c->nb;
   int64_t s0 = 0, s1 = 0, t0 = 0, nt = 0, h0 = 0, h1 = 0;
@@ -756,6 +813,32 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
     add((const void* const*)&v->hit_idx, c->at<int32_t>(L.o_hit_idx) + h0, 4 * (size_t)(h1 - h0));
     v->trk_stride = host ? nt : c->CS;
   }
+  if (done & TPCCA_STAGE_SELECT) {
+    const int64_t k0 = S.sel_off[sector], nk = S.sel_off[sector + 1] - k0;
+    const int64_t g0 = S.sel_hit_off[sector], g1 = S.sel_hit_off[sector + 1];
+    v->n_selected = nk; v->n_sel_hits = g1 - g0;
+    if (what & TPCCA_OUT_SELECTION) {
+      add((const void* const*)&v->owner, reinterpret_cast<const int32_t*>(c->ws + L.rec + 8 * (size_t)c->N) + off, 4 * (size_t)n);
+      add((const void* const*)&v->n_own, c->at<int32_t>(L.sel_n_own) + t0, 4 * (size_t)nt);
+      add((const void* const*)&v->sel_track, c->at<int32_t>(L.sel_track) + k0, 4 * (size_t)nk);
+    }
+    if (what & TPCCA_OUT_TRACKS_SEL) {       // the S5 fields of the view, filled from the compact table of the selected tracks
+      const SelOut so = sel_out(c);
+      add((const void* const*)&v->x_ref, so.o.x_ref + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->z_ref, so.o.z_ref + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->chi2, so.o.chi2 + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->par, so.o.par + k0, 4 * (size_t)nk, 5);
+      add((const void* const*)&v->cov, so.o.cov + k0, 4 * (size_t)nk, 15);
+      add((const void* const*)&v->n_hits_trk, so.o.n_hits + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->n_fit, so.o.n_fit + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->first_row, so.o.first_row + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->last_row, so.o.last_row + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->trk_start_hit, so.o.start_hit + k0, 4 * (size_t)nk);
+      add((const void* const*)&v->hit_offset, so.o.hit_offset + k0 + sector, 4 * (size_t)(nk + 1));
+      add((const void* const*)&v->hit_idx, so.o.hit_idx + g0, 4 * (size_t)(g1 - g0));
+      v->trk_stride = host ? nk : c->CS;
+    }
+  }
   if (!host) {
     for (auto& it : items) *it.dst = it.src;
     return TPCCA_OK;
@@ -795,7 +878,7 @@ void tpcca_destroy(tpcca_ctx* c) {
   DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing; ++k)
-    for (int i = 0; i < 6; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
+    for (int i = 0; i < 7; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
   if (c->arena) cudaFreeHost(c->arena);
   if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
   delete c;

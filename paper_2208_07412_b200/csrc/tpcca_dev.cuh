@@ -30,6 +30,7 @@ struct DevTables {
   int32_t n_rows, n_sectors;
   int32_t bins_per_sector;              // nb = sum_r ny_r * nz_r
   int32_t tc_max_gap, tc_min_hits;
+  int32_t sel_permille;                 // S6: max shared hits of a selected tracklet, in 1/1000 of its hits
   float grid_z_lo;
   float Bc, err2_y, err2_z;
   float init_cov[5];
@@ -70,6 +71,8 @@ struct DevStatus {
   int32_t trk_off[kMaxSectors + 1];     // first track of each sector
   int64_t hit_off[kMaxSectors + 1];     // first hit of each sector (global CSR base)
   unsigned long long work[5];           // S5 work counters: propagations, updates, gates, searches, candidates
+  int32_t sel_off[kMaxSectors + 1];     // S6: first selected track of each sector
+  int64_t sel_hit_off[kMaxSectors + 1]; // S6: first hit of each sector in the selected hit CSR
 };
 
 // ---- S1 key: by = clamp(floor((y - y_lo) * inv_bin_y), 0, ny - 1) ------------

@@ -126,3 +126,31 @@ def compare_timeframe(tracker, tf, oracle_obj, sectors=None, stages=0x1F) -> dic
         tot["par_bit_exact"] &= rep.get("par_bit_exact", True)
         tot["cov_bit_exact"] &= rep.get("cov_bit_exact", True)
     return tot
+
+
+def compare_selection(tracker, tf, oracle_obj, sectors=None) -> dict:
+    """S6 (tracklet selector): owner / n_own / selected bit-exact against the oracle; the compact table of the
+    selected tracks must be the S5 table gathered at `selected` (bit-exact, hit lists included)."""
+    from paper_2208_07412_b200 import binding as B
+    tot = dict(sectors=0, n_tracks=0, n_selected=0)
+    for s in (range(tf.n_sectors) if sectors is None else sectors):
+        o = oracle_obj.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x3F)
+        g = tracker.get_tracks(s, B.OUT_TRACKS | B.OUT_SELECTION)
+        c = tracker.get_tracks(s, B.OUT_TRACKS_SEL)
+        rep = {}
+        try:
+            _eq("owner", g.owner, o.owner, rep)
+            _eq("n_own", g.n_own, o.n_own, rep)
+            _eq("selected", g.selected, o.selected, rep)
+            sel = o.selected
+            for f in ("x_ref", "z_ref", "chi2", "par", "cov", "n_hits", "n_fit", "first_row", "last_row", "trk_start_hit"):
+                _eq("sel." + f, getattr(c, f), getattr(g, f)[sel], rep)
+            off = np.concatenate([[0], np.cumsum(o.n_hits[sel])]).astype(np.int32)
+            _eq("sel.hit_offset", c.hit_offset, off, rep)
+            idx = (np.concatenate([o.hit_idx[o.hit_offset[t]:o.hit_offset[t + 1]] for t in sel]) if len(sel)
+                   else np.empty(0, np.int32))
+            _eq("sel.hit_idx", c.hit_idx, idx, rep)
+        except ParityError as e:
+            raise ParityError(f"sector {s}: {e}") from None
+        tot["sectors"] += 1; tot["n_tracks"] += int(o.n_tracks); tot["n_selected"] += int(len(o.selected))
+    return tot

@@ -421,3 +421,72 @@ def test_config2_full_size_six_sectors(pkg):
     assert tf.n_clusters > 25_000_000
     rep = check(pkg, tf, sectors=(0, 7, 13, 18, 26, 35))
     assert rep["sectors"] == 6 and rep["n_clusters"] > 4_000_000 and rep["links_differing"] == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# S6 tracklet selector
+# ------------------------------------------------------------------------------------------------
+def run_gpu_select(pkg, tf, **kw):
+    trk = pkg.Tracker(tf.params, max_clusters=max(tf.n_clusters, 1), **kw)
+    trk.load_timeframe(tf)
+    trk.run(0x3F)
+    trk.sync()
+    return trk
+
+
+def test_selector_config0_and_config1(pkg, cfg0, cfg1_small):
+    from parity import compare_selection
+    for tf in (cfg0, cfg1_small):
+        trk = run_gpu_select(pkg, tf)
+        orc = Oracle(tf.params)
+        compare_timeframe(trk, tf, orc)                    # S1-S5 outputs are untouched by S6
+        rep = compare_selection(trk, tf, orc)
+        cnt = trk.counts()
+        assert cnt["n_selected"] == rep["n_selected"] and 0 < rep["n_selected"] < rep["n_tracks"]
+        assert trk.timings()[6] > 0.0
+        trk.close()
+
+
+def test_selector_separate_run_and_thresholds(pkg, cfg1_small):
+    """S6 on its own after an S1-S5 run; other thresholds (0 = no shared hit allowed, 1000 = keep all)."""
+    from parity import compare_selection
+    tf = cfg1_small
+    for permille in (0, 250, 1000):
+        P = tf.params.copy(sel_max_shared_permille=permille)
+        tf2 = ArrTF(P, [(tf.y[s], tf.z[s], tf.row[s]) for s in (2, 11, 29)])
+        trk = run_gpu(pkg, tf2)
+        trk.run(0x20)
+        trk.sync()
+        rep = compare_selection(trk, tf2, Oracle(P))
+        if permille == 1000:
+            assert rep["n_selected"] == rep["n_tracks"]
+        # re-running S5 alone invalidates the selection (its tables alias S5 scratch)
+        trk.run(0x10)
+        trk.sync()
+        assert trk.counts()["n_selected"] == 0
+        trk.close()
+
+
+def test_selector_dense_stress_and_empty(pkg):
+    from parity import compare_selection
+    tf = tpcsynth.generate(4, n_tracks=1500)
+    trk = run_gpu_select(pkg, tf)
+    rep = compare_selection(trk, tf, Oracle(tf.params))
+    assert rep["n_selected"] > 300
+    trk.close()
+    P = tpcsynth.default_params(n_sectors=3)
+    e = (np.empty(0, np.float32), np.empty(0, np.float32), np.empty(0, np.uint16))
+    one = (np.array([0.5], np.float32), np.array([10.0], np.float32), np.array([7], np.uint16))
+    for secs in ([e, e, e], [one, e, one]):
+        tf = ArrTF(P, secs)
+        trk = run_gpu_select(pkg, tf)
+        assert compare_selection(trk, tf, Oracle(P))["n_selected"] == 0
+        trk.close()
+    rng = np.random.default_rng(2)
+    n = 6000
+    tf = ArrTF(tpcsynth.default_params(n_sectors=1), [((rng.random(n) * 16.0 - 8.0).astype(np.float32),
+                                                       (rng.random(n) * 12.0).astype(np.float32),
+                                                       rng.integers(0, 12, n).astype(np.uint16))])
+    trk = run_gpu_select(pkg, tf)
+    compare_selection(trk, tf, Oracle(tf.params))
+    trk.close()

@@ -784,3 +784,92 @@ def test_jacobian_n14_arc_term():
     n14 = s[6 + tri(4, 1)]                                            # C'_41 = J_14 * J_44
     want = p[3] * Bc * (p4 * Bc * 30.0) * 900.0 / 12.0                # p3 Bc (k d) d^2 / 12 with d = dx
     assert abs(fd - want) < 0.02 * want and abs(n14 - fd) < 0.02 * abs(fd), (n14, fd, want)
+
+
+# ----------------------------------------------------------------------------------------
+# S6 tracklet selector
+# ----------------------------------------------------------------------------------------
+def _read_selector_toy():
+    import os
+    tracks, exp = [], {}
+    owner = n_own = None
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "toy_selector.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        head, _, body = line.partition(":")
+        vals = [int(v) for v in body.split()]
+        if head.startswith("track"):
+            tracks.append(vals)
+        elif head == "owner":
+            owner = vals
+        elif head == "n_own":
+            n_own = vals
+        else:
+            exp[int(head.split()[1])] = vals
+    return tracks, owner, n_own, exp
+
+
+def test_selector_toy_worked_example():
+    from oracle import select_tracks
+    tracks, owner, n_own, exp = _read_selector_toy()
+    off = np.concatenate([[0], np.cumsum([len(t) for t in tracks])])
+    idx = np.concatenate(tracks)
+    for permille, want in exp.items():
+        o, w, s = select_tracks(len(owner), off, idx, permille)
+        assert o.tolist() == owner and w.tolist() == n_own and s.tolist() == want, permille
+
+
+def numpy_selector(n_clusters, hit_offset, hit_idx, permille):
+    """Independent formulation: sort all (cluster, -n_hits, track) triples; the first of every cluster owns it."""
+    nt = len(hit_offset) - 1
+    nh = np.diff(hit_offset).astype(np.int64)
+    trk = np.repeat(np.arange(nt), nh)
+    order = np.lexsort((trk, -nh[trk], hit_idx))
+    c_sorted = hit_idx[order]
+    first = np.ones(len(order), bool); first[1:] = c_sorted[1:] != c_sorted[:-1]
+    owner = np.full(n_clusters, -1, np.int64)
+    owner[c_sorted[first]] = trk[order][first]
+    n_own = np.bincount(trk[owner[hit_idx] == trk], minlength=nt)
+    sel = np.nonzero((nh - n_own) * 1000 <= permille * nh)[0]
+    return owner, n_own, sel
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_selector_equals_sort_formulation(seed):
+    from oracle import select_tracks
+    rng = np.random.default_rng(seed)
+    n, nt = 400, 120
+    lists = []
+    for t in range(nt):
+        k = int(rng.integers(1, 30))
+        base = int(rng.integers(0, n - 40))
+        lists.append(np.sort(rng.choice(np.arange(base, base + 40), size=k, replace=False)))   # overlapping neighbourhoods
+    off = np.concatenate([[0], np.cumsum([len(l) for l in lists])]).astype(np.int32)
+    idx = np.concatenate(lists).astype(np.int32)
+    for permille in (0, 250, 500, 900):
+        o, w, s = select_tracks(n, off, idx, permille)
+        o2, w2, s2 = numpy_selector(n, off, idx, permille)
+        assert np.array_equal(o, o2) and np.array_equal(w, w2) and np.array_equal(s, s2)
+        covered = np.zeros(n, bool); covered[idx] = True
+        assert np.array_equal(o >= 0, covered) and w.sum() == covered.sum()       # every covered cluster has one owner
+
+
+def test_selector_removes_clones_and_keeps_efficiency(cfg1_tracks):
+    """Generator truth (P10) before and after S6 on config-1 kinematics: about four clones per particle
+    (reading N3) fall to about one, the efficiency is unchanged, fakes do not grow."""
+    tf, secs, _ = cfg1_tracks
+    orc = Oracle(tf.params)
+    before, after = [], []
+    for s in secs:
+        r = orc.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x3F)
+        assert r.selected.shape[0] > 0 and np.all(np.diff(r.selected) > 0)
+        before.append(sector_metrics(tf.label[s], r.order, r.hit_offset, r.hit_idx))
+        off = np.concatenate([[0], np.cumsum(r.n_hits[r.selected])]).astype(np.int32)
+        idx = np.concatenate([r.hit_idx[r.hit_offset[t]:r.hit_offset[t + 1]] for t in r.selected])
+        after.append(sector_metrics(tf.label[s], r.order, off, idx))
+    b, a = summarize(before), summarize(after)
+    assert b["clone_rate"] > 0.6, b                       # >= 2.5 found tracks per matched particle
+    assert a["clone_rate"] < 0.05, a
+    assert a["efficiency"] >= b["efficiency"] - 0.005 and a["efficiency"] >= 0.97, (a, b)
+    assert a["fake_rate"] <= b["fake_rate"] + 0.01, (a, b)

@@ -75,6 +75,7 @@ class TrackerParams:
     grid_margin: float
     tc_max_gap: int
     tc_min_hits: int
+    sel_max_shared_permille: int = 500   # S6 selector: a tracklet survives iff at most this share of its hits is not its own
     # informative (not consumed by the tracker)
     sigma: float = 0.1
     z_hi: float = 250.0
