@@ -12,7 +12,7 @@ tpcsynth recipe of DESIGN.md 6).  N>1: one time frame per GPU (the paper's own s
               order + cleaned links + start hits + track table + hit CSR inside the timed region
   roofline  : neighbour finder (S2; the stage BASELINE.json's metric names) vs the measured HBM peak;
   roofline_dominant : the stage that takes the most time (S5 tracklets), plain-ALU bound
-  cpu_baseline : the oracle as it stands, one single-threaded oracle per host core, over 4 sectors of the same
+  cpu_baseline : the oracle as it stands, one single-threaded oracle per host core, over 8 sectors of the same
                  time frame spread over both sides (also the full-size parity check of those sectors)
 """
 from __future__ import annotations
@@ -383,20 +383,25 @@ def run_tpcca(args, env_cls=CudaEnv):
     # ---- end to end: host buffers in, host buffers out, through the public API ---------------------
     h2d = int(10 * N)
 
-    def e2e_step(t):
-        """One whole step through the public API: pinned HOST inputs in, HOST outputs out."""
+    def e2e_step(t, selected=False):
+        """One whole step through the public API: pinned HOST inputs in, HOST outputs out.  selected: the step also
+        runs S6 and ships the selected tracks (compact table) + per-cluster owner instead of every tracklet."""
         t.reset()
         for s, (a, b, c) in enumerate(host):
             t.load_clusters(s, a, b, c)
-        t.run()
+        t.run(0x3F if selected else 0x1F)
         out = 0
         early = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START          # ready after S4: copied while S5 runs
         for s in range(tf.n_sectors):
             v = t.get_tracks_view(s, B.MEM_HOST, early)
             out += 12 * v.n_clusters + 4 * v.n_start
         for s in range(tf.n_sectors):
-            v = t.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS)
-            out += 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
+            if selected:
+                v = t.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS_SEL | B.OUT_SELECTION)
+                out += 4 * v.n_sel_hits + (4 * 28 + 4) * v.n_selected + 4 + 4 * v.n_clusters + 4 * v.n_tracks + 4 * v.n_selected
+            else:
+                v = t.get_tracks_view(s, B.MEM_HOST, B.OUT_TRACKS)
+                out += 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4
         return int(out)
 
     # (a) serial: one context, step after step
@@ -410,6 +415,19 @@ def run_tpcca(args, env_cls=CudaEnv):
     env.synchronize()
     barrier()
     e2e_serial_ms = max_over_ranks(ev0.elapsed_time(ev1))
+
+    # (a') the same serial step with S6 on: the consumer downloads the selected tracks only
+    d2h_sel = e2e_step(trk, True)
+    barrier()
+    ev0.record()
+    for _ in range(e2e_steps):
+        e2e_step(trk, True)
+    ev1.record()
+    env.synchronize()
+    barrier()
+    e2e_sel_serial_ms = max_over_ranks(ev0.elapsed_time(ev1))
+    s6_ms = float(trk.timings(0)[6])
+    counts_sel = trk.counts()
 
     # (b) streaming (the EPN operating mode: time frames follow each other): two contexts on two
     # streams, each step still does its own H2D, S1-S5 and D2H, but the copies of one time frame overlap the
@@ -493,6 +511,12 @@ def run_tpcca(args, env_cls=CudaEnv):
                      ms_per_step=e2e_ms / e2e_steps, mode=e2e_mode,
                      serial_value=n_all * e2e_steps_serial / (e2e_serial_ms * 1e-3),
                      serial_ms_per_step=e2e_serial_ms / e2e_steps_serial),
+            selector=dict(stage_ms_S6=round(s6_ms, 4), n_selected=counts_sel["n_selected"], n_sel_hits=counts_sel["n_sel_hits"],
+                          note="S6 (SURVEY 8(f)-1) is outside the timed step; e2e_selected = serial step S1-S6 shipping the "
+                               "selected tracks + owner instead of every tracklet",
+                          e2e_selected=dict(value=n_all * e2e_steps_serial / (e2e_sel_serial_ms * 1e-3), unit=UNIT,
+                                            ms_per_step=e2e_sel_serial_ms / e2e_steps_serial, d2h_bytes_per_step=d2h_sel,
+                                            h2d_bytes_per_step=h2d, mode="serial, 1 context")),
             gpu_launches=int(launches_per_step * args.steps),
             clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1),
         )
@@ -531,7 +555,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--ref-z-frac", type=float, default=0.25)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-sectors", type=int, default=4, help="sectors of the CPU-baseline / full-size parity sample")
+    ap.add_argument("--cpu-sectors", type=int, default=8, help="sectors of the CPU-baseline / full-size parity sample")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")
     args = ap.parse_args()
@@ -542,6 +566,9 @@ def parse_args():
 
 def main():
     args = parse_args()
+    if "WORLD_SIZE" in os.environ:      # one line per rank on stderr: the launch can be counted from the log
+        print(f"bench.py rank {os.environ.get('RANK', '0')}/{os.environ['WORLD_SIZE']} started (pid {os.getpid()}, "
+              f"impl {args.impl})", file=sys.stderr, flush=True)
     if args.impl == "reference":
         run_reference(args)
     elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:

@@ -83,6 +83,7 @@ def test_reference_arm_prints_on_rank0_only():
 class _FakeView:
     def __init__(self, n):
         self.n_clusters, self.n_start, self.n_tracks, self.n_hits = n, n // 30, n // 40, n // 2
+        self.n_selected, self.n_sel_hits = n // 160, n // 8
 
 
 class _FakeTracker:
@@ -107,11 +108,12 @@ class _FakeTracker:
         return 30
 
     def counts(self):
-        return dict(n_clusters=self.n, n_start=self.n // 30, n_tracks=self.n // 40, n_hits=self.n // 2, n_bins=1000)
+        return dict(n_clusters=self.n, n_start=self.n // 30, n_tracks=self.n // 40, n_hits=self.n // 2, n_bins=1000,
+                    n_selected=self.n // 160, n_sel_hits=self.n // 8)
 
     def timings(self, i=0):
         t = self.env.step_ms
-        return [0.1 * t, 0.1 * t, 0.05 * t, 0.05 * t, 0.7 * t, t]
+        return [0.1 * t, 0.1 * t, 0.05 * t, 0.05 * t, 0.7 * t, t, 0.02 * t]
 
     def work_counters(self):
         return dict(propagations=10, updates=10, gates=1, searches=5, candidates=9)
@@ -237,4 +239,5 @@ def test_bench_gpus_n_starts_n_ranks():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--config", "0"],
                        env=env, capture_output=True, text=True, timeout=300)
     assert r.returncode != 0
-    assert "bench.py rank 0/2: needs a CUDA device" in r.stderr and "bench.py rank 1/2: needs a CUDA device" in r.stderr
+    assert "bench.py rank 0/2 started" in r.stderr and "bench.py rank 1/2 started" in r.stderr
+    assert "needs a CUDA device: tpcca has no CPU path" in r.stderr     # (the launcher stops the other rank at the first failure)
