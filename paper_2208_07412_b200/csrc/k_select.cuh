@@ -16,25 +16,37 @@ __device__ __forceinline__ int sector_of_track(const DevStatus* __restrict__ st,
   return lo;
 }
 
-// ownership key of track t_local with nh hits: larger = better; ties in nh -> the smaller track number wins
-__device__ __forceinline__ unsigned long long sel_key(int nh, int t_local) {
-  return ((unsigned long long)(uint32_t)nh << 32) | (unsigned long long)(0xFFFFFFFFu - (uint32_t)t_local);
+// ownership key of track t_local with nh hits: larger = better; ties in nh -> the smaller track number wins.
+// 32 bits: nh (<= TPCCA_MAX_ROWS = 256: 9 bits) | 0x7FFFFF - t_local (a sector with 2^23 or more tracks is refused:
+// DevStatus::err_select).  0 = unclaimed (a real key has nh >= 1 in its top bits).
+constexpr int kSelTrackBits = 23;
+__device__ __forceinline__ uint32_t sel_key(int nh, int t_local) {
+  return ((uint32_t)nh << kSelTrackBits) | (uint32_t)(((1 << kSelTrackBits) - 1) - t_local);
 }
 
+// Both passes walk the tracks in the PROCESSING ORDER of S5 (perm: sector by sector in ascending z), not in output
+// order: the three or four clones of a particle then touch its ~100 clusters within a short time and the scattered
+// 4-byte accesses hit L2 instead of DRAM.  slot_trk[slot] = global track of the start-hit slot (-1: rejected).
 // ---- K6a: claim.  One warp per track: own_key[cluster] = max over the tracks holding it ---------------
 __global__ void __launch_bounds__(256)
-k_sel_claim(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
+k_sel_claim(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, DevStatus* __restrict__ st,
+            const int4* __restrict__ perm, const int32_t* __restrict__ slot_trk,
             const int32_t* __restrict__ n_hits, const int32_t* __restrict__ hit_offset, const int32_t* __restrict__ hit_idx,
-            unsigned long long* __restrict__ own_key) {
-  const int ns = T->n_sectors;
-  const int n_trk = st->trk_off[ns];
+            uint32_t* __restrict__ own_key) {
+  if (st->err_capacity || st->err_range) return;
+  const int n_start = st->n_start;
   const int lane = threadIdx.x & 31;
-  for (int t = blockIdx.x * 8 + (threadIdx.x >> 5); t < n_trk; t += gridDim.x * 8) {
-    const int s = sector_of_track(st, ns, t);
+  for (int j = blockIdx.x * 8 + (threadIdx.x >> 5); j < n_start; j += gridDim.x * 8) {
+    const int4 pr = __ldg(&perm[j]);
+    const int t = slot_trk[pr.x];
+    if (t < 0) continue;
+    const int s = pr.y >> 16;
+    const int t_local = t - st->trk_off[s];
+    if (t_local >= (1 << kSelTrackBits) - 1) { if (lane == 0) st->err_select = 1; continue; }
     const int nh = n_hits[t];
     const long long h0 = st->hit_off[s] + hit_offset[t + s];
-    const unsigned long long key = sel_key(nh, t - st->trk_off[s]);
-    unsigned long long* ok = own_key + sec[s].off;
+    const uint32_t key = sel_key(nh, t_local);
+    uint32_t* ok = own_key + sec[s].off;
     for (int k = lane; k < nh; k += 32) {
       const int c = hit_idx[h0 + k];
       // (plain read first: most clusters are claimed by three or four clones and only the first few raise the key)
@@ -46,17 +58,21 @@ k_sel_claim(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
 // ---- K6b: count.  One warp per track: n_own[t] = hits whose key is the track's own ----------------------
 __global__ void __launch_bounds__(256)
 k_sel_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
+            const int4* __restrict__ perm, const int32_t* __restrict__ slot_trk,
             const int32_t* __restrict__ n_hits, const int32_t* __restrict__ hit_offset, const int32_t* __restrict__ hit_idx,
-            const unsigned long long* __restrict__ own_key, int32_t* __restrict__ n_own) {
-  const int ns = T->n_sectors;
-  const int n_trk = st->trk_off[ns];
+            const uint32_t* __restrict__ own_key, int32_t* __restrict__ n_own) {
+  if (st->err_capacity || st->err_range) return;
+  const int n_start = st->n_start;
   const int lane = threadIdx.x & 31;
-  for (int t = blockIdx.x * 8 + (threadIdx.x >> 5); t < n_trk; t += gridDim.x * 8) {
-    const int s = sector_of_track(st, ns, t);
+  for (int j = blockIdx.x * 8 + (threadIdx.x >> 5); j < n_start; j += gridDim.x * 8) {
+    const int4 pr = __ldg(&perm[j]);
+    const int t = slot_trk[pr.x];
+    if (t < 0) continue;
+    const int s = pr.y >> 16;
     const int nh = n_hits[t];
     const long long h0 = st->hit_off[s] + hit_offset[t + s];
-    const unsigned long long key = sel_key(nh, t - st->trk_off[s]);
-    const unsigned long long* ok = own_key + sec[s].off;
+    const uint32_t key = sel_key(nh, t - st->trk_off[s]);
+    const uint32_t* ok = own_key + sec[s].off;
     int cnt = 0;
     for (int k = lane; k < nh; k += 32) cnt += (ok[hit_idx[h0 + k]] == key) ? 1 : 0;
 #pragma unroll
@@ -166,12 +182,12 @@ __global__ void k_sel_close_empty(const DevTables* __restrict__ T, const DevStat
   if (st->trk_off[s] == st->trk_off[s + 1]) out.o.hit_offset[st->sel_off[s] + s] = 0;
 }
 
-// ---- K6f: owner[c] = track number decoded from the key (-1: the cluster is in no track) ----------------
+// ---- K6f: in place: owner[c] = track number decoded from the key (-1: the cluster is in no track) --------
 __global__ void __launch_bounds__(256)
-k_sel_owner(const unsigned long long* __restrict__ own_key, int32_t* __restrict__ owner, size_t n) {
+k_sel_owner(uint32_t* __restrict__ key_owner, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const unsigned long long k = own_key[i];
-    owner[i] = k ? (int32_t)(0xFFFFFFFFu - (uint32_t)k) : -1;
+    const uint32_t k = key_owner[i];
+    key_owner[i] = k ? (uint32_t)(((1 << kSelTrackBits) - 1) - (int)(k & ((1u << kSelTrackBits) - 1u))) : 0xFFFFFFFFu;
   }
 }
 

@@ -647,7 +647,7 @@ __global__ void __launch_bounds__(1024)
 k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st,
                const int32_t* __restrict__ start_hit, int32_t cap, const int32_t* __restrict__ hits,
                const float4* __restrict__ trk_v, const int32_t* __restrict__ trk_n,
-               const longlong2* __restrict__ tile_off, TrackOut o) {
+               const longlong2* __restrict__ tile_off, TrackOut o, int32_t* __restrict__ slot_trk /*[cap]: slot -> track, -1*/) {
   __shared__ int ws[33];
   const int ns = T->n_sectors, n_rows_g = T->n_rows;
   const int n_start = st->err_capacity ? 0 : st->n_start;
@@ -668,6 +668,7 @@ k_track_gather(const DevTables* __restrict__ T, const DevStatus* __restrict__ st
   const long long h = tile_off[blockIdx.x].y + eb;       // global hit index
   int first = 0, last = -1;
   if (valid) {
+    slot_trk[slot] = nh > 0 ? (int32_t)t : -1;
     const long long hloc = h - st->hit_off[s];
     // hit_offset of sector s lives at [trk_off[s] + s, trk_off[s+1] + s + 1)
     if (nh > 0) {

@@ -29,7 +29,7 @@ struct Layout {
   size_t tile_cnt, tile_off, start_bits;
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
-  size_t sel_n_own, sel_track;   // S6 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
+  size_t sel_n_own, sel_track, slot_trk;   // S6 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
 };
@@ -115,6 +115,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.o_hit_idx = take(4 * (size_t)(nr * CS));
   L.sel_n_own = take(4 * (size_t)CS);
   L.sel_track = take(4 * (size_t)CS);
+  L.slot_trk = take(4 * (size_t)CS);     // start-hit slot -> global track (S5 gather), -1 = rejected
   L.total = cur;
   return L;
 }
@@ -228,6 +229,7 @@ int status_errors(tpcca_ctx* c) {
   if (c->status.err_capacity)
     return set_err(c, TPCCA_E_WORKSPACE, "start-hit capacity exceeded: %d start hits > max_start_hits %lld",
                    c->status.n_start, (long long)c->CS);
+  if (c->status.err_select) return set_err(c, TPCCA_E_WORKSPACE, "S6: a sector holds 2^23 or more tracks (selector key capacity)");
   return TPCCA_OK;
 }
 
@@ -250,11 +252,7 @@ int fetch_status(tpcca_ctx* c) {
   CU(c, cudaMemcpyAsync(&c->status, c->at<DevStatus>(c->L.status), sizeof(DevStatus), cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
   c->status_valid = true;
-  if (c->status.err_range) return set_err(c, TPCCA_E_RANGE, "a cluster has row >= n_rows (%d)", c->nr);
-  if (c->status.err_capacity)
-    return set_err(c, TPCCA_E_WORKSPACE, "start-hit capacity exceeded: %d start hits > max_start_hits %lld",
-                   c->status.n_start, (long long)c->CS);
-  return TPCCA_OK;
+  return status_errors(c);
 }
 
 // S6 compact table of the selected tracks: 28 planes of CS words in the S5 slot-record buffer (trk_v: exactly
@@ -641,7 +639,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     k_track_tile_sums<<<cap_tiles, 1024, 0, st>>>(status, trk_i, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 2);
     k_track_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, trk_i, tile_off, tot + 2);
-    k_track_gather<<<cap_tiles, 1024, 0, st>>>(T, status, start_hit, cap, hits, trk_f, trk_i, tile_off, o);
+    k_track_gather<<<cap_tiles, 1024, 0, st>>>(T, status, start_hit, cap, hits, trk_f, trk_i, tile_off, o, c->at<int32_t>(L.slot_trk));
     k_track_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, o);
     c->launches += 9;
   }
@@ -655,21 +653,22 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     in.n_fit = c->at<int32_t>(L.o_n_fit); in.first_row = c->at<int32_t>(L.o_first); in.last_row = c->at<int32_t>(L.o_last);
     in.start_hit = c->at<int32_t>(L.o_start); in.hit_offset = c->at<int32_t>(L.o_hit_offset); in.hit_idx = c->at<int32_t>(L.o_hit_idx);
     SelOut so = sel_out(c);
-    unsigned long long* own_key = c->at<unsigned long long>(L.rec);
-    int32_t* owner = reinterpret_cast<int32_t*>(c->ws + L.rec + 8 * (size_t)c->N);
+    uint32_t* own_key = c->at<uint32_t>(L.rec);          // ownership keys, decoded in place to `owner` at the end
     int32_t* n_own = c->at<int32_t>(L.sel_n_own);
+    const int32_t* slot_trk = c->at<int32_t>(L.slot_trk);
+    const int4* perm = c->at<int4>(L.perm);
     const int cap_tiles = (int)((c->CS + 1023) / 1024);
     const size_t nk = (size_t)std::max<int64_t>(c->n_total, 1);
-    k_zero_words<<<(unsigned)std::min<size_t>((2 * nk + 1023) / 1024, (size_t)c->sm_count * 32), 256, 0, st>>>(reinterpret_cast<uint32_t*>(own_key), 2 * nk);
-    const int warp_grid = (int)std::min<int64_t>((c->CS + 7) / 8, (int64_t)c->sm_count * 64);
-    k_sel_claim<<<warp_grid, 256, 0, st>>>(T, sec, status, in.n_hits, in.hit_offset, in.hit_idx, own_key);
-    k_sel_count<<<warp_grid, 256, 0, st>>>(T, sec, status, in.n_hits, in.hit_offset, in.hit_idx, own_key, n_own);
+    k_zero_words<<<(unsigned)std::min<size_t>((nk + 1023) / 1024, (size_t)c->sm_count * 32), 256, 0, st>>>(own_key, nk);
+    const int warp_grid = (int)std::min<int64_t>((c->CS + 7) / 8, (int64_t)c->sm_count * 8);
+    k_sel_claim<<<warp_grid, 256, 0, st>>>(T, sec, status, perm, slot_trk, in.n_hits, in.hit_offset, in.hit_idx, own_key);
+    k_sel_count<<<warp_grid, 256, 0, st>>>(T, sec, status, perm, slot_trk, in.n_hits, in.hit_offset, in.hit_idx, own_key, n_own);
     k_sel_tile_sums<<<cap_tiles, 1024, 0, st>>>(T, status, in.n_hits, n_own, tile_cnt);
     k_scan_pairs<<<1, 1024, 0, st>>>(tile_cnt, tile_off, cap_tiles, tot + 6);
     k_sel_sector_bases<<<1, kMaxSectors + 1, 0, st>>>(T, status, in.n_hits, n_own, tile_off, tot + 6);
     k_sel_gather<<<cap_tiles, 1024, 0, st>>>(T, status, cap, n_own, tile_off, in, so);
     k_sel_close_empty<<<1, kMaxSectors, 0, st>>>(T, status, so);
-    k_sel_owner<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(own_key, owner, nk);
+    k_sel_owner<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(own_key, nk);
     c->launches += 9;
   }
   mark(6);
@@ -818,7 +817,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
     const int64_t g0 = S.sel_hit_off[sector], g1 = S.sel_hit_off[sector + 1];
     v->n_selected = nk; v->n_sel_hits = g1 - g0;
     if (what & TPCCA_OUT_SELECTION) {
-      add((const void* const*)&v->owner, reinterpret_cast<const int32_t*>(c->ws + L.rec + 8 * (size_t)c->N) + off, 4 * (size_t)n);
+      add((const void* const*)&v->owner, c->at<int32_t>(L.rec) + off, 4 * (size_t)n);
       add((const void* const*)&v->n_own, c->at<int32_t>(L.sel_n_own) + t0, 4 * (size_t)nt);
       add((const void* const*)&v->sel_track, c->at<int32_t>(L.sel_track) + k0, 4 * (size_t)nk);
     }

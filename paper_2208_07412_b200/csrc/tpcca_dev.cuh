@@ -64,6 +64,7 @@ struct SectorDesc {
 struct DevStatus {
   int32_t err_range;       // some cluster had row >= n_rows
   int32_t err_capacity;    // n_start exceeded max_start_hits
+  int32_t err_select;      // S6: a sector holds 2^23 or more tracks (ownership key overflow)
   uint32_t n_big;          // S1 coarse buckets too large for the shared-memory sort
   int32_t n_start;         // total start hits
   int32_t work_counter[8]; // S5 dynamic work distribution: one counter per kernel mode (index 1..4)
