@@ -13,6 +13,7 @@
  *   S5 tracklet construction + fp32 Kalman helix fit   (Bz = 0.5 T)
  * and, beyond the five (SURVEY.md 8(f) "next" rows):
  *   S6 tracklet selector: per-cluster ownership, clone removal
+ *   S7 track-residual front end of a track-model cluster compression
  * "clusters per sector and pad row in, links and fitted tracks out" (BASELINE.json:5).
  *
  * Every stage runs in hand-written CUDA kernels for sm_100a; there is NO CPU fallback: every
@@ -63,6 +64,7 @@ extern "C" {
 #define TPCCA_STAGE_TRACKLETS  0x10u
 #define TPCCA_STAGE_ALL        0x1Fu   /* the five stages of the hot path (BASELINE.json:5)             */
 #define TPCCA_STAGE_SELECT     0x20u   /* S6 tracklet selector; needs S1-S5           */
+#define TPCCA_STAGE_RESIDUALS  0x40u   /* S7 cluster residuals to the selected tracks; needs S1-S6 */
 
 /* which output groups tpcca_get_tracks delivers (HOST: copies) */
 #define TPCCA_OUT_ORDER      0x01u  /* order                                      (S1)            */
@@ -76,6 +78,7 @@ extern "C" {
 #define TPCCA_OUT_TRACKS_SEL 0x80u  /* the track table + hit CSR of the SELECTED tracks only (S6): fills the S5    */
                                     /* fields of the view from the compact table (array lengths: n_selected and    */
                                     /* n_sel_hits instead of n_tracks and n_hits); not together with OUT_TRACKS   */
+#define TPCCA_OUT_RESIDUALS  0x100u /* res_trk, res_y, res_z, q_y, q_z            (S7)            */
 
 typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
 
@@ -105,6 +108,7 @@ typedef struct {
   int32_t tc_max_gap;              /* S5: consecutive rows without a hit before stopping          */
   int32_t tc_min_hits;             /* S5: minimum hits of an emitted track                        */
   int32_t sel_max_shared_permille; /* S6: a tracklet is selected iff (n_hits - n_own) * 1000 <= this * n_hits     */
+  float res_inv_quantum;           /* S7: residuals are quantised to rint(res * this), 16 bits (> 0)              */
 } tpcca_params;
 
 /* Outputs of ONE sector.  With mem_space == TPCCA_MEM_DEVICE the pointers are DEVICE pointers
@@ -147,6 +151,10 @@ typedef struct {
   const int32_t  *owner;      /* [n_clusters] track (sector-local number) owning the cluster; -1 */
   const int32_t  *n_own;      /* [n_tracks] hits of each S5 track that the track owns            */
   const int32_t  *sel_track;  /* [n_selected] ascending sector-local numbers of the selected     */
+  /* S7: residual front end, per cluster (sorted position) */
+  const int32_t  *res_trk;    /* [n_clusters] selected track (sector-local number) the cluster is attached to; -1 */
+  const float    *res_y, *res_z;   /* [n_clusters] y_c - y_track, z_c - z_track at the cluster's row; 0 if -1    */
+  const int16_t  *q_y, *q_z;  /* [n_clusters] rint(res * res_inv_quantum), clamped to +-32767    */
 } tpcca_tracks_view;
 
 /* Bytes of DEVICE workspace that tpcca_create needs for at most `max_clusters_total` clusters
@@ -182,7 +190,7 @@ int tpcca_load_clusters(tpcca_ctx *ctx, int sector, int64_t n, const float *x, c
 /* Start a new time frame: forget all loaded sectors and all outputs (no device work). */
 int tpcca_reset(tpcca_ctx *ctx);
 
-/* Run the stages in `stage_mask` (bit i = stage i+1; TPCCA_STAGE_SELECT = S6) over all sectors, asynchronously on the
+/* Run the stages in `stage_mask` (bit i = stage i+1; S6, S7: TPCCA_STAGE_SELECT, TPCCA_STAGE_RESIDUALS) over all sectors, asynchronously on the
  * context's stream.  A stage needs the outputs of the stages before it from this or an earlier
  * run on the same clusters (TPCCA_E_STATE otherwise).  Device-side failures (row out of range,
  * start-hit capacity overflow) are reported by the next tpcca_get_* / tpcca_sync call.
@@ -211,10 +219,10 @@ int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[7]);
 
 /* Device time of each stage [ms] of the run `runs_back` runs ago (0 = the last tpcca_run; the
  * context keeps the events of its last 16 runs), from CUDA events recorded on the context's
- * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6 (0 if not run).
+ * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6, ms[7] = S7 (0 if not run).
  * Synchronises the stream.
  * Errors: TPCCA_E_ARG (runs_back outside 0..15), TPCCA_E_STATE (no such run). */
-int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[7]);
+int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[8]);
 
 /* Work counters of the last run's S5 kernel, for the ALU roofline:
  * out[0] = Kalman propagations that moved the state, out[1] = Kalman updates,

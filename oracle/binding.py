@@ -23,7 +23,7 @@ class _Params(C.Structure):
         ("tc_win_y", C.c_double), ("tc_win_z", C.c_double), ("tc_gate", C.c_double),
         ("max_sinphi", C.c_double), ("grid_margin", C.c_double),
         ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32),
-        ("sel_max_shared_permille", C.c_int32),
+        ("sel_max_shared_permille", C.c_int32), ("res_inv_quantum", C.c_double),
     ]
 
 
@@ -53,6 +53,7 @@ def _load():
         lib.oracle_n_selected.argtypes = [C.c_void_p]
         lib.oracle_n_selected.restype = C.c_int64
         lib.oracle_get_selection.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+        lib.oracle_get_residuals.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         lib.oracle_select.argtypes = [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 3
         lib.oracle_select.restype = C.c_int64
         _lib = lib
@@ -88,6 +89,11 @@ class OracleResult:
     owner: np.ndarray = None        # S6: [n] track owning each cluster (-1 none)
     n_own: np.ndarray = None        # S6: [n_tracks]
     selected: np.ndarray = None     # S6: [n_selected] ascending track numbers
+    res_trk: np.ndarray = None      # S7: [n] selected track owning the cluster (-1: stored raw)
+    res_y: np.ndarray = None        # S7: [n] residuals to the track model
+    res_z: np.ndarray = None
+    q_y: np.ndarray = None          # S7: [n] int16 quantised residuals
+    q_z: np.ndarray = None
 
     @property
     def n_tracks(self) -> int:
@@ -132,6 +138,7 @@ class Oracle:
         p.grid_margin = float(params.grid_margin)
         p.tc_max_gap = int(params.tc_max_gap); p.tc_min_hits = int(params.tc_min_hits)
         p.sel_max_shared_permille = int(getattr(params, "sel_max_shared_permille", 500))
+        p.res_inv_quantum = float(getattr(params, "res_inv_quantum", 128.0))
         self._h = lib.oracle_create(C.byref(p), self.precision)
         if not self._h:
             raise RuntimeError("oracle_create failed")
@@ -187,6 +194,11 @@ class Oracle:
             res.owner = np.empty(n, np.int32); res.n_own = np.empty(n_trk, np.int32)
             res.selected = np.empty(int(self._lib.oracle_n_selected(self._h)), np.int32)
             self._lib.oracle_get_selection(self._h, res.owner.ctypes.data, res.n_own.ctypes.data, res.selected.ctypes.data)
+        if "tracks" in want and (stage_mask & 64):
+            res.res_trk = np.empty(n, np.int32); res.res_y = np.empty(n); res.res_z = np.empty(n)
+            res.q_y = np.empty(n, np.int16); res.q_z = np.empty(n, np.int16)
+            self._lib.oracle_get_residuals(self._h, res.res_trk.ctypes.data, res.res_y.ctypes.data, res.res_z.ctypes.data,
+                                           res.q_y.ctypes.data, res.q_z.ctypes.data)
         return res
 
     # ---- unit entry points (pins) ---------------------------------------------------

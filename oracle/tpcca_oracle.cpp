@@ -56,6 +56,7 @@ struct oracle_params {      // all tables are double arrays holding the (fp32-re
   double tc_win_y, tc_win_z, tc_gate, max_sinphi, grid_margin;
   int32_t tc_max_gap, tc_min_hits;
   int32_t sel_max_shared_permille;   // S6: a tracklet survives iff shared hits * 1000 <= this * n_hits
+  double res_inv_quantum;            // S7: residuals are quantised to round(res * this), 16 bits
 };
 }
 
@@ -136,6 +137,7 @@ class Oracle {
     max_sinphi = (R)q.max_sinphi; margin = (R)q.grid_margin;
     max_gap = q.tc_max_gap; min_hits = q.tc_min_hits;
     sel_permille = q.sel_max_shared_permille;
+    res_inv_q = (R)q.res_inv_quantum;
     row_bin_base.resize(n_rows + 1);
     row_bin_base[0] = 0;
     for (int r = 0; r < n_rows; ++r) row_bin_base[r + 1] = row_bin_base[r] + (int64_t)ny[r] * nz[r];
@@ -479,6 +481,41 @@ class Oracle {
     }
   }
 
+  // ----------------------------------------------------------------------------- S7: track residuals
+  // SURVEY.md 8(f)-4 / DESIGN.md 3.7: the front end of a track-model cluster compression ("data
+  // compression rely on the information from TPC tracking").  For every SELECTED track t (S6), starting from its
+  // fitted state (x_ref, p) and walking its hits in ascending row, the state is transported hit to hit with
+  // Propagate (mean only: the covariance is not needed) and, for every hit c that t OWNS,
+  //   res_y[c] = y_c - p0,   res_z[c] = (z_c - z_ref) - p1,   q_y = clamp(rint(res_y * inv_quantum), +-32767), q_z likewise
+  // (rint = round half to even, the fp32 decision), res_trk[c] = t.  A failed transport ends the track's walk.
+  // Clusters no selected track owns keep res_trk = -1, residuals 0 (a codec stores them raw).
+  void track_residuals() {
+    res_trk.assign(n, -1); res_y.assign(n, (R)0); res_z.assign(n, (R)0); q_y.assign(n, 0); q_z.assign(n, 0);
+    for (int32_t t : selected) {
+      const Track<R>& T = tracks[t];
+      KFState<R> s;
+      s.x = T.x_ref;
+      for (int i = 0; i < 5; ++i) s.p[i] = T.p[i];
+      for (int i = 0; i < 15; ++i) s.C[i] = (R)0;
+      s.chi2 = (R)0; s.n = 0;
+      for (int32_t k = hit_offset[t]; k < hit_offset[t + 1]; ++k) {
+        const int32_t c = hit_idx[k];
+        if (!propagate(s, row_x[srow[c]])) break;
+        if (owner[c] != t) continue;
+        const R ry = sy[c] - s.p[0];
+        const R rz = (sz[c] - T.z_ref) - s.p[1];
+        res_trk[c] = t; res_y[c] = ry; res_z[c] = rz;
+        q_y[c] = quantise(ry); q_z[c] = quantise(rz);
+      }
+    }
+  }
+  int16_t quantise(R r) const {
+    R v = std::nearbyint(r * res_inv_q);          // default rounding mode: half to even
+    if (v > (R)32767) v = (R)32767;
+    if (v < (R)-32767) v = (R)-32767;
+    return (int16_t)v;
+  }
+
   void run(uint32_t stage_mask, bool brute) {
     if (stage_mask & 1u) build_grid();
     if (stage_mask & 2u) find_neighbours(brute);
@@ -487,6 +524,7 @@ class Oracle {
     if (stage_mask & 16u) construct_tracklets();
     if (stage_mask & 32u)
       select_tracks_plain(n, (int64_t)tracks.size(), hit_offset.data(), hit_idx.data(), sel_permille, owner, n_own, selected);
+    if (stage_mask & 64u) track_residuals();
   }
 
   // tables
@@ -497,6 +535,7 @@ class Oracle {
   R grid_z_lo, Bc, err2_y, err2_z, init_cov[5], win_y, win_z, gate, max_sinphi, margin;
   R c24, c640, c12;
   int max_gap, min_hits, sel_permille;
+  R res_inv_q;
   // data
   int64_t n = 0;
   std::vector<R> y, z, sy, sz;
@@ -507,6 +546,9 @@ class Oracle {
   std::vector<Track<R>> tracks;
   std::vector<int32_t> hit_offset, hit_idx;
   std::vector<int32_t> owner, n_own, selected;   // S6
+  std::vector<int32_t> res_trk;                  // S7
+  std::vector<R> res_y, res_z;
+  std::vector<int16_t> q_y, q_z;
 };
 
 struct Handle {
@@ -627,6 +669,16 @@ void oracle_get_selection(void* hv, int32_t* owner, int32_t* n_own, int32_t* sel
     std::copy((o)->selected.begin(), (o)->selected.end(), selected); } while (0)
   if (h->precision == 0) GS(h->f); else GS(h->d);
 #undef GS
+}
+// S7 outputs of the last run with stage bit 64, per cluster: res_trk i32, res_y / res_z double, q_y / q_z i16
+void oracle_get_residuals(void* hv, int32_t* res_trk, double* res_y, double* res_z, int16_t* q_y, int16_t* q_z) {
+  Handle* h = (Handle*)hv;
+#define GR(o) do { \
+    std::copy((o)->res_trk.begin(), (o)->res_trk.end(), res_trk); \
+    copy_out(res_y, (o)->res_y); copy_out(res_z, (o)->res_z); \
+    std::copy((o)->q_y.begin(), (o)->q_y.end(), q_y); std::copy((o)->q_z.begin(), (o)->q_z.end(), q_z); } while (0)
+  if (h->precision == 0) GR(h->f); else GR(h->d);
+#undef GR
 }
 // the selector on its own, on hit lists given by the caller (pins): returns the number of selected tracks
 int64_t oracle_select(int64_t n_clusters, int64_t n_tracks, const int32_t* hit_offset, const int32_t* hit_idx,

@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 STAGE_GRID, STAGE_NEIGHBOURS, STAGE_CLEAN, STAGE_START, STAGE_TRACKLETS, STAGE_ALL = 1, 2, 4, 8, 16, 31
-STAGE_SELECT = 32
+STAGE_SELECT, STAGE_RESIDUALS = 32, 64
 MEM_HOST, MEM_DEVICE, MEM_DEVICE_BORROW = 0, 1, 2
 
 _fp = C.POINTER(C.c_float)
@@ -27,7 +27,7 @@ ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "
                "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
                "tpcca_get_launch_count", "tpcca_get_info", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
-OUT_SELECTION, OUT_TRACKS_SEL = 64, 128
+OUT_SELECTION, OUT_TRACKS_SEL, OUT_RESIDUALS = 64, 128, 256
 
 
 class TpccaError(RuntimeError):
@@ -47,6 +47,7 @@ class _Params(C.Structure):
         ("tc_win_y", C.c_float), ("tc_win_z", C.c_float), ("tc_gate", C.c_float),
         ("max_sinphi", C.c_float), ("grid_margin", C.c_float),
         ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32), ("sel_max_shared_permille", C.c_int32),
+        ("res_inv_quantum", C.c_float),
     ]
 
 
@@ -61,6 +62,7 @@ class _View(C.Structure):
         ("n_hits_trk", _ip), ("n_fit", _ip), ("first_row", _ip), ("last_row", _ip), ("trk_start_hit", _ip),
         ("hit_offset", _ip), ("hit_idx", _ip),
         ("n_selected", C.c_int64), ("n_sel_hits", C.c_int64), ("owner", _ip), ("n_own", _ip), ("sel_track", _ip),
+        ("res_trk", _ip), ("res_y", _fp), ("res_z", _fp), ("q_y", C.POINTER(C.c_int16)), ("q_z", C.POINTER(C.c_int16)),
     ]
 
 
@@ -134,6 +136,7 @@ def _make_params(P):
     p.max_sinphi = float(P.max_sinphi); p.grid_margin = float(P.grid_margin)
     p.tc_max_gap = int(P.tc_max_gap); p.tc_min_hits = int(P.tc_min_hits)
     p.sel_max_shared_permille = int(getattr(P, "sel_max_shared_permille", 500))
+    p.res_inv_quantum = float(getattr(P, "res_inv_quantum", 128.0))
     return p, keep
 
 
@@ -178,6 +181,11 @@ class SectorOutput:
     owner: np.ndarray = None       # S6
     n_own: np.ndarray = None
     selected: np.ndarray = None
+    res_trk: np.ndarray = None     # S7
+    res_y: np.ndarray = None
+    res_z: np.ndarray = None
+    q_y: np.ndarray = None
+    q_z: np.ndarray = None
 
     @property
     def n_tracks(self) -> int:
@@ -299,8 +307,8 @@ class Tracker:
                     n_bins=int(out[4]), n_selected=int(out[5]), n_sel_hits=int(out[6]))
 
     def timings(self, runs_back: int = 0):
-        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, S1..S5, S6]."""
-        out = (C.c_float * 7)()
+        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, S1..S5, S6, S7]."""
+        out = (C.c_float * 8)()
         self._check(self._lib.tpcca_get_timings(self._h, int(runs_back), out))
         return [float(v) for v in out]
 
@@ -349,6 +357,9 @@ class Tracker:
         if v.owner:
             o.owner = _np(v.owner, n, np.int32); o.n_own = _np(v.n_own, int(v.n_tracks), np.int32)
             o.selected = _np(v.sel_track, int(v.n_selected), np.int32)
+        if v.res_trk:
+            o.res_trk = _np(v.res_trk, n, np.int32); o.res_y = _np(v.res_y, n, np.float32); o.res_z = _np(v.res_z, n, np.float32)
+            o.q_y = _np(v.q_y, n, np.int16); o.q_z = _np(v.q_z, n, np.int16)
         if v.x_ref:
             o.x_ref = _np(v.x_ref, nt, np.float32); o.z_ref = _np(v.z_ref, nt, np.float32)
             o.chi2 = _np(v.chi2, nt, np.float32)

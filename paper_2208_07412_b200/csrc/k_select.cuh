@@ -191,4 +191,74 @@ k_sel_owner(uint32_t* __restrict__ key_owner, size_t n) {
   }
 }
 
+// ---- S7: track-residual front end --------------------------------------
+// Per cluster: res_trk = the SELECTED track owning it (-1: none), residuals to that track's helix, quantised.
+struct ResOut {
+  int32_t* res_trk;     // [N]
+  float* res_y;         // [N]
+  float* res_z;         // [N]
+  int16_t* q_y;         // [N]
+  int16_t* q_z;         // [N]
+};
+
+__global__ void __launch_bounds__(256)
+k_res_init(ResOut o, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    o.res_trk[i] = -1; o.res_y[i] = 0.0f; o.res_z[i] = 0.0f; o.q_y[i] = 0; o.q_z[i] = 0;
+  }
+}
+
+__device__ __forceinline__ int16_t res_quantise(float r, float inv_q) {
+  float v = rintf(__fmul_rn(r, inv_q));       // round half to even
+  v = v > 32767.0f ? 32767.0f : v;
+  v = v < -32767.0f ? -32767.0f : v;
+  return (int16_t)(int)v;
+}
+
+// One thread per selected track: the fitted state is transported hit to hit (mean only, the operations of
+// kf_prop_mean = DESIGN.md 3.5 Propagate) and every hit the track owns gets its residual.
+__global__ void __launch_bounds__(128)
+k_residuals(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
+            const float2* __restrict__ syz, const int32_t* __restrict__ row_start, const int32_t* __restrict__ owner,
+            SelOut sel, int32_t cap, ResOut o) {
+  const int ns = T->n_sectors, n_rows = T->n_rows;
+  const int n_sel = st->sel_off[ns];
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n_sel) return;
+  int s = 0;
+  {
+    int lo = 0, hi = ns - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (st->sel_off[mid] <= k) lo = mid; else hi = mid - 1; }
+    s = lo;
+  }
+  const int t_local = sel.sel_track[k];
+  const size_t cs = (size_t)cap;
+  KF f;
+  f.x = sel.o.x_ref[k];
+  const float z_ref = sel.o.z_ref[k];
+  f.p0 = sel.o.par[k]; f.p1 = sel.o.par[cs + k]; f.p2 = sel.o.par[2 * cs + k]; f.p3 = sel.o.par[3 * cs + k]; f.p4 = sel.o.par[4 * cs + k];
+  KFConst K;
+  K.Bc = T->Bc; K.err2_y = 0.f; K.err2_z = 0.f; K.max_sinphi = T->max_sinphi;
+  K.c24 = (float)(1.0 / 24.0); K.c640 = (float)(3.0 / 640.0); K.c12 = (float)(1.0 / 12.0);
+  K.ic0 = K.ic1 = K.ic2 = K.ic3 = K.ic4 = 0.f;
+  const float inv_q = T->res_inv_q;
+  const int nh = sel.o.n_hits[k];
+  const int32_t* hl = sel.o.hit_idx + (st->sel_hit_off[s] + sel.o.hit_offset[k + s]);
+  const int off = sec[s].off;
+  const int32_t* rs = row_start + (size_t)s * (n_rows + 1);
+  int r = sel.o.first_row[k];
+  for (int q = 0; q < nh; ++q) {
+    const int c = hl[q];
+    while (r + 1 < n_rows && c >= __ldg(&rs[r + 1])) ++r;     // hits ascend in row
+    const float2 h = __ldg(&syz[off + c]);
+    KFJac J;
+    if (!kf_prop_mean(f, __ldg(&T->row_x[r]), K, J)) break;
+    if (owner[off + c] != t_local) continue;
+    const float ry = h.x - f.p0;
+    const float rz = (h.y - z_ref) - f.p1;
+    o.res_trk[off + c] = t_local; o.res_y[off + c] = ry; o.res_z[off + c] = rz;
+    o.q_y[off + c] = res_quantise(ry, inv_q); o.q_z[off + c] = res_quantise(rz, inv_q);
+  }
+}
+
 }  // namespace tpcca

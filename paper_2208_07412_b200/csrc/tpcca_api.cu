@@ -29,7 +29,8 @@ struct Layout {
   size_t tile_cnt, tile_off, start_bits;
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
-  size_t sel_n_own, sel_track, slot_trk;   // S6 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
+  size_t sel_n_own, sel_track, slot_trk;   // S6
+  size_t res_trk, res_y, res_z, res_qy, res_qz;   // S7 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
 };
@@ -116,6 +117,8 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.sel_n_own = take(4 * (size_t)CS);
   L.sel_track = take(4 * (size_t)CS);
   L.slot_trk = take(4 * (size_t)CS);     // start-hit slot -> global track (S5 gather), -1 = rejected
+  L.res_trk = take(4 * (size_t)N); L.res_y = take(4 * (size_t)N); L.res_z = take(4 * (size_t)N);
+  L.res_qy = take(2 * (size_t)N); L.res_qz = take(2 * (size_t)N);
   L.total = cur;
   return L;
 }
@@ -138,6 +141,7 @@ int check_params(const tpcca_params* p, std::string& err) {
   if ((nb + 1) * (int64_t)p->n_sectors >= (int64_t)0xFFFFFFF0u) return fail("too many grid bins (n_sectors * (bins + 1) must fit 32 bits)");
   if (nb >= 0x7FFFFFF0) return fail("too many grid bins per sector");
   if (p->sel_max_shared_permille < 0 || p->sel_max_shared_permille > 1000) return fail("sel_max_shared_permille must be in 0..1000");
+  if (!(p->res_inv_quantum > 0.0f)) return fail("res_inv_quantum must be > 0");
   return TPCCA_OK;
 }
 
@@ -175,7 +179,7 @@ struct tpcca_ctx {
   uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
   bool desc_valid = false;
   static constexpr int kRing = 16;
-  cudaEvent_t ev[kRing][7]{};
+  cudaEvent_t ev[kRing][8]{};
   uint32_t ev_mask[kRing]{};          // stage mask of the run that used the slot (0 = unused)
   int64_t run_count = 0;
   char* arena = nullptr;              // pinned host arena of tpcca_get_tracks(HOST)
@@ -273,6 +277,14 @@ SelOut sel_out(const tpcca_ctx* c) {
   return so;
 }
 
+ResOut res_out(const tpcca_ctx* c) {
+  const Layout& L = c->L;
+  ResOut ro;
+  ro.res_trk = c->at<int32_t>(L.res_trk); ro.res_y = c->at<float>(L.res_y); ro.res_z = c->at<float>(L.res_z);
+  ro.q_y = c->at<int16_t>(L.res_qy); ro.q_z = c->at<int16_t>(L.res_qz);
+  return ro;
+}
+
 }  // namespace
 
 extern "C" {
@@ -334,7 +346,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   DevTables& t = c->tab;
   memset(&t, 0, sizeof t);
   t.n_rows = p->n_rows; t.n_sectors = p->n_sectors; t.bins_per_sector = (int32_t)c->nb;
-  t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits; t.sel_permille = p->sel_max_shared_permille;
+  t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits; t.sel_permille = p->sel_max_shared_permille; t.res_inv_q = p->res_inv_quantum;
   t.grid_z_lo = p->grid_z_lo; t.Bc = p->kappa_per_qpt; t.err2_y = p->err2_y; t.err2_z = p->err2_z;
   for (int i = 0; i < 5; ++i) t.init_cov[i] = p->init_cov[i];
   t.win_y = p->tc_win_y; t.win_z = p->tc_win_z; t.gate = p->tc_gate; t.max_sinphi = p->max_sinphi;
@@ -393,7 +405,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
-    for (int i = 0; i < 7 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
+    for (int i = 0; i < 8 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
     tpcca_destroy(c);
@@ -467,10 +479,10 @@ int tpcca_load_clusters(tpcca_ctx* c, int sector, int64_t n, const float* x, con
 
 int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   if (!c) return TPCCA_E_ARG;
-  mask &= (TPCCA_STAGE_ALL | TPCCA_STAGE_SELECT);
+  mask &= (TPCCA_STAGE_ALL | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS);
   if (!mask) return set_err(c, TPCCA_E_ARG, "empty stage mask");
   // a stage needs everything before it
-  for (int i = 0; i < 6; ++i)
+  for (int i = 0; i < 7; ++i)
     if (mask & (1u << i)) {
       const uint32_t need = (1u << i) - 1u;
       if ((need & ~(c->done_mask | mask)) != 0)
@@ -514,7 +526,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   const int slot_ev = (int)(c->run_count % tpcca_ctx::kRing);
   c->ev_mask[slot_ev] = 0;
   // end of a stage: its event, and the launch errors of ITS kernels (so a failed launch names its stage)
-  static const char* const kStageName[7] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets", "S6 selector"};
+  static const char* const kStageName[8] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets", "S6 selector", "S7 residuals"};
   cudaError_t stage_err = cudaSuccess;
   int stage_bad = -1;
   auto mark = [&](int i) {
@@ -672,12 +684,21 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     c->launches += 9;
   }
   mark(6);
+  if (mask & TPCCA_STAGE_RESIDUALS) {
+    const ResOut ro = res_out(c);
+    const size_t nk = (size_t)std::max<int64_t>(c->n_total, 1);
+    k_res_init<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(ro, nk);
+    k_residuals<<<(unsigned)((c->CS + 127) / 128), 128, 0, st>>>(T, sec, status, syz, row_start, c->at<int32_t>(L.rec), sel_out(c), cap, ro);
+    c->launches += 2;
+  }
+  mark(7);
   if (stage_err != cudaSuccess)
     return set_err(c, TPCCA_E_CUDA, "tpcca_run: stage %s failed: %s", kStageName[stage_bad], cudaGetErrorString(stage_err));
   c->ev_mask[slot_ev] = mask;
   ++c->run_count;
   // S6's outputs alias S1 / S5 scratch: re-running either without S6 leaves no valid selection
-  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS)) && !(mask & TPCCA_STAGE_SELECT)) c->done_mask &= ~TPCCA_STAGE_SELECT;
+  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS)) && !(mask & TPCCA_STAGE_SELECT)) c->done_mask &= ~(TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS);
+  if ((mask & TPCCA_STAGE_SELECT) && !(mask & TPCCA_STAGE_RESIDUALS)) c->done_mask &= ~TPCCA_STAGE_RESIDUALS;
   c->done_mask |= mask;
   return TPCCA_OK;
 }
@@ -703,10 +724,10 @@ int tpcca_get_counts(tpcca_ctx* c, int64_t out[7]) {
   return TPCCA_OK;
 }
 
-int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[7]) {
+int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[8]) {
   if (!c || !ms) return TPCCA_E_ARG;
   if (runs_back < 0 || runs_back >= tpcca_ctx::kRing) return set_err(c, TPCCA_E_ARG, "runs_back must be in 0..15");
-  for (int i = 0; i < 7; ++i) ms[i] = 0.f;
+  for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   if (runs_back >= c->run_count) return set_err(c, TPCCA_E_STATE, "no such run");
   const int k = (int)((c->run_count - 1 - runs_back) % tpcca_ctx::kRing);
   if (!c->ev_mask[k]) return set_err(c, TPCCA_E_STATE, "no such run");
@@ -715,6 +736,7 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[7]) {
   for (int i = 0; i < 5; ++i) CU(c, cudaEventElapsedTime(&ms[i], c->ev[k][i], c->ev[k][i + 1]));
   CU(c, cudaEventElapsedTime(&ms[5], c->ev[k][0], c->ev[k][5]));
   CU(c, cudaEventElapsedTime(&ms[6], c->ev[k][5], c->ev[k][6]));
+  CU(c, cudaEventElapsedTime(&ms[7], c->ev[k][6], c->ev[k][7]));
   return TPCCA_OK;
 }
 
@@ -755,6 +777,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   if (what & TPCCA_OUT_START) need_stage = 4;
   if (what & TPCCA_OUT_TRACKS) need_stage = 5;
   if ((what & (TPCCA_OUT_SELECTION | TPCCA_OUT_TRACKS_SEL)) && (c->done_mask & TPCCA_STAGE_SELECT)) need_stage = 6;
+  if ((what & TPCCA_OUT_RESIDUALS) && (c->done_mask & TPCCA_STAGE_RESIDUALS)) need_stage = 7;
   if ((what & TPCCA_OUT_TRACKS) && (what & TPCCA_OUT_TRACKS_SEL))
     return set_err(c, TPCCA_E_ARG, "TPCCA_OUT_TRACKS and TPCCA_OUT_TRACKS_SEL fill the same fields: ask for one");
   while (need_stage > 1 && need_stage <= 5 && !(c->done_mask & (1u << (need_stage - 1)))) --need_stage;     // stages that were never run deliver nothing
@@ -765,7 +788,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   const Layout& L = c->L;
   const DevStatus& S = c->status;
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
-  const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT)) : c->done_mask;
+  const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS)) : c->done_mask;
   v->n_clusters = n;
   v->n_bins = c->nb;
   int64_t s0 = 0, s1 = 0, t0 = 0, nt = 0, h0 = 0, h1 = 0;
@@ -838,6 +861,14 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
       v->trk_stride = host ? nk : c->CS;
     }
   }
+  if ((done & TPCCA_STAGE_RESIDUALS) && (what & TPCCA_OUT_RESIDUALS)) {
+    const ResOut ro = res_out(c);
+    add((const void* const*)&v->res_trk, ro.res_trk + off, 4 * (size_t)n);
+    add((const void* const*)&v->res_y, ro.res_y + off, 4 * (size_t)n);
+    add((const void* const*)&v->res_z, ro.res_z + off, 4 * (size_t)n);
+    add((const void* const*)&v->q_y, ro.q_y + off, 2 * (size_t)n);
+    add((const void* const*)&v->q_z, ro.q_z + off, 2 * (size_t)n);
+  }
   if (!host) {
     for (auto& it : items) *it.dst = it.src;
     return TPCCA_OK;
@@ -877,7 +908,7 @@ void tpcca_destroy(tpcca_ctx* c) {
   DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing; ++k)
-    for (int i = 0; i < 7; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
+    for (int i = 0; i < 8; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
   if (c->arena) cudaFreeHost(c->arena);
   if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
   delete c;

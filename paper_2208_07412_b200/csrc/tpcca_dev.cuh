@@ -31,6 +31,7 @@ struct DevTables {
   int32_t bins_per_sector;              // nb = sum_r ny_r * nz_r
   int32_t tc_max_gap, tc_min_hits;
   int32_t sel_permille;                 // S6: max shared hits of a selected tracklet, in 1/1000 of its hits
+  float res_inv_q;                      // S7: residual quantisation, 1 / quantum
   float grid_z_lo;
   float Bc, err2_y, err2_z;
   float init_cov[5];

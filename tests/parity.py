@@ -154,3 +154,24 @@ def compare_selection(tracker, tf, oracle_obj, sectors=None) -> dict:
             raise ParityError(f"sector {s}: {e}") from None
         tot["sectors"] += 1; tot["n_tracks"] += int(o.n_tracks); tot["n_selected"] += int(len(o.selected))
     return tot
+
+
+def compare_residuals(tracker, tf, oracle_obj, sectors=None) -> dict:
+    """S7 (track-residual front end): res_trk and the quantised residuals bit-exact (integers), the fp32
+    residuals bit-exact as well (same operation order; the bar would allow 1e-4 relative)."""
+    from paper_2208_07412_b200 import binding as B
+    tot = dict(sectors=0, n_clusters=0, n_attached=0)
+    for s in (range(tf.n_sectors) if sectors is None else sectors):
+        o = oracle_obj.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x7F)
+        g = tracker.get_tracks(s, B.OUT_RESIDUALS)
+        rep = {}
+        try:
+            _eq("res_trk", g.res_trk, o.res_trk, rep)
+            _eq("q_y", g.q_y, o.q_y, rep)
+            _eq("q_z", g.q_z, o.q_z, rep)
+            _eq("res_y", g.res_y, o.res_y.astype(np.float32), rep)
+            _eq("res_z", g.res_z, o.res_z.astype(np.float32), rep)
+        except ParityError as e:
+            raise ParityError(f"sector {s}: {e}") from None
+        tot["sectors"] += 1; tot["n_clusters"] += int(o.n); tot["n_attached"] += int((o.res_trk >= 0).sum())
+    return tot

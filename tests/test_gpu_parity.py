@@ -490,3 +490,44 @@ def test_selector_dense_stress_and_empty(pkg):
     trk = run_gpu_select(pkg, tf)
     compare_selection(trk, tf, Oracle(tf.params))
     trk.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# S7 track-residual front end
+# ------------------------------------------------------------------------------------------------
+def test_residuals_config0_config1_config4(pkg, cfg0, cfg1_small):
+    from parity import compare_residuals, compare_selection
+    for tf in (cfg0, cfg1_small, tpcsynth.generate(4, n_tracks=1500)):
+        trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+        trk.load_timeframe(tf)
+        trk.run(0x7F)
+        trk.sync()
+        orc = Oracle(tf.params)
+        rep = compare_residuals(trk, tf, orc)
+        assert rep["n_attached"] > 0.7 * rep["n_clusters"]
+        compare_selection(trk, tf, orc)
+        assert trk.timings()[7] > 0.0
+        trk.close()
+
+
+def test_residuals_separate_run_quantum_and_empty(pkg, cfg1_small):
+    from parity import compare_residuals
+    tf = cfg1_small
+    P = tf.params.copy(res_inv_quantum=32.0, sel_max_shared_permille=300)
+    tf2 = ArrTF(P, [(tf.y[s], tf.z[s], tf.row[s]) for s in (4, 22)])
+    trk = run_gpu(pkg, tf2)
+    trk.run(0x20)
+    trk.run(0x40)
+    trk.sync()
+    compare_residuals(trk, tf2, Oracle(P))
+    trk.close()
+    P3 = tpcsynth.default_params(n_sectors=2)
+    e = (np.empty(0, np.float32), np.empty(0, np.float32), np.empty(0, np.uint16))
+    one = (np.array([0.5], np.float32), np.array([10.0], np.float32), np.array([7], np.uint16))
+    tf3 = ArrTF(P3, [e, one])
+    trk = pkg.Tracker(P3, max_clusters=4)
+    trk.load_timeframe(tf3)
+    trk.run(0x7F)
+    trk.sync()
+    compare_residuals(trk, tf3, Oracle(P3))
+    trk.close()

@@ -873,3 +873,72 @@ def test_selector_removes_clones_and_keeps_efficiency(cfg1_tracks):
     assert a["clone_rate"] < 0.05, a
     assert a["efficiency"] >= b["efficiency"] - 0.005 and a["efficiency"] >= 0.97, (a, b)
     assert a["fake_rate"] <= b["fake_rate"] + 0.01, (a, b)
+
+
+# ----------------------------------------------------------------------------------------
+# S7 track-residual front end
+# ----------------------------------------------------------------------------------------
+def test_residuals_vanish_on_exact_helices():
+    """Noise-free helices (P6 fixture, double): every cluster is owned by its track and its residual to the
+    fitted helix is zero to 2e-5 cm (the fit itself recovers the helix to 1e-5 relative, P6); the quantised
+    residuals are all 0."""
+    P = tpcsynth.default_params(n_sectors=1)
+    y, z, row, lab = _helix_sector(P, HELIX_TRACKS, np.float64)
+    res = Oracle(P, "f64").run(y, z, row, stage_mask=0x7F)
+    assert res.n_tracks == len(HELIX_TRACKS) and len(res.selected) == len(HELIX_TRACKS)
+    assert np.all(res.res_trk >= 0)
+    assert np.abs(res.res_y).max() < 2e-5 and np.abs(res.res_z).max() < 2e-5
+    assert not res.q_y.any() and not res.q_z.any()
+
+
+def test_residuals_equal_closed_form_circle(cfg0):
+    """Residual of every attached cluster vs the closed-form helix through the fitted state (x_ref, par):
+    sin phi(x) = sin phi0 + kappa (x - x0); y(x) = y0 + (cos phi0 - cos phi(x)) / kappa;
+    z(x) = z0 + dz/ds * (phi(x) - phi0) / kappa -- circle geometry with asin, independent of the oracle's
+    hit-to-hit chord transport.  Pins which state is transported, the walk, the signs and K-rule Z."""
+    tf = cfg0
+    P = tf.params
+    res = Oracle(P, "f64").run(tf.y[0], tf.z[0], tf.row[0], stage_mask=0x7F)
+    Bc = float(P.kappa_per_qpt)
+    rx = P.row_x.astype(np.float64)
+    srow = tf.row[0][res.order].astype(np.int64)
+    m = np.nonzero(res.res_trk >= 0)[0]
+    assert m.size > 3000
+    t = res.res_trk[m]
+    assert np.all(np.isin(t, res.selected)) and np.array_equal(res.owner[m], t)
+    x0 = res.x_ref[t]; p = res.par[t]
+    kappa = p[:, 4] * Bc
+    sp = p[:, 2] + kappa * (rx[srow[m]] - x0)
+    ok = np.abs(kappa) > 1e-9
+    yh = np.where(ok, p[:, 0] + (np.sqrt(1 - p[:, 2] ** 2) - np.sqrt(1 - sp ** 2)) / np.where(ok, kappa, 1.0), np.nan)
+    zh = np.where(ok, p[:, 1] + p[:, 3] * (np.arcsin(sp) - np.arcsin(p[:, 2])) / np.where(ok, kappa, 1.0), np.nan)
+    assert ok.mean() > 0.99
+    assert np.nanmax(np.abs(res.res_y[m] - (res.sy[m] - yh))) < 1e-7
+    assert np.nanmax(np.abs(res.res_z[m] - ((res.sz[m] - res.z_ref[t]) - zh))) < 1e-6
+    # every cluster a selected track owns is attached (no transport failed on this input)
+    owned = np.isin(res.owner, res.selected) & (res.owner >= 0)
+    assert np.array_equal(owned, res.res_trk >= 0)
+
+
+def test_residual_statistics_and_quantiser(cfg1_tracks):
+    """fp32, config-1 kinematics: residuals of attached clusters are centred with the cluster resolution
+    (sigma = 0.1 cm, slightly less: the fit absorbs part of it); q = rint(res * 128) with numpy's round-half-even."""
+    tf, secs, _ = cfg1_tracks
+    orc = Oracle(tf.params)
+    ry, rz = [], []
+    for s in secs[:3]:
+        r = orc.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x7F)
+        m = r.res_trk >= 0
+        assert m.mean() > 0.85                                   # most clusters are attached to a selected track
+        f32 = np.float32
+        assert np.array_equal(r.q_y[m], np.clip(np.rint(r.res_y[m].astype(f32) * f32(128.0)), -32767, 32767).astype(np.int16))
+        assert np.array_equal(r.q_z[m], np.clip(np.rint(r.res_z[m].astype(f32) * f32(128.0)), -32767, 32767).astype(np.int16))
+        assert not r.q_y[~m].any() and not r.res_y[~m].any()
+        lab = tf.label[s][r.order]
+        good = m & (lab >= 0)
+        ry.append(r.res_y[good]); rz.append(r.res_z[good])
+    ry = np.concatenate(ry); rz = np.concatenate(rz)
+    core_y = ry[np.abs(ry) < 0.5]; core_z = rz[np.abs(rz) < 0.5]
+    assert core_y.size > 0.98 * ry.size
+    assert abs(core_y.mean()) < 0.003 and abs(core_z.mean()) < 0.003
+    assert 0.085 < core_y.std() < 0.105 and 0.085 < core_z.std() < 0.105

@@ -76,6 +76,7 @@ class TrackerParams:
     tc_max_gap: int
     tc_min_hits: int
     sel_max_shared_permille: int = 500   # S6 selector: a tracklet survives iff at most this share of its hits is not its own
+    res_inv_quantum: float = 128.0       # S7 residual front end: residuals are quantised to round(res * this) (1/128 cm)
     # informative (not consumed by the tracker)
     sigma: float = 0.1
     z_hi: float = 250.0
