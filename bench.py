@@ -272,6 +272,9 @@ class CudaEnv:
     def tracker(self, params, max_clusters, max_start_hits, stream=None):
         return self.pkg.Tracker(params, max_clusters=max_clusters, max_start_hits=max_start_hits, device=self.local, stream=stream)
 
+    def pipeline(self, params, n_groups, max_clusters_group, max_start_hits_group):
+        return self.pkg.Pipeline(params, n_groups, max_clusters_group, max_start_hits_group, device=self.local)
+
     def pin(self, a):
         return self.torch.from_numpy(a).pin_memory()
 
@@ -480,6 +483,34 @@ def run_tpcca(args, env_cls=CudaEnv):
                 t.close()
         else:
             e2e_mode = "serial, 1 context (no device memory for a second time frame)"
+    # (c) one time frame through the sector-group pipeline of the library (tpcca_pipeline_run: SURVEY 8(f)-3): latency of
+    # ONE time frame, host buffers in, host views out, the groups' copies overlapping each other's kernels
+    pipe_res = None
+    if args.pipeline_groups > 1 and world == 1:
+        G = min(args.pipeline_groups, tf.n_sectors)
+        first = [g * tf.n_sectors // G for g in range(G + 1)]
+        sc = tf.sector_counts()
+        cap_g = int(max(sc[first[g]:first[g + 1]].sum() for g in range(G)) * 1.05) + 1024
+        try:
+            pipe = env.pipeline(tf.params, G, cap_g, cap_g // 8 + 1024)
+        except env.oom_error:
+            pipe = None
+        if pipe is not None:
+            hy = [h[0] for h in host]; hz = [h[1] for h in host]; hr = [h[2] for h in host]
+            what = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START | B.OUT_TRACKS
+            pipe.run_views(hy, hz, hr, 0x1F, what)          # warm-up: grows the pinned arenas
+            env.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                views = pipe.run_views(hy, hz, hr, 0x1F, what)
+            env.synchronize()
+            dt = (time.perf_counter() - t0) / e2e_steps
+            d2h_p = int(sum(12 * v.n_clusters + 4 * v.n_start + 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4 for v in views))
+            pipe_res = dict(value=N / dt, unit=UNIT, ms_per_step=1e3 * dt, n_groups=G, h2d_bytes_per_step=h2d,
+                            d2h_bytes_per_step=d2h_p, group_ms=[round(v, 1) for v in pipe.groups()[1]],
+                            mode=f"one time frame at a time, {G} sector groups on {G} streams / host threads (host wall clock)")
+            pipe.close()
+            env.empty_cache()
     e2e_value = n_all * e2e_n / (e2e_ms * 1e-3)
     e2e_steps_serial = e2e_steps
     e2e_steps = e2e_n
@@ -512,7 +543,7 @@ def run_tpcca(args, env_cls=CudaEnv):
             e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h, steps=e2e_steps,
                      ms_per_step=e2e_ms / e2e_steps, mode=e2e_mode,
                      serial_value=n_all * e2e_steps_serial / (e2e_serial_ms * 1e-3),
-                     serial_ms_per_step=e2e_serial_ms / e2e_steps_serial),
+                     serial_ms_per_step=e2e_serial_ms / e2e_steps_serial, pipelined=pipe_res),
             selector=dict(stage_ms_S6=round(s6_ms, 4), stage_ms_S7_residuals=round(s7_ms, 4), n_selected=counts_sel["n_selected"], n_sel_hits=counts_sel["n_sel_hits"],
                           note="S6 (SURVEY 8(f)-1) is outside the timed step; e2e_selected = serial step S1-S6 shipping the "
                                "selected tracks + owner instead of every tracklet",
@@ -559,6 +590,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sectors", type=int, default=8, help="sectors of the CPU-baseline / full-size parity sample")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
+    ap.add_argument("--pipeline-groups", type=int, default=4, help="sector groups of the tpcca_pipeline e2e leg (0/1: off)")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "tpcca":

@@ -212,6 +212,11 @@ int tpcca_sync(tpcca_ctx *ctx);
  * always filled.  Errors: TPCCA_E_ARG, TPCCA_E_STATE (nothing was run), plus those of tpcca_sync. */
 int tpcca_get_tracks(tpcca_ctx *ctx, int sector, int mem_space, uint32_t what, tpcca_tracks_view *out);
 
+/* The outputs of ALL sectors in one call: views[s] for s = 0 .. n_sectors - 1, otherwise as tpcca_get_tracks.  HOST:
+ * every array of every sector lands in ONE pinned arena behind one synchronise of the copy stream (valid until the
+ * next tpcca_get_* (HOST) call on this context). */
+int tpcca_get_tracks_all(tpcca_ctx *ctx, int mem_space, uint32_t what, tpcca_tracks_view *views);
+
 /* Totals over all sectors after a run: out[0..6] = n_clusters, n_start, n_tracks, n_hits,
  * n_bins (per sector), n_selected, n_sel_hits (S6; 0 if not run).  Synchronises the stream.
  * Errors as tpcca_sync. */
@@ -245,6 +250,44 @@ const char *tpcca_last_error(const tpcca_ctx *ctx);
 
 /* Release the context (not the workspace, not borrowed inputs).  NULL is allowed. */
 void tpcca_destroy(tpcca_ctx *ctx);
+
+/* ---- time-frame streaming: sector-group pipeline --------------------------------
+ * A pipeline owns n_groups contexts; group g handles the sectors [g * n_sectors / n_groups, (g + 1) * n_sectors /
+ * n_groups) of every time frame on its own stream and its own host thread: H2D load, tpcca_run, D2H delivery.
+ * Sectors are independent units (no halo, no exchange), so the copies of one group overlap the kernels of the
+ * others, the first tracks are on the host after 1 / n_groups of the work, and one workspace holds 1 / n_groups of
+ * the time frame. */
+typedef struct tpcca_pipeline tpcca_pipeline;
+
+/* Bytes of DEVICE workspace EACH group needs for at most max_clusters_group clusters / max_start_hits_group start
+ * hits in one group (tpcca_workspace_bytes for the largest group).  HOST call.  Errors: TPCCA_E_ARG. */
+int tpcca_pipeline_workspace_bytes(const tpcca_params *params, int n_groups, int64_t max_clusters_group,
+                                   int64_t max_start_hits_group, size_t *out_bytes);
+
+/* cuda_streams[g] (distinct cudaStream_t of cuda_device) and workspaces[g] (DEVICE, 256-byte aligned,
+ * workspace_bytes_each bytes) are owned by the caller until tpcca_pipeline_destroy.  Errors as tpcca_create. */
+int tpcca_pipeline_create(const tpcca_params *params, int cuda_device, int n_groups, void *const *cuda_streams,
+                          void *const *workspaces, size_t workspace_bytes_each, int64_t max_clusters_group,
+                          int64_t max_start_hits_group, tpcca_pipeline **out);
+
+/* One time frame through the pipeline.  n[s], y[s], z[s], row[s]: the clusters of sector s (arrays of n_sectors
+ * entries; HOST -- pinned memory lets the copies overlap -- or DEVICE per mem_space; they must stay valid until the
+ * call returns).  stage_mask / what as for tpcca_run / tpcca_get_tracks.  views[s] (HOST array of n_sectors views)
+ * receives HOST pointers into the pinned arenas of the groups, valid until the next run of this pipeline.  Blocks
+ * until every group has delivered.  Errors: those of tpcca_load_clusters / tpcca_run / tpcca_get_tracks of any group
+ * (message names the group). */
+int tpcca_pipeline_run(tpcca_pipeline *p, const int64_t *n, const float *const *y, const float *const *z,
+                       const uint16_t *const *row, int mem_space, uint32_t stage_mask, uint32_t what,
+                       tpcca_tracks_view *views);
+
+/* Sector ranges of the groups (first_sector[n_groups + 1], may be NULL) and the host wall time [ms] each group's
+ * thread spent in the last run (ms[n_groups], may be NULL).  Returns n_groups (or TPCCA_E_ARG). */
+int tpcca_pipeline_get_groups(const tpcca_pipeline *p, int32_t *first_sector, float *ms);
+
+/* Message of the last failing call (p == NULL: of the last failing create / workspace_bytes of this thread). */
+const char *tpcca_pipeline_last_error(const tpcca_pipeline *p);
+
+void tpcca_pipeline_destroy(tpcca_pipeline *p);
 
 /* Library version string, e.g. "tpcca 0.1 (sm_100a)". */
 const char *tpcca_version(void);

@@ -25,7 +25,9 @@ _up = C.POINTER(C.c_uint32)
 #: every symbol include/tpcca.h declares
 ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "tpcca_reset", "tpcca_run",
                "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
-               "tpcca_get_launch_count", "tpcca_get_info", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
+               "tpcca_get_launch_count", "tpcca_get_info", "tpcca_get_tracks_all", "tpcca_pipeline_workspace_bytes",
+               "tpcca_pipeline_create", "tpcca_pipeline_run", "tpcca_pipeline_get_groups", "tpcca_pipeline_last_error",
+               "tpcca_pipeline_destroy", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
 OUT_SELECTION, OUT_TRACKS_SEL, OUT_RESIDUALS = 64, 128, 256
 
@@ -95,6 +97,17 @@ def load_library():
     lib.tpcca_get_work_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_get_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
     lib.tpcca_get_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+    lib.tpcca_get_tracks_all.argtypes = [C.c_void_p, C.c_int, C.c_uint32, C.POINTER(_View)]
+    lib.tpcca_pipeline_workspace_bytes.argtypes = [C.POINTER(_Params), C.c_int, C.c_int64, C.c_int64, C.POINTER(C.c_size_t)]
+    lib.tpcca_pipeline_create.argtypes = [C.POINTER(_Params), C.c_int, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                          C.c_size_t, C.c_int64, C.c_int64, C.POINTER(C.c_void_p)]
+    lib.tpcca_pipeline_run.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                       C.POINTER(C.c_void_p), C.c_int, C.c_uint32, C.c_uint32, C.POINTER(_View)]
+    lib.tpcca_pipeline_get_groups.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_float)]
+    lib.tpcca_pipeline_last_error.argtypes = [C.c_void_p]
+    lib.tpcca_pipeline_last_error.restype = C.c_char_p
+    lib.tpcca_pipeline_destroy.argtypes = [C.c_void_p]
+    lib.tpcca_pipeline_destroy.restype = None
     lib.tpcca_last_error.argtypes = [C.c_void_p]
     lib.tpcca_last_error.restype = C.c_char_p
     lib.tpcca_destroy.argtypes = [C.c_void_p]
@@ -196,6 +209,44 @@ def _np(ptr, n, dtype):
     if not ptr or n == 0:
         return np.empty(0, dtype) if ptr else None
     return np.ctypeslib.as_array(ptr, shape=(n,)).astype(dtype, copy=True)
+
+
+def output_from_view(v, what: int, n_rows: int) -> SectorOutput:
+    """HOST tpcca_tracks_view -> numpy copies (argument marshalling only)."""
+    n, nt = int(v.n_clusters), int(v.n_tracks)
+    o = SectorOutput(n=n, n_bins=int(v.n_bins))
+    o.order = _np(v.order, n, np.int32)
+    if v.syz:
+        syz = _np(v.syz, 2 * n, np.float32).reshape(n, 2)
+        o.sy, o.sz = np.ascontiguousarray(syz[:, 0]), np.ascontiguousarray(syz[:, 1])
+    o.bin_start = _np(v.bin_start, int(v.n_bins) + 1, np.uint32) if v.bin_start else None
+    o.row_start = _np(v.row_start, n_rows + 1, np.int32) if v.row_start else None
+    o.link_up_raw = _np(v.link_up_raw, n, np.int32); o.link_dn_raw = _np(v.link_dn_raw, n, np.int32)
+    o.link_up = _np(v.link_up, n, np.int32); o.link_dn = _np(v.link_dn, n, np.int32)
+    o.start_hit = _np(v.start_hit, int(v.n_start), np.int32)
+    if what & OUT_TRACKS_SEL:          # the S5 fields hold the selected tracks only
+        nt = int(v.n_selected)
+    n_hits_total = int(v.n_sel_hits) if what & OUT_TRACKS_SEL else int(v.n_hits)
+    if v.owner:
+        o.owner = _np(v.owner, n, np.int32); o.n_own = _np(v.n_own, int(v.n_tracks), np.int32)
+        o.selected = _np(v.sel_track, int(v.n_selected), np.int32)
+    if v.res_trk:
+        o.res_trk = _np(v.res_trk, n, np.int32); o.res_y = _np(v.res_y, n, np.float32); o.res_z = _np(v.res_z, n, np.float32)
+        o.q_y = _np(v.q_y, n, np.int16); o.q_z = _np(v.q_z, n, np.int16)
+    if v.x_ref:
+        o.x_ref = _np(v.x_ref, nt, np.float32); o.z_ref = _np(v.z_ref, nt, np.float32)
+        o.chi2 = _np(v.chi2, nt, np.float32)
+        stride = int(v.trk_stride)
+        o.par = (_np(v.par, 5 * stride, np.float32).reshape(5, stride)[:, :nt].T.copy() if nt
+                 else np.empty((0, 5), np.float32))
+        o.cov = (_np(v.cov, 15 * stride, np.float32).reshape(15, stride)[:, :nt].T.copy() if nt
+                 else np.empty((0, 15), np.float32))
+        o.n_hits = _np(v.n_hits_trk, nt, np.int32); o.n_fit = _np(v.n_fit, nt, np.int32)
+        o.first_row = _np(v.first_row, nt, np.int32); o.last_row = _np(v.last_row, nt, np.int32)
+        o.trk_start_hit = _np(v.trk_start_hit, nt, np.int32)
+        o.hit_offset = _np(v.hit_offset, nt + 1, np.int32)
+        o.hit_idx = _np(v.hit_idx, n_hits_total, np.int32)
+    return o
 
 
 class Tracker:
@@ -339,38 +390,84 @@ class Tracker:
 
     def get_tracks(self, sector: int, what: int = OUT_ALL) -> SectorOutput:
         """tpcca_get_tracks(HOST) -> numpy copies."""
-        v = self.get_tracks_view(sector, MEM_HOST, what)
-        n, nt = int(v.n_clusters), int(v.n_tracks)
-        o = SectorOutput(n=n, n_bins=int(v.n_bins))
-        o.order = _np(v.order, n, np.int32)
-        if v.syz:
-            syz = _np(v.syz, 2 * n, np.float32).reshape(n, 2)
-            o.sy, o.sz = np.ascontiguousarray(syz[:, 0]), np.ascontiguousarray(syz[:, 1])
-        o.bin_start = _np(v.bin_start, int(v.n_bins) + 1, np.uint32) if v.bin_start else None
-        o.row_start = _np(v.row_start, self.n_rows + 1, np.int32) if v.row_start else None
-        o.link_up_raw = _np(v.link_up_raw, n, np.int32); o.link_dn_raw = _np(v.link_dn_raw, n, np.int32)
-        o.link_up = _np(v.link_up, n, np.int32); o.link_dn = _np(v.link_dn, n, np.int32)
-        o.start_hit = _np(v.start_hit, int(v.n_start), np.int32)
-        if what & OUT_TRACKS_SEL:          # the S5 fields hold the selected tracks only
-            nt = int(v.n_selected)
-        n_hits_total = int(v.n_sel_hits) if what & OUT_TRACKS_SEL else int(v.n_hits)
-        if v.owner:
-            o.owner = _np(v.owner, n, np.int32); o.n_own = _np(v.n_own, int(v.n_tracks), np.int32)
-            o.selected = _np(v.sel_track, int(v.n_selected), np.int32)
-        if v.res_trk:
-            o.res_trk = _np(v.res_trk, n, np.int32); o.res_y = _np(v.res_y, n, np.float32); o.res_z = _np(v.res_z, n, np.float32)
-            o.q_y = _np(v.q_y, n, np.int16); o.q_z = _np(v.q_z, n, np.int16)
-        if v.x_ref:
-            o.x_ref = _np(v.x_ref, nt, np.float32); o.z_ref = _np(v.z_ref, nt, np.float32)
-            o.chi2 = _np(v.chi2, nt, np.float32)
-            stride = int(v.trk_stride)
-            o.par = (_np(v.par, 5 * stride, np.float32).reshape(5, stride)[:, :nt].T.copy() if nt
-                     else np.empty((0, 5), np.float32))
-            o.cov = (_np(v.cov, 15 * stride, np.float32).reshape(15, stride)[:, :nt].T.copy() if nt
-                     else np.empty((0, 15), np.float32))
-            o.n_hits = _np(v.n_hits_trk, nt, np.int32); o.n_fit = _np(v.n_fit, nt, np.int32)
-            o.first_row = _np(v.first_row, nt, np.int32); o.last_row = _np(v.last_row, nt, np.int32)
-            o.trk_start_hit = _np(v.trk_start_hit, nt, np.int32)
-            o.hit_offset = _np(v.hit_offset, nt + 1, np.int32)
-            o.hit_idx = _np(v.hit_idx, n_hits_total, np.int32)
-        return o
+        return output_from_view(self.get_tracks_view(sector, MEM_HOST, what), what, self.n_rows)
+
+    def get_tracks_all(self, what: int = OUT_ALL):
+        """tpcca_get_tracks_all(HOST): every sector behind one synchronise -> list of SectorOutput."""
+        views = (_View * self.n_sectors)()
+        self._check(self._lib.tpcca_get_tracks_all(self._h, MEM_HOST, int(what), views))
+        return [output_from_view(views[s], what, self.n_rows) for s in range(self.n_sectors)]
+
+
+class Pipeline:
+    """tpcca_pipeline: a time frame streamed through n_groups sector groups (one context, stream, host thread and
+    workspace each).  PyTorch lends the streams and the workspaces."""
+
+    def __init__(self, params, n_groups: int, max_clusters_group: int, max_start_hits_group: int = 0, device: int = 0):
+        import torch
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise TpccaError(-3, "no CUDA device: tpcca has no CPU path")
+        self.n_sectors, self.n_rows, self.n_groups = int(params.n_sectors), int(params.n_rows), int(n_groups)
+        p, self._keep = _make_params(params)
+        nbytes = C.c_size_t(0)
+        rc = self._lib.tpcca_pipeline_workspace_bytes(C.byref(p), self.n_groups, int(max_clusters_group), int(max_start_hits_group),
+                                                      C.byref(nbytes))
+        if rc:
+            raise TpccaError(rc, self._lib.tpcca_pipeline_last_error(None).decode())
+        self.workspace_bytes_each = int(nbytes.value)
+        with torch.cuda.device(device):
+            self._streams = [torch.cuda.Stream(device=device) for _ in range(self.n_groups)]
+            self._ws = [torch.empty(self.workspace_bytes_each + 256, dtype=torch.uint8, device=f"cuda:{device}")
+                        for _ in range(self.n_groups)]
+        st = (C.c_void_p * self.n_groups)(*[s.cuda_stream for s in self._streams])
+        ws = (C.c_void_p * self.n_groups)(*[(w.data_ptr() + 255) // 256 * 256 for w in self._ws])
+        h = C.c_void_p()
+        rc = self._lib.tpcca_pipeline_create(C.byref(p), int(device), self.n_groups, st, ws, self.workspace_bytes_each,
+                                             int(max_clusters_group), int(max_start_hits_group), C.byref(h))
+        if rc:
+            raise TpccaError(rc, self._lib.tpcca_pipeline_last_error(None).decode())
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.tpcca_pipeline_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def run_views(self, y, z, row, stage_mask: int = STAGE_ALL, what: int = OUT_ALL):
+        """tpcca_pipeline_run on per-sector arrays (numpy / pinned torch CPU tensors: HOST; torch CUDA tensors: DEVICE).
+        Returns the raw views (HOST pointers, valid until the next run)."""
+        ns = self.n_sectors
+        assert len(y) == ns and len(z) == ns and len(row) == ns
+        is_t = hasattr(y[0], "data_ptr")
+        dev = is_t and y[0].is_cuda
+        ptr = (lambda a: a.data_ptr() if a.numel() else None) if is_t else (lambda a: a.ctypes.data if a.size else None)
+        if not is_t:
+            y = [_f32(a) for a in y]; z = [_f32(a) for a in z]
+            row = [np.ascontiguousarray(a, dtype=np.uint16) for a in row]
+        self._inputs = (y, z, row)
+        n = (C.c_int64 * ns)(*[int(a.shape[0]) for a in y])
+        py = (C.c_void_p * ns)(*[ptr(a) for a in y]); pz = (C.c_void_p * ns)(*[ptr(a) for a in z])
+        pr = (C.c_void_p * ns)(*[ptr(a) for a in row])
+        views = (_View * ns)()
+        rc = self._lib.tpcca_pipeline_run(self._h, n, py, pz, pr, MEM_DEVICE if dev else MEM_HOST, int(stage_mask), int(what), views)
+        if rc:
+            raise TpccaError(rc, self._lib.tpcca_pipeline_last_error(self._h).decode())
+        return views
+
+    def run(self, y, z, row, stage_mask: int = STAGE_ALL, what: int = OUT_ALL):
+        views = self.run_views(y, z, row, stage_mask, what)
+        return [output_from_view(views[s], what, self.n_rows) for s in range(self.n_sectors)]
+
+    def groups(self):
+        first = (C.c_int32 * (self.n_groups + 1))()
+        ms = (C.c_float * self.n_groups)()
+        self._lib.tpcca_pipeline_get_groups(self._h, first, ms)
+        return list(first), [float(v) for v in ms]

@@ -1,6 +1,7 @@
 // Host side of the tpcca C-ABI (include/tpcca.h): workspace carving, stage scheduling on the
 // caller's stream, per-stage CUDA events, error mapping.  No torch types, no CPU compute path:
 // every stage of the hot path runs in the kernels of k_grid.cuh / k_links.cuh / k_tracklets.cuh.
+#include <chrono>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -762,9 +763,11 @@ int tpcca_get_launch_count(const tpcca_ctx* c, int64_t* out) {
   return TPCCA_OK;
 }
 
-int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpcca_tracks_view* v) {
-  if (!c || !v) return TPCCA_E_ARG;
-  if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
+// Outputs of sectors [sec0, sec1) into views[0 .. sec1 - sec0): DEVICE pointers, or HOST copies into ONE pinned arena
+// followed by one synchronise of the copy stream.
+static int get_tracks_range(tpcca_ctx* c, int sec0, int sec1, int mem_space, uint32_t what, tpcca_tracks_view* views) {
+  if (!c || !views) return TPCCA_E_ARG;
+  if (sec0 < 0 || sec1 > c->ns || sec0 >= sec1) return set_err(c, TPCCA_E_ARG, "sector range %d..%d out of range", sec0, sec1);
   if (mem_space != TPCCA_MEM_HOST && mem_space != TPCCA_MEM_DEVICE) return set_err(c, TPCCA_E_ARG, "bad mem_space");
   if (!c->done_mask || !c->desc_valid) return set_err(c, TPCCA_E_STATE, "nothing was run");
   GUARD(c);
@@ -784,9 +787,17 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   const bool partial = host && need_stage < 5 && (c->done_mask & TPCCA_STAGE_TRACKLETS) && c->run_count > 0;
   int rc = partial ? fetch_status_after(c, std::max(need_stage, (c->done_mask & TPCCA_STAGE_START) ? 4 : need_stage)) : fetch_status(c);
   if (rc) return rc;
-  memset(v, 0, sizeof *v);
   const Layout& L = c->L;
   const DevStatus& S = c->status;
+  // the arrays to deliver: (destination field, device source, bytes); par / cov are strided planes
+  struct Item { const void** dst; const void* src; size_t bytes; int planes; };
+  std::vector<Item> items;
+  auto add = [&](const void* const* dst, const void* src, size_t bytes, int planes = 1) {
+    items.push_back(Item{(const void**)dst, src, bytes, planes});
+  };
+  for (int sector = sec0; sector < sec1; ++sector) {
+  tpcca_tracks_view* v = views + (sector - sec0);
+  memset(v, 0, sizeof *v);
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
   const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS)) : c->done_mask;
   v->n_clusters = n;
@@ -797,12 +808,6 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
     t0 = S.trk_off[sector]; nt = S.trk_off[sector + 1] - t0; h0 = S.hit_off[sector]; h1 = S.hit_off[sector + 1];
     v->n_tracks = nt; v->n_hits = h1 - h0;
   }
-  // the arrays to deliver: (destination field, device source, bytes); par / cov are strided planes
-  struct Item { const void** dst; const void* src; size_t bytes; int planes; };
-  std::vector<Item> items;
-  auto add = [&](const void* const* dst, const void* src, size_t bytes, int planes = 1) {
-    items.push_back(Item{(const void**)dst, src, bytes, planes});
-  };
   if ((what & TPCCA_OUT_ORDER) && (done & TPCCA_STAGE_GRID))
     add((const void* const*)&v->order, c->at<int32_t>(L.order) + off, 4 * (size_t)n);
   if ((what & TPCCA_OUT_GRID) && (done & TPCCA_STAGE_GRID)) {
@@ -869,6 +874,7 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
     add((const void* const*)&v->q_y, ro.q_y + off, 2 * (size_t)n);
     add((const void* const*)&v->q_z, ro.q_z + off, 2 * (size_t)n);
   }
+  }   // sectors
   if (!host) {
     for (auto& it : items) *it.dst = it.src;
     return TPCCA_OK;
@@ -903,6 +909,17 @@ int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpc
   return TPCCA_OK;
 }
 
+int tpcca_get_tracks(tpcca_ctx* c, int sector, int mem_space, uint32_t what, tpcca_tracks_view* v) {
+  if (!c || !v) return TPCCA_E_ARG;
+  if (sector < 0 || sector >= c->ns) return set_err(c, TPCCA_E_ARG, "sector %d out of range", sector);
+  return get_tracks_range(c, sector, sector + 1, mem_space, what, v);
+}
+
+int tpcca_get_tracks_all(tpcca_ctx* c, int mem_space, uint32_t what, tpcca_tracks_view* views) {
+  if (!c || !views) return TPCCA_E_ARG;
+  return get_tracks_range(c, 0, c->ns, mem_space, what, views);
+}
+
 void tpcca_destroy(tpcca_ctx* c) {
   if (!c) return;
   DeviceGuard guard(c->device);
@@ -915,3 +932,5 @@ void tpcca_destroy(tpcca_ctx* c) {
 }
 
 }  // extern "C"
+
+#include "tpcca_pipeline.cuh"

@@ -531,3 +531,67 @@ def test_residuals_separate_run_quantum_and_empty(pkg, cfg1_small):
     trk.sync()
     compare_residuals(trk, tf3, Oracle(P3))
     trk.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# time-frame streaming: sector-group pipeline
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_groups", [1, 4, 5])
+def test_pipeline_equals_oracle(pkg, cfg1_small, n_groups):
+    """Every sector delivered by the pipeline (S1-S7 per sector group on its own stream / thread) equals the
+    oracle element by element; 5 groups: uneven group sizes (36 sectors)."""
+    from paper_2208_07412_b200 import binding as B
+    from parity import _eq
+    tf = cfg1_small
+    cap = int(max(tf.sector_counts().reshape(-1).sum() // n_groups * 1.5, 1000))
+    pipe = pkg.Pipeline(tf.params, n_groups, max_clusters_group=cap)
+    first, _ = pipe.groups()
+    assert first[0] == 0 and first[-1] == 36 and len(first) == n_groups + 1
+    what = B.OUT_ALL | B.OUT_SELECTION | B.OUT_RESIDUALS
+    orc = Oracle(tf.params)
+    for rep in range(2):                       # a pipeline is reusable: second time frame through the same contexts
+        outs = pipe.run(tf.y, tf.z, tf.row, stage_mask=0x7F, what=what)
+        for s in (range(36) if rep == 0 else (0, 17, 35)):
+            o = orc.run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x7F)
+            try:
+                compare_sector(outs[s], o, orc, tf.row[s][o.order])
+                r = {}
+                _eq("owner", outs[s].owner, o.owner, r); _eq("selected", outs[s].selected, o.selected, r)
+                _eq("res_trk", outs[s].res_trk, o.res_trk, r); _eq("q_y", outs[s].q_y, o.q_y, r)
+            except ParityError as e:
+                raise ParityError(f"groups {n_groups} sector {s}: {e}") from None
+    pipe.close()
+
+
+def test_pipeline_device_inputs_and_errors(pkg, cfg1_small):
+    import torch
+    from paper_2208_07412_b200 import binding as B
+    tf = cfg1_small
+    pipe = pkg.Pipeline(tf.params, 3, max_clusters_group=tf.n_clusters)
+    y = [torch.from_numpy(a).cuda() for a in tf.y]; z = [torch.from_numpy(a).cuda() for a in tf.z]
+    row = [torch.from_numpy(a.astype(np.int16)).cuda().view(torch.uint16) for a in tf.row]
+    outs = pipe.run(y, z, row)
+    orc = Oracle(tf.params)
+    for s in (5, 20):
+        o = orc.run(tf.y[s], tf.z[s], tf.row[s])
+        compare_sector(outs[s], o, orc, tf.row[s][o.order])
+    pipe.close()
+    # a group whose capacity is too small reports it (nothing is truncated)
+    pipe = pkg.Pipeline(tf.params, 4, max_clusters_group=1000)
+    with pytest.raises(pkg.TpccaError) as e:
+        pipe.run(tf.y, tf.z, tf.row)
+    assert e.value.code == -4 and "group" in str(e.value)
+    pipe.close()
+    with pytest.raises(pkg.TpccaError):
+        pkg.Pipeline(tf.params, 99, max_clusters_group=1000)
+
+
+def test_get_tracks_all_equals_per_sector(pkg, cfg1_small):
+    tf = cfg1_small
+    trk = run_gpu(pkg, tf)
+    allv = trk.get_tracks_all()
+    for s in (0, 9, 35):
+        one = trk.get_tracks(s)
+        for f in ("order", "link_up", "start_hit", "par", "cov", "hit_idx", "hit_offset"):
+            assert np.array_equal(getattr(allv[s], f), getattr(one, f)), f
+    trk.close()

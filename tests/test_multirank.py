@@ -154,6 +154,9 @@ class FakeEnv:
     def tracker(self, params, max_clusters, max_start_hits, stream=None):
         return _FakeTracker(self, params)
 
+    def pipeline(self, *a):
+        raise AssertionError("the pipeline leg runs at N = 1 only")
+
     def pin(self, a):
         return torch.from_numpy(a)
 
