@@ -24,6 +24,8 @@ class _Params(C.Structure):
         ("max_sinphi", C.c_double), ("grid_margin", C.c_double),
         ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32),
         ("sel_max_shared_permille", C.c_int32), ("res_inv_quantum", C.c_double),
+        ("sectors_per_side", C.c_int32), ("sector_cos", C.c_double), ("sector_sin", C.c_double),
+        ("mg_max_row_gap", C.c_int32), ("mg_dy", C.c_double), ("mg_dz", C.c_double), ("mg_dsin", C.c_double),
     ]
 
 
@@ -53,6 +55,11 @@ def _load():
         lib.oracle_n_selected.argtypes = [C.c_void_p]
         lib.oracle_n_selected.restype = C.c_int64
         lib.oracle_get_selection.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+        lib.oracle_merge.argtypes = [C.POINTER(C.c_void_p), C.c_int]
+        lib.oracle_get_merge_links.argtypes = [C.c_void_p] + [C.c_void_p] * 4 + [C.POINTER(C.c_int64)]
+        lib.oracle_get_merged.argtypes = [C.c_void_p] + [C.c_void_p] * 9
+        lib.oracle_kf_rotate.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
+        lib.oracle_kf_rotate.restype = C.c_int
         lib.oracle_get_residuals.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         lib.oracle_select.argtypes = [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int32] + [C.c_void_p] * 3
         lib.oracle_select.restype = C.c_int64
@@ -139,6 +146,12 @@ class Oracle:
         p.tc_max_gap = int(params.tc_max_gap); p.tc_min_hits = int(params.tc_min_hits)
         p.sel_max_shared_permille = int(getattr(params, "sel_max_shared_permille", 500))
         p.res_inv_quantum = float(getattr(params, "res_inv_quantum", 128.0))
+        p.sectors_per_side = int(getattr(params, "sectors_per_side", 18))
+        p.sector_cos = float(getattr(params, "sector_cos", np.float32(np.cos(np.pi / 9))))
+        p.sector_sin = float(getattr(params, "sector_sin", np.float32(np.sin(np.pi / 9))))
+        p.mg_max_row_gap = int(getattr(params, "mg_max_row_gap", 8))
+        p.mg_dy = float(getattr(params, "mg_dy", 1.0)); p.mg_dz = float(getattr(params, "mg_dz", 1.0))
+        p.mg_dsin = float(getattr(params, "mg_dsin", 0.05))
         self._h = lib.oracle_create(C.byref(p), self.precision)
         if not self._h:
             raise RuntimeError("oracle_create failed")
@@ -216,8 +229,68 @@ class Oracle:
         st = np.ascontiguousarray(state, dtype=np.float64)
         return float(self._lib.oracle_kf_dist2(self._h, st.ctypes.data_as(_dp), float(ym), float(zm)))
 
+    def kf_rotate(self, state, ca, sa):
+        st = np.ascontiguousarray(state, dtype=np.float64).copy()
+        ok = self._lib.oracle_kf_rotate(self._h, st.ctypes.data_as(_dp), float(ca), float(sa))
+        return bool(ok), st
+
     def score(self, r, yc, zc, yu, zu, yd, zd):
         return float(self._lib.oracle_score(self._h, int(r), yc, zc, yu, zu, yd, zd))
+
+
+@dataclasses.dataclass
+class MergeResult:
+    """S8 outputs of one sector: links per SELECTED track and the merged chains headed in the sector."""
+    next_sec: np.ndarray = None
+    next_trk: np.ndarray = None
+    prev_sec: np.ndarray = None
+    prev_trk: np.ndarray = None
+    head: np.ndarray = None       # [n_merged] selected index of the lowest segment
+    n_seg: np.ndarray = None
+    n_hits: np.ndarray = None
+    n_fit: np.ndarray = None
+    first_row: np.ndarray = None
+    last_row: np.ndarray = None
+    frame_seg: np.ndarray = None  # segment (index in the chain) whose frame / z_ref the parameters are in
+    x_ref: np.ndarray = None
+    z_ref: np.ndarray = None
+    par: np.ndarray = None
+    cov: np.ndarray = None
+    chi2: np.ndarray = None
+    seg_offset: np.ndarray = None
+    seg_sec: np.ndarray = None
+    seg_trk: np.ndarray = None
+
+
+def run_timeframe_merged(tf, precision="f32", sectors=None):
+    """S1-S8 over a whole time frame: per-sector OracleResult (stage mask 0x7F) + MergeResult.  Keeps one oracle
+    per sector alive for the cross-sector step."""
+    lib = _load()
+    ns = tf.n_sectors
+    orcs = [Oracle(tf.params, precision) for _ in range(ns)]
+    res = [orcs[s].run(tf.y[s], tf.z[s], tf.row[s], stage_mask=0x7F) for s in range(ns)]
+    handles = (C.c_void_p * ns)(*[o._h for o in orcs])
+    lib.oracle_merge(handles, ns)
+    out = []
+    for s in range(ns):
+        k = int(res[s].selected.shape[0])
+        m = MergeResult(next_sec=np.empty(k, np.int32), next_trk=np.empty(k, np.int32), prev_sec=np.empty(k, np.int32),
+                        prev_trk=np.empty(k, np.int32))
+        cnt = (C.c_int64 * 2)()
+        lib.oracle_get_merge_links(orcs[s]._h, m.next_sec.ctypes.data, m.next_trk.ctypes.data, m.prev_sec.ctypes.data,
+                                   m.prev_trk.ctypes.data, cnt)
+        nm, nseg = int(cnt[0]), int(cnt[1])
+        ints = np.empty((nm, 7), np.int32)
+        m.x_ref = np.empty(nm); m.z_ref = np.empty(nm); m.chi2 = np.empty(nm); m.par = np.empty((nm, 5)); m.cov = np.empty((nm, 15))
+        m.seg_offset = np.empty(nm + 1, np.int32); m.seg_sec = np.empty(nseg, np.int32); m.seg_trk = np.empty(nseg, np.int32)
+        lib.oracle_get_merged(orcs[s]._h, ints.ctypes.data, m.x_ref.ctypes.data, m.z_ref.ctypes.data, m.par.ctypes.data,
+                              m.cov.ctypes.data, m.chi2.ctypes.data, m.seg_offset.ctypes.data, m.seg_sec.ctypes.data,
+                              m.seg_trk.ctypes.data)
+        m.head, m.n_seg, m.n_hits, m.n_fit, m.first_row, m.last_row, m.frame_seg = (np.ascontiguousarray(ints[:, i]) for i in range(7))
+        out.append(m)
+    for o in orcs:
+        o.close()
+    return res, out
 
 
 def select_tracks(n_clusters, hit_offset, hit_idx, max_shared_permille=500):

@@ -57,6 +57,11 @@ struct oracle_params {      // all tables are double arrays holding the (fp32-re
   int32_t tc_max_gap, tc_min_hits;
   int32_t sel_max_shared_permille;   // S6: a tracklet survives iff shared hits * 1000 <= this * n_hits
   double res_inv_quantum;            // S7: residuals are quantised to round(res * this), 16 bits
+  // S8: cross-sector merging
+  int32_t sectors_per_side;          // sectors s and s' are neighbours iff same side (s / this) and |s - s'| = 1 mod this
+  double sector_cos, sector_sin;     // cos / sin of the angle between neighbouring sectors (20 degrees)
+  int32_t mg_max_row_gap;            // the upper segment starts 1 .. this rows above the last row of the lower one
+  double mg_dy, mg_dz, mg_dsin;      // match windows on y, z, sin(phi) at the upper segment's reference plane
 };
 }
 
@@ -138,6 +143,8 @@ class Oracle {
     max_gap = q.tc_max_gap; min_hits = q.tc_min_hits;
     sel_permille = q.sel_max_shared_permille;
     res_inv_q = (R)q.res_inv_quantum;
+    per_side = q.sectors_per_side; sec_cos = (R)q.sector_cos; sec_sin = (R)q.sector_sin;
+    mg_gap = q.mg_max_row_gap; mg_dy = (R)q.mg_dy; mg_dz = (R)q.mg_dz; mg_ds = (R)q.mg_dsin;
     row_bin_base.resize(n_rows + 1);
     row_bin_base[0] = 0;
     for (int r = 0; r < n_rows; ++r) row_bin_base[r + 1] = row_bin_base[r] + (int64_t)ny[r] * nz[r];
@@ -491,6 +498,9 @@ class Oracle {
   // Clusters no selected track owns keep res_trk = -1, residuals 0 (a codec stores them raw).
   void track_residuals() {
     res_trk.assign(n, -1); res_y.assign(n, (R)0); res_z.assign(n, (R)0); q_y.assign(n, 0); q_z.assign(n, 0);
+    out_state.assign(selected.size(), KFState<R>());
+    out_ok.assign(selected.size(), 0);
+    size_t ksel = 0;
     for (int32_t t : selected) {
       const Track<R>& T = tracks[t];
       KFState<R> s;
@@ -498,15 +508,19 @@ class Oracle {
       for (int i = 0; i < 5; ++i) s.p[i] = T.p[i];
       for (int i = 0; i < 15; ++i) s.C[i] = (R)0;
       s.chi2 = (R)0; s.n = 0;
+      bool walked = true;
       for (int32_t k = hit_offset[t]; k < hit_offset[t + 1]; ++k) {
         const int32_t c = hit_idx[k];
-        if (!propagate(s, row_x[srow[c]])) break;
+        if (!propagate(s, row_x[srow[c]])) { walked = false; break; }
+        if (k + 1 == hit_offset[t + 1]) { out_state[ksel] = s; out_ok[ksel] = 1; }   // S8: state on the last row
         if (owner[c] != t) continue;
         const R ry = sy[c] - s.p[0];
         const R rz = (sz[c] - T.z_ref) - s.p[1];
         res_trk[c] = t; res_y[c] = ry; res_z[c] = rz;
         q_y[c] = quantise(ry); q_z[c] = quantise(rz);
       }
+      (void)walked;
+      ++ksel;
     }
   }
   int16_t quantise(R r) const {
@@ -514,6 +528,46 @@ class Oracle {
     if (v > (R)32767) v = (R)32767;
     if (v < (R)-32767) v = (R)-32767;
     return (int16_t)v;
+  }
+
+  // ----------------------------------------------------------------------------- S8: cross-sector merging
+  // DESIGN.md 3.7 "Rotate": the state at plane x of a frame is re-expressed in the frame turned by the angle
+  // whose cosine / sine are (ca, sa) (sa > 0: towards the next sector in azimuth), at the plane through the SAME
+  // space point:  x' = x ca + y sa,  y' = y ca - x sa,  sin phi' = sin phi ca - cos phi sa  (cos phi > 0: the
+  // track moves outward).  Covariance: a shift dy of the point moves it by (dy sa, dy ca) in the new frame; back
+  // on the fixed plane x' that is  dY = dy cos phi / cos phi',  dZ = -dy p3 sa / cos phi',
+  // d sin phi' = -dy (Bc p4) sa;  and  d sin phi' / d sin phi = cos phi' / cos phi.  Fails (state untouched) if
+  // |sin phi| or |sin phi'| exceeds max_sinphi.
+  bool rotate(KFState<R>& s, R ca, R sa) const {
+    const R sf = s.p[2];
+    if (!(std::fabs(sf) <= max_sinphi)) return false;
+    const R cf = std::sqrt((R)1 - sf * sf);
+    const R sf2 = sf * ca - cf * sa;
+    if (!(std::fabs(sf2) <= max_sinphi)) return false;
+    const R cf2 = std::sqrt((R)1 - sf2 * sf2);
+    const R x2 = s.x * ca + s.p[0] * sa;
+    const R y2 = s.p[0] * ca - s.x * sa;
+    const R j00 = cf / cf2;
+    const R j10 = -((s.p[3] * sa) / cf2);
+    const R j20 = -((s.p[4] * Bc) * sa);
+    const R j22 = cf2 / cf;
+    R A[5][5];
+    for (int j = 0; j < 5; ++j) {
+      A[0][j] = j00 * s.c(0, j);
+      A[1][j] = j10 * s.c(0, j) + s.c(1, j);
+      A[2][j] = j20 * s.c(0, j) + j22 * s.c(2, j);
+      A[3][j] = s.c(3, j);
+      A[4][j] = s.c(4, j);
+    }
+    for (int i = 0; i < 5; ++i) {
+      s.C[tri(i, 0)] = A[i][0] * j00;
+      if (i >= 1) s.C[tri(i, 1)] = A[i][0] * j10 + A[i][1];
+      if (i >= 2) s.C[tri(i, 2)] = A[i][0] * j20 + A[i][2] * j22;
+      if (i >= 3) s.C[tri(i, 3)] = A[i][3];
+      if (i >= 4) s.C[tri(i, 4)] = A[i][4];
+    }
+    s.x = x2; s.p[0] = y2; s.p[2] = sf2;
+    return true;
   }
 
   void run(uint32_t stage_mask, bool brute) {
@@ -536,6 +590,8 @@ class Oracle {
   R c24, c640, c12;
   int max_gap, min_hits, sel_permille;
   R res_inv_q;
+  int per_side = 0, mg_gap = 0;
+  R sec_cos = 0, sec_sin = 0, mg_dy = 0, mg_dz = 0, mg_ds = 0;
   // data
   int64_t n = 0;
   std::vector<R> y, z, sy, sz;
@@ -549,7 +605,147 @@ class Oracle {
   std::vector<int32_t> res_trk;                  // S7
   std::vector<R> res_y, res_z;
   std::vector<int16_t> q_y, q_z;
+  std::vector<KFState<R>> out_state;             // S7 by-product for S8: state of each selected track on its last row
+  std::vector<char> out_ok;
+  // S8, per selected track: neighbour-sector partner above (next) / below (prev), -1 none
+  std::vector<int32_t> mg_next_sec, mg_next_trk, mg_prev_sec, mg_prev_trk;
+  struct Merged { int32_t head; std::vector<int32_t> seg_sec, seg_trk; Track<R> t; };
+  std::vector<Merged> merged;                     // chains whose lowest segment lives in this sector
 };
+
+// S8: match the selected tracks of neighbouring sectors and refit the chains.
+//  Matching.  a = selected track of sector s with an outer state (S7 walk), b = selected track of a neighbour
+//  sector n (same side, next or previous in azimuth) with 1 <= first_row(b) - last_row(a) <= mg_max_row_gap:
+//  a's outer state is rotated into n's frame and propagated to x_ref(b) (either failing: no candidate), then
+//    dy = p0(b) - p0',  dz = (z_ref(b) - z_ref(a)) + (p1(b) - p1'),  ds = p2(b) - p2';
+//  candidate iff |dy| <= mg_dy, |dz| <= mg_dz, |ds| <= mg_dsin;  score = (dy/mg_dy)^2 + (dz/mg_dz)^2 + (ds/mg_dsin)^2.
+//  next(a) = the candidate with the smallest score (ties: smaller sector, then smaller track), prev(b) likewise
+//  over the a's that have b as a candidate; the link a -> b is kept iff next(a) = b and prev(b) = a.
+//  Refit.  For every chain g1 -> ... -> gk (g1 has no prev): start from gk's outer state with the reset
+//  covariance and run the Kalman filter downward over the hits of gk, ..., g1 (propagate to the hit's row,
+//  update; no gate, no search); between segments the state is rotated into the lower segment's frame and p1 is
+//  re-referenced: p1 += z_ref(upper) - z_ref(lower).  A failed transport / rotation ends the refit (the chain
+//  is emitted with what was fitted if at least one update happened).
+template <class R>
+void merge_sectors(std::vector<Oracle<R>*>& S) {
+  const int ns = (int)S.size();
+  for (auto* o : S) {
+    const size_t k = o->selected.size();
+    o->mg_next_sec.assign(k, -1); o->mg_next_trk.assign(k, -1); o->mg_prev_sec.assign(k, -1); o->mg_prev_trk.assign(k, -1);
+    o->merged.clear();
+  }
+  if (ns == 0) return;
+  const int per = S[0]->per_side;
+  if (per < 2 || ns % per != 0) return;                 // no neighbour relation defined
+  struct Best { bool have = false; R score = 0; int sec = -1, trk = -1; };
+  std::vector<std::vector<Best>> nxt(ns), prv(ns);
+  for (int s = 0; s < ns; ++s) { nxt[s].assign(S[s]->selected.size(), Best()); prv[s].assign(S[s]->selected.size(), Best()); }
+  auto better = [](const Best& b, R sc, int sec, int trk) {
+    if (!b.have) return true;
+    if (sc != b.score) return sc < b.score;
+    if (sec != b.sec) return sec < b.sec;
+    return trk < b.trk;
+  };
+  for (int s = 0; s < ns; ++s) {
+    Oracle<R>& A = *S[s];
+    const int side = s / per, loc = s % per;
+    for (int dir = 0; dir < 2; ++dir) {
+      const int nsec = side * per + (dir == 0 ? (loc + 1) % per : (loc + per - 1) % per);
+      if (nsec == s) continue;
+      if (per == 2 && dir == 1) continue;               // two sectors per side: one neighbour, reached once
+      Oracle<R>& B = *S[nsec];
+      const R sa = dir == 0 ? A.sec_sin : -A.sec_sin;
+      for (size_t ia = 0; ia < A.selected.size(); ++ia) {
+        if (!A.out_ok[ia]) continue;
+        const Track<R>& ta = A.tracks[A.selected[ia]];
+        for (size_t ib = 0; ib < B.selected.size(); ++ib) {
+          const Track<R>& tb = B.tracks[B.selected[ib]];
+          const int gap = tb.first_row - ta.last_row;
+          if (gap < 1 || gap > A.mg_gap) continue;
+          KFState<R> st = A.out_state[ia];
+          if (!A.rotate(st, A.sec_cos, sa)) continue;
+          if (!A.propagate(st, tb.x_ref)) continue;
+          const R dy = tb.p[0] - st.p[0];
+          const R dz = (tb.z_ref - ta.z_ref) + (tb.p[1] - st.p[1]);
+          const R ds = tb.p[2] - st.p[2];
+          if (!(std::fabs(dy) <= A.mg_dy && std::fabs(dz) <= A.mg_dz && std::fabs(ds) <= A.mg_ds)) continue;
+          const R qy = dy / A.mg_dy, qz = dz / A.mg_dz, qs = ds / A.mg_ds;
+          const R sc = qy * qy + qz * qz + qs * qs;
+          if (better(nxt[s][ia], sc, nsec, (int)ib)) { nxt[s][ia].have = true; nxt[s][ia].score = sc; nxt[s][ia].sec = nsec; nxt[s][ia].trk = (int)ib; }
+          if (better(prv[nsec][ib], sc, s, (int)ia)) { prv[nsec][ib].have = true; prv[nsec][ib].score = sc; prv[nsec][ib].sec = s; prv[nsec][ib].trk = (int)ia; }
+        }
+      }
+    }
+  }
+  for (int s = 0; s < ns; ++s)
+    for (size_t ia = 0; ia < S[s]->selected.size(); ++ia) {
+      const Best& b = nxt[s][ia];
+      if (!b.have) continue;
+      const Best& back = prv[b.sec][b.trk];
+      if (back.have && back.sec == s && back.trk == (int)ia) {
+        S[s]->mg_next_sec[ia] = b.sec; S[s]->mg_next_trk[ia] = b.trk;
+        S[b.sec]->mg_prev_sec[b.trk] = s; S[b.sec]->mg_prev_trk[b.trk] = (int32_t)ia;
+      }
+    }
+  // ---- refit of the chains
+  for (int s = 0; s < ns; ++s) {
+    Oracle<R>& H = *S[s];
+    for (size_t ih = 0; ih < H.selected.size(); ++ih) {
+      if (H.mg_prev_sec[ih] != -1 || H.mg_next_sec[ih] == -1) continue;       // heads of chains with >= 2 segments
+      typename Oracle<R>::Merged M;
+      M.head = (int32_t)ih;
+      int cs = s, ct = (int)ih;
+      while (cs != -1) {
+        M.seg_sec.push_back(cs); M.seg_trk.push_back(ct);
+        const int ns2 = S[cs]->mg_next_sec[ct], nt2 = S[cs]->mg_next_trk[ct];
+        cs = ns2; ct = nt2;
+      }
+      const int k = (int)M.seg_sec.size();
+      Oracle<R>& Top = *S[M.seg_sec[k - 1]];
+      KFState<R> st = Top.out_state[M.seg_trk[k - 1]];       // exists: the top segment was matched through it or ...
+      bool ok = Top.out_ok[M.seg_trk[k - 1]] != 0;
+      H.reset_cov(st);
+      KFState<R> snap = st;
+      bool have_snap = false;
+      int n_hits = 0, first = -1, last = -1, g_snap = k - 1;
+      for (int g = k - 1; g >= 0 && ok; --g) {
+        Oracle<R>& G = *S[M.seg_sec[g]];
+        const int32_t t = G.selected[M.seg_trk[g]];
+        const Track<R>& tg = G.tracks[t];
+        if (g < k - 1) {
+          // into the lower segment's frame: the inverse of the rotation that led from it to the upper one
+          const int up = M.seg_sec[g + 1], lo = M.seg_sec[g];
+          const int per_ = G.per_side;
+          const bool up_is_next = (up % per_) == ((lo % per_) + 1) % per_;
+          const R sa = up_is_next ? -G.sec_sin : G.sec_sin;
+          if (!G.rotate(st, G.sec_cos, sa)) { ok = false; break; }
+          const Track<R>& tu = S[up]->tracks[S[up]->selected[M.seg_trk[g + 1]]];
+          st.p[1] = st.p[1] + (tu.z_ref - tg.z_ref);
+        }
+        for (int32_t q = G.hit_offset[t + 1] - 1; q >= G.hit_offset[t]; --q) {
+          const int32_t c = G.hit_idx[q];
+          if (!G.propagate(st, G.row_x[G.srow[c]])) { ok = false; break; }
+          G.update(st, G.sy[c], G.sz[c] - tg.z_ref);
+          snap = st; have_snap = true; g_snap = g;
+          if (last < 0) last = G.srow[c];
+          first = G.srow[c];
+          ++n_hits;
+        }
+      }
+      if (!have_snap) continue;
+      M.t.x_ref = snap.x;
+      {   // the parameters are in the frame (and relative to the z_ref) of the lowest segment the refit reached
+        Oracle<R>& G = *S[M.seg_sec[g_snap]];
+        M.t.z_ref = G.tracks[G.selected[M.seg_trk[g_snap]]].z_ref;
+        M.t.start_hit = g_snap;                     // index of that segment in the chain (0 = head: the normal case)
+      }
+      for (int i = 0; i < 5; ++i) M.t.p[i] = snap.p[i];
+      for (int i = 0; i < 15; ++i) M.t.C[i] = snap.C[i];
+      M.t.chi2 = snap.chi2; M.t.n_fit = snap.n; M.t.n_hits = n_hits; M.t.first_row = first; M.t.last_row = last;
+      H.merged.push_back(M);
+    }
+  }
+}
 
 struct Handle {
   int precision;           // 0 = float, 1 = double
@@ -670,6 +866,59 @@ void oracle_get_selection(void* hv, int32_t* owner, int32_t* n_own, int32_t* sel
   if (h->precision == 0) GS(h->f); else GS(h->d);
 #undef GS
 }
+// S8: match and refit across the sectors held by `handles` (each after a run with stage bits up to 64)
+int oracle_merge(void** handles, int n_sectors) {
+  if (n_sectors <= 0) return 0;
+  const int prec = ((Handle*)handles[0])->precision;
+  if (prec == 0) {
+    std::vector<Oracle<float>*> S;
+    for (int i = 0; i < n_sectors; ++i) S.push_back(((Handle*)handles[i])->f);
+    merge_sectors(S);
+  } else {
+    std::vector<Oracle<double>*> S;
+    for (int i = 0; i < n_sectors; ++i) S.push_back(((Handle*)handles[i])->d);
+    merge_sectors(S);
+  }
+  return 0;
+}
+// per selected track of the sector: partner above / below; returns the number of merged chains headed here and
+// (out[1]) the total number of their segments
+void oracle_get_merge_links(void* hv, int32_t* next_sec, int32_t* next_trk, int32_t* prev_sec, int32_t* prev_trk, int64_t* out) {
+  Handle* h = (Handle*)hv;
+#define GM(o) do { \
+    std::copy((o)->mg_next_sec.begin(), (o)->mg_next_sec.end(), next_sec); std::copy((o)->mg_next_trk.begin(), (o)->mg_next_trk.end(), next_trk); \
+    std::copy((o)->mg_prev_sec.begin(), (o)->mg_prev_sec.end(), prev_sec); std::copy((o)->mg_prev_trk.begin(), (o)->mg_prev_trk.end(), prev_trk); \
+    out[0] = (int64_t)(o)->merged.size(); out[1] = 0; for (auto& m : (o)->merged) out[1] += (int64_t)m.seg_sec.size(); } while (0)
+  if (h->precision == 0) GM(h->f); else GM(h->d);
+#undef GM
+}
+// merged chains headed in this sector: ints [n][6] = head (selected index), n_seg, n_hits, n_fit, first_row, last_row + frame segment;
+// seg_offset [n + 1], seg_sec / seg_trk [total segments]
+void oracle_get_merged(void* hv, int32_t* ints, double* x_ref, double* z_ref, double* par, double* cov, double* chi2,
+                       int32_t* seg_offset, int32_t* seg_sec, int32_t* seg_trk) {
+  Handle* h = (Handle*)hv;
+#define GG2(o) do { \
+    int32_t off = 0; size_t i = 0; \
+    for (auto& m : (o)->merged) { \
+      ints[i * 7 + 0] = m.head; ints[i * 7 + 1] = (int32_t)m.seg_sec.size(); ints[i * 7 + 2] = m.t.n_hits; ints[i * 7 + 3] = m.t.n_fit; \
+      ints[i * 7 + 4] = m.t.first_row; ints[i * 7 + 5] = m.t.last_row; ints[i * 7 + 6] = m.t.start_hit; \
+      x_ref[i] = (double)m.t.x_ref; z_ref[i] = (double)m.t.z_ref; chi2[i] = (double)m.t.chi2; \
+      for (int q = 0; q < 5; ++q) par[i * 5 + q] = (double)m.t.p[q]; \
+      for (int q = 0; q < 15; ++q) cov[i * 15 + q] = (double)m.t.C[q]; \
+      seg_offset[i] = off; \
+      for (size_t q = 0; q < m.seg_sec.size(); ++q) { seg_sec[off] = m.seg_sec[q]; seg_trk[off] = m.seg_trk[q]; ++off; } \
+      ++i; } \
+    seg_offset[i] = off; } while (0)
+  if (h->precision == 0) GG2(h->f); else GG2(h->d);
+#undef GG2
+}
+// unit entry point for the pins: rotate a state [x, p0..p4, C0..C14, chi2] by (ca, sa)
+int oracle_kf_rotate(void* hv, double* st, double ca, double sa) {
+  Handle* h = (Handle*)hv;
+  if (h->precision == 0) { KFState<float> s; st_in(s, st); bool ok = h->f->rotate(s, (float)ca, (float)sa); st_out(s, st); return ok; }
+  KFState<double> s; st_in(s, st); bool ok = h->d->rotate(s, ca, sa); st_out(s, st); return ok;
+}
+
 // S7 outputs of the last run with stage bit 64, per cluster: res_trk i32, res_y / res_z double, q_y / q_z i16
 void oracle_get_residuals(void* hv, int32_t* res_trk, double* res_y, double* res_z, int16_t* q_y, int16_t* q_z) {
   Handle* h = (Handle*)hv;

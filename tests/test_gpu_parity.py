@@ -25,9 +25,14 @@ def pkg():
     return p
 
 
+#: TPCCA_TEST_WS_FILL=0xff (or 0x7f, ...) poisons every workspace before tpcca_create: the stand-in for
+#: `compute-sanitizer --tool initcheck`, which is closed on this GPU pool (profiles/r2_sanitizers.md)
+WS_FILL = int(os.environ["TPCCA_TEST_WS_FILL"], 0) if os.environ.get("TPCCA_TEST_WS_FILL") else None
+
+
 def run_gpu(pkg, tf, stages=0x1F, max_start_hits=0):
     n = max(tf.n_clusters, 1)
-    trk = pkg.Tracker(tf.params, max_clusters=n, max_start_hits=max_start_hits)
+    trk = pkg.Tracker(tf.params, max_clusters=n, max_start_hits=max_start_hits, workspace_fill=WS_FILL)
     trk.load_timeframe(tf)
     trk.run(stages)
     trk.sync()
@@ -427,7 +432,7 @@ def test_config2_full_size_six_sectors(pkg):
 # S6 tracklet selector
 # ------------------------------------------------------------------------------------------------
 def run_gpu_select(pkg, tf, **kw):
-    trk = pkg.Tracker(tf.params, max_clusters=max(tf.n_clusters, 1), **kw)
+    trk = pkg.Tracker(tf.params, max_clusters=max(tf.n_clusters, 1), workspace_fill=WS_FILL, **kw)
     trk.load_timeframe(tf)
     trk.run(0x3F)
     trk.sync()

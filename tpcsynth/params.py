@@ -77,6 +77,14 @@ class TrackerParams:
     tc_min_hits: int
     sel_max_shared_permille: int = 500   # S6 selector: a tracklet survives iff at most this share of its hits is not its own
     res_inv_quantum: float = 128.0       # S7 residual front end: residuals are quantised to round(res * this) (1/128 cm)
+    # S8 cross-sector merging: neighbour relation (18 sectors per side, 20 degrees apart) and match windows
+    sectors_per_side: int = 18
+    sector_cos: float = float(np.float32(math.cos(math.pi / 9.0)))
+    sector_sin: float = float(np.float32(math.sin(math.pi / 9.0)))
+    mg_max_row_gap: int = 8
+    mg_dy: float = 1.0
+    mg_dz: float = 1.0
+    mg_dsin: float = 0.05
     # informative (not consumed by the tracker)
     sigma: float = 0.1
     z_hi: float = 250.0
