@@ -26,6 +26,7 @@ class _Params(C.Structure):
         ("sel_max_shared_permille", C.c_int32), ("res_inv_quantum", C.c_double),
         ("sectors_per_side", C.c_int32), ("sector_cos", C.c_double), ("sector_sin", C.c_double),
         ("mg_max_row_gap", C.c_int32), ("mg_dy", C.c_double), ("mg_dz", C.c_double), ("mg_dsin", C.c_double),
+        ("mg_zpre", C.c_double),
     ]
 
 
@@ -151,7 +152,7 @@ class Oracle:
         p.sector_sin = float(getattr(params, "sector_sin", np.float32(np.sin(np.pi / 9))))
         p.mg_max_row_gap = int(getattr(params, "mg_max_row_gap", 8))
         p.mg_dy = float(getattr(params, "mg_dy", 1.0)); p.mg_dz = float(getattr(params, "mg_dz", 1.0))
-        p.mg_dsin = float(getattr(params, "mg_dsin", 0.05))
+        p.mg_dsin = float(getattr(params, "mg_dsin", 0.05)); p.mg_zpre = float(getattr(params, "mg_zpre", 32.0))
         self._h = lib.oracle_create(C.byref(p), self.precision)
         if not self._h:
             raise RuntimeError("oracle_create failed")

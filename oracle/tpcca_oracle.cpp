@@ -62,6 +62,7 @@ struct oracle_params {      // all tables are double arrays holding the (fp32-re
   double sector_cos, sector_sin;     // cos / sin of the angle between neighbouring sectors (20 degrees)
   int32_t mg_max_row_gap;            // the upper segment starts 1 .. this rows above the last row of the lower one
   double mg_dy, mg_dz, mg_dsin;      // match windows on y, z, sin(phi) at the upper segment's reference plane
+  double mg_zpre;                    // pre-cut on |z(b at x_ref) - z(a on its last row)| before any transport
 };
 }
 
@@ -144,7 +145,7 @@ class Oracle {
     sel_permille = q.sel_max_shared_permille;
     res_inv_q = (R)q.res_inv_quantum;
     per_side = q.sectors_per_side; sec_cos = (R)q.sector_cos; sec_sin = (R)q.sector_sin;
-    mg_gap = q.mg_max_row_gap; mg_dy = (R)q.mg_dy; mg_dz = (R)q.mg_dz; mg_ds = (R)q.mg_dsin;
+    mg_gap = q.mg_max_row_gap; mg_dy = (R)q.mg_dy; mg_dz = (R)q.mg_dz; mg_ds = (R)q.mg_dsin; mg_zpre = (R)q.mg_zpre;
     row_bin_base.resize(n_rows + 1);
     row_bin_base[0] = 0;
     for (int r = 0; r < n_rows; ++r) row_bin_base[r + 1] = row_bin_base[r] + (int64_t)ny[r] * nz[r];
@@ -591,7 +592,7 @@ class Oracle {
   int max_gap, min_hits, sel_permille;
   R res_inv_q;
   int per_side = 0, mg_gap = 0;
-  R sec_cos = 0, sec_sin = 0, mg_dy = 0, mg_dz = 0, mg_ds = 0;
+  R sec_cos = 0, sec_sin = 0, mg_dy = 0, mg_dz = 0, mg_ds = 0, mg_zpre = 0;
   // data
   int64_t n = 0;
   std::vector<R> y, z, sy, sz;
@@ -615,7 +616,8 @@ class Oracle {
 
 // S8: match the selected tracks of neighbouring sectors and refit the chains.
 //  Matching.  a = selected track of sector s with an outer state (S7 walk), b = selected track of a neighbour
-//  sector n (same side, next or previous in azimuth) with 1 <= first_row(b) - last_row(a) <= mg_max_row_gap:
+//  sector n (same side, next or previous in azimuth) with 1 <= first_row(b) - last_row(a) <= mg_max_row_gap and
+//  |(z_ref(b) + p1(b)) - (z_ref(a) + p1_out(a))| <= mg_zpre (a cheap pre-cut an index can serve):
 //  a's outer state is rotated into n's frame and propagated to x_ref(b) (either failing: no candidate), then
 //    dy = p0(b) - p0',  dz = (z_ref(b) - z_ref(a)) + (p1(b) - p1'),  ds = p2(b) - p2';
 //  candidate iff |dy| <= mg_dy, |dz| <= mg_dz, |ds| <= mg_dsin;  score = (dy/mg_dy)^2 + (dz/mg_dz)^2 + (ds/mg_dsin)^2.
@@ -662,6 +664,8 @@ void merge_sectors(std::vector<Oracle<R>*>& S) {
           const Track<R>& tb = B.tracks[B.selected[ib]];
           const int gap = tb.first_row - ta.last_row;
           if (gap < 1 || gap > A.mg_gap) continue;
+          const R za = ta.z_ref + A.out_state[ia].p[1], zb = tb.z_ref + tb.p[1];
+          if (!(std::fabs(zb - za) <= A.mg_zpre)) continue;
           KFState<R> st = A.out_state[ia];
           if (!A.rotate(st, A.sec_cos, sa)) continue;
           if (!A.propagate(st, tb.x_ref)) continue;

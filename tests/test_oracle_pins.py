@@ -942,3 +942,181 @@ def test_residual_statistics_and_quantiser(cfg1_tracks):
     assert core_y.size > 0.98 * ry.size
     assert abs(core_y.mean()) < 0.003 and abs(core_z.mean()) < 0.003
     assert 0.085 < core_y.std() < 0.105 and 0.085 < core_z.std() < 0.105
+
+
+# ----------------------------------------------------------------------------------------
+# S8 cross-sector merging + refit
+# ----------------------------------------------------------------------------------------
+def test_rotate_follows_exact_circle_geometry():
+    """Rotate + Propagate vs the generator's exact circle geometry (tpcsynth.truth_state: double precision,
+    atan2 / sinh, the same helix expressed in the local frames of two neighbouring sectors)."""
+    tf = tpcsynth.generate(1, n_tracks=400)
+    P = tf.params
+    orc = Oracle(P, "f64")
+    rx = P.row_x.astype(np.float64)
+    ca, sa = math.cos(math.pi / 9), math.sin(math.pi / 9)
+    n_ok = 0
+    for trk in range(tf.trk_pt.shape[0]):
+        if tf.trk_pt[trk] < 0.4:
+            continue
+        for s in range(0, 36, 3):
+            for x in (rx[10], rx[40], rx[75], rx[110], rx[140]):
+                a = tpcsynth.truth_state(tf, trk, s, float(x))
+                if a is None or not (0.165 * x <= abs(a["y"]) <= 0.19 * x) or abs(a["sinphi"]) > 0.6:   # at the edge of sector s
+                    continue
+                up = a["y"] > 0                                                     # leaves towards s+1 (y > 0) or s-1
+                n_sec = (s // 18) * 18 + ((s % 18) + (1 if up else 17)) % 18
+                st = _state(x, [a["y"], a["z"], a["sinphi"], a["dzds"], a["p4"]])
+                ok, r = orc.kf_rotate(st, ca, sa if up else -sa)
+                assert ok
+                x2 = float(rx[np.argmin(np.abs(rx - r[0]))])                        # nearest pad row of the neighbour
+                b = tpcsynth.truth_state(tf, trk, n_sec, x2)
+                if b is None or abs(b["sinphi"]) > 0.9:
+                    continue
+                ok, q = orc.kf_propagate(r, x2)
+                assert ok
+                assert abs(q[1] - b["y"]) < 1e-8 and abs(q[3] - b["sinphi"]) < 1e-10, (trk, s, q[1], b["y"])
+                assert abs(q[2] - b["z"]) < 1e-6 and q[4] == a["dzds"] and q[5] == a["p4"]
+                n_ok += 1
+    assert n_ok > 25
+
+
+def test_rotate_covariance_jacobian_finite_differences():
+    """C' = J C J^T of Rotate vs central differences of (rotate, then back onto the unperturbed plane)."""
+    P = tpcsynth.default_params(n_sectors=1)
+    orc = Oracle(P, "f64")
+    ca, sa = math.cos(math.pi / 9), -math.sin(math.pi / 9)
+    x = 150.0
+    p = np.array([24.0, -3.0, 0.35, 0.6, -2.0])
+    ok, base = orc.kf_rotate(_state(x, p), ca, sa)
+    assert ok
+    x_new = base[0]
+
+    def image(q):
+        ok, r = orc.kf_rotate(_state(x, q), ca, sa)
+        assert ok
+        ok, r = orc.kf_propagate(r, x_new)           # the perturbed point lies on another plane: bring it back
+        assert ok
+        return r[1:6]
+    tri = lambda i, j: i * (i + 1) // 2 + j
+    J_fd = np.zeros((5, 5))
+    for j in range(5):
+        h = 1e-6
+        dp = np.zeros(5); dp[j] = h
+        J_fd[:, j] = (image(p + dp) - image(p - dp)) / (2 * h)
+    # J from the covariance transform: for C = e_j e_j^T + e_k e_k^T ... use single-entry covariances
+    J = np.zeros((5, 5))
+    for j in range(5):
+        C = np.zeros(15); C[tri(j, j)] = 1.0
+        ok, r = orc.kf_rotate(_state(x, p, C), ca, sa)
+        Cn = r[6:21]
+        d = np.array([Cn[tri(i, i)] for i in range(5)])          # J[i,j]^2
+        jj = int(np.argmax(d))
+        col = np.array([Cn[tri(max(i, jj), min(i, jj))] for i in range(5)]) / math.sqrt(d[jj])
+        if col @ J_fd[:, j] < 0:
+            col = -col
+        J[:, j] = col
+    assert np.allclose(J, J_fd, rtol=1e-6, atol=1e-7), (J, J_fd)
+    assert abs(J[0, 0] - 1) > 0.05 and abs(J[2, 0]) > 1e-4 and abs(J[1, 0]) > 0.05      # the non-trivial terms are exercised
+
+
+@pytest.fixture(scope="module")
+def merged_cfg1():
+    from oracle import run_timeframe_merged
+    tf = tpcsynth.generate(1, n_tracks=4000)
+    res, mg = run_timeframe_merged(tf)
+    return tf, res, mg
+
+
+def _selected_majority(tf, res, s):
+    from tpcsynth.truth import match_tracks
+    r = res[s]
+    lab = tf.label[s][r.order]
+    off = np.concatenate([[0], np.cumsum(r.n_hits[r.selected])]).astype(np.int32)
+    idx = (np.concatenate([r.hit_idx[r.hit_offset[t]:r.hit_offset[t + 1]] for t in r.selected]) if len(r.selected)
+           else np.empty(0, np.int32))
+    return match_tracks(lab, off, idx)[0]
+
+
+def test_merge_links_invariants_and_truth(merged_cfg1):
+    tf, res, mg = merged_cfg1
+    maj = [_selected_majority(tf, res, s) for s in range(36)]
+    n_links = good = 0
+    gaps = []
+    for s in range(36):
+        m, r = mg[s], res[s]
+        for ia in np.nonzero(m.next_sec >= 0)[0]:
+            ns_, ib = int(m.next_sec[ia]), int(m.next_trk[ia])
+            # neighbours on the same side; links are mutual; the upper segment starts 1..8 rows above the lower one
+            assert ns_ // 18 == s // 18 and (ns_ % 18 - s % 18) % 18 in (1, 17)
+            assert mg[ns_].prev_sec[ib] == s and mg[ns_].prev_trk[ib] == ia
+            gap = res[ns_].first_row[res[ns_].selected[ib]] - r.last_row[r.selected[ia]]
+            assert 1 <= gap <= 8
+            gaps.append(gap)
+            n_links += 1
+            good += int(maj[s][ia] >= 0 and maj[s][ia] == maj[ns_][ib])
+        assert (m.prev_sec >= 0).sum() == sum(int((mg[t].next_sec == s).sum()) for t in range(36))
+    assert n_links > 3000 and good >= 0.99 * n_links, (n_links, good)
+    assert min(gaps) == 1 and max(gaps) >= 4
+    # efficiency: pairs of selected tracks of neighbouring sectors with the same particle, consecutive in row
+    # (upper starts 1..8 rows above the lower one's end), are linked
+    want = have = 0
+    for s in range(36):
+        r = res[s]
+        for d in (1, 17):
+            t = (s // 18) * 18 + (s % 18 + d) % 18
+            rt = res[t]
+            by_label = {}
+            for ib, lb in enumerate(maj[t]):
+                if lb >= 0:
+                    by_label.setdefault(int(lb), []).append(ib)
+            for ia, la in enumerate(maj[s]):
+                for ib in by_label.get(int(la), []) if la >= 0 else []:
+                    gap = rt.first_row[rt.selected[ib]] - r.last_row[r.selected[ia]]
+                    if 1 <= gap <= 8:
+                        want += 1
+                        have += int(mg[s].next_sec[ia] == t and mg[s].next_trk[ia] == ib)
+    assert want > 3000 and have >= 0.93 * want, (want, have)
+
+
+def test_merged_refit_statistics(merged_cfg1):
+    """The refit over the union of the segments: unit pulls against generator truth at the reference plane of the
+    lowest segment, chi2 / ndf = 1, every hit of every segment fitted, covariance smaller than the head's own."""
+    tf, res, mg = merged_cfg1
+    maj = [_selected_majority(tf, res, s) for s in range(36)]
+    pulls, red, shrink = [], [], []
+    tri = lambda i: i * (i + 1) // 2 + i
+    n_chain = 0
+    for s in range(36):
+        m, r = mg[s], res[s]
+        for k in range(len(m.head)):
+            segs = list(zip(m.seg_sec[m.seg_offset[k]:m.seg_offset[k + 1]], m.seg_trk[m.seg_offset[k]:m.seg_offset[k + 1]]))
+            assert segs[0] == (s, m.head[k]) and len(segs) == m.n_seg[k] >= 2
+            tot = sum(int(res[a].n_hits[res[a].selected[b]]) for a, b in segs)
+            n_chain += 1
+            if m.n_fit[k] != tot:
+                continue                                        # a transport failed on the way down (rare)
+            assert m.frame_seg[k] == 0 and m.n_hits[k] == tot
+            t_head = r.selected[m.head[k]]
+            assert m.x_ref[k] == r.x_ref[t_head] and m.z_ref[k] == r.z_ref[t_head]
+            labs = {int(maj[a][b]) for a, b in segs}
+            if len(labs) != 1 or -1 in labs or tot < 60:
+                continue
+            tr = tpcsynth.truth_state(tf, labs.pop(), s, float(m.x_ref[k]))
+            if tr is None:
+                continue
+            got = np.array([m.par[k, 0], m.z_ref[k] + m.par[k, 1], m.par[k, 2], m.par[k, 3], m.par[k, 4]])
+            want = np.array([tr["y"], tr["z"], tr["sinphi"], tr["dzds"], tr["p4"]])
+            err = np.sqrt(np.array([m.cov[k][tri(i)] for i in range(5)]))
+            pulls.append((got - want) / err)
+            red.append(m.chi2[k] / (2 * m.n_fit[k] - 5))
+            shrink.append(m.cov[k][tri(4)] / r.cov[t_head][tri(4)])
+    pulls = np.array(pulls)
+    assert n_chain > 1500 and pulls.shape[0] > 800
+    core = np.all(np.abs(pulls) < 5, axis=1)
+    assert core.mean() > 0.95
+    pc = pulls[core]
+    assert np.all(np.abs(pc.mean(axis=0)) < 0.12), pc.mean(axis=0)
+    assert np.all(np.abs(pc.std(axis=0) - 1.0) < 0.12), pc.std(axis=0)
+    assert abs(np.mean(np.array(red)[core]) - 1.0) < 0.06
+    assert np.median(shrink) < 0.5                              # the longer lever arm pins q/pT down

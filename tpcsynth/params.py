@@ -85,6 +85,7 @@ class TrackerParams:
     mg_dy: float = 1.0
     mg_dz: float = 1.0
     mg_dsin: float = 0.05
+    mg_zpre: float = 32.0
     # informative (not consumed by the tracker)
     sigma: float = 0.1
     z_hi: float = 250.0
