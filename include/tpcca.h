@@ -14,6 +14,7 @@
  * and, beyond the five (SURVEY.md 8(f) "next" rows):
  *   S6 tracklet selector: per-cluster ownership, clone removal
  *   S7 track-residual front end of a track-model cluster compression
+ *   S8 cross-sector merging of the selected tracks + Kalman refit of the merged chains
  * "clusters per sector and pad row in, links and fitted tracks out" (BASELINE.json:5).
  *
  * Every stage runs in hand-written CUDA kernels for sm_100a; there is NO CPU fallback: every
@@ -65,6 +66,7 @@ extern "C" {
 #define TPCCA_STAGE_ALL        0x1Fu   /* the five stages of the hot path (BASELINE.json:5)             */
 #define TPCCA_STAGE_SELECT     0x20u   /* S6 tracklet selector; needs S1-S5           */
 #define TPCCA_STAGE_RESIDUALS  0x40u   /* S7 cluster residuals to the selected tracks; needs S1-S6 */
+#define TPCCA_STAGE_MERGE      0x80u   /* S8 cross-sector merging + chain refit; needs S1-S7       */
 
 /* which output groups tpcca_get_tracks delivers (HOST: copies) */
 #define TPCCA_OUT_ORDER      0x01u  /* order                                      (S1)            */
@@ -79,6 +81,7 @@ extern "C" {
                                     /* fields of the view from the compact table (array lengths: n_selected and    */
                                     /* n_sel_hits instead of n_tracks and n_hits); not together with OUT_TRACKS   */
 #define TPCCA_OUT_RESIDUALS  0x100u /* res_trk, res_y, res_z, q_y, q_z            (S7)            */
+#define TPCCA_OUT_MERGE      0x200u /* mg_* links and merged chains               (S8)            */
 
 typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
 
@@ -109,6 +112,13 @@ typedef struct {
   int32_t tc_min_hits;             /* S5: minimum hits of an emitted track                        */
   int32_t sel_max_shared_permille; /* S6: a tracklet is selected iff (n_hits - n_own) * 1000 <= this * n_hits     */
   float res_inv_quantum;           /* S7: residuals are quantised to rint(res * this), 16 bits (> 0)              */
+  /* S8: sectors s, s' are neighbours iff s / sectors_per_side == s' / sectors_per_side and they are adjacent (cyclic)  */
+  /* inside the side; no merging if sectors_per_side < 2 or n_sectors is not a multiple of it                           */
+  int32_t sectors_per_side;        /* 18 for the ALICE TPC                                                        */
+  float sector_cos, sector_sin;    /* cos / sin of the angle between neighbouring sectors (20 degrees)            */
+  int32_t mg_max_row_gap;          /* the upper segment starts 1 .. this rows above the lower segment's last row  */
+  float mg_dy, mg_dz, mg_dsin;     /* match windows at the upper segment's reference plane (> 0)                  */
+  float mg_zpre;                   /* pre-cut on |z(upper at x_ref) - z(lower on its last row)| (> 0)             */
 } tpcca_params;
 
 /* Outputs of ONE sector.  With mem_space == TPCCA_MEM_DEVICE the pointers are DEVICE pointers
@@ -155,6 +165,14 @@ typedef struct {
   const int32_t  *res_trk;    /* [n_clusters] selected track (sector-local number) the cluster is attached to; -1 */
   const float    *res_y, *res_z;   /* [n_clusters] y_c - y_track, z_c - z_track at the cluster's row; 0 if -1    */
   const int16_t  *q_y, *q_z;  /* [n_clusters] rint(res * res_inv_quantum), clamped to +-32767    */
+  /* S8, per SELECTED track of the sector (n_selected entries each): the partner segment in a
+   * neighbour sector above / below (sector, selected-track number there; -1 none), and -- for tracks that are the
+   * lowest segment of a chain of >= 2 segments (mg_n_seg > 0) -- the Kalman refit over all hits of the chain,
+   * expressed in the frame and relative to the z_ref of segment mg_frame_seg of the chain (0 = this track) */
+  int64_t mg_stride;          /* elements between consecutive planes of mg_par / mg_cov          */
+  const int32_t  *mg_next_sec, *mg_next_trk, *mg_prev_sec, *mg_prev_trk;
+  const int32_t  *mg_n_seg, *mg_n_hits, *mg_n_fit, *mg_first_row, *mg_last_row, *mg_frame_seg;
+  const float    *mg_x_ref, *mg_z_ref, *mg_chi2, *mg_par, *mg_cov;
 } tpcca_tracks_view;
 
 /* Bytes of DEVICE workspace that tpcca_create needs for at most `max_clusters_total` clusters
@@ -190,7 +208,7 @@ int tpcca_load_clusters(tpcca_ctx *ctx, int sector, int64_t n, const float *x, c
 /* Start a new time frame: forget all loaded sectors and all outputs (no device work). */
 int tpcca_reset(tpcca_ctx *ctx);
 
-/* Run the stages in `stage_mask` (bit i = stage i+1; S6, S7: TPCCA_STAGE_SELECT, TPCCA_STAGE_RESIDUALS) over all sectors, asynchronously on the
+/* Run the stages in `stage_mask` (bit i = stage i+1; S6-S8: TPCCA_STAGE_SELECT, _RESIDUALS, _MERGE) over all sectors, asynchronously on the
  * context's stream.  A stage needs the outputs of the stages before it from this or an earlier
  * run on the same clusters (TPCCA_E_STATE otherwise).  Device-side failures (row out of range,
  * start-hit capacity overflow) are reported by the next tpcca_get_* / tpcca_sync call.
@@ -224,10 +242,10 @@ int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[7]);
 
 /* Device time of each stage [ms] of the run `runs_back` runs ago (0 = the last tpcca_run; the
  * context keeps the events of its last 16 runs), from CUDA events recorded on the context's
- * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6, ms[7] = S7 (0 if not run).
+ * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6, ms[7] = S7, ms[8] = S8 (0 if not run).
  * Synchronises the stream.
  * Errors: TPCCA_E_ARG (runs_back outside 0..15), TPCCA_E_STATE (no such run). */
-int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[8]);
+int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[9]);
 
 /* Work counters of the last run's S5 kernel, for the ALU roofline:
  * out[0] = Kalman propagations that moved the state, out[1] = Kalman updates,

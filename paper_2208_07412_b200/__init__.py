@@ -6,7 +6,7 @@ marshals arguments.  PyTorch lends device memory (the workspace) and the stream.
 CPU fallback: without the built library or without a CUDA device every entry point raises.
 """
 from .binding import (TpccaError, Tracker, Pipeline, SectorOutput, load_library, library_path, abi_symbols,
-                      STAGE_GRID, STAGE_NEIGHBOURS, STAGE_CLEAN, STAGE_START, STAGE_TRACKLETS, STAGE_ALL, STAGE_SELECT, STAGE_RESIDUALS)
+                      STAGE_GRID, STAGE_NEIGHBOURS, STAGE_CLEAN, STAGE_START, STAGE_TRACKLETS, STAGE_ALL, STAGE_SELECT, STAGE_RESIDUALS, STAGE_MERGE)
 
 __all__ = ["TpccaError", "Tracker", "Pipeline", "SectorOutput", "load_library", "library_path", "abi_symbols",
-           "STAGE_GRID", "STAGE_NEIGHBOURS", "STAGE_CLEAN", "STAGE_START", "STAGE_TRACKLETS", "STAGE_ALL", "STAGE_SELECT", "STAGE_RESIDUALS"]
+           "STAGE_GRID", "STAGE_NEIGHBOURS", "STAGE_CLEAN", "STAGE_START", "STAGE_TRACKLETS", "STAGE_ALL", "STAGE_SELECT", "STAGE_RESIDUALS", "STAGE_MERGE"]

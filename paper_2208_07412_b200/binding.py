@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 STAGE_GRID, STAGE_NEIGHBOURS, STAGE_CLEAN, STAGE_START, STAGE_TRACKLETS, STAGE_ALL = 1, 2, 4, 8, 16, 31
-STAGE_SELECT, STAGE_RESIDUALS = 32, 64
+STAGE_SELECT, STAGE_RESIDUALS, STAGE_MERGE = 32, 64, 128
 MEM_HOST, MEM_DEVICE, MEM_DEVICE_BORROW = 0, 1, 2
 
 _fp = C.POINTER(C.c_float)
@@ -29,7 +29,7 @@ ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "
                "tpcca_pipeline_create", "tpcca_pipeline_run", "tpcca_pipeline_get_groups", "tpcca_pipeline_last_error",
                "tpcca_pipeline_destroy", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
-OUT_SELECTION, OUT_TRACKS_SEL, OUT_RESIDUALS = 64, 128, 256
+OUT_SELECTION, OUT_TRACKS_SEL, OUT_RESIDUALS, OUT_MERGE = 64, 128, 256, 512
 
 
 class TpccaError(RuntimeError):
@@ -50,6 +50,9 @@ class _Params(C.Structure):
         ("max_sinphi", C.c_float), ("grid_margin", C.c_float),
         ("tc_max_gap", C.c_int32), ("tc_min_hits", C.c_int32), ("sel_max_shared_permille", C.c_int32),
         ("res_inv_quantum", C.c_float),
+        ("sectors_per_side", C.c_int32), ("sector_cos", C.c_float), ("sector_sin", C.c_float),
+        ("mg_max_row_gap", C.c_int32), ("mg_dy", C.c_float), ("mg_dz", C.c_float), ("mg_dsin", C.c_float),
+        ("mg_zpre", C.c_float),
     ]
 
 
@@ -65,6 +68,10 @@ class _View(C.Structure):
         ("hit_offset", _ip), ("hit_idx", _ip),
         ("n_selected", C.c_int64), ("n_sel_hits", C.c_int64), ("owner", _ip), ("n_own", _ip), ("sel_track", _ip),
         ("res_trk", _ip), ("res_y", _fp), ("res_z", _fp), ("q_y", C.POINTER(C.c_int16)), ("q_z", C.POINTER(C.c_int16)),
+        ("mg_stride", C.c_int64),
+        ("mg_next_sec", _ip), ("mg_next_trk", _ip), ("mg_prev_sec", _ip), ("mg_prev_trk", _ip),
+        ("mg_n_seg", _ip), ("mg_n_hits", _ip), ("mg_n_fit", _ip), ("mg_first_row", _ip), ("mg_last_row", _ip), ("mg_frame_seg", _ip),
+        ("mg_x_ref", _fp), ("mg_z_ref", _fp), ("mg_chi2", _fp), ("mg_par", _fp), ("mg_cov", _fp),
     ]
 
 
@@ -150,6 +157,12 @@ def _make_params(P):
     p.tc_max_gap = int(P.tc_max_gap); p.tc_min_hits = int(P.tc_min_hits)
     p.sel_max_shared_permille = int(getattr(P, "sel_max_shared_permille", 500))
     p.res_inv_quantum = float(getattr(P, "res_inv_quantum", 128.0))
+    p.sectors_per_side = int(getattr(P, "sectors_per_side", 18))
+    p.sector_cos = float(getattr(P, "sector_cos", np.float32(np.cos(np.pi / 9))))
+    p.sector_sin = float(getattr(P, "sector_sin", np.float32(np.sin(np.pi / 9))))
+    p.mg_max_row_gap = int(getattr(P, "mg_max_row_gap", 8))
+    p.mg_dy = float(getattr(P, "mg_dy", 1.0)); p.mg_dz = float(getattr(P, "mg_dz", 1.0))
+    p.mg_dsin = float(getattr(P, "mg_dsin", 0.05)); p.mg_zpre = float(getattr(P, "mg_zpre", 32.0))
     return p, keep
 
 
@@ -199,6 +212,7 @@ class SectorOutput:
     res_z: np.ndarray = None
     q_y: np.ndarray = None
     q_z: np.ndarray = None
+    merge: dict = None             # S8: per selected track: next_sec, next_trk, prev_sec, prev_trk, n_seg, ..., par, cov
 
     @property
     def n_tracks(self) -> int:
@@ -233,6 +247,15 @@ def output_from_view(v, what: int, n_rows: int) -> SectorOutput:
     if v.res_trk:
         o.res_trk = _np(v.res_trk, n, np.int32); o.res_y = _np(v.res_y, n, np.float32); o.res_z = _np(v.res_z, n, np.float32)
         o.q_y = _np(v.q_y, n, np.int16); o.q_z = _np(v.q_z, n, np.int16)
+    if v.mg_next_sec:
+        nk = int(v.n_selected)
+        o.merge = {f: _np(getattr(v, "mg_" + f), nk, np.int32) for f in ("next_sec", "next_trk", "prev_sec", "prev_trk", "n_seg",
+                                                                          "n_hits", "n_fit", "first_row", "last_row", "frame_seg")}
+        for f in ("x_ref", "z_ref", "chi2"):
+            o.merge[f] = _np(getattr(v, "mg_" + f), nk, np.float32)
+        ms = int(v.mg_stride)
+        o.merge["par"] = _np(v.mg_par, 5 * ms, np.float32).reshape(5, ms)[:, :nk].T.copy() if nk else np.empty((0, 5), np.float32)
+        o.merge["cov"] = _np(v.mg_cov, 15 * ms, np.float32).reshape(15, ms)[:, :nk].T.copy() if nk else np.empty((0, 15), np.float32)
     if v.x_ref:
         o.x_ref = _np(v.x_ref, nt, np.float32); o.z_ref = _np(v.z_ref, nt, np.float32)
         o.chi2 = _np(v.chi2, nt, np.float32)
@@ -358,8 +381,8 @@ class Tracker:
                     n_bins=int(out[4]), n_selected=int(out[5]), n_sel_hits=int(out[6]))
 
     def timings(self, runs_back: int = 0):
-        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, S1..S5, S6, S7]."""
-        out = (C.c_float * 8)()
+        """Per-stage device ms of a recent run (0 = last): [S1, S2, S3, S4, S5, S1..S5, S6, S7, S8]."""
+        out = (C.c_float * 9)()
         self._check(self._lib.tpcca_get_timings(self._h, int(runs_back), out))
         return [float(v) for v in out]
 

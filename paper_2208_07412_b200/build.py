@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpcca.so")
 SOURCES = ["tpcca_api.cu"]
-DEPS = ["tpcca_api.cu", "tpcca_pipeline.cuh", "tpcca_dev.cuh", "k_grid.cuh", "k_links.cuh", "k_tracklets.cuh", "k_select.cuh"]
+DEPS = ["tpcca_api.cu", "tpcca_pipeline.cuh", "tpcca_dev.cuh", "k_grid.cuh", "k_links.cuh", "k_tracklets.cuh", "k_select.cuh", "k_merge.cuh"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "--fmad=false", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",

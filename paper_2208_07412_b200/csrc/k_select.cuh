@@ -220,7 +220,8 @@ __device__ __forceinline__ int16_t res_quantise(float r, float inv_q) {
 __global__ void __launch_bounds__(128)
 k_residuals(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
             const float2* __restrict__ syz, const int32_t* __restrict__ row_start, const int32_t* __restrict__ owner,
-            SelOut sel, int32_t cap, ResOut o) {
+            SelOut sel, int32_t cap, ResOut o, float* __restrict__ out_x /*[cap]*/, float* __restrict__ out_p /*[5][cap]*/,
+            int32_t* __restrict__ out_ok /*[cap]: S8 needs the state on the last row*/) {
   const int ns = T->n_sectors, n_rows = T->n_rows;
   const int n_sel = st->sel_off[ns];
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -247,18 +248,22 @@ k_residuals(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   const int off = sec[s].off;
   const int32_t* rs = row_start + (size_t)s * (n_rows + 1);
   int r = sel.o.first_row[k];
+  bool walked = true;
   for (int q = 0; q < nh; ++q) {
     const int c = hl[q];
     while (r + 1 < n_rows && c >= __ldg(&rs[r + 1])) ++r;     // hits ascend in row
     const float2 h = __ldg(&syz[off + c]);
     KFJac J;
-    if (!kf_prop_mean(f, __ldg(&T->row_x[r]), K, J)) break;
+    if (!kf_prop_mean(f, __ldg(&T->row_x[r]), K, J)) { walked = false; break; }
     if (owner[off + c] != t_local) continue;
     const float ry = h.x - f.p0;
     const float rz = (h.y - z_ref) - f.p1;
     o.res_trk[off + c] = t_local; o.res_y[off + c] = ry; o.res_z[off + c] = rz;
     o.q_y[off + c] = res_quantise(ry, inv_q); o.q_z[off + c] = res_quantise(rz, inv_q);
   }
+  out_ok[k] = (walked && nh > 0) ? 1 : 0;
+  out_x[k] = f.x;
+  out_p[k] = f.p0; out_p[cs + k] = f.p1; out_p[2 * cs + k] = f.p2; out_p[3 * cs + k] = f.p3; out_p[4 * cs + k] = f.p4;
 }
 
 }  // namespace tpcca

@@ -2,6 +2,7 @@
 // caller's stream, per-stage CUDA events, error mapping.  No torch types, no CPU compute path:
 // every stage of the hot path runs in the kernels of k_grid.cuh / k_links.cuh / k_tracklets.cuh.
 #include <chrono>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -10,7 +11,7 @@
 #include <utility>
 #include <vector>
 
-#include "k_select.cuh"
+#include "k_merge.cuh"
 
 using namespace tpcca;
 
@@ -30,11 +31,24 @@ struct Layout {
   size_t tile_cnt, tile_off, start_bits;
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
-  size_t sel_n_own, sel_track, slot_trk;   // S6
-  size_t res_trk, res_y, res_z, res_qy, res_qz;   // S7 (its other buffers alias S1 / S5 scratch: see sel_* in tpcca_run)
+  size_t sel_n_own, sel_track, slot_trk;   // S6 (its other buffers alias S1 / S5 scratch: see sel_out)
+  size_t res_trk, res_y, res_z, res_qy, res_qz;   // S7
+  size_t mg_out, mg_ok, mg_cnt, mg_cur, mg_list, mg_keys, mg_links;   // S8 (chain outputs alias the parked-tracklet buffer)
+  int64_t mg_nzb;
   size_t total;
   int64_t n_tiles_max, nf_tiles_max, n_cb;
 };
+
+// S8 candidate index: z buckets of width max(mg_zpre, 8 cm, range / 4096) over the z range of the grid
+int64_t mg_z_buckets(const tpcca_params* p, float* lo, float* inv) {
+  double zmax = p->grid_z_lo;
+  for (int r = 0; r < p->n_rows; ++r) zmax = std::max(zmax, (double)p->grid_z_lo + (double)p->grid_nz[r] / (double)p->grid_inv_bin_z[r]);
+  const double range = std::max(zmax - (double)p->grid_z_lo, 1.0);
+  const double width = std::max({(double)p->mg_zpre, 8.0, range / 4096.0});
+  if (lo) *lo = p->grid_z_lo;
+  if (inv) *inv = (float)(1.0 / width);
+  return (int64_t)std::ceil(range / width) + 1;
+}
 
 int64_t bins_per_sector(const tpcca_params* p) {
   int64_t nb = 0;
@@ -120,6 +134,10 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.slot_trk = take(4 * (size_t)CS);     // start-hit slot -> global track (S5 gather), -1 = rejected
   L.res_trk = take(4 * (size_t)N); L.res_y = take(4 * (size_t)N); L.res_z = take(4 * (size_t)N);
   L.res_qy = take(2 * (size_t)N); L.res_qz = take(2 * (size_t)N);
+  L.mg_nzb = mg_z_buckets(p, nullptr, nullptr);
+  L.mg_out = take(4 * (size_t)(6 * CS)); L.mg_ok = take(4 * (size_t)CS);
+  L.mg_cnt = take(4 * (size_t)(ns * nr * L.mg_nzb + 2)); L.mg_cur = take(4 * (size_t)(ns * nr * L.mg_nzb + 2));
+  L.mg_list = take(4 * (size_t)CS); L.mg_keys = take(8 * (size_t)(2 * CS)); L.mg_links = take(4 * (size_t)(4 * CS));
   L.total = cur;
   return L;
 }
@@ -143,6 +161,8 @@ int check_params(const tpcca_params* p, std::string& err) {
   if (nb >= 0x7FFFFFF0) return fail("too many grid bins per sector");
   if (p->sel_max_shared_permille < 0 || p->sel_max_shared_permille > 1000) return fail("sel_max_shared_permille must be in 0..1000");
   if (!(p->res_inv_quantum > 0.0f)) return fail("res_inv_quantum must be > 0");
+  if (p->sectors_per_side < 0 || p->mg_max_row_gap < 0) return fail("sectors_per_side / mg_max_row_gap must be >= 0");
+  if (!(p->mg_dy > 0.0f) || !(p->mg_dz > 0.0f) || !(p->mg_dsin > 0.0f) || !(p->mg_zpre > 0.0f)) return fail("mg_dy / mg_dz / mg_dsin / mg_zpre must be > 0");
   return TPCCA_OK;
 }
 
@@ -180,7 +200,8 @@ struct tpcca_ctx {
   uint32_t done_mask = 0;             // stages whose outputs are valid for the loaded clusters
   bool desc_valid = false;
   static constexpr int kRing = 16;
-  cudaEvent_t ev[kRing][8]{};
+  cudaEvent_t ev[kRing][9]{};
+  MgParams mgp{};
   uint32_t ev_mask[kRing]{};          // stage mask of the run that used the slot (0 = unused)
   int64_t run_count = 0;
   char* arena = nullptr;              // pinned host arena of tpcca_get_tracks(HOST)
@@ -278,6 +299,26 @@ SelOut sel_out(const tpcca_ctx* c) {
   return so;
 }
 
+// S8 buffers; the per-chain outputs (29 planes of CS words) alias the parked-tracklet buffer behind the selected
+// table's hit_offset (free after S5, like the rest of the S6 tables)
+MgBuf mg_buf(const tpcca_ctx* c) {
+  static_assert(kHsV * 16 >= 4 + 29 * 4 + 8, "chain outputs fit the parked-tracklet buffer");
+  const Layout& L = c->L;
+  const size_t cs = (size_t)c->CS;
+  MgBuf b;
+  b.out_x = c->at<float>(L.mg_out); b.out_p = b.out_x + cs; b.out_ok = c->at<int32_t>(L.mg_ok);
+  b.bk_cnt = c->at<uint32_t>(L.mg_cnt); b.bk_list = c->at<int32_t>(L.mg_list);
+  b.next_key = c->at<unsigned long long>(L.mg_keys); b.prev_key = b.next_key + cs;
+  int32_t* l = c->at<int32_t>(L.mg_links);
+  b.next_sec = l; b.next_trk = l + cs; b.prev_sec = l + 2 * cs; b.prev_trk = l + 3 * cs;
+  char* base = c->ws + L.hs + align_up(4 * (cs + (size_t)c->ns + 1));
+  int32_t* i32 = reinterpret_cast<int32_t*>(base);
+  float* f = reinterpret_cast<float*>(base);
+  b.n_seg = i32; b.n_hits = i32 + cs; b.n_fit = i32 + 2 * cs; b.first_row = i32 + 3 * cs; b.last_row = i32 + 4 * cs; b.frame_seg = i32 + 5 * cs;
+  b.x_ref = f + 6 * cs; b.z_ref = f + 7 * cs; b.chi2 = f + 8 * cs; b.par = f + 9 * cs; b.cov = f + 14 * cs;
+  return b;
+}
+
 ResOut res_out(const tpcca_ctx* c) {
   const Layout& L = c->L;
   ResOut ro;
@@ -348,6 +389,12 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   memset(&t, 0, sizeof t);
   t.n_rows = p->n_rows; t.n_sectors = p->n_sectors; t.bins_per_sector = (int32_t)c->nb;
   t.tc_max_gap = p->tc_max_gap; t.tc_min_hits = p->tc_min_hits; t.sel_permille = p->sel_max_shared_permille; t.res_inv_q = p->res_inv_quantum;
+  {
+    MgParams& m = c->mgp;
+    m.per_side = p->sectors_per_side; m.max_row_gap = p->mg_max_row_gap; m.ca = p->sector_cos; m.sa = p->sector_sin;
+    m.dy = p->mg_dy; m.dz = p->mg_dz; m.ds = p->mg_dsin; m.zpre = p->mg_zpre;
+    m.n_zb = (int32_t)mg_z_buckets(p, &m.zb_lo, &m.zb_inv);
+  }
   t.grid_z_lo = p->grid_z_lo; t.Bc = p->kappa_per_qpt; t.err2_y = p->err2_y; t.err2_z = p->err2_z;
   for (int i = 0; i < 5; ++i) t.init_cov[i] = p->init_cov[i];
   t.win_y = p->tc_win_y; t.win_z = p->tc_win_z; t.gate = p->tc_gate; t.max_sinphi = p->max_sinphi;
@@ -406,7 +453,7 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(c->stream);
   if (e1 == cudaSuccess) e1 = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
   for (int k = 0; k < tpcca_ctx::kRing && e1 == cudaSuccess; ++k)
-    for (int i = 0; i < 8 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
+    for (int i = 0; i < 9 && e1 == cudaSuccess; ++i) e1 = cudaEventCreate(&c->ev[k][i]);
   if (e1 != cudaSuccess) {
     set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: %s", cudaGetErrorString(e1));
     tpcca_destroy(c);
@@ -480,10 +527,10 @@ int tpcca_load_clusters(tpcca_ctx* c, int sector, int64_t n, const float* x, con
 
 int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   if (!c) return TPCCA_E_ARG;
-  mask &= (TPCCA_STAGE_ALL | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS);
+  mask &= (TPCCA_STAGE_ALL | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS | TPCCA_STAGE_MERGE);
   if (!mask) return set_err(c, TPCCA_E_ARG, "empty stage mask");
   // a stage needs everything before it
-  for (int i = 0; i < 7; ++i)
+  for (int i = 0; i < 8; ++i)
     if (mask & (1u << i)) {
       const uint32_t need = (1u << i) - 1u;
       if ((need & ~(c->done_mask | mask)) != 0)
@@ -527,7 +574,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   const int slot_ev = (int)(c->run_count % tpcca_ctx::kRing);
   c->ev_mask[slot_ev] = 0;
   // end of a stage: its event, and the launch errors of ITS kernels (so a failed launch names its stage)
-  static const char* const kStageName[8] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets", "S6 selector", "S7 residuals"};
+  static const char* const kStageName[9] = {"start", "S1 grid", "S2 neighbours", "S3 clean", "S4 start hits", "S5 tracklets", "S6 selector", "S7 residuals", "S8 merge"};
   cudaError_t stage_err = cudaSuccess;
   int stage_bad = -1;
   auto mark = [&](int i) {
@@ -689,17 +736,37 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     const ResOut ro = res_out(c);
     const size_t nk = (size_t)std::max<int64_t>(c->n_total, 1);
     k_res_init<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(ro, nk);
-    k_residuals<<<(unsigned)((c->CS + 127) / 128), 128, 0, st>>>(T, sec, status, syz, row_start, c->at<int32_t>(L.rec), sel_out(c), cap, ro);
+    const MgBuf mb = mg_buf(c);
+    k_residuals<<<(unsigned)((c->CS + 127) / 128), 128, 0, st>>>(T, sec, status, syz, row_start, c->at<int32_t>(L.rec), sel_out(c), cap, ro,
+                                                                 mb.out_x, mb.out_p, mb.out_ok);
     c->launches += 2;
   }
   mark(7);
+  if (mask & TPCCA_STAGE_MERGE) {
+    const MgBuf mb = mg_buf(c);
+    const SelOut so = sel_out(c);
+    const size_t nbk = (size_t)c->ns * c->nr * c->mgp.n_zb + 1;
+    uint32_t* cursor = c->at<uint32_t>(L.mg_cur);
+    const unsigned g256 = (unsigned)((c->CS + 255) / 256), g128 = (unsigned)((c->CS + 127) / 128);
+    k_zero_words<<<(unsigned)std::min<size_t>((nbk + 1023) / 1024, (size_t)c->sm_count * 8), 256, 0, st>>>(mb.bk_cnt, nbk + 1);
+    k_zero_words<<<(unsigned)std::min<size_t>((nbk + 1023) / 1024, (size_t)c->sm_count * 8), 256, 0, st>>>(cursor, nbk + 1);
+    k_mg_count<<<g256, 256, 0, st>>>(T, status, so, cap, c->mgp, mb);
+    k_mg_scan<<<1, 1024, 0, st>>>(mb.bk_cnt, (int)(nbk - 1));
+    k_mg_scatter<<<g256, 256, 0, st>>>(T, status, so, cap, c->mgp, mb, cursor);
+    k_mg_match<<<g128, 128, 0, st>>>(T, status, so, cap, c->mgp, mb);
+    k_mg_link<<<g256, 256, 0, st>>>(T, status, mb);
+    k_mg_refit<<<g128, 128, 0, st>>>(T, sec, status, syz, row_start, so, cap, c->mgp, mb);
+    c->launches += 8;
+  }
+  mark(8);
   if (stage_err != cudaSuccess)
     return set_err(c, TPCCA_E_CUDA, "tpcca_run: stage %s failed: %s", kStageName[stage_bad], cudaGetErrorString(stage_err));
   c->ev_mask[slot_ev] = mask;
   ++c->run_count;
   // S6's outputs alias S1 / S5 scratch: re-running either without S6 leaves no valid selection
-  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS)) && !(mask & TPCCA_STAGE_SELECT)) c->done_mask &= ~(TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS);
-  if ((mask & TPCCA_STAGE_SELECT) && !(mask & TPCCA_STAGE_RESIDUALS)) c->done_mask &= ~TPCCA_STAGE_RESIDUALS;
+  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS)) && !(mask & TPCCA_STAGE_SELECT)) c->done_mask &= ~(TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS | TPCCA_STAGE_MERGE);
+  if ((mask & TPCCA_STAGE_SELECT) && !(mask & TPCCA_STAGE_RESIDUALS)) c->done_mask &= ~(TPCCA_STAGE_RESIDUALS | TPCCA_STAGE_MERGE);
+  if ((mask & (TPCCA_STAGE_GRID | TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_RESIDUALS)) && !(mask & TPCCA_STAGE_MERGE)) c->done_mask &= ~TPCCA_STAGE_MERGE;
   c->done_mask |= mask;
   return TPCCA_OK;
 }
@@ -725,10 +792,10 @@ int tpcca_get_counts(tpcca_ctx* c, int64_t out[7]) {
   return TPCCA_OK;
 }
 
-int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[8]) {
+int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[9]) {
   if (!c || !ms) return TPCCA_E_ARG;
   if (runs_back < 0 || runs_back >= tpcca_ctx::kRing) return set_err(c, TPCCA_E_ARG, "runs_back must be in 0..15");
-  for (int i = 0; i < 8; ++i) ms[i] = 0.f;
+  for (int i = 0; i < 9; ++i) ms[i] = 0.f;
   if (runs_back >= c->run_count) return set_err(c, TPCCA_E_STATE, "no such run");
   const int k = (int)((c->run_count - 1 - runs_back) % tpcca_ctx::kRing);
   if (!c->ev_mask[k]) return set_err(c, TPCCA_E_STATE, "no such run");
@@ -738,6 +805,7 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[8]) {
   CU(c, cudaEventElapsedTime(&ms[5], c->ev[k][0], c->ev[k][5]));
   CU(c, cudaEventElapsedTime(&ms[6], c->ev[k][5], c->ev[k][6]));
   CU(c, cudaEventElapsedTime(&ms[7], c->ev[k][6], c->ev[k][7]));
+  CU(c, cudaEventElapsedTime(&ms[8], c->ev[k][7], c->ev[k][8]));
   return TPCCA_OK;
 }
 
@@ -781,6 +849,7 @@ static int get_tracks_range(tpcca_ctx* c, int sec0, int sec1, int mem_space, uin
   if (what & TPCCA_OUT_TRACKS) need_stage = 5;
   if ((what & (TPCCA_OUT_SELECTION | TPCCA_OUT_TRACKS_SEL)) && (c->done_mask & TPCCA_STAGE_SELECT)) need_stage = 6;
   if ((what & TPCCA_OUT_RESIDUALS) && (c->done_mask & TPCCA_STAGE_RESIDUALS)) need_stage = 7;
+  if ((what & TPCCA_OUT_MERGE) && (c->done_mask & TPCCA_STAGE_MERGE)) need_stage = 8;
   if ((what & TPCCA_OUT_TRACKS) && (what & TPCCA_OUT_TRACKS_SEL))
     return set_err(c, TPCCA_E_ARG, "TPCCA_OUT_TRACKS and TPCCA_OUT_TRACKS_SEL fill the same fields: ask for one");
   while (need_stage > 1 && need_stage <= 5 && !(c->done_mask & (1u << (need_stage - 1)))) --need_stage;     // stages that were never run deliver nothing
@@ -799,7 +868,7 @@ static int get_tracks_range(tpcca_ctx* c, int sec0, int sec1, int mem_space, uin
   tpcca_tracks_view* v = views + (sector - sec0);
   memset(v, 0, sizeof *v);
   const int64_t n = c->desc[sector].n, off = c->desc[sector].off;
-  const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS)) : c->done_mask;
+  const uint32_t done = partial ? (c->done_mask & ~(TPCCA_STAGE_TRACKLETS | TPCCA_STAGE_SELECT | TPCCA_STAGE_RESIDUALS | TPCCA_STAGE_MERGE)) : c->done_mask;
   v->n_clusters = n;
   v->n_bins = c->nb;
   int64_t s0 = 0, s1 = 0, t0 = 0, nt = 0, h0 = 0, h1 = 0;
@@ -874,6 +943,20 @@ static int get_tracks_range(tpcca_ctx* c, int sec0, int sec1, int mem_space, uin
     add((const void* const*)&v->q_y, ro.q_y + off, 2 * (size_t)n);
     add((const void* const*)&v->q_z, ro.q_z + off, 2 * (size_t)n);
   }
+  if ((done & TPCCA_STAGE_MERGE) && (what & TPCCA_OUT_MERGE)) {
+    const MgBuf mb = mg_buf(c);
+    const int64_t k0 = S.sel_off[sector], nk = S.sel_off[sector + 1] - k0;
+    const size_t by = 4 * (size_t)nk;
+    add((const void* const*)&v->mg_next_sec, mb.next_sec + k0, by); add((const void* const*)&v->mg_next_trk, mb.next_trk + k0, by);
+    add((const void* const*)&v->mg_prev_sec, mb.prev_sec + k0, by); add((const void* const*)&v->mg_prev_trk, mb.prev_trk + k0, by);
+    add((const void* const*)&v->mg_n_seg, mb.n_seg + k0, by); add((const void* const*)&v->mg_n_hits, mb.n_hits + k0, by);
+    add((const void* const*)&v->mg_n_fit, mb.n_fit + k0, by); add((const void* const*)&v->mg_first_row, mb.first_row + k0, by);
+    add((const void* const*)&v->mg_last_row, mb.last_row + k0, by); add((const void* const*)&v->mg_frame_seg, mb.frame_seg + k0, by);
+    add((const void* const*)&v->mg_x_ref, mb.x_ref + k0, by); add((const void* const*)&v->mg_z_ref, mb.z_ref + k0, by);
+    add((const void* const*)&v->mg_chi2, mb.chi2 + k0, by);
+    add((const void* const*)&v->mg_par, mb.par + k0, by, 5); add((const void* const*)&v->mg_cov, mb.cov + k0, by, 15);
+    v->mg_stride = host ? nk : c->CS;
+  }
   }   // sectors
   if (!host) {
     for (auto& it : items) *it.dst = it.src;
@@ -925,7 +1008,7 @@ void tpcca_destroy(tpcca_ctx* c) {
   DeviceGuard guard(c->device);
   cudaStreamSynchronize(c->stream);
   for (int k = 0; k < tpcca_ctx::kRing; ++k)
-    for (int i = 0; i < 8; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
+    for (int i = 0; i < 9; ++i) if (c->ev[k][i]) cudaEventDestroy(c->ev[k][i]);
   if (c->arena) cudaFreeHost(c->arena);
   if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
   delete c;

@@ -175,3 +175,63 @@ def compare_residuals(tracker, tf, oracle_obj, sectors=None) -> dict:
             raise ParityError(f"sector {s}: {e}") from None
         tot["sectors"] += 1; tot["n_clusters"] += int(o.n); tot["n_attached"] += int((o.res_trk >= 0).sum())
     return tot
+
+
+def compare_merge(tracker, tf, precision="f32") -> dict:
+    """S8 (cross-sector merging + chain refit): the links per selected track bit-exact; per chain head the segment
+    count, hit counts, rows, reference plane bit-exact and the refitted parameters / covariance / chi2 within the
+    1e-4 bar of N5 (same operation order: observed bit-exact is reported)."""
+    from oracle import run_timeframe_merged
+    from paper_2208_07412_b200 import binding as B
+    res, mg = run_timeframe_merged(tf, precision)
+    tot = dict(sectors=0, n_selected=0, n_links=0, n_chains=0, par_bit_exact=True, cov_bit_exact=True)
+    for s in range(tf.n_sectors):
+        g = tracker.get_tracks(s, B.OUT_MERGE | B.OUT_SELECTION).merge
+        m = mg[s]
+        rep = {}
+        try:
+            if g is None:
+                raise ParityError("no S8 outputs delivered")
+            for f in ("next_sec", "next_trk", "prev_sec", "prev_trk"):
+                _eq("mg_" + f, g[f], getattr(m, f), rep)
+            nk = len(m.next_sec)
+            n_seg = np.zeros(nk, np.int32); n_seg[m.head] = m.n_seg
+            _eq("mg_n_seg", g["n_seg"], n_seg, rep)
+            h = m.head
+            for f in ("n_hits", "n_fit", "first_row", "last_row", "frame_seg"):
+                _eq("mg_" + f, g[f][h], getattr(m, f), rep)
+            _eq("mg_x_ref", g["x_ref"][h], m.x_ref.astype(np.float32), rep)
+            _eq("mg_z_ref", g["z_ref"][h], m.z_ref.astype(np.float32), rep)
+            # the chain of every head, rebuilt from the GPU's links, equals the oracle's segment list
+            for k, ih in enumerate(h):
+                segs = [(s, int(ih))]
+                while True:
+                    a, b = segs[-1]
+                    ma = mg[a]
+                    if ma.next_sec[b] < 0:
+                        break
+                    segs.append((int(ma.next_sec[b]), int(ma.next_trk[b])))
+                want = list(zip(m.seg_sec[m.seg_offset[k]:m.seg_offset[k + 1]].tolist(), m.seg_trk[m.seg_offset[k]:m.seg_offset[k + 1]].tolist()))
+                if segs != want:
+                    raise ParityError(f"chain of head {ih}: {segs} vs {want}")
+            if len(h):
+                gp = g["par"][h].astype(np.float64); op = m.par
+                tol = 1e-4 * np.maximum(np.maximum(np.abs(gp), np.abs(op)), PAR_FLOOR[None, :])
+                if (np.abs(gp - op) > tol).any():
+                    t, i = np.argwhere(np.abs(gp - op) > tol)[0]
+                    raise ParityError(f"mg_par[{t},{i}]: gpu {gp[t, i]} oracle {op[t, i]}")
+                gc = g["cov"][h].astype(np.float64); oc = m.cov
+                diag = np.stack([oc[:, i * (i + 1) // 2 + i] for i in range(5)], axis=1)
+                for kk, (i, j) in enumerate(TRI):
+                    lim = 1e-4 * np.sqrt(np.abs(diag[:, i] * diag[:, j]))
+                    if (np.abs(gc[:, kk] - oc[:, kk]) > lim).any():
+                        raise ParityError(f"mg_cov[{kk}] differs")
+                g2 = g["chi2"][h].astype(np.float64)
+                if (np.abs(g2 - m.chi2) > 1e-4 * np.maximum(np.maximum(np.abs(g2), np.abs(m.chi2)), 1e-3)).any():
+                    raise ParityError("mg_chi2 differs")
+                tot["par_bit_exact"] &= bool(np.array_equal(g["par"][h], op.astype(np.float32)))
+                tot["cov_bit_exact"] &= bool(np.array_equal(g["cov"][h], oc.astype(np.float32)))
+        except ParityError as e:
+            raise ParityError(f"sector {s}: {e}") from None
+        tot["sectors"] += 1; tot["n_selected"] += nk; tot["n_links"] += int((m.next_sec >= 0).sum()); tot["n_chains"] += len(h)
+    return tot

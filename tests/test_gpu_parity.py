@@ -600,3 +600,47 @@ def test_get_tracks_all_equals_per_sector(pkg, cfg1_small):
         for f in ("order", "link_up", "start_hit", "par", "cov", "hit_idx", "hit_offset"):
             assert np.array_equal(getattr(allv[s], f), getattr(one, f)), f
     trk.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# S8 cross-sector merging + chain refit
+# ------------------------------------------------------------------------------------------------
+def test_merge_config1_and_config4(pkg, cfg1_small):
+    from parity import compare_merge
+    for tf in (cfg1_small, tpcsynth.generate(1, n_tracks=4000), tpcsynth.generate(4, n_tracks=2500)):
+        trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters, workspace_fill=WS_FILL)
+        trk.load_timeframe(tf)
+        trk.run(0xFF)
+        trk.sync()
+        rep = compare_merge(trk, tf)
+        assert rep["n_links"] > 0.2 * rep["n_selected"] and rep["n_chains"] > 0
+        assert trk.timings()[8] > 0.0
+        compare_timeframe(trk, tf, Oracle(tf.params), sectors=(0, 19))       # S1-S5 outputs untouched by S6-S8
+        trk.close()
+
+
+def test_merge_time_frame_and_degenerate_layouts(pkg):
+    """Several collisions along the 128-orbit z axis (candidate index over 900+ z buckets); sector layouts without a
+    neighbour relation (1 or 3 sectors: S8 is a no-op) and with two sectors per side."""
+    from parity import compare_merge
+    T = 128 * tpcsynth.ORBIT_US
+    tf = tpcsynth.generate(3, coll_times=[0.0, 0.2 * T, 0.2 * T + 9.0, 0.77 * T, T], coll_mult=900)
+    trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+    trk.load_timeframe(tf)
+    trk.run(0xFF)
+    trk.sync()
+    rep = compare_merge(trk, tf)
+    assert rep["n_links"] > 500
+    trk.close()
+    base = tpcsynth.generate(1, n_tracks=1500)
+    for nsec, per in ((1, 18), (3, 18), (4, 2), (6, 3)):
+        P = base.params.copy(n_sectors=nsec, sectors_per_side=per)
+        tf2 = ArrTF(P, [(base.y[s], base.z[s], base.row[s]) for s in range(nsec)])
+        trk = pkg.Tracker(P, max_clusters=tf2.n_clusters)
+        trk.load_timeframe(tf2)
+        trk.run(0xFF)
+        trk.sync()
+        rep = compare_merge(trk, tf2)
+        if nsec % per:
+            assert rep["n_links"] == 0
+        trk.close()

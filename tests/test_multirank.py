@@ -113,7 +113,7 @@ class _FakeTracker:
 
     def timings(self, i=0):
         t = self.env.step_ms
-        return [0.1 * t, 0.1 * t, 0.05 * t, 0.05 * t, 0.7 * t, t, 0.02 * t, 0.01 * t]
+        return [0.1 * t, 0.1 * t, 0.05 * t, 0.05 * t, 0.7 * t, t, 0.02 * t, 0.01 * t, 0.01 * t]
 
     def work_counters(self):
         return dict(propagations=10, updates=10, gates=1, searches=5, candidates=9)
