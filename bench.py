@@ -433,6 +433,8 @@ def run_tpcca(args, env_cls=CudaEnv):
     counts_sel = trk.counts()
     trk.run(0x40)                       # S7 residual front end on the same time frame (outside every timed region)
     s7_ms = float(trk.timings(0)[7])
+    trk.run(0x80)                       # S8 cross-sector merging + chain refit
+    s8_ms = float(trk.timings(0)[8])
 
     # (b) streaming (the EPN operating mode: time frames follow each other): two contexts on two
     # streams, each step still does its own H2D, S1-S5 and D2H, but the copies of one time frame overlap the
@@ -544,7 +546,7 @@ def run_tpcca(args, env_cls=CudaEnv):
                      ms_per_step=e2e_ms / e2e_steps, mode=e2e_mode,
                      serial_value=n_all * e2e_steps_serial / (e2e_serial_ms * 1e-3),
                      serial_ms_per_step=e2e_serial_ms / e2e_steps_serial, pipelined=pipe_res),
-            selector=dict(stage_ms_S6=round(s6_ms, 4), stage_ms_S7_residuals=round(s7_ms, 4), n_selected=counts_sel["n_selected"], n_sel_hits=counts_sel["n_sel_hits"],
+            selector=dict(stage_ms_S6=round(s6_ms, 4), stage_ms_S7_residuals=round(s7_ms, 4), stage_ms_S8_merge=round(s8_ms, 4), n_selected=counts_sel["n_selected"], n_sel_hits=counts_sel["n_sel_hits"],
                           note="S6 (SURVEY 8(f)-1) is outside the timed step; e2e_selected = serial step S1-S6 shipping the "
                                "selected tracks + owner instead of every tracklet",
                           e2e_selected=dict(value=n_all * e2e_steps_serial / (e2e_sel_serial_ms * 1e-3), unit=UNIT,
