@@ -80,10 +80,18 @@ extern "C" {
 #define TPCCA_OUT_TRACKS_SEL 0x80u  /* the track table + hit CSR of the SELECTED tracks only (S6): fills the S5    */
                                     /* fields of the view from the compact table (array lengths: n_selected and    */
                                     /* n_sel_hits instead of n_tracks and n_hits); not together with OUT_TRACKS   */
-#define TPCCA_OUT_RESIDUALS  0x100u /* res_trk, res_y, res_z, q_y, q_z            (S7)            */
+#define TPCCA_OUT_RESIDUALS  0x100u /* res (tpcca_residual records)                (S7)            */
 #define TPCCA_OUT_MERGE      0x200u /* mg_* links and merged chains               (S8)            */
 
 typedef struct tpcca_ctx tpcca_ctx;   /* opaque; owned by the library */
+
+/* S7: one 16-byte record per cluster (sorted position): the selected track the cluster is attached to and its
+ * residuals to that track's helix at the cluster's pad row. */
+typedef struct {
+  int32_t trk;            /* sector-local number of the SELECTED track owning the cluster; -1: none (stored raw)   */
+  float   res_y, res_z;   /* y_c - y_track, (z_c - z_ref) - z_track; 0 if trk == -1                                */
+  int16_t q_y, q_z;       /* rint(res * res_inv_quantum) (round half to even), clamped to +-32767                  */
+} tpcca_residual;
 
 /* Tracker tables (DESIGN.md 3 "Derived tables").  All table pointers are HOST arrays of length
  * n_rows, owned by the caller and copied by tpcca_create.  The tables are DATA: geometry, grid,
@@ -162,9 +170,7 @@ typedef struct {
   const int32_t  *n_own;      /* [n_tracks] hits of each S5 track that the track owns            */
   const int32_t  *sel_track;  /* [n_selected] ascending sector-local numbers of the selected     */
   /* S7: residual front end, per cluster (sorted position) */
-  const int32_t  *res_trk;    /* [n_clusters] selected track (sector-local number) the cluster is attached to; -1 */
-  const float    *res_y, *res_z;   /* [n_clusters] y_c - y_track, z_c - z_track at the cluster's row; 0 if -1    */
-  const int16_t  *q_y, *q_z;  /* [n_clusters] rint(res * res_inv_quantum), clamped to +-32767    */
+  const tpcca_residual *res;  /* [n_clusters] one record per cluster                              */
   /* S8, per SELECTED track of the sector (n_selected entries each): the partner segment in a
    * neighbour sector above / below (sector, selected-track number there; -1 none), and -- for tracks that are the
    * lowest segment of a chain of >= 2 segments (mg_n_seg > 0) -- the Kalman refit over all hits of the chain,

@@ -67,13 +67,16 @@ class _View(C.Structure):
         ("n_hits_trk", _ip), ("n_fit", _ip), ("first_row", _ip), ("last_row", _ip), ("trk_start_hit", _ip),
         ("hit_offset", _ip), ("hit_idx", _ip),
         ("n_selected", C.c_int64), ("n_sel_hits", C.c_int64), ("owner", _ip), ("n_own", _ip), ("sel_track", _ip),
-        ("res_trk", _ip), ("res_y", _fp), ("res_z", _fp), ("q_y", C.POINTER(C.c_int16)), ("q_z", C.POINTER(C.c_int16)),
+        ("res", C.c_void_p),
         ("mg_stride", C.c_int64),
         ("mg_next_sec", _ip), ("mg_next_trk", _ip), ("mg_prev_sec", _ip), ("mg_prev_trk", _ip),
         ("mg_n_seg", _ip), ("mg_n_hits", _ip), ("mg_n_fit", _ip), ("mg_first_row", _ip), ("mg_last_row", _ip), ("mg_frame_seg", _ip),
         ("mg_x_ref", _fp), ("mg_z_ref", _fp), ("mg_chi2", _fp), ("mg_par", _fp), ("mg_cov", _fp),
     ]
 
+
+#: numpy view of tpcca_residual (include/tpcca.h)
+RESIDUAL_DTYPE = np.dtype([("trk", np.int32), ("res_y", np.float32), ("res_z", np.float32), ("q_y", np.int16), ("q_z", np.int16)])
 
 _lib = None
 
@@ -244,9 +247,9 @@ def output_from_view(v, what: int, n_rows: int) -> SectorOutput:
     if v.owner:
         o.owner = _np(v.owner, n, np.int32); o.n_own = _np(v.n_own, int(v.n_tracks), np.int32)
         o.selected = _np(v.sel_track, int(v.n_selected), np.int32)
-    if v.res_trk:
-        o.res_trk = _np(v.res_trk, n, np.int32); o.res_y = _np(v.res_y, n, np.float32); o.res_z = _np(v.res_z, n, np.float32)
-        o.q_y = _np(v.q_y, n, np.int16); o.q_z = _np(v.q_z, n, np.int16)
+    if v.res:
+        rec = np.frombuffer((C.c_char * (16 * n)).from_address(v.res), dtype=RESIDUAL_DTYPE, count=n) if n else np.empty(0, RESIDUAL_DTYPE)
+        o.res_trk, o.res_y, o.res_z, o.q_y, o.q_z = (np.ascontiguousarray(rec[f]) for f in ("trk", "res_y", "res_z", "q_y", "q_z"))
     if v.mg_next_sec:
         nk = int(v.n_selected)
         o.merge = {f: _np(getattr(v, "mg_" + f), nk, np.int32) for f in ("next_sec", "next_trk", "prev_sec", "prev_trk", "n_seg",

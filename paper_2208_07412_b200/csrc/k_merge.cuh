@@ -83,23 +83,26 @@ k_mg_count(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, Se
   B.next_sec[k] = -1; B.next_trk[k] = -1; B.prev_sec[k] = -1; B.prev_trk[k] = -1; B.n_seg[k] = 0;
 }
 
-// exclusive scan of n counters in place (one block; n up to a few million: ~n / 1024 rounds)
+// exclusive scan of the bucket counters in place, one block per sector: the first bucket of sector s starts at
+// sel_off[s] (every selected track of the sector sits in one of its buckets), so the sectors need no carry
 __global__ void __launch_bounds__(1024)
-k_mg_scan(uint32_t* __restrict__ cnt, int n) {
+k_mg_scan(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, uint32_t* __restrict__ cnt, int per_sector) {
   __shared__ uint32_t ws[33];
-  uint32_t carry = 0;
-  for (int b0 = 0; b0 < n; b0 += 8192) {
+  const int s = blockIdx.x;
+  uint32_t* c = cnt + (size_t)s * per_sector;
+  uint32_t carry = (uint32_t)st->sel_off[s];
+  for (int b0 = 0; b0 < per_sector; b0 += 8192) {
     const int i0 = b0 + threadIdx.x * 8;
     uint32_t v[8], sum = 0;
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { v[j] = (i0 + j < n) ? cnt[i0 + j] : 0u; sum += v[j]; }
+    for (int j = 0; j < 8; ++j) { v[j] = (i0 + j < per_sector) ? c[i0 + j] : 0u; sum += v[j]; }
     uint32_t total;
     uint32_t run = carry + block_exclusive_scan<uint32_t>(sum, ws, total);
 #pragma unroll
-    for (int j = 0; j < 8; ++j) { if (i0 + j < n) cnt[i0 + j] = run; run += v[j]; }
+    for (int j = 0; j < 8; ++j) { if (i0 + j < per_sector) c[i0 + j] = run; run += v[j]; }
     carry += total;
   }
-  if (threadIdx.x == 0) cnt[n] = carry;
+  if (s == T->n_sectors - 1 && threadIdx.x == 0) c[per_sector] = carry;      // closing entry
 }
 
 // pass 2: scatter (the order inside a bucket is arbitrary: no result depends on it)
@@ -196,15 +199,31 @@ k_mg_link(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, MgB
   }
 }
 
+// ---- K8c': the heads of chains (no partner below, one above), compacted (any order: outputs are indexed by the head)
+__global__ void __launch_bounds__(256)
+k_mg_heads(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, MgBuf B, int32_t* __restrict__ head_list,
+           uint32_t* __restrict__ n_heads) {
+  const int n_sel = st->sel_off[T->n_sectors];
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool head = k < n_sel && B.prev_sec[k] == -1 && B.next_sec[k] != -1;
+  const unsigned m = __ballot_sync(0xffffffffu, head);
+  if (!m) return;
+  const int lane = threadIdx.x & 31;
+  uint32_t base = 0;
+  if (lane == 0) base = atomicAdd(n_heads, (uint32_t)__popc(m));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (head) head_list[base + __popc(m & ((1u << lane) - 1u))] = k;
+}
+
 // ---- K8d: refit of the chains.  One thread per chain head --------------------------------------------------------
 __global__ void __launch_bounds__(128)
 k_mg_refit(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
-           const float2* __restrict__ syz, const int32_t* __restrict__ row_start, SelOut sel, int32_t cap, MgParams M, MgBuf B) {
+           const float2* __restrict__ syz, const int32_t* __restrict__ row_start, SelOut sel, int32_t cap, MgParams M, MgBuf B,
+           const int32_t* __restrict__ head_list, const uint32_t* __restrict__ n_heads) {
   const int ns = T->n_sectors, nr = T->n_rows;
-  const int n_sel = st->sel_off[ns];
-  const int kh = blockIdx.x * blockDim.x + threadIdx.x;
-  if (kh >= n_sel) return;
-  if (B.prev_sec[kh] != -1 || B.next_sec[kh] == -1) return;
+  const int ih = blockIdx.x * blockDim.x + threadIdx.x;
+  if (ih >= (int)*n_heads) return;
+  const int kh = head_list[ih];
   const size_t cs = (size_t)cap;
   // walk up to the top segment
   int n_seg = 1, ktop = kh;

@@ -193,19 +193,12 @@ k_sel_owner(uint32_t* __restrict__ key_owner, size_t n) {
 
 // ---- S7: track-residual front end --------------------------------------
 // Per cluster: res_trk = the SELECTED track owning it (-1: none), residuals to that track's helix, quantised.
-struct ResOut {
-  int32_t* res_trk;     // [N]
-  float* res_y;         // [N]
-  float* res_z;         // [N]
-  int16_t* q_y;         // [N]
-  int16_t* q_z;         // [N]
-};
+static_assert(sizeof(tpcca_residual) == 16, "tpcca_residual is one 16-byte record");
 
 __global__ void __launch_bounds__(256)
-k_res_init(ResOut o, size_t n) {
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    o.res_trk[i] = -1; o.res_y[i] = 0.0f; o.res_z[i] = 0.0f; o.q_y[i] = 0; o.q_z[i] = 0;
-  }
+k_res_init(tpcca_residual* __restrict__ o, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    reinterpret_cast<int4*>(o)[i] = make_int4(-1, 0, 0, 0);
 }
 
 __device__ __forceinline__ int16_t res_quantise(float r, float inv_q) {
@@ -220,7 +213,7 @@ __device__ __forceinline__ int16_t res_quantise(float r, float inv_q) {
 __global__ void __launch_bounds__(128)
 k_residuals(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, const DevStatus* __restrict__ st,
             const float2* __restrict__ syz, const int32_t* __restrict__ row_start, const int32_t* __restrict__ owner,
-            SelOut sel, int32_t cap, ResOut o, float* __restrict__ out_x /*[cap]*/, float* __restrict__ out_p /*[5][cap]*/,
+            SelOut sel, int32_t cap, tpcca_residual* __restrict__ o, float* __restrict__ out_x /*[cap]*/, float* __restrict__ out_p /*[5][cap]*/,
             int32_t* __restrict__ out_ok /*[cap]: S8 needs the state on the last row*/) {
   const int ns = T->n_sectors, n_rows = T->n_rows;
   const int n_sel = st->sel_off[ns];
@@ -249,17 +242,23 @@ k_residuals(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
   const int32_t* rs = row_start + (size_t)s * (n_rows + 1);
   int r = sel.o.first_row[k];
   bool walked = true;
+  // the hit, its cluster and its owner are read one step ahead of the transport (their latency is off the chain)
+  int c_n = nh > 0 ? hl[0] : 0;
+  float2 h_n = nh > 0 ? __ldg(&syz[off + c_n]) : make_float2(0.f, 0.f);
+  int own_n = nh > 0 ? owner[off + c_n] : -1;
   for (int q = 0; q < nh; ++q) {
-    const int c = hl[q];
+    const int c = c_n;
+    const float2 h = h_n;
+    const int own = own_n;
+    if (q + 1 < nh) { c_n = hl[q + 1]; h_n = __ldg(&syz[off + c_n]); own_n = owner[off + c_n]; }
     while (r + 1 < n_rows && c >= __ldg(&rs[r + 1])) ++r;     // hits ascend in row
-    const float2 h = __ldg(&syz[off + c]);
     KFJac J;
     if (!kf_prop_mean(f, __ldg(&T->row_x[r]), K, J)) { walked = false; break; }
-    if (owner[off + c] != t_local) continue;
+    if (own != t_local) continue;
     const float ry = h.x - f.p0;
     const float rz = (h.y - z_ref) - f.p1;
-    o.res_trk[off + c] = t_local; o.res_y[off + c] = ry; o.res_z[off + c] = rz;
-    o.q_y[off + c] = res_quantise(ry, inv_q); o.q_z[off + c] = res_quantise(rz, inv_q);
+    const int qq = (int)(uint16_t)res_quantise(ry, inv_q) | ((int)(uint16_t)res_quantise(rz, inv_q) << 16);
+    reinterpret_cast<int4*>(o)[off + c] = make_int4(t_local, __float_as_int(ry), __float_as_int(rz), qq);   // one 16-byte store
   }
   out_ok[k] = (walked && nh > 0) ? 1 : 0;
   out_x[k] = f.x;

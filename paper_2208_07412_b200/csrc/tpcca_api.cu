@@ -32,7 +32,7 @@ struct Layout {
   size_t start_hit, hits, trk_v, trk_n, hs;
   size_t o_x_ref, o_z_ref, o_chi2, o_par, o_cov, o_n_hits, o_n_fit, o_first, o_last, o_start, o_hit_offset, o_hit_idx;
   size_t sel_n_own, sel_track, slot_trk;   // S6 (its other buffers alias S1 / S5 scratch: see sel_out)
-  size_t res_trk, res_y, res_z, res_qy, res_qz;   // S7
+  size_t res;   // S7: tpcca_residual[N]
   size_t mg_out, mg_ok, mg_cnt, mg_cur, mg_list, mg_keys, mg_links;   // S8 (chain outputs alias the parked-tracklet buffer)
   int64_t mg_nzb;
   size_t total;
@@ -132,8 +132,7 @@ Layout make_layout(const tpcca_params* p, int64_t N, int64_t CS) {
   L.sel_n_own = take(4 * (size_t)CS);
   L.sel_track = take(4 * (size_t)CS);
   L.slot_trk = take(4 * (size_t)CS);     // start-hit slot -> global track (S5 gather), -1 = rejected
-  L.res_trk = take(4 * (size_t)N); L.res_y = take(4 * (size_t)N); L.res_z = take(4 * (size_t)N);
-  L.res_qy = take(2 * (size_t)N); L.res_qz = take(2 * (size_t)N);
+  L.res = take(sizeof(tpcca_residual) * (size_t)N);
   L.mg_nzb = mg_z_buckets(p, nullptr, nullptr);
   L.mg_out = take(4 * (size_t)(6 * CS)); L.mg_ok = take(4 * (size_t)CS);
   L.mg_cnt = take(4 * (size_t)(ns * nr * L.mg_nzb + 2)); L.mg_cur = take(4 * (size_t)(ns * nr * L.mg_nzb + 2));
@@ -317,14 +316,6 @@ MgBuf mg_buf(const tpcca_ctx* c) {
   b.n_seg = i32; b.n_hits = i32 + cs; b.n_fit = i32 + 2 * cs; b.first_row = i32 + 3 * cs; b.last_row = i32 + 4 * cs; b.frame_seg = i32 + 5 * cs;
   b.x_ref = f + 6 * cs; b.z_ref = f + 7 * cs; b.chi2 = f + 8 * cs; b.par = f + 9 * cs; b.cov = f + 14 * cs;
   return b;
-}
-
-ResOut res_out(const tpcca_ctx* c) {
-  const Layout& L = c->L;
-  ResOut ro;
-  ro.res_trk = c->at<int32_t>(L.res_trk); ro.res_y = c->at<float>(L.res_y); ro.res_z = c->at<float>(L.res_z);
-  ro.q_y = c->at<int16_t>(L.res_qy); ro.q_z = c->at<int16_t>(L.res_qz);
-  return ro;
 }
 
 }  // namespace
@@ -733,7 +724,7 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
   }
   mark(6);
   if (mask & TPCCA_STAGE_RESIDUALS) {
-    const ResOut ro = res_out(c);
+    tpcca_residual* ro = c->at<tpcca_residual>(L.res);
     const size_t nk = (size_t)std::max<int64_t>(c->n_total, 1);
     k_res_init<<<(unsigned)std::min<size_t>((nk + 255) / 256, (size_t)c->sm_count * 32), 256, 0, st>>>(ro, nk);
     const MgBuf mb = mg_buf(c);
@@ -751,12 +742,16 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     k_zero_words<<<(unsigned)std::min<size_t>((nbk + 1023) / 1024, (size_t)c->sm_count * 8), 256, 0, st>>>(mb.bk_cnt, nbk + 1);
     k_zero_words<<<(unsigned)std::min<size_t>((nbk + 1023) / 1024, (size_t)c->sm_count * 8), 256, 0, st>>>(cursor, nbk + 1);
     k_mg_count<<<g256, 256, 0, st>>>(T, status, so, cap, c->mgp, mb);
-    k_mg_scan<<<1, 1024, 0, st>>>(mb.bk_cnt, (int)(nbk - 1));
+    k_mg_scan<<<c->ns, 1024, 0, st>>>(T, status, mb.bk_cnt, (int)((nbk - 1) / c->ns));
     k_mg_scatter<<<g256, 256, 0, st>>>(T, status, so, cap, c->mgp, mb, cursor);
     k_mg_match<<<g128, 128, 0, st>>>(T, status, so, cap, c->mgp, mb);
     k_mg_link<<<g256, 256, 0, st>>>(T, status, mb);
-    k_mg_refit<<<g128, 128, 0, st>>>(T, sec, status, syz, row_start, so, cap, c->mgp, mb);
-    c->launches += 8;
+    // chain heads, compacted: bk_list is free once the matching is done; the cursor array's last word counts them
+    int32_t* head_list = mb.bk_list;
+    uint32_t* n_heads = cursor + nbk;
+    k_mg_heads<<<g256, 256, 0, st>>>(T, status, mb, head_list, n_heads);
+    k_mg_refit<<<g128, 128, 0, st>>>(T, sec, status, syz, row_start, so, cap, c->mgp, mb, head_list, n_heads);
+    c->launches += 9;
   }
   mark(8);
   if (stage_err != cudaSuccess)
@@ -936,12 +931,7 @@ static int get_tracks_range(tpcca_ctx* c, int sec0, int sec1, int mem_space, uin
     }
   }
   if ((done & TPCCA_STAGE_RESIDUALS) && (what & TPCCA_OUT_RESIDUALS)) {
-    const ResOut ro = res_out(c);
-    add((const void* const*)&v->res_trk, ro.res_trk + off, 4 * (size_t)n);
-    add((const void* const*)&v->res_y, ro.res_y + off, 4 * (size_t)n);
-    add((const void* const*)&v->res_z, ro.res_z + off, 4 * (size_t)n);
-    add((const void* const*)&v->q_y, ro.q_y + off, 2 * (size_t)n);
-    add((const void* const*)&v->q_z, ro.q_z + off, 2 * (size_t)n);
+    add((const void* const*)&v->res, c->at<tpcca_residual>(L.res) + off, sizeof(tpcca_residual) * (size_t)n);
   }
   if ((done & TPCCA_STAGE_MERGE) && (what & TPCCA_OUT_MERGE)) {
     const MgBuf mb = mg_buf(c);
