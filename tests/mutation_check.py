@@ -27,6 +27,23 @@ M = [
  ("c640 changed", lambda s: s.replace("c640 = (R)(3.0 / 640.0)", "c640 = (R)(3.0 / 64.0)")),
  ("C starts at last", lambda s: s.replace("for (int r = top; r >= 0; --r) {", "for (int r = last; r >= 0; --r) {")),
  ("R2: top -> n_rows-1 start", lambda s: s.replace("for (int r = top; r >= 0; --r) {", "for (int r = n_rows - 1; r >= 0; --r) {")),
+ # ---- S6 / S7 / S8 (round 2)
+ ("S6 tie -> larger track", lambda s: s.replace("if (o < 0 || nh > hit_offset[o + 1] - hit_offset[o]) owner[c] = (int32_t)t;", "if (o < 0 || nh >= hit_offset[o + 1] - hit_offset[o]) owner[c] = (int32_t)t;")),
+ ("S6 keep <", lambda s: s.replace("if (shared * 1000 <= (int64_t)max_shared_permille * nh)", "if (shared * 1000 < (int64_t)max_shared_permille * nh)")),
+ ("S7 residual of every hit", lambda s: s.replace("        if (owner[c] != t) continue;\n        const R ry", "        const R ry")),
+ ("S7 z residual ignores z_ref", lambda s: s.replace("const R rz = (sz[c] - T.z_ref) - s.p[1];", "const R rz = sz[c] - s.p[1];")),
+ ("S7 quantiser truncates", lambda s: s.replace("R v = std::nearbyint(r * res_inv_q);", "R v = std::trunc(r * res_inv_q);")),
+ ("S8 gap from 2", lambda s: s.replace("if (gap < 1 || gap > A.mg_gap) continue;", "if (gap < 2 || gap > A.mg_gap) continue;")),
+ ("S8 gap >=", lambda s: s.replace("if (gap < 1 || gap > A.mg_gap) continue;", "if (gap < 1 || gap >= A.mg_gap) continue;")),
+ ("S8 rotation sign", lambda s: s.replace("const R sa = dir == 0 ? A.sec_sin : -A.sec_sin;", "const R sa = dir == 0 ? -A.sec_sin : A.sec_sin;")),
+ ("S8 no mutual check", lambda s: s.replace("if (back.have && back.sec == s && back.trk == (int)ia) {", "if (back.have) {")),
+ ("S8 windows halved", lambda s: s.replace("if (!(std::fabs(dy) <= A.mg_dy && std::fabs(dz) <= A.mg_dz && std::fabs(ds) <= A.mg_ds)) continue;", "if (!(std::fabs(dy) <= A.mg_dy * (R)0.25 && std::fabs(dz) <= A.mg_dz * (R)0.25 && std::fabs(ds) <= A.mg_ds * (R)0.25)) continue;")),
+ ("S8 z re-reference sign", lambda s: s.replace("st.p[1] = st.p[1] + (tu.z_ref - tg.z_ref);", "st.p[1] = st.p[1] - (tu.z_ref - tg.z_ref);")),
+ ("S8 refit rotation sign", lambda s: s.replace("const R sa = up_is_next ? -G.sec_sin : G.sec_sin;", "const R sa = up_is_next ? G.sec_sin : -G.sec_sin;")),
+ ("S8 rotate drops j10", lambda s: s.replace("const R j10 = -((s.p[3] * sa) / cf2);", "const R j10 = (R)0 * ((s.p[3] * sa) / cf2);")),
+ ("S8 rotate drops j20", lambda s: s.replace("const R j20 = -((s.p[4] * Bc) * sa);", "const R j20 = (R)0 * ((s.p[4] * Bc) * sa);")),
+ ("S8 rotate j22 inverted", lambda s: s.replace("const R j22 = cf2 / cf;", "const R j22 = cf / cf2;")),
+ ("S8 tie -> larger sector/track", lambda s: s.replace("    if (sec != b.sec) return sec < b.sec;\n    return trk < b.trk;", "    if (sec != b.sec) return sec > b.sec;\n    return trk > b.trk;")),
 ]
 src = open(os.path.join(ROOT, "oracle", "tpcca_oracle.cpp")).read()
 only = sys.argv[1:]

@@ -1120,3 +1120,17 @@ def test_merged_refit_statistics(merged_cfg1):
     assert np.all(np.abs(pc.std(axis=0) - 1.0) < 0.12), pc.std(axis=0)
     assert abs(np.mean(np.array(red)[core]) - 1.0) < 0.06
     assert np.median(shrink) < 0.5                              # the longer lever arm pins q/pT down
+
+
+def test_merge_row_gap_bounds_are_inclusive():
+    """mg_max_row_gap is data: with 2, links with a gap of exactly 2 rows exist and none is larger (pins `1 <= gap <= max`)."""
+    from oracle import run_timeframe_merged
+    tf = tpcsynth.generate(1, n_tracks=2500)
+    tf.params = tf.params.copy(mg_max_row_gap=2)
+    res, mg = run_timeframe_merged(tf)
+    gaps = []
+    for s in range(36):
+        for ia in np.nonzero(mg[s].next_sec >= 0)[0]:
+            b = res[mg[s].next_sec[ia]]
+            gaps.append(int(b.first_row[b.selected[mg[s].next_trk[ia]]] - res[s].last_row[res[s].selected[ia]]))
+    assert len(gaps) > 300 and min(gaps) == 1 and max(gaps) == 2 and gaps.count(2) > 20
