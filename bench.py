@@ -499,18 +499,28 @@ def run_tpcca(args, env_cls=CudaEnv):
             pipe = None
         if pipe is not None:
             hy = [h[0] for h in host]; hz = [h[1] for h in host]; hr = [h[2] for h in host]
-            what = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START | B.OUT_TRACKS
-            pipe.run_views(hy, hz, hr, 0x1F, what)          # warm-up: grows the pinned arenas
-            env.synchronize()
-            t0 = time.perf_counter()
-            for _ in range(e2e_steps):
-                views = pipe.run_views(hy, hz, hr, 0x1F, what)
-            env.synchronize()
-            dt = (time.perf_counter() - t0) / e2e_steps
-            d2h_p = int(sum(12 * v.n_clusters + 4 * v.n_start + 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4 for v in views))
-            pipe_res = dict(value=N / dt, unit=UNIT, ms_per_step=1e3 * dt, n_groups=G, h2d_bytes_per_step=h2d,
-                            d2h_bytes_per_step=d2h_p, group_ms=[round(v, 1) for v in pipe.groups()[1]],
-                            mode=f"one time frame at a time, {G} sector groups on {G} streams / host threads (host wall clock)")
+
+            def pipe_leg(mask, what, selected):
+                pipe.run_views(hy, hz, hr, mask, what)          # warm-up: grows the pinned arenas
+                env.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(e2e_steps):
+                    views = pipe.run_views(hy, hz, hr, mask, what)
+                env.synchronize()
+                dt = (time.perf_counter() - t0) / e2e_steps
+                if selected:
+                    nb = sum(12 * v.n_clusters + 4 * v.n_start + 4 * v.n_sel_hits + (4 * 28 + 4) * v.n_selected + 4
+                             + 4 * v.n_clusters + 4 * v.n_tracks + 4 * v.n_selected for v in views)
+                else:
+                    nb = sum(12 * v.n_clusters + 4 * v.n_start + 4 * v.n_hits + (4 * 28 + 4) * v.n_tracks + 4 for v in views)
+                return dict(value=N / dt, unit=UNIT, ms_per_step=1e3 * dt, d2h_bytes_per_step=int(nb),
+                            group_ms=[round(v, 1) for v in pipe.groups()[1]])
+
+            early = B.OUT_ORDER | B.OUT_LINKS | B.OUT_START
+            pipe_res = pipe_leg(0x1F, early | B.OUT_TRACKS, False)
+            pipe_res.update(n_groups=G, h2d_bytes_per_step=h2d,
+                            mode=f"one time frame at a time, {G} sector groups on {G} streams / host threads (host wall clock)",
+                            selected=pipe_leg(0x3F, early | B.OUT_TRACKS_SEL | B.OUT_SELECTION, True))
             pipe.close()
             env.empty_cache()
     e2e_value = n_all * e2e_n / (e2e_ms * 1e-3)
@@ -592,7 +602,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sectors", type=int, default=8, help="sectors of the CPU-baseline / full-size parity sample")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
-    ap.add_argument("--pipeline-groups", type=int, default=4, help="sector groups of the tpcca_pipeline e2e leg (0/1: off)")
+    ap.add_argument("--pipeline-groups", type=int, default=3, help="sector groups of the tpcca_pipeline e2e leg (0/1: off)")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "tpcca":

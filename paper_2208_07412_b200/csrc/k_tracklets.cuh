@@ -171,6 +171,10 @@ constexpr int kS5Refill = TPCCA_S5_REFILL;      // idle lanes of a warp that tri
 #define TPCCA_S5_UNROLL 5
 #endif
 constexpr int kS5Unroll = TPCCA_S5_UNROLL;   // candidate loads in flight per lane in the S5 search
+#ifndef TPCCA_S5_SEARCH_BATCH
+#define TPCCA_S5_SEARCH_BATCH 4
+#endif
+constexpr int kS5SearchBatch = TPCCA_S5_SEARCH_BATCH;   // phase-C1 lanes that wait for each other before a search is issued
 constexpr int kSnapF = 22;        // floats of a saved Kalman state: x, p[5], c[15], chi2
 
 // scalars of S5, passed by value (constant bank: no registers)
@@ -492,6 +496,19 @@ k_tracklets(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
       }
     }
     __syncwarp();
+    if (MODE == MODE_C1) {
+      // Refit over known hits: only the few lanes on a hit-less row search, and each such step would issue the whole
+      // search code for one or two lanes (23 % of this kernel's instructions ran at < 4 active lanes).  A lane that
+      // needs a search therefore WAITS on its row (the state already sits there: repeating the step is a no-op up to
+      // this point) until kS5SearchBatch lanes of the warp wait, or every live lane does.
+      const unsigned want = __ballot_sync(0xffffffffu, need_search);
+      if (want) {
+        const unsigned live = __ballot_sync(0xffffffffu, alive);
+        if (__popc(want) < kS5SearchBatch && want != live) {
+          if (need_search) { need_search = false; go = false; }
+        }
+      }
+    }
     if (MODE != MODE_A && need_search) {
       // search: best cluster of row r in the tc window around the prediction
       const float yc = f.p0;
