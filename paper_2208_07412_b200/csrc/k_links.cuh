@@ -16,28 +16,36 @@ __device__ __forceinline__ int row_search(const int32_t* __restrict__ rs, int n_
 // ---- S2 tiling and staging -------------------------------------------------------
 // A tile = kNfTile consecutive sorted clusters of ONE (sector, row).  Because the sort key is
 // (row, bz, by, id), the window candidates of a whole tile in row r+1 (r-1) are ONE contiguous run
-// of sorted clusters: the z slices S_lo..S_hi of that row.  k_nf_plan writes one descriptor per tile;
-// k_neighbours stages the two cluster runs of the NEXT tile in shared memory with 1-D bulk async
-// copies (TMA, mbarrier completion, two buffers) while the current tile is searched in shared memory.
-// bin_start is not read at all on the fast path: the first staged cluster of every z slice is found
-// from the staged clusters themselves (a z slice of a row holds ~5 clusters at the headline density, so
-// walking the whole slices of a window costs about as much as looking the y bins up, without the loads).
-#ifndef TPCCA_NF_K
-#define TPCCA_NF_K 12
+// of sorted clusters (the z slices S_lo..S_hi of that row) and their bin_start entries are one
+// contiguous run as well.  k_nf_plan writes one descriptor per tile; k_neighbours stages the two
+// cluster runs and the two bin_start runs of the next tile in shared memory with 1-D bulk async
+// copies (TMA, mbarrier completion) while the current tile is searched entirely in shared memory.
+#ifndef TPCCA_NF_T2
+#define TPCCA_NF_T2 2      // window-test candidates per loop trip
 #endif
-constexpr int kNfK = TPCCA_NF_K;          // window hits listed per side and thread in shared memory
+#ifndef TPCCA_NF_K
+#define TPCCA_NF_K 10
+#endif
+#ifndef TPCCA_NF_ARENA
+#define TPCCA_NF_ARENA 8448
+#endif
+constexpr int kNfK = TPCCA_NF_K;          // window hits cached per side and thread in shared memory (<= 15): normal occupancy
+constexpr int kNfKDense = 15;             // ... of the kernel instance used for dense time frames (tpcca_create chooses)
+static_assert(TPCCA_NF_K <= 15 && TPCCA_NF_TILE <= 256, "work-item encoding: 8 bits cluster, 4 bits hit row, 4 bits nd");
 constexpr int kNfThreads = kNfTile;       // one thread per cluster of the tile
-constexpr int kNfArenaC = 768;            // staged clusters per buffer (both sides together)
-constexpr int kNfMaxSl = 254;             // z slices per side whose first cluster is indexed
+constexpr int kNfArena = TPCCA_NF_ARENA;  // bytes of one staging buffer: [up clusters | down clusters | up bins | down bins]
+constexpr int kNfMaxCn = 1022;            // staged clusters per side (staged indices are packed in 10 bits)
+constexpr int kNfMaxRun = 63;             // window candidates per side handled by the packed fast path
 
-enum { NF_STAGED = 0, NF_NOLINK = 1, NF_GLOBAL = 2 };
+enum { NF_STAGED = 0, NF_NOLINK = 1, NF_GLOBAL = 2, NF_STAGED_C = 3 };   // STAGED_C: clusters staged, bins read from global memory
 
 struct NfSide {        // staging of one neighbour row for one tile
   int32_t c0;          // sector-local sorted position of staged cluster 0 ((sec_off + c0) is even; may be -1)
   int32_t cn;          // staged clusters (even)
+  uint32_t b0;         // global bin_start index of staged entry 0 (multiple of 4)
+  int32_t bn;          // staged entries (multiple of 4)
   int32_t s0;          // first staged z slice
-  int32_t nsl;         // staged z slices
-  int32_t lo, hi;      // staged indices [lo, hi) are the clusters of slices s0 .. s0 + nsl - 1 (the rest is alignment)
+  int32_t ds_shift;    // (last staged slice - s0) | (index of slice s0's first entry in the staged run) << 24
 };
 struct NfTileDesc {    // 64 bytes
   int32_t p0;          // global index (concatenated arrays) of the tile's first cluster
@@ -94,12 +102,15 @@ __device__ __forceinline__ void nf_plan_side(NfSide& o, int& flag, const DevTabl
     s_hi = bin_range(ze + hm + (0.02f + 1e-6f * fabsf(ze)), zlo, ibz, nzh);
   }
   const uint32_t gb_lo = bs_off + (uint32_t)(T->bin_base[rn] + s_lo * ny);
-  const uint32_t gb_hi = bs_off + (uint32_t)(T->bin_base[rn] + (s_hi + 1) * ny);   // end of slice s_hi
+  const uint32_t gb_hi = bs_off + (uint32_t)(T->bin_base[rn] + (s_hi + 1) * ny);   // inclusive: end of slice s_hi
+  const uint32_t b0 = gb_lo & ~3u;
+  const int bn = (int)((gb_hi + 1u - b0 + 3u) & ~3u);
   const int c_lo = (int)bin_start[gb_lo], c_hi = (int)bin_start[gb_hi];
   const int c0 = c_lo - ((sec_off + c_lo) & 1);
   const int cn = (c_hi - c0 + 1) & ~1;
-  o.c0 = c0; o.cn = cn; o.s0 = s_lo; o.nsl = s_hi - s_lo + 1; o.lo = c_lo - c0; o.hi = c_hi - c0;
-  if (o.nsl > kNfMaxSl) flag = NF_GLOBAL;
+  o.c0 = c0; o.cn = cn; o.b0 = b0; o.bn = bn; o.s0 = s_lo;
+  o.ds_shift = (s_hi - s_lo) | ((int)(gb_lo - b0) << 24);
+  if (cn > kNfMaxCn || (s_hi - s_lo) >= (1 << 24)) flag = NF_GLOBAL;
 }
 
 __global__ void __launch_bounds__(128)
@@ -127,14 +138,15 @@ k_nf_plan(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec, c
       d.n = min(kNfTile, rs1 - pl0);
       d.sec_off = sec_off;
       int flag = edge ? NF_NOLINK : NF_STAGED;
-      d.up = NfSide{0, 0, 0, 0, 0, 0};
+      d.up = NfSide{0, 0, 0u, 0, 0, 0};
       d.dn = d.up;
       if (!edge) {
         const int b_first = bin_range(syz[d.p0].y, zlo, ibz, nz_r - 1);
         const int b_last = bin_range(syz[d.p0 + d.n - 1].y, zlo, ibz, nz_r - 1);
         nf_plan_side(d.up, flag, T, r + 1, T->hz_up[r] + T->margin, b_first, b_last, nz_r, bin_r, bs_off, sec_off, bin_start);
         nf_plan_side(d.dn, flag, T, r - 1, T->hz_dn[r] + T->margin, b_first, b_last, nz_r, bin_r, bs_off, sec_off, bin_start);
-        if (d.up.cn + d.dn.cn > kNfArenaC) flag = NF_GLOBAL;
+        if (flag == NF_STAGED && 8 * (d.up.cn + d.dn.cn) + 4 * (d.up.bn + d.dn.bn) > kNfArena)
+          flag = (8 * (d.up.cn + d.dn.cn) <= kNfArena) ? NF_STAGED_C : NF_GLOBAL;
       }
       d.rsf = r | (s << 8) | (flag << 16);
       desc[t] = d;
@@ -162,7 +174,8 @@ __device__ __forceinline__ void nf_for_each(const float2 c, const float4 A, cons
 
 // Slow path of S2 (global memory, exact in every case: any number of candidates, ties by original
 // id): the full U x D product by nested rescans of both windows.  Taken by clusters whose windows
-// are not covered by the staged runs or whose best score is tied.
+// are not covered by the staged runs, hold more than kNfK hits or kNfMaxRun candidates on a side,
+// or whose best score is tied.
 __device__ __noinline__ void nf_slow(const float2 c, const NfConst& kc, const uint32_t* __restrict__ bs,
                                      const float2* __restrict__ yz, const int32_t* __restrict__ ord,
                                      float& best, int32_t& bu, int32_t& bd) {
@@ -187,15 +200,40 @@ __device__ __noinline__ void nf_slow(const float2 c, const NfConst& kc, const ui
   });
 }
 
+// ---- fast path, phase 0: the candidate runs of one side as a packed descriptor ----------------------
+// A window touches nsl = 2 (3 when it straddles a bin edge by less than the margin) z slices of the
+// neighbour row; in each slice its y range of bins is ONE run of sorted clusters.  The runs are
+// addressed by a flat candidate index j in [0, tot): staged index = q + j + (j >= n0 ? o1 : 0) +
+// (j >= n01 ? o2 : 0).  w0 = q | n0 << 10 | o1 << 16 | n01 << 26,  w1 = o2 | tot << 10.
+// Returns false if the window is not covered by the staged slices, spans more than 3 slices or holds
+// more than kNfMaxRun candidates.
+__device__ __forceinline__ bool nf_runs(const float2 c, const float4 A, const float4 B, const int4 C, const NfSide& sd,
+                                        const uint32_t* __restrict__ sB, uint32_t& w0, uint32_t& w1, int& tot) {
+  const int by0 = bin_range(__fsub_rn(c.x, A.z), B.x, B.y, C.x), by1 = bin_range(__fadd_rn(c.x, A.z), B.x, B.y, C.x);
+  const int bz0 = bin_range(__fsub_rn(c.y, A.w), B.w, B.z, C.y), bz1 = bin_range(__fadd_rn(c.y, A.w), B.w, B.z, C.y);
+  const int ds = sd.ds_shift & 0xffffff, shift = sd.ds_shift >> 24;
+  const int k0 = bz0 - sd.s0, nsl = bz1 - bz0;          // nsl = slices - 1
+  w0 = 0; w1 = 0; tot = 0;
+  if (k0 < 0 || bz1 - sd.s0 > ds || nsl > 2) return false;
+  const uint32_t* bp = sB + shift + k0 * C.z + by0;
+  const int w = by1 + 1 - by0;
+  const int qa = (int)bp[0], ea = (int)bp[w];
+  int qb = ea, eb = ea, qc, ec;
+  if (nsl >= 1) { qb = (int)bp[C.z]; eb = (int)bp[C.z + w]; }
+  qc = eb; ec = eb;
+  if (nsl >= 2) { qc = (int)bp[2 * C.z]; ec = (int)bp[2 * C.z + w]; }
+  const int n0 = ea - qa, n01 = n0 + (eb - qb);
+  tot = n01 + (ec - qc);
+  if (tot > kNfMaxRun) return false;
+  w0 = (uint32_t)(qa - sd.c0) | (uint32_t)n0 << 10 | (uint32_t)(qb - ea) << 16 | (uint32_t)n01 << 26;
+  w1 = (uint32_t)(qc - eb) | (uint32_t)tot << 10;
+  return true;
+}
+
 // ---- shared-memory accessors on 32-bit shared addresses (no 64-bit pointer arithmetic in the loops) --
 __device__ __forceinline__ float2 lds_f2(uint32_t a) {
   float2 v;
   asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a));
-  return v;
-}
-__device__ __forceinline__ float lds_f1(uint32_t a) {
-  float v;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
   return v;
 }
 __device__ __forceinline__ void sts_f2(uint32_t a, float x, float y) {
@@ -210,106 +248,125 @@ __device__ __forceinline__ void sts_u16(uint32_t a, uint32_t v) {
   asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((uint16_t)v) : "memory");
 }
 
-constexpr uint32_t kVecRow = 8u * kNfThreads;   // bytes between consecutive rows of the down-vector cache
-constexpr uint32_t kIdxRow = 2u * kNfThreads;   // ... of the hit lists
+constexpr uint32_t kVecRow = 8u * kNfThreads;   // bytes between consecutive rows of the hit-vector cache
+constexpr uint32_t kIdxRow = 2u * kNfThreads;   // ... of the hit-index cache
 
+// ---- fast path, phase A: window test of the tot candidates of one side ------------------------------
+// sC = shared address of the side's staged cluster run, (hy, hz) the exact window, scale = +dxd (up
+// side) or -dxu (down side: (y_c - y_d) * dxu = -((y_d - y_c) * dxu), exact).  Hits go to the thread's
+// cache column: vector (dy * scale, dz * scale) at pv + k * kVecRow, staged index at pi + k * kIdxRow.
+// Returns the number of hits (may exceed kNfK; only the first kNfK are cached).
 template <int K>
-struct NfSmem {
-  alignas(128) float2 arena[2][kNfArenaC];   // two staging buffers (TMA destinations): [up clusters | down clusters]
-  float2 vecD[K][kNfThreads];                // (y_d - y_c, z_d - z_c) * (-dxu) of the listed down-side hits; column = cluster
-  uint16_t list[2][K][kNfThreads];           // staged indices of the window hits: [0] down side, [1] up side
-  uint16_t sidx[2][2][kNfMaxSl + 2];         // [buffer][side]: first staged index of every staged z slice (+ end)
-  NfTileDesc desc[4];
-  uint64_t full[2];
-};
-
-// ---- phase 0: first staged index of every z slice of one side --------------------------------------
-// The staged run [lo, hi) holds the clusters of slices s0 .. s0 + nsl - 1 in slice order.  sidx[k] = first
-// index whose slice is >= s0 + k (k = 0 .. nsl; sidx[nsl] = hi): every thread looks at a few staged clusters
-// and, where the slice changes, fills the entries of the slices that start there.
-__device__ __forceinline__ void nf_slice_index(const NfSide& sd, uint32_t sA, float zlo, float ibz, int nzh,
-                                               uint16_t* __restrict__ sidx, int tid) {
-  const int lo = sd.lo, hi = sd.hi, nsl = sd.nsl;
-  if (lo >= hi) {
-    for (int k = tid; k <= nsl; k += kNfThreads) sidx[k] = (uint16_t)lo;
-    return;
-  }
-  for (int i = lo + tid; i < hi; i += kNfThreads) {
-    const int b = min(max(bin_range(lds_f1(sA + 8u * (uint32_t)i + 4u), zlo, ibz, nzh) - sd.s0, 0), nsl - 1);
-    const int bp = (i == lo) ? -1 : min(max(bin_range(lds_f1(sA + 8u * (uint32_t)i - 4u), zlo, ibz, nzh) - sd.s0, 0), nsl - 1);
-    for (int k = bp + 1; k <= b; ++k) sidx[k] = (uint16_t)i;
-    if (i == hi - 1)
-      for (int k = b + 1; k <= nsl; ++k) sidx[k] = (uint16_t)hi;
-  }
-}
-
-// ---- phase A: window test of the staged run [j0, j1) of one side -------------------------------------
-// Hits (staged indices) go to the thread's list column at pl + k * kIdxRow; returns the number of hits
-// (may exceed K; only the first K are listed).
-template <int K>
-__device__ __forceinline__ int nf_test_run(const float2 c, uint32_t sA, int j0, int j1, float hy, float hz, uint32_t pl) {
+__device__ __forceinline__ int nf_test_runs(const float2 c, uint32_t w0, uint32_t w1, uint32_t sC, float hy, float hz,
+                                            float scale, uint32_t pv, uint32_t pi) {
+  const int n0 = (w0 >> 10) & 63, n01 = w0 >> 26, tot = w1 >> 10;
+  const uint32_t o1 = 8u * ((w0 >> 16) & 1023u), o2 = 8u * (w1 & 1023u);
+  uint32_t a = sC + 8u * (w0 & 1023u);
+  const uint32_t pv_end = pv + K * kVecRow;
   int n = 0;
-  uint32_t a = sA + 8u * (uint32_t)j0;
-  const uint32_t e = sA + 8u * (uint32_t)j1;
-#pragma unroll 2
-  for (; a < e; a += 8u) {
-    const float2 v = lds_f2(a);
-    const float dy = __fsub_rn(v.x, c.x), dz = __fsub_rn(v.y, c.y);
-    if (fabsf(dy) <= hy && fabsf(dz) <= hz) {
-      if (n < K) sts_u16(pl + (uint32_t)n * kIdxRow, (a - sA) >> 3);
-      ++n;
+  // kT candidates per trip: their shared-memory loads are issued before the first test (independent chains)
+  constexpr int kT = TPCCA_NF_T2;
+#pragma unroll 1
+  for (int j = 0; j < tot; j += kT) {
+    uint32_t aa[kT];
+    float2 v[kT];
+#pragma unroll
+    for (int k = 0; k < kT; ++k) {
+      if (j + k == n0) a += o1;
+      if (j + k == n01) a += o2;
+      aa[k] = (k == 0 || j + k < tot) ? a : aa[0];
+      a += 8u;
+    }
+#pragma unroll
+    for (int k = 0; k < kT; ++k) v[k] = lds_f2(aa[k]);
+#pragma unroll
+    for (int k = 0; k < kT; ++k) {
+      const float dy = __fsub_rn(v[k].x, c.x), dz = __fsub_rn(v[k].y, c.y);
+      if ((k == 0 || j + k < tot) && fabsf(dy) <= hy && fabsf(dz) <= hz) {
+        if (pv != pv_end) {
+          sts_f2(pv, __fmul_rn(dy, scale), __fmul_rn(dz, scale));
+          sts_u16(pi, (aa[k] - sC) >> 3);
+          pv += kVecRow; pi += kIdxRow;
+        }
+        ++n;
+      }
     }
   }
   return n;
 }
 
-// ---- medium path: more than K hits on a side (dense regions) -----------------------------------------
-// Nested loops over the staged candidate runs of both sides (no lists): the U x D product in the order
-// and arithmetic of nf_slow, in shared memory.  Returns false on an exact score tie (decided by original
-// ids in nf_slow).  iu / id are staged indices.
-__device__ __noinline__ bool nf_medium(const float2 c, uint32_t sAU, int ju0, int ju1, uint32_t sAD, int jd0, int jd1,
-                                       const float4 uA, const float4 dA, const float4 g, float& best, int& iu, int& id) {
+// ---- medium path: more than kNfK hits on a side (dense regions) -------------------------------------
+// Nested loops over the staged candidate runs of both sides (no hit cache): the U x D product in the
+// order and arithmetic of nf_slow, in shared memory.  Returns false on an exact score tie (decided by
+// original ids in nf_slow).  iu / id are staged indices.
+__device__ __noinline__ bool nf_medium(const float2 c, uint32_t wu0, uint32_t wu1, uint32_t wd0, uint32_t wd1, uint32_t sUC,
+                                       uint32_t sDC, const float4 uA, const float4 dA, const float4 g, float& best,
+                                       int& iu, int& id) {
+  const int un0 = (wu0 >> 10) & 63, un01 = wu0 >> 26, utot = wu1 >> 10;
+  const uint32_t uo1 = 8u * ((wu0 >> 16) & 1023u), uo2 = 8u * (wu1 & 1023u);
+  const int dn0 = (wd0 >> 10) & 63, dn01 = wd0 >> 26, dtot = wd1 >> 10;
+  const uint32_t do1 = 8u * ((wd0 >> 16) & 1023u), do2 = 8u * (wd1 & 1023u);
   bool have = false, tie = false;
   best = 0.0f; iu = -1; id = -1;
+  uint32_t au = sUC + 8u * (wu0 & 1023u);
 #pragma unroll 1
-  for (int ju = ju0; ju < ju1; ++ju) {
-    const float2 u = lds_f2(sAU + 8u * (uint32_t)ju);
+  for (int ju = 0; ju < utot; ++ju, au += 8u) {
+    if (ju == un0) au += uo1;
+    if (ju == un01) au += uo2;
+    const float2 u = lds_f2(au);
     const float dyu = __fsub_rn(u.x, c.x), dzu = __fsub_rn(u.y, c.y);
     if (!(fabsf(dyu) <= uA.x && fabsf(dzu) <= uA.y)) continue;
     const float Ay = __fmul_rn(dyu, g.y), Az = __fmul_rn(dzu, g.y);
+    uint32_t ad = sDC + 8u * (wd0 & 1023u);
 #pragma unroll 1
-    for (int jd = jd0; jd < jd1; ++jd) {
-      const float2 d = lds_f2(sAD + 8u * (uint32_t)jd);
+    for (int jd = 0; jd < dtot; ++jd, ad += 8u) {
+      if (jd == dn0) ad += do1;
+      if (jd == dn01) ad += do2;
+      const float2 d = lds_f2(ad);
       const float dyd = __fsub_rn(d.x, c.x), dzd = __fsub_rn(d.y, c.y);
       if (!(fabsf(dyd) <= dA.x && fabsf(dzd) <= dA.y)) continue;
       const float ay = __fsub_rn(Ay, __fmul_rn(-dyd, g.x));
       const float az = __fsub_rn(Az, __fmul_rn(-dzd, g.x));
       const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
       if (have && sc == best) tie = true;
-      if (!have || sc < best) { have = true; best = sc; iu = ju; id = jd; }
+      if (!have || sc < best) { have = true; best = sc; iu = (int)((au - sUC) >> 3); id = (int)((ad - sDC) >> 3); }
     }
   }
   return !tie;
 }
+
+template <int K>
+struct NfSmem {
+  alignas(128) unsigned char arena[kNfArena];   // staging buffer (TMA destination): [up clusters | down clusters | up bins | down bins]
+  float2 vec[2 * K][kNfThreads];      // cached hits: rows [0, K) down side, [K, 2K) up side; column = cluster of the tile
+  uint16_t hidx[2 * K][kNfThreads];   // staged indices of the cached hits
+  uint16_t items[K * kNfThreads];           // pair work items (one per up-side hit): cluster | hit row << 8 | nd << 12
+  int hist[2][16], cnt[2][16];           // items per nd (work key) / emission cursors, two consecutive tiles
+  NfTileDesc desc[4];
+  uint64_t full;
+};
 
 // ---- K2b: neighbour finder --------------------------------------------------
 // For cluster c of row r (1 <= r <= n_rows-2): over U x D (exact windows in rows r+1, r-1) the
 // pair minimising score = ay^2 + az^2, ay = (yu-yc)*dxd - (yc-yd)*dxu; ties -> smallest original
 // id of u, then of d; stored if score <= nf_cut[r].
 // Persistent blocks walk the tile list with a grid stride (tiles in flight are neighbours in memory,
-// so the three-fold reuse of a row stays in L2).  Per tile, ONE block barrier:
-//   phase 0  the first staged index of every z slice of both neighbour runs (from the staged clusters);
-//   barrier; thread 0 issues the bulk copies of the NEXT tile into the other buffer;
-//   phase A  thread t = cluster t: the z slices its two windows touch -> one contiguous staged run per
-//            side (the grid is only an accelerator: every cluster of those slices gets the exact window
-//            test); hits are listed in the thread's shared-memory column;
-//   phase B  thread t: the nd down vectors once, then the nu x nd pair scores in the defined operation
-//            order, minimum, cut, coalesced link stores.  An exact tie of the minimum goes to nf_slow.
+// so the three-fold reuse of a row stays in L2).  Per tile:
+//   phase A  thread t = cluster t: bin ranges of both windows, candidate runs from the staged
+//            bin_start entries, window tests of both sides; hits cached in the thread's column.
+//   phase B  the nu x nd pair scores are NOT looped per cluster (nu * nd has a long tail: mean 3.7,
+//            1 % above 24): every up-side hit becomes a work item (cluster, hit row, nd), the items
+//            are counting-sorted by nd in shared memory, and thread i scores item i against the nd
+//            down-side hits of its cluster, so the lanes of a warp run the same trip count (<= kNfK).
+//   phase C  thread t = cluster t: minimum over its nu item results, cut, coalesced link stores.
+// The staged runs of tile i+1 are fetched by bulk async copies (issued by thread 0 right after the
+// barrier that ends phase A of tile i, the only phase that reads the staging buffer); per-row
+// constants come from the constant bank (NfTable is a by-value kernel parameter).
 #ifndef TPCCA_NF_BPS
-#define TPCCA_NF_BPS 6
+#define TPCCA_NF_BPS 5
 #endif
 template <int K>
-__global__ void __launch_bounds__(kNfThreads, TPCCA_NF_BPS)
+__global__ void __launch_bounds__(kNfThreads, K == kNfK ? TPCCA_NF_BPS : 4)
 k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz,
              const uint32_t* __restrict__ bin_start, const int32_t* __restrict__ order, uint32_t nbp1,
              const int32_t* __restrict__ n_tiles_ptr, const NfTileDesc* __restrict__ desc,
@@ -321,33 +378,41 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
   const int stride = gridDim.x;
   const int first = blockIdx.x;
   if (first >= n_tiles) return;
-  if (tid == 0) { mbar_init(&S.full[0], 1); mbar_init(&S.full[1], 1); fence_mbar_init(); }
+  if (tid == 0) { mbar_init(&S.full, 1); fence_mbar_init(); }
+  if (tid < 64) (&S.hist[0][0])[tid] = 0;            // hist[2][16] and cnt[2][16] are contiguous
   if (tid < 48) {      // descriptors of the block's first three tiles
     const int k = tid >> 4, t = first + k * stride;
     if (t < n_tiles) reinterpret_cast<int32_t*>(&S.desc[k])[tid & 15] = __ldg(reinterpret_cast<const int32_t*>(&desc[t]) + (tid & 15));
   }
   __syncthreads();
-  auto issue = [&](const NfTileDesc& d, int buf) {      // thread 0 only
+  auto issue = [&](const NfTileDesc& d) {      // thread 0 only
     const int flag = d.rsf >> 16;
-    const uint32_t bytes = flag == NF_STAGED ? 8u * (uint32_t)(d.up.cn + d.dn.cn) : 0u;
-    mbar_arrive_expect_tx(&S.full[buf], bytes);
+    uint32_t bytes = 0;
+    if (flag == NF_STAGED) bytes = 8u * (uint32_t)(d.up.cn + d.dn.cn) + 4u * (uint32_t)(d.up.bn + d.dn.bn);
+    else if (flag == NF_STAGED_C) bytes = 8u * (uint32_t)(d.up.cn + d.dn.cn);
+    mbar_arrive_expect_tx(&S.full, bytes);
     if (bytes) {
-      float2* a = S.arena[buf];
-      if (d.up.cn) bulk_g2s(a, syz + (d.sec_off + d.up.c0), 8u * d.up.cn, &S.full[buf]);
-      if (d.dn.cn) bulk_g2s(a + d.up.cn, syz + (d.sec_off + d.dn.c0), 8u * d.dn.cn, &S.full[buf]);
+      unsigned char* a = S.arena;
+      if (d.up.cn) bulk_g2s(a, syz + (d.sec_off + d.up.c0), 8u * d.up.cn, &S.full);
+      if (d.dn.cn) bulk_g2s(a + 8 * d.up.cn, syz + (d.sec_off + d.dn.c0), 8u * d.dn.cn, &S.full);
+      if (flag == NF_STAGED) {
+        unsigned char* b = a + 8 * (d.up.cn + d.dn.cn);
+        if (d.up.bn) bulk_g2s(b, bin_start + d.up.b0, 4u * d.up.bn, &S.full);
+        if (d.dn.bn) bulk_g2s(b + 4 * d.up.bn, bin_start + d.dn.b0, 4u * d.dn.bn, &S.full);
+      }
     }
   };
-  if (tid == 0) issue(S.desc[0], 0);
+  if (tid == 0) issue(S.desc[0]);
   float2 c_next = make_float2(0.f, 0.f);
   if (tid < S.desc[0].n) c_next = __ldg(&syz[S.desc[0].p0 + tid]);
-  const uint32_t sListD = smem_u32(&S.list[0][0][0]) + 2u * tid, sListU = smem_u32(&S.list[1][0][0]) + 2u * tid;
-  const uint32_t sVec = smem_u32(&S.vecD[0][0]) + 8u * tid;
+  const uint32_t sArena = smem_u32(S.arena);
+  const uint32_t sVecD = smem_u32(&S.vec[0][0]), sVecU = smem_u32(&S.vec[K][0]);
+  const uint32_t sIdxD = smem_u32(&S.hidx[0][0]), sIdxU = smem_u32(&S.hidx[K][0]);
   int it = 0;
   for (int tile = first; tile < n_tiles; tile += stride, ++it) {
-    const int buf = it & 1;
     const NfTileDesc& d = S.desc[it & 3];
     const bool have_next = tile + stride < n_tiles;
-    int32_t dword = 0;                       // descriptor of tile it+3 (stored after the barrier)
+    int32_t dword = 0;                       // descriptor of tile it+3 (stored at the end of the iteration)
     const bool fetch3 = tid < 16 && (long long)tile + 3ll * stride < n_tiles;
     if (fetch3) dword = __ldg(reinterpret_cast<const int32_t*>(&desc[tile + 3 * stride]) + tid);
     const float2 c = c_next;
@@ -358,74 +423,110 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
     const int r = d.rsf & 0xff, flag = d.rsf >> 16, n = d.n;
     const NfConst& kc = tab.row[r];
     const float4 g = kc.g;
-    const uint32_t sAU = smem_u32(S.arena[buf]), sAD = sAU + 8u * (uint32_t)d.up.cn;
-    uint16_t* sxD = S.sidx[buf][0];
-    uint16_t* sxU = S.sidx[buf][1];
-    // wait for the staged runs of this tile (each barrier serves every other tile)
-    while (!mbar_try_wait(&S.full[buf], (uint32_t)((it >> 1) & 1))) {}
-    // ---- phase 0 -------------------------------------------------------------------------------
-    if (flag == NF_STAGED) {
-      nf_slice_index(d.up, sAU, kc.uB.w, kc.uB.z, kc.uC.y, sxU, tid);
-      nf_slice_index(d.dn, sAD, kc.dB.w, kc.dB.z, kc.dC.y, sxD, tid);
-    }
-    __syncthreads();          // slice index complete; every thread is done with the previous tile (other buffer free)
-    if (tid == 0 && have_next) issue(S.desc[(it + 1) & 3], buf ^ 1);
-    if (fetch3) reinterpret_cast<int32_t*>(&S.desc[(it + 3) & 3])[tid] = dword;
-    // ---- phases A + B (thread = cluster) ---------------------------------------------------------
-    if (tid < n) {
-      int32_t bu = -1, bd = -1;
-      float best = 0.0f;
-      bool slow = false;
+    int* hist = S.hist[it & 1];
+    int* cnt = S.cnt[it & 1];
+    // wait for the staged runs of this tile (one barrier phase per tile)
+    while (!mbar_try_wait(&S.full, (uint32_t)(it & 1))) {}
+    // ---- phase A -------------------------------------------------------------------------------
+    int nu = 0, nd = 0;
+    bool slow = false;                         // m_*: result of the medium path (more than kNfK hits on a side)
+    int32_t m_bu = -1, m_bd = -1;
+    float m_best = 0.0f;
+    if (tid < n && flag != NF_NOLINK) {
+      uint32_t wd0, wd1, wu0, wu1;
+      int td, tu;
+      bool ok;
       if (flag == NF_STAGED) {
-        // z slices the two windows touch (monotone key function: a superset of the window), as staged runs
-        const int ud0 = bin_range(__fsub_rn(c.y, kc.uA.w), kc.uB.w, kc.uB.z, kc.uC.y) - d.up.s0;
-        const int ud1 = bin_range(__fadd_rn(c.y, kc.uA.w), kc.uB.w, kc.uB.z, kc.uC.y) - d.up.s0;
-        const int dd0 = bin_range(__fsub_rn(c.y, kc.dA.w), kc.dB.w, kc.dB.z, kc.dC.y) - d.dn.s0;
-        const int dd1 = bin_range(__fadd_rn(c.y, kc.dA.w), kc.dB.w, kc.dB.z, kc.dC.y) - d.dn.s0;
-        if (ud0 < 0 || ud1 >= d.up.nsl || dd0 < 0 || dd1 >= d.dn.nsl) {
-          slow = true;                                  // not covered by the staged slices
+        const uint32_t* sUB = reinterpret_cast<const uint32_t*>(S.arena + 8 * (d.up.cn + d.dn.cn));
+        ok = nf_runs(c, kc.dA, kc.dB, kc.dC, d.dn, sUB + d.up.bn, wd0, wd1, td);
+        ok = nf_runs(c, kc.uA, kc.uB, kc.uC, d.up, sUB, wu0, wu1, tu) && ok;
+      } else if (flag == NF_STAGED_C) {
+        ok = nf_runs(c, kc.dA, kc.dB, kc.dC, d.dn, bin_start + d.dn.b0, wd0, wd1, td);
+        ok = nf_runs(c, kc.uA, kc.uB, kc.uC, d.up, bin_start + d.up.b0, wu0, wu1, tu) && ok;
+      } else {
+        ok = false; wd0 = wd1 = wu0 = wu1 = 0;
+      }
+      if (ok) {
+        nd = nf_test_runs<K>(c, wd0, wd1, sArena + 8u * (uint32_t)d.up.cn, kc.dA.x, kc.dA.y, -g.x, sVecD + 8u * tid, sIdxD + 2u * tid);
+        nu = nf_test_runs<K>(c, wu0, wu1, sArena, kc.uA.x, kc.uA.y, g.y, sVecU + 8u * tid, sIdxU + 2u * tid);
+      }
+      if (ok && (nd > K || nu > K)) {               // dense region: decide now, while the staged runs are here
+        int iu, id;
+        if (nf_medium(c, wu0, wu1, wd0, wd1, sArena, sArena + 8u * (uint32_t)d.up.cn, kc.uA, kc.dA, g, m_best, iu, id)) {
+          if (iu >= 0) { m_bu = iu + d.up.c0; m_bd = id + d.dn.c0; }
         } else {
-          const int ju0 = sxU[ud0], ju1 = sxU[ud1 + 1], jd0 = sxD[dd0], jd1 = sxD[dd1 + 1];
-          const int nd = nf_test_run<K>(c, sAD, jd0, jd1, kc.dA.x, kc.dA.y, sListD);
-          const int nu = nd > 0 ? nf_test_run<K>(c, sAU, ju0, ju1, kc.uA.x, kc.uA.y, sListU) : 0;
-          if (nd > K || nu > K) {                       // dense region: no lists, nested loops over the runs
-            int iu, id;
-            if (nf_medium(c, sAU, ju0, ju1, sAD, jd0, jd1, kc.uA, kc.dA, g, best, iu, id)) {
-              if (iu >= 0) { bu = iu + d.up.c0; bd = id + d.dn.c0; }
-            } else {
-              slow = true;
-            }
-          } else if (nu > 0) {
-            // down vectors once: (y_c - y_d) * dxu = (y_d - y_c) * (-dxu), exact
-#pragma unroll 1
-            for (int k = 0; k < nd; ++k) {
-              const float2 v = lds_f2(sAD + 8u * lds_u16(sListD + (uint32_t)k * kIdxRow));
-              sts_f2(sVec + (uint32_t)k * kVecRow, __fmul_rn(__fsub_rn(v.x, c.x), -g.x), __fmul_rn(__fsub_rn(v.y, c.y), -g.x));
-            }
-            best = __int_as_float(0x7f800000);
-            int bi = 0, bk = 0;
-            bool tie = false;
-#pragma unroll 1
-            for (int i = 0; i < nu; ++i) {
-              const uint32_t ju = lds_u16(sListU + (uint32_t)i * kIdxRow);
-              const float2 v = lds_f2(sAU + 8u * ju);
-              const float Ay = __fmul_rn(__fsub_rn(v.x, c.x), g.y), Az = __fmul_rn(__fsub_rn(v.y, c.y), g.y);
-              uint32_t pb = sVec;
-#pragma unroll 1
-              for (int k = 0; k < nd; ++k, pb += kVecRow) {
-                const float2 b = lds_f2(pb);
-                const float ay = __fsub_rn(Ay, b.x), az = __fsub_rn(Az, b.y);
-                const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
-                tie = tie || (sc == best);
-                if (sc < best) { best = sc; bi = (int)ju; bk = k; }
-              }
-            }
-            if (tie) slow = true;
-            else { bu = bi + d.up.c0; bd = (int32_t)lds_u16(sListD + (uint32_t)bk * kIdxRow) + d.dn.c0; }
-          }
+          ok = false;                                       // exact tie: global slow path
         }
-      } else if (flag == NF_GLOBAL) {
-        slow = true;
+        nu = 0; nd = 0;
+      }
+      slow = !ok;
+      if (slow) { nu = 0; nd = 0; }
+      if (nu > 0 && nd > 0) atomicAdd(&hist[nd], nu);
+    }
+    __syncthreads();                                          // (1) phase A done: staging buffer free, histogram complete
+    if (tid == 0 && have_next) issue(S.desc[(it + 1) & 3]);
+    // ---- phase B1: emit one work item per up-side hit, counting-sorted by nd (descending) -------------
+    int n_items = 0;
+    {
+      int above = 0;                                          // items with a larger nd than this thread's
+#pragma unroll
+      for (int k = K; k >= 1; --k) {
+        const int h = hist[k];
+        if (k > nd) above += h;
+        n_items += h;
+      }
+      if (nu > 0 && nd > 0) {
+        const int slot = above + atomicAdd(&cnt[nd], nu);
+        const uint32_t code = (uint32_t)tid | (uint32_t)nd << 12;
+#pragma unroll 1
+        for (int k = 0; k < nu; ++k) S.items[slot + k] = (uint16_t)(code | (uint32_t)k << 8);
+      }
+    }
+    __syncthreads();                                          // (2) work items complete
+    if (tid < 16) { S.hist[(it + 1) & 1][tid] = 0; S.cnt[(it + 1) & 1][tid] = 0; }   // rows of the next tile
+    // ---- phase B2: thread i scores item i: one up-side hit against the nd down-side hits ---------------
+#pragma unroll 1
+    for (int i = tid; i < n_items; i += kNfThreads) {
+      const uint32_t item = S.items[i];
+      const uint32_t col = 8u * (item & 255u);
+      const uint32_t pa = sVecU + ((item >> 8) & 15u) * kVecRow + col;
+      const int ndd = (int)(item >> 12);
+      const float2 a = lds_f2(pa);
+      uint32_t pb = sVecD + col;
+      float best = __int_as_float(0x7f800000);
+      int bid = 0, tie = 0;
+#pragma unroll 1
+      for (int k = 0; k < ndd; ++k, pb += kVecRow) {
+        const float2 b = lds_f2(pb);
+        const float ay = __fsub_rn(a.x, b.x), az = __fsub_rn(a.y, b.y);
+        const float sc = __fadd_rn(__fmul_rn(ay, ay), __fmul_rn(az, az));
+        if (sc == best) tie = 256;
+        if (sc < best) { best = sc; bid = k; }
+      }
+      sts_f2(pa, best, __int_as_float(bid | tie));           // the hit's vector is consumed: reuse its slot
+    }
+    __syncthreads();                                          // (3) item results complete
+    // ---- phase C: minimum over the cluster's items, cut, stores -----------------------------------------
+    if (tid < n) {
+      int32_t bu = m_bu, bd = m_bd;
+      float best = m_best;
+      if (nu > 0 && nd > 0) {
+        best = __int_as_float(0x7f800000);
+        int bk = 0, bcode = 0, tie = 0;
+        uint32_t pr = sVecU + 8u * tid;
+#pragma unroll 1
+        for (int k = 0; k < nu; ++k, pr += kVecRow) {
+          const float2 res = lds_f2(pr);
+          const int code = __float_as_int(res.y);
+          if (res.x == best) tie = 256;
+          if (res.x < best) { best = res.x; bk = k; bcode = code; }
+          tie |= code & 256;
+        }
+        if (tie) slow = true;
+        else {
+          bu = (int32_t)lds_u16(sIdxU + (uint32_t)bk * kIdxRow + 2u * tid) + d.up.c0;
+          bd = (int32_t)lds_u16(sIdxD + (uint32_t)(bcode & 255) * kIdxRow + 2u * tid) + d.dn.c0;
+        }
       }
       if (slow) {
         const int s = (d.rsf >> 8) & 0xff;
@@ -435,8 +536,9 @@ k_neighbours(const __grid_constant__ NfTable tab, const float2* __restrict__ syz
       link_up[d.p0 + tid] = bu;
       link_dn[d.p0 + tid] = bd;
     }
-    // no barrier here: the next tile uses the other staging buffer and the other slice index; its phases A / B
-    // write only the thread's own list / vector columns.
+    if (fetch3) reinterpret_cast<int32_t*>(&S.desc[(it + 3) & 3])[tid] = dword;
+    // no barrier here: phase A of the next tile writes only the thread's own cache column, the other
+    // histogram row and (after its mbarrier wait) reads the staging buffer refilled after barrier (1).
   }
 }
 

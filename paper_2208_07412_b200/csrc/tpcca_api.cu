@@ -452,8 +452,12 @@ int tpcca_create(const tpcca_params* p, int cuda_device, void* cuda_stream, void
   }
   {
     int occ = 0;
-    const void* nf_fn = (const void*)k_neighbours<kNfK>;
-    const size_t nf_smem = sizeof(NfSmem<kNfK>);
+    // S2 kernel instance: the hit cache holds kNfK hits per side (5 blocks per SM) or, for dense time frames (more
+    // than ~0.7 clusters per grid bin at the context's capacity: windows with more than kNfK hits are common there
+    // and each one stalls its warp in the uncached path), kNfKDense hits (4 blocks per SM)
+    c->nf_dense = (double)c->N > 0.7 * (double)c->ns * (double)c->nb;
+    const void* nf_fn = c->nf_dense ? (const void*)k_neighbours<kNfKDense> : (const void*)k_neighbours<kNfK>;
+    const size_t nf_smem = c->nf_dense ? sizeof(NfSmem<kNfKDense>) : sizeof(NfSmem<kNfK>);
     cudaError_t e2 = cudaFuncSetAttribute(nf_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)nf_smem);
     if (e2 != cudaSuccess) {
       set_err(nullptr, TPCCA_E_CUDA, "tpcca_create: shared memory opt-in of k_neighbours failed: %s", cudaGetErrorString(e2));
@@ -607,9 +611,14 @@ int tpcca_run(tpcca_ctx* c, uint32_t mask) {
     NfTileDesc* nfd = c->at<NfTileDesc>(L.nf_desc);
     const int32_t* nf_ts = c->at<int32_t>(L.nf_tile_start);
     k_nf_plan<<<std::min(c->ns * c->nr, c->sm_count * 64), 128, 0, st>>>(T, sec, syz, bin_start, row_start, nf_ts, nfd);
-    k_neighbours<kNfK><<<grid, kNfThreads, sizeof(NfSmem<kNfK>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
-                                                                       nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
-                                                                       c->at<int32_t>(L.dn_raw));
+    if (c->nf_dense)
+      k_neighbours<kNfKDense><<<grid, kNfThreads, sizeof(NfSmem<kNfKDense>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
+                                                                                   nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
+                                                                                   c->at<int32_t>(L.dn_raw));
+    else
+      k_neighbours<kNfK><<<grid, kNfThreads, sizeof(NfSmem<kNfK>), st>>>(c->nftab, syz, bin_start, order, (uint32_t)(c->nb + 1),
+                                                                         nf_ts + (size_t)c->ns * c->nr, nfd, c->at<int32_t>(L.up_raw),
+                                                                         c->at<int32_t>(L.dn_raw));
     c->launches += 2;
   }
   mark(2);
@@ -806,7 +815,7 @@ int tpcca_get_work_counters(tpcca_ctx* c, int64_t out[5]) {
 
 int tpcca_get_info(const tpcca_ctx* c, int64_t out[8]) {
   if (!c || !out) return TPCCA_E_ARG;
-  out[0] = c->tab.slab_shift; out[1] = c->tab.n_cb; out[2] = kNfK; out[3] = c->sm_count;
+  out[0] = c->tab.slab_shift; out[1] = c->tab.n_cb; out[2] = c->nf_dense ? kNfKDense : kNfK; out[3] = c->sm_count;
   out[4] = c->nf_blocks_per_sm; out[5] = c->N; out[6] = c->CS; out[7] = (int64_t)c->L.total;
   return TPCCA_OK;
 }
