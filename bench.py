@@ -195,9 +195,45 @@ def _oracle_sector_job(job):
     from oracle import Oracle
     orc = Oracle(params)
     t0 = time.time()
-    orc.run(y, z, row, want=())
+    orc.run(y, z, row, want=())                      # the timed run: S1-S5, the five stages of the hot path
     dt = time.time() - t0
-    return dt, orc.run(y, z, row)
+    return dt, orc.run(y, z, row, stage_mask=0x7F)   # outputs for the parity check, S6 / S7 included
+
+
+def merge_properties(trk, tf, B):
+    """S8 at full size, where the oracle's all-pairs matching is out of reach: properties that hold at any size.  Links are
+    mutual, join neighbouring sectors of one side, the upper segment starts 1 .. mg_max_row_gap rows above the lower one,
+    and every chain head's segment count equals the length of its link chain."""
+    P = tf.params
+    per, ns = P.sectors_per_side, tf.n_sectors
+    outs = [trk.get_tracks(s, B.OUT_MERGE | B.OUT_TRACKS_SEL) for s in range(ns)]
+    n_links = n_chains = 0
+    for s, o in enumerate(outs):
+        m = o.merge
+        a = np.nonzero(m["next_sec"] >= 0)[0]
+        if a.size == 0:
+            continue
+        nsec, ntrk = m["next_sec"][a], m["next_trk"][a]
+        assert np.all(nsec // per == s // per) and np.all(np.isin((nsec % per - s % per) % per, (1, per - 1))), "not neighbours"
+        for t in np.unique(nsec):
+            sel = nsec == t
+            b = outs[t]
+            assert np.array_equal(b.merge["prev_sec"][ntrk[sel]], np.full(sel.sum(), s)), "prev_sec not mutual"
+            assert np.array_equal(b.merge["prev_trk"][ntrk[sel]], a[sel]), "prev_trk not mutual"
+            gap = b.first_row[ntrk[sel]] - o.last_row[a[sel]]
+            assert gap.min() >= 1 and gap.max() <= P.mg_max_row_gap, "row gap out of range"
+        n_links += int(a.size)
+        heads = np.nonzero((m["prev_sec"] < 0) & (m["next_sec"] >= 0))[0]
+        fitted = np.nonzero(m["n_seg"] > 0)[0]                  # (a chain whose top segment has no outer state is not refitted)
+        assert np.all(np.isin(fitted, heads)) and fitted.size >= 0.98 * heads.size, "chain heads"
+        for h in fitted[:: max(1, fitted.size // 200)]:        # a sample of the chains is walked
+            k, cs, ct = 1, s, int(h)
+            while outs[cs].merge["next_sec"][ct] >= 0:
+                cs, ct = int(outs[cs].merge["next_sec"][ct]), int(outs[cs].merge["next_trk"][ct])
+                k += 1
+            assert k == m["n_seg"][h], "n_seg"
+        n_chains += int(heads.size)
+    return dict(status="pass", n_links=n_links, n_chains=n_chains)
 
 
 def cpu_baseline_and_parity(args, tf, trk):
@@ -232,11 +268,25 @@ def cpu_baseline_and_parity(args, tf, trk):
                one_core_value=float(n_s / busy))
     orc = Oracle(tf.params)
     parity = dict(sectors=sectors, n_clusters=0, n_tracks=0, links_differing=0, membership="bit-exact",
-                  par_bit_exact=True, status="pass")
+                  par_bit_exact=True, n_selected=0, n_attached=0, s6_s7="bit-exact", status="pass")
+    B = sys.modules["paper_2208_07412_b200.binding"]
+    trk.run(0xFF)                                    # the same time frame once more, S6 - S8 included
+    trk.sync()
+    try:
+        parity["s8_properties"] = merge_properties(trk, tf, B)
+    except AssertionError as e:
+        parity.update(status="FAIL", error=f"S8 properties: {str(e)[:300]}")
     for s, (_, o) in zip(sectors, out):
-        g = trk.get_tracks(s)
+        g = trk.get_tracks(s, B.OUT_ALL | B.OUT_SELECTION | B.OUT_RESIDUALS)
         try:
             rep = compare_sector(g, o, orc, tf.row[s][o.order])
+            for f in ("owner", "n_own", "selected", "res_trk", "q_y", "q_z"):
+                if not np.array_equal(getattr(g, f), getattr(o, f)):
+                    raise AssertionError(f"S6/S7 output {f} differs")
+            for f in ("res_y", "res_z"):
+                if not np.array_equal(getattr(g, f), getattr(o, f).astype(np.float32)):
+                    raise AssertionError(f"S7 output {f} differs")
+            parity["n_selected"] += int(len(o.selected)); parity["n_attached"] += int((o.res_trk >= 0).sum())
         except AssertionError as e:
             parity.update(status="FAIL", error=f"sector {s}: {str(e)[:300]}")
             break
