@@ -491,6 +491,7 @@ def run_tpcca(args, env_cls=CudaEnv):
     # kernels of the other (PCIe is full duplex).  One host thread per context (ctypes releases the GIL).
     e2e_ms, e2e_n = e2e_serial_ms, e2e_steps
     e2e_mode = "serial, 1 context"
+    e2e_sel_stream_ms = None
     if not args.no_streaming:
         n_ctx = max(2, args.e2e_contexts)
         sides = [env.stream() for _ in range(n_ctx - 1)]
@@ -504,33 +505,38 @@ def run_tpcca(args, env_cls=CudaEnv):
             extra = None
             env.empty_cache()
         if extra:
-            for t in extra:
-                e2e_step(t)
-            env.synchronize()
             per = e2e_steps
 
-            def worker(t, delay):
-                env.set_thread_device()
-                time.sleep(delay)              # the contexts start a fraction of a step apart: the copies of one meet the kernels of another
-                for _ in range(per):
-                    e2e_step(t)
+            def stream_leg(selected, serial_ms):
+                for t in extra:
+                    e2e_step(t, selected)          # warm-up: grows the pinned arenas
+                env.synchronize()
 
-            barrier()
-            ev0.record()
-            step_s = 1e-3 * e2e_serial_ms / e2e_steps
-            th = [threading.Thread(target=worker, args=(t, i * step_s / n_ctx)) for i, t in enumerate([trk] + extra)]
-            for t in th:
-                t.start()
-            for t in th:
-                t.join()
-            for sd in sides:
-                env.wait_stream(sd)
-            ev1.record()
-            env.synchronize()
-            barrier()
-            e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
+                def worker(t, delay):
+                    env.set_thread_device()
+                    time.sleep(delay)              # the contexts start a fraction of a step apart: the copies of one meet the kernels of another
+                    for _ in range(per):
+                        e2e_step(t, selected)
+
+                barrier()
+                ev0.record()
+                step_s = 1e-3 * serial_ms / e2e_steps
+                th = [threading.Thread(target=worker, args=(t, i * step_s / n_ctx)) for i, t in enumerate([trk] + extra)]
+                for t in th:
+                    t.start()
+                for t in th:
+                    t.join()
+                for sd in sides:
+                    env.wait_stream(sd)
+                ev1.record()
+                env.synchronize()
+                barrier()
+                return max_over_ranks(ev0.elapsed_time(ev1))
+
+            e2e_ms = stream_leg(False, e2e_serial_ms)
             e2e_n = n_ctx * per
             e2e_mode = "streaming, %d contexts on %d streams" % (n_ctx, n_ctx)
+            e2e_sel_stream_ms = stream_leg(True, e2e_sel_serial_ms)
             for t in extra:
                 t.close()
         else:
@@ -611,7 +617,9 @@ def run_tpcca(args, env_cls=CudaEnv):
                                "selected tracks + owner instead of every tracklet",
                           e2e_selected=dict(value=n_all * e2e_steps_serial / (e2e_sel_serial_ms * 1e-3), unit=UNIT,
                                             ms_per_step=e2e_sel_serial_ms / e2e_steps_serial, d2h_bytes_per_step=d2h_sel,
-                                            h2d_bytes_per_step=h2d, mode="serial, 1 context")),
+                                            h2d_bytes_per_step=h2d, mode="serial, 1 context",
+                                            streaming_value=(n_all * e2e_n / (e2e_sel_stream_ms * 1e-3) if e2e_sel_stream_ms else None),
+                                            streaming_ms_per_step=(e2e_sel_stream_ms / e2e_n if e2e_sel_stream_ms else None))),
             gpu_launches=int(launches_per_step * args.steps),
             clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1),
         )
