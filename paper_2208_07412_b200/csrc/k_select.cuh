@@ -48,7 +48,7 @@ k_sel_claim(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     const uint32_t key = sel_key(nh, t_local);
     uint32_t* ok = own_key + sec[s].off;
     for (int k = lane; k < nh; k += 32) {
-      const int c = hit_idx[h0 + k];
+      const int c = __ldcs(&hit_idx[h0 + k]);      // streamed once: keep L2 for the keys
       // (plain read first: most clusters are claimed by three or four clones and only the first few raise the key)
       if (ok[c] < key) atomicMax(&ok[c], key);
     }
@@ -74,7 +74,7 @@ k_sel_count(const DevTables* __restrict__ T, const SectorDesc* __restrict__ sec,
     const uint32_t key = sel_key(nh, t - st->trk_off[s]);
     const uint32_t* ok = own_key + sec[s].off;
     int cnt = 0;
-    for (int k = lane; k < nh; k += 32) cnt += (ok[hit_idx[h0 + k]] == key) ? 1 : 0;
+    for (int k = lane; k < nh; k += 32) cnt += (ok[__ldcs(&hit_idx[h0 + k])] == key) ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) cnt += __shfl_down_sync(0xffffffffu, cnt, o);
     if (lane == 0) n_own[t] = cnt;
