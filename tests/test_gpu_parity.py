@@ -644,3 +644,21 @@ def test_merge_time_frame_and_degenerate_layouts(pkg):
         if nsec % per:
             assert rep["n_links"] == 0
         trk.close()
+
+
+def test_dense_slice_all_stages(pkg):
+    """S6-S8 at the occupancy of the ~4e8-cluster footprint (one orbit of the time-frame recipe at 2.75x
+    multiplicity, 36 sectors): selection, residual codes and merge links bit-exact, chain refits within 1e-4."""
+    from parity import compare_merge, compare_residuals, compare_selection
+    tf = tpcsynth.generate(2, n_orbits=1, mult_scale=2.75, seed=220807499)
+    trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters, workspace_fill=WS_FILL)
+    trk.load_timeframe(tf)
+    trk.run(0xFF)
+    trk.sync()
+    orc = Oracle(tf.params)
+    sel = compare_selection(trk, tf, orc, sectors=(0, 8, 17, 18, 30))
+    assert sel["n_selected"] > 200
+    compare_residuals(trk, tf, orc, sectors=(3, 21))
+    rep = compare_merge(trk, tf)
+    assert rep["n_links"] > 300 and rep["n_chains"] > 200
+    trk.close()
