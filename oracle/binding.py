@@ -57,6 +57,7 @@ def _load():
         lib.oracle_n_selected.restype = C.c_int64
         lib.oracle_get_selection.argtypes = [C.c_void_p] + [C.c_void_p] * 3
         lib.oracle_merge.argtypes = [C.POINTER(C.c_void_p), C.c_int]
+        lib.oracle_inject_selected.argtypes = [C.c_void_p, C.c_int32] + [C.c_void_p] * 4
         lib.oracle_get_merge_links.argtypes = [C.c_void_p] + [C.c_void_p] * 4 + [C.POINTER(C.c_int64)]
         lib.oracle_get_merged.argtypes = [C.c_void_p] + [C.c_void_p] * 9
         lib.oracle_kf_rotate.argtypes = [C.c_void_p, _dp, C.c_double, C.c_double]
@@ -292,6 +293,32 @@ def run_timeframe_merged(tf, precision="f32", sectors=None):
     for o in orcs:
         o.close()
     return res, out
+
+
+def merge_links_of_tables(params, sectors, precision="f32"):
+    """S8 matching on hand-made selected tracks (pins of the match decisions).  `sectors`: per sector a list of dicts
+    with first_row, last_row, x_ref, z_ref, par[5] and, for tracks that may be a lower segment, out = (x, p0..p4).
+    Returns per sector (next_sec, next_trk, prev_sec, prev_trk)."""
+    lib = _load()
+    orcs = [Oracle(params, precision) for _ in sectors]
+    for o, trks in zip(orcs, sectors):
+        n = len(trks)
+        ints = np.array([[t["first_row"], t["last_row"], 1 if t.get("out") is not None else 0] for t in trks], np.int32).reshape(n, 3)
+        ref = np.array([[t["x_ref"], t["z_ref"]] for t in trks], np.float64).reshape(n, 2)
+        par = np.array([t["par"] for t in trks], np.float64).reshape(n, 5)
+        out = np.array([t["out"] if t.get("out") is not None else [0.0] * 6 for t in trks], np.float64).reshape(n, 6)
+        lib.oracle_inject_selected(o._h, n, ints.ctypes.data, ref.ctypes.data, par.ctypes.data, out.ctypes.data)
+    handles = (C.c_void_p * len(orcs))(*[o._h for o in orcs])
+    lib.oracle_merge(handles, len(orcs))
+    res = []
+    for o, trks in zip(orcs, sectors):
+        k = len(trks)
+        a = [np.empty(k, np.int32) for _ in range(4)]
+        cnt = (C.c_int64 * 2)()
+        lib.oracle_get_merge_links(o._h, a[0].ctypes.data, a[1].ctypes.data, a[2].ctypes.data, a[3].ctypes.data, cnt)
+        res.append(tuple(x.tolist() for x in a))
+        o.close()
+    return res
 
 
 def select_tracks(n_clusters, hit_offset, hit_idx, max_shared_permille=500):

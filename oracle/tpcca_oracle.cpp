@@ -27,8 +27,10 @@
 // gate, tc_min_hits, search window / tie-break, chi2 gate, readings R2 / R3) by the
 // hand-worked toy tests/golden/toy_tracklets.txt and by the one-bin-per-row (brute-force
 // search) metamorphic pin; tests/mutation_check.py re-checks that one-line mutations of
-// those decisions fail a pin.  Nothing can be pinned to values the paper prints (it prints
-// none) -- "parity unpinned to the paper" in that sense only.
+// those decisions fail a pin.  S6 / S7 / S8 (added in round 2 as new code below the five
+// stages): hand-worked toys toy_selector.txt / toy_merge.txt, sort formulation, closed-form circle, exact circle
+// geometry in two sector frames, finite-difference Jacobian of Rotate, generator truth.  Nothing can be pinned to
+// values the paper prints (it prints none) -- "parity unpinned to the paper" in that sense only.
 // =========================================================================================
 #include <algorithm>
 #include <cmath>
@@ -884,6 +886,25 @@ int oracle_merge(void** handles, int n_sectors) {
     merge_sectors(S);
   }
   return 0;
+}
+// TEST HOOK for the S8 decision pins: replace the sector's selected tracks by hand-made ones (no clusters, no hit lists:
+// the chain refit then has nothing to fit).  Per track: ints = first_row, last_row, out_ok; ref = x_ref, z_ref;
+// par[5] = fitted state at x_ref; out[6] = outer state x, p0..p4.  No arithmetic happens here.
+void oracle_inject_selected(void* hv, int32_t n, const int32_t* ints, const double* ref, const double* par, const double* out) {
+  Handle* h = (Handle*)hv;
+#define INJ(o, R) do { \
+    (o)->n = 0; (o)->tracks.clear(); (o)->selected.clear(); (o)->out_state.clear(); (o)->out_ok.clear(); \
+    (o)->hit_offset.assign(1, 0); (o)->hit_idx.clear(); \
+    for (int32_t i = 0; i < n; ++i) { \
+      Track<R> t{}; t.x_ref = (R)ref[2 * i]; t.z_ref = (R)ref[2 * i + 1]; \
+      for (int q = 0; q < 5; ++q) t.p[q] = (R)par[5 * i + q]; \
+      t.first_row = ints[3 * i]; t.last_row = ints[3 * i + 1]; t.n_hits = 0; t.n_fit = 0; t.start_hit = -1; \
+      (o)->tracks.push_back(t); (o)->selected.push_back(i); (o)->hit_offset.push_back(0); \
+      KFState<R> st{}; st.x = (R)out[6 * i]; for (int q = 0; q < 5; ++q) st.p[q] = (R)out[6 * i + 1 + q]; \
+      for (int q = 0; q < 15; ++q) st.C[q] = (R)0; st.chi2 = (R)0; st.n = 0; \
+      (o)->out_state.push_back(st); (o)->out_ok.push_back((char)ints[3 * i + 2]); } } while (0)
+  if (h->precision == 0) INJ(h->f, float); else INJ(h->d, double);
+#undef INJ
 }
 // per selected track of the sector: partner above / below; returns the number of merged chains headed here and
 // (out[1]) the total number of their segments

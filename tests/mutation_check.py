@@ -43,6 +43,8 @@ M = [
  ("S8 rotate drops j10", lambda s: s.replace("const R j10 = -((s.p[3] * sa) / cf2);", "const R j10 = (R)0 * ((s.p[3] * sa) / cf2);")),
  ("S8 rotate drops j20", lambda s: s.replace("const R j20 = -((s.p[4] * Bc) * sa);", "const R j20 = (R)0 * ((s.p[4] * Bc) * sa);")),
  ("S8 rotate j22 inverted", lambda s: s.replace("const R j22 = cf2 / cf;", "const R j22 = cf / cf2;")),
+ ("S8 z pre-cut dropped", lambda s: s.replace("          if (!(std::fabs(zb - za) <= A.mg_zpre)) continue;\n", "")),
+ ("S8 dy window strict", lambda s: s.replace("if (!(std::fabs(dy) <= A.mg_dy && ", "if (!(std::fabs(dy) < A.mg_dy && ")),
  ("S8 tie -> larger sector/track", lambda s: s.replace("    if (sec != b.sec) return sec < b.sec;\n    return trk < b.trk;", "    if (sec != b.sec) return sec > b.sec;\n    return trk > b.trk;")),
 ]
 src = open(os.path.join(ROOT, "oracle", "tpcca_oracle.cpp")).read()

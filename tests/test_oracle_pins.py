@@ -1134,3 +1134,49 @@ def test_merge_row_gap_bounds_are_inclusive():
             b = res[mg[s].next_sec[ia]]
             gaps.append(int(b.first_row[b.selected[mg[s].next_trk[ia]]] - res[s].last_row[res[s].selected[ia]]))
     assert len(gaps) > 300 and min(gaps) == 1 and max(gaps) == 2 and gaps.count(2) > 20
+
+
+def test_merge_toy_worked_example():
+    """S8 match decisions on hand-made tracks (tests/golden/toy_merge.txt): inclusive window edges, row-gap bounds,
+    the z pre-cut, mutual best without fall-back, ties by (sector, track), chains through three sectors."""
+    import os
+    from oracle import merge_links_of_tables
+    P = tpcsynth.default_params(n_sectors=6, row_x=64.0 + np.arange(32), sigma=0.125)
+    P = P.copy(sectors_per_side=3, sector_cos=1.0, sector_sin=0.0, mg_max_row_gap=8, mg_dy=1.0, mg_dz=1.0, mg_dsin=0.0625,
+               mg_zpre=32.0)
+    sectors = [[] for _ in range(6)]
+    where, links = {}, []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "toy_merge.txt")):
+        f = line.split("#")[0].split()
+        if not f:
+            continue
+        if f[0] == "link":
+            links.append((f[1], f[2]))
+            continue
+        kind, name, s = f[0], f[1], int(f[2])
+        if kind == "lower":
+            last, y, zref = int(f[3]), float(f[4]), float(f[5])
+            noout = "noout" in f
+            p3 = float(f[6]) if len(f) > 6 and f[6] != "noout" else 0.0
+            t = dict(first_row=0, last_row=last, x_ref=64.0, z_ref=zref, par=[y, 0.0, 0.0, p3, 0.0],
+                     out=None if noout else [64.0 + last, y, 0.0, 0.0, p3, 0.0])
+        elif kind == "upper":
+            first, y, zref = int(f[3]), float(f[4]), float(f[5])
+            p1 = float(f[6]) if len(f) > 6 else 0.0
+            sp = float(f[7]) if len(f) > 7 else 0.0
+            t = dict(first_row=first, last_row=31, x_ref=64.0 + first, z_ref=zref, par=[y, p1, sp, 0.0, 0.0], out=None)
+        else:   # mid: first_row last_row y z_ref -- both an upper and a lower segment
+            first, last, y, zref = int(f[3]), int(f[4]), float(f[5]), float(f[6])
+            t = dict(first_row=first, last_row=last, x_ref=64.0 + first, z_ref=zref, par=[y, 0.0, 0.0, 0.0, 0.0],
+                     out=[64.0 + last, y, 0.0, 0.0, 0.0, 0.0])
+        where[name] = (s, len(sectors[s]))
+        sectors[s].append(t)
+    assert len(links) == 13 and len(where) == 42
+    for precision in ("f32", "f64"):
+        got = merge_links_of_tables(P, sectors, precision)
+        want = [([-1] * len(t), [-1] * len(t), [-1] * len(t), [-1] * len(t)) for t in sectors]
+        for lo, up in links:
+            (sa, ia), (sb, ib) = where[lo], where[up]
+            want[sa][0][ia] = sb; want[sa][1][ia] = ib; want[sb][2][ib] = sa; want[sb][3][ib] = ia
+        for s in range(6):
+            assert got[s] == tuple(want[s]), (precision, s, got[s], want[s])
