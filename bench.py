@@ -51,8 +51,8 @@ def load_peaks():
 
 def ncu_traffic(args, n_clusters):
     """dram bytes read + written per launch of the S2 kernels from the committed ncu capture of this workload
-    (profiles/r1_traffic.txt), or None when the workload differs from the captured one."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.txt")
+    (profiles/r2_traffic.txt), or None when the workload differs from the captured one."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.txt")
     if not os.path.exists(p):
         return None
     d = json.load(open(p))
