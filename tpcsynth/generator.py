@@ -248,6 +248,9 @@ def generate(config: int, seed: int | None = None, mult_scale: float = 1.0,
             parts = list(ex.map(one, range(n_coll)))
     else:
         parts = [one(c) for c in range(n_coll)]
+    if not parts:       # a Poisson draw of zero collisions: an empty time frame is a legal input (reading N8)
+        e = np.empty(0)
+        parts = [(e.astype(np.uint8), e.astype(np.uint8), e.astype(np.float32), e.astype(np.float32), e.astype(np.int32))]
     sec = np.concatenate([p[0] for p in parts])
     row = np.concatenate([p[1] for p in parts])
     y = np.concatenate([p[2] for p in parts])
