@@ -901,7 +901,8 @@ void oracle_inject_selected(void* hv, int32_t n, const int32_t* ints, const doub
       t.first_row = ints[3 * i]; t.last_row = ints[3 * i + 1]; t.n_hits = 0; t.n_fit = 0; t.start_hit = -1; \
       (o)->tracks.push_back(t); (o)->selected.push_back(i); (o)->hit_offset.push_back(0); \
       KFState<R> st{}; st.x = (R)out[6 * i]; for (int q = 0; q < 5; ++q) st.p[q] = (R)out[6 * i + 1 + q]; \
-      for (int q = 0; q < 15; ++q) st.C[q] = (R)0; st.chi2 = (R)0; st.n = 0; \
+      for (int q = 0; q < 15; ++q) { st.C[q] = (R)0; } \
+      st.chi2 = (R)0; st.n = 0; \
       (o)->out_state.push_back(st); (o)->out_ok.push_back((char)ints[3 * i + 2]); } } while (0)
   if (h->precision == 0) INJ(h->f, float); else INJ(h->d, double);
 #undef INJ
