@@ -218,7 +218,9 @@ int tpcca_reset(tpcca_ctx *ctx);
  * context's stream.  A stage needs the outputs of the stages before it from this or an earlier
  * run on the same clusters (TPCCA_E_STATE otherwise).  Device-side failures (row out of range,
  * start-hit capacity overflow) are reported by the next tpcca_get_* / tpcca_sync call.
- * Errors: TPCCA_E_STATE, TPCCA_E_CUDA. */
+ * The tables of S6-S8 live in workspace regions that S1 / S5 use as scratch: a later run of S1 or S5 without S6 (S7,
+ * S8) invalidates them (they are then reported as not run, never delivered stale).
+ * Errors: TPCCA_E_STATE, TPCCA_E_CUDA (the message names the stage whose launch failed). */
 int tpcca_run(tpcca_ctx *ctx, uint32_t stage_mask);
 
 /* Wait for the stream and report device-side failures of the last run (TPCCA_E_RANGE,
