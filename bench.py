@@ -46,7 +46,7 @@ def load_peaks():
     if os.path.exists(p):
         d = json.load(open(p))
         return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
-    return dict(hbm_gbs=7700.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md nominal)")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback (B200_PROFILING.md: 6.65 TB/s)")
 
 
 def ncu_traffic(args, n_clusters):
