@@ -418,6 +418,13 @@ class Tracker:
         """tpcca_get_tracks(HOST) -> numpy copies."""
         return output_from_view(self.get_tracks_view(sector, MEM_HOST, what), what, self.n_rows)
 
+    def get_tracks_all_views(self, mem_space: int = MEM_HOST, what: int = OUT_ALL):
+        """Raw tpcca_get_tracks_all: the views of every sector (HOST: one arena, one synchronise; valid until the next
+        HOST fetch)."""
+        views = (_View * self.n_sectors)()
+        self._check(self._lib.tpcca_get_tracks_all(self._h, int(mem_space), int(what), views))
+        return views
+
     def get_tracks_all(self, what: int = OUT_ALL):
         """tpcca_get_tracks_all(HOST): every sector behind one synchronise -> list of SectorOutput."""
         views = (_View * self.n_sectors)()

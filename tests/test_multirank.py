@@ -121,6 +121,9 @@ class _FakeTracker:
     def get_tracks_view(self, s, mem, what):
         return _FakeView(self.sec[s])
 
+    def get_tracks_all_views(self, mem, what):
+        return [_FakeView(n) for n in self.sec]
+
     def close(self):
         pass
 
