@@ -315,6 +315,50 @@ const char *tpcca_pipeline_last_error(const tpcca_pipeline *p);
 
 void tpcca_pipeline_destroy(tpcca_pipeline *p);
 
+/* ---- S4 start-hit selection without any allocation (BASELINE.json:5 "start-hit selection") ------
+ * For callers that cannot obtain device memory of their own at the moment of the call and hold no tpcca context:
+ * a step of an online framework whose GPU memory was handed out once, in full, at start of run (a cudaMalloc there
+ * has nothing left to take, and cudaMalloc / cudaFree stall all streams of the GPU while other time frames are being
+ * processed); a plug-in living under a caching allocator (e.g. PyTorch's), which cannot see or reuse memory taken
+ * behind its back; a monitoring hook that has the two link arrays of a sector and nothing else.  The regular path
+ * (tpcca_create + tpcca_run) does not serve them: it needs a caller-allocated workspace and creates events, a copy
+ * stream and pinned host buffers.
+ *
+ * This call creates and allocates NOTHING (no cudaMalloc / cudaFree / cudaMallocHost, no stream or event, no
+ * allocating library routine).  The scratch the stage needs -- one count and one offset per 2048-cluster tile --
+ * is a fixed 64 KiB array inside the library image; every GPU the library is used on holds those 64 KiB until the
+ * process exits.  That fixes the limit: n_clusters <= TPCCA_NOALLOC_MAX_CLUSTERS (16 777 216, four config-3
+ * sectors); a larger n_clusters is refused with TPCCA_E_ARG before anything is launched.
+ *
+ * Computes  start_hit = [ c ascending in [0, n_clusters) : link_dn[c] == -1 and link_up[c] >= 0 ]  on the CLEANED
+ * links of ONE sector (the link_up / link_dn of tpcca_tracks_view, or the caller's own), i.e. exactly what stage S4
+ * of tpcca_run writes.
+ *   cuda_device, cuda_stream  device and cudaStream_t (NULL = default stream) the three kernels are queued on; the
+ *                             call is asynchronous and leaves the caller's current device as it found it.
+ *   link_up, link_dn          DEVICE, int32[n_clusters], read only (may be NULL when n_clusters == 0).
+ *   start_hit                 DEVICE, int32[max_start_hits], output; slots >= *n_start are not written.
+ *   n_start                   DEVICE, int32[1], output: the number of start hits FOUND.  If it exceeds
+ *                             max_start_hits only the first max_start_hits were stored; the caller compares (the call
+ *                             does not wait for the GPU, so it cannot report this itself).
+ *   err_msg, err_msg_len      HOST buffer for the message of a failing call (may be NULL / 0); "" on success.
+ * All arrays are the caller's and must stay valid until the stream has passed the call.
+ *
+ * The scratch is ONE array per GPU, shared by every call in the process, and keeps the numbers of the previous
+ * call.  No part of it has to be zero on entry (each call overwrites what it later reads), so consecutive calls on
+ * one stream, of any sizes, are independent.  Calls that can be on the same GPU at the same time -- two streams, or
+ * two host threads with their own streams -- overwrite each other's counts and give wrong start hits: put them on one
+ * stream or order them with events.
+ *
+ * The first call on a device does a one-time set-up: it asks the CUDA runtime for the device address of the scratch
+ * (which makes the runtime load the library's code on that device if it has not yet).  Make that first call during
+ * initialisation, outside any stream capture; later calls only queue three kernels.
+ * Errors: TPCCA_E_ARG (negative or too large sizes, NULL pointers, cuda_device outside 0..63), TPCCA_E_CUDA (no
+ * device -- there is no CPU path --, set-up or launch failure). */
+#define TPCCA_NOALLOC_MAX_CLUSTERS 16777216
+int tpcca_start_hits_noalloc(int cuda_device, void *cuda_stream, const int32_t *link_up, const int32_t *link_dn,
+                             int64_t n_clusters, int32_t *start_hit, int64_t max_start_hits, int32_t *n_start,
+                             char *err_msg, size_t err_msg_len);
+
 /* Library version string, e.g. "tpcca 0.1 (sm_100a)". */
 const char *tpcca_version(void);
 

@@ -27,7 +27,7 @@ ABI_SYMBOLS = ("tpcca_workspace_bytes", "tpcca_create", "tpcca_load_clusters", "
                "tpcca_sync", "tpcca_get_tracks", "tpcca_get_counts", "tpcca_get_timings", "tpcca_get_work_counters",
                "tpcca_get_launch_count", "tpcca_get_info", "tpcca_get_tracks_all", "tpcca_pipeline_workspace_bytes",
                "tpcca_pipeline_create", "tpcca_pipeline_run", "tpcca_pipeline_get_groups", "tpcca_pipeline_last_error",
-               "tpcca_pipeline_destroy", "tpcca_last_error", "tpcca_destroy", "tpcca_version")
+               "tpcca_pipeline_destroy", "tpcca_last_error", "tpcca_destroy", "tpcca_version", "tpcca_start_hits_noalloc")
 OUT_ORDER, OUT_GRID, OUT_LINKS_RAW, OUT_LINKS, OUT_START, OUT_TRACKS, OUT_ALL = 1, 2, 4, 8, 16, 32, 63
 OUT_SELECTION, OUT_TRACKS_SEL, OUT_RESIDUALS, OUT_MERGE = 64, 128, 256, 512
 
@@ -123,6 +123,8 @@ def load_library():
     lib.tpcca_destroy.argtypes = [C.c_void_p]
     lib.tpcca_destroy.restype = None
     lib.tpcca_version.restype = C.c_char_p
+    lib.tpcca_start_hits_noalloc.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_int64,
+                                             C.c_void_p, C.c_char_p, C.c_size_t]
     _lib = lib
     return lib
 
@@ -178,6 +180,41 @@ def workspace_bytes(params, max_clusters: int, max_start_hits: int = 0) -> int:
     if rc:
         raise TpccaError(rc, lib.tpcca_last_error(None).decode())
     return int(out.value)
+
+
+#: size limit of start_hits_noalloc (TPCCA_NOALLOC_MAX_CLUSTERS in include/tpcca.h)
+NOALLOC_MAX_CLUSTERS = 1 << 24
+
+
+def start_hits_noalloc(link_up, link_dn, start_hit, n_start, stream=None):
+    """tpcca_start_hits_noalloc: S4 start-hit selection on the cleaned links of one sector, for callers that may
+    not allocate device memory (a step inside a framework that owns all of the GPU's memory, a plug-in under a
+    caching allocator, a hook without a tpcca context) -- include/tpcca.h says who they are and why.
+
+    Every buffer is the caller's: `link_up`, `link_dn` int32 CUDA tensors of equal length (inputs), `start_hit` an
+    int32 CUDA tensor whose length is the capacity, `n_start` an int32 CUDA tensor of one element.  Neither this
+    wrapper nor the C call allocates; the call queues three kernels on `stream` (default: torch's current stream)
+    and returns.  Afterwards n_start[0] holds the number of start hits found and start_hit[:n_start[0]] the hits in
+    ascending position (only the first len(start_hit) are stored if more were found).  At most
+    NOALLOC_MAX_CLUSTERS links per call (TpccaError beyond); calls that overlap on one GPU share the library's
+    fixed scratch and race -- keep them on one stream.  Argument marshalling only."""
+    import torch
+    lib = load_library()
+    for name, t in (("link_up", link_up), ("link_dn", link_dn), ("start_hit", start_hit), ("n_start", n_start)):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous()):
+            raise TypeError(f"{name} must be a contiguous int32 CUDA tensor")
+    if link_up.numel() != link_dn.numel() or n_start.numel() != 1:
+        raise ValueError("link_up and link_dn must have the same length, n_start exactly one element")
+    dev = link_up.device
+    if any(t.device != dev for t in (link_dn, start_hit, n_start)):
+        raise ValueError("all tensors must be on the same device")
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    msg = C.create_string_buffer(512)
+    rc = lib.tpcca_start_hits_noalloc(dev.index, C.c_void_p(st.cuda_stream), C.c_void_p(link_up.data_ptr()),
+                                      C.c_void_p(link_dn.data_ptr()), link_up.numel(), C.c_void_p(start_hit.data_ptr()),
+                                      start_hit.numel(), C.c_void_p(n_start.data_ptr()), msg, len(msg))
+    if rc:
+        raise TpccaError(rc, msg.value.decode())
 
 
 @dataclasses.dataclass

@@ -15,8 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpcca.so")
-SOURCES = ["tpcca_api.cu"]
-DEPS = ["tpcca_api.cu", "tpcca_pipeline.cuh", "tpcca_dev.cuh", "k_grid.cuh", "k_links.cuh", "k_tracklets.cuh", "k_select.cuh", "k_merge.cuh"]
+SOURCES = ["tpcca_api.cu", "tpcca_noalloc.cu"]
+DEPS = ["tpcca_api.cu", "tpcca_noalloc.cu", "tpcca_pipeline.cuh", "tpcca_dev.cuh", "k_grid.cuh", "k_links.cuh", "k_tracklets.cuh", "k_select.cuh", "k_merge.cuh"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "--fmad=false", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",
