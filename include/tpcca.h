@@ -250,7 +250,8 @@ int tpcca_get_counts(tpcca_ctx *ctx, int64_t out[7]);
 
 /* Device time of each stage [ms] of the run `runs_back` runs ago (0 = the last tpcca_run; the
  * context keeps the events of its last 16 runs), from CUDA events recorded on the context's
- * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6, ms[7] = S7, ms[8] = S8 (0 if not run).
+ * stream around the stages; ms[0..4] = S1..S5, ms[5] = S1..S5 together, ms[6] = S6, ms[7] = S7, ms[8] = S8.  A stage
+ * that was not in that run's stage_mask reports exactly 0 (ms[5] spans whichever of S1..S5 ran).
  * Synchronises the stream.
  * Errors: TPCCA_E_ARG (runs_back outside 0..15), TPCCA_E_STATE (no such run). */
 int tpcca_get_timings(tpcca_ctx *ctx, int runs_back, float ms[9]);
@@ -290,17 +291,22 @@ typedef struct tpcca_pipeline tpcca_pipeline;
 int tpcca_pipeline_workspace_bytes(const tpcca_params *params, int n_groups, int64_t max_clusters_group,
                                    int64_t max_start_hits_group, size_t *out_bytes);
 
-/* cuda_streams[g] (distinct cudaStream_t of cuda_device) and workspaces[g] (DEVICE, 256-byte aligned,
- * workspace_bytes_each bytes) are owned by the caller until tpcca_pipeline_destroy.  Errors as tpcca_create. */
+/* cuda_streams[g] (n_groups pairwise distinct cudaStream_t of cuda_device; TPCCA_E_ARG if any two are equal) and
+ * workspaces[g] (DEVICE, 256-byte aligned, workspace_bytes_each bytes) are owned by the caller until
+ * tpcca_pipeline_destroy.  Errors as tpcca_create. */
 int tpcca_pipeline_create(const tpcca_params *params, int cuda_device, int n_groups, void *const *cuda_streams,
                           void *const *workspaces, size_t workspace_bytes_each, int64_t max_clusters_group,
                           int64_t max_start_hits_group, tpcca_pipeline **out);
 
 /* One time frame through the pipeline.  n[s], y[s], z[s], row[s]: the clusters of sector s (arrays of n_sectors
  * entries; HOST -- pinned memory lets the copies overlap -- or DEVICE per mem_space; they must stay valid until the
- * call returns).  stage_mask / what as for tpcca_run / tpcca_get_tracks.  views[s] (HOST array of n_sectors views)
- * receives HOST pointers into the pinned arenas of the groups, valid until the next run of this pipeline.  Blocks
- * until every group has delivered.  Errors: those of tpcca_load_clusters / tpcca_run / tpcca_get_tracks of any group
+ * call returns; DEVICE arrays are copied on the groups' streams, which know nothing of the stream that produced them:
+ * the producer must have finished, or every group stream must be made to wait for it (cudaStreamWaitEvent), before
+ * the call -- the Python binding does the latter with torch's current stream).  stage_mask / what as for tpcca_run /
+ * tpcca_get_tracks, EXCEPT cross-sector merging: the groups are separate contexts that never see each other's tracks,
+ * so TPCCA_STAGE_MERGE / TPCCA_OUT_MERGE are refused with TPCCA_E_ARG (run S8 on one context over all sectors).
+ * views[s] (HOST array of n_sectors views) receives HOST pointers into the pinned arenas of the groups, valid until
+ * the next run of this pipeline.  Blocks until every group has delivered.  Errors: those of tpcca_load_clusters / tpcca_run / tpcca_get_tracks of any group
  * (message names the group). */
 int tpcca_pipeline_run(tpcca_pipeline *p, const int64_t *n, const float *const *y, const float *const *z,
                        const uint16_t *const *row, int mem_space, uint32_t stage_mask, uint32_t what,

@@ -143,7 +143,10 @@ k_mg_match(const DevTables* __restrict__ T, const DevStatus* __restrict__ st, Se
   out.p0 = B.out_p[ka]; out.p1 = B.out_p[cs + ka]; out.p2 = B.out_p[2 * cs + ka]; out.p3 = B.out_p[3 * cs + ka]; out.p4 = B.out_p[4 * cs + ka];
   kf_reset_cov(out, K);                     // zero covariance: only the mean is used
   const float za = zref_a + out.p1;
-  const int zb0 = mg_zbucket(za - M.zpre, M), zb1 = mg_zbucket(za + M.zpre, M);
+  // One bucket more on each side than fl(za -+ zpre) fall in: the pre-cut below is |fl(zb - za)| <= zpre, and a zb one
+  // ulp beyond fl(za + zpre) can still pass it after rounding while sitting across a bucket edge.  The extra
+  // buckets only add candidates that the exact pre-cut then rejects, so no other result changes.
+  const int zb0 = max(mg_zbucket(za - M.zpre, M) - 1, 0), zb1 = min(mg_zbucket(za + M.zpre, M) + 1, M.n_zb - 1);
   unsigned long long best = ~0ull;
   for (int dir = 0; dir < 2; ++dir) {
     const int nsec = side * per + (dir == 0 ? (loc + 1) % per : (loc + per - 1) % per);

@@ -801,6 +801,11 @@ int tpcca_get_timings(tpcca_ctx* c, int runs_back, float ms[9]) {
   CU(c, cudaEventElapsedTime(&ms[6], c->ev[k][5], c->ev[k][6]));
   CU(c, cudaEventElapsedTime(&ms[7], c->ev[k][6], c->ev[k][7]));
   CU(c, cudaEventElapsedTime(&ms[8], c->ev[k][7], c->ev[k][8]));
+  // the events around a stage are recorded whether or not the stage ran: a stage outside the run's mask would show
+  // the few microseconds between two records.  The header promises 0 for it.
+  const uint32_t m = c->ev_mask[k];
+  for (int i = 0; i < 5; ++i) if (!(m & (1u << i))) ms[i] = 0.f;
+  for (int i = 6; i < 9; ++i) if (!(m & (1u << (i - 1)))) ms[i] = 0.f;
   return TPCCA_OK;
 }
 

@@ -51,11 +51,14 @@ int tpcca_pipeline_create(const tpcca_params* params, int cuda_device, int n_gro
   p->first.resize(n_groups + 1);
   for (int g = 0; g <= n_groups; ++g) p->first[g] = (int)((int64_t)g * p->ns / n_groups);
   p->ms.assign(n_groups, 0.f);
+  for (int g = 1; g < n_groups; ++g)
+    for (int h = 0; h < g; ++h)
+      if (cuda_streams[g] == cuda_streams[h]) {      // any two groups on one stream would run one after the other
+        tpcca_pipeline_destroy(p);
+        return pipe_err(nullptr, TPCCA_E_ARG, "every group needs its own stream (groups " + std::to_string(h) + " and " +
+                                              std::to_string(g) + " share one)");
+      }
   for (int g = 0; g < n_groups; ++g) {
-    if (g > 0 && cuda_streams[g] == cuda_streams[g - 1]) {
-      tpcca_pipeline_destroy(p);
-      return pipe_err(nullptr, TPCCA_E_ARG, "every group needs its own stream");
-    }
     tpcca_params q = *params;
     q.n_sectors = p->first[g + 1] - p->first[g];
     tpcca_ctx* c = nullptr;
@@ -76,6 +79,11 @@ int tpcca_pipeline_run(tpcca_pipeline* p, const int64_t* n, const float* const* 
                        const uint16_t* const* row, int mem_space, uint32_t stage_mask, uint32_t what,
                        tpcca_tracks_view* views) {
   if (!p || !n || !y || !z || !row || !views) return pipe_err(p, TPCCA_E_ARG, "NULL argument");
+  // S8 links tracks ACROSS sectors; a group is a context of its own with group-local sector numbers, so it would
+  // miss every link over a group boundary and number the others wrongly.  Refused instead of delivered wrong.
+  if ((stage_mask & TPCCA_STAGE_MERGE) || (what & TPCCA_OUT_MERGE))
+    return pipe_err(p, TPCCA_E_ARG, "the pipeline runs sector groups independently: TPCCA_STAGE_MERGE / TPCCA_OUT_MERGE "
+                                    "(cross-sector merging) need one context over all sectors (tpcca_run)");
   std::vector<int> rc(p->ng, TPCCA_OK);
   std::vector<std::string> msg(p->ng);
   // the groups issue their loads in group order (group g + 1 queues its H2D copies after group g), so the copy

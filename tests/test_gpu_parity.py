@@ -591,6 +591,81 @@ def test_pipeline_device_inputs_and_errors(pkg, cfg1_small):
         pkg.Pipeline(tf.params, 99, max_clusters_group=1000)
 
 
+def test_pipeline_device_inputs_still_being_written(pkg, cfg1_small):
+    """Device inputs whose upload is still queued on the caller's stream when the pipeline is called: the groups'
+    streams must wait for it (they used to copy at once and could read the buffers before the data had arrived)."""
+    import torch
+    tf = cfg1_small
+    pipe = pkg.Pipeline(tf.params, 3, max_clusters_group=tf.n_clusters)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    hy = [pin(a) for a in tf.y]; hz = [pin(a) for a in tf.z]; hr = [pin(a.astype(np.int16)) for a in tf.row]
+    y = [torch.zeros_like(a, device="cuda") for a in hy]; z = [torch.zeros_like(a, device="cuda") for a in hz]
+    row = [torch.zeros_like(a, device="cuda") for a in hr]
+    torch.cuda.synchronize()
+    torch.cuda._sleep(400_000_000)                  # ~0.2 s of busy waiting on the current stream, then the uploads
+    for d, h in zip(y + z + row, hy + hz + hr):
+        d.copy_(h, non_blocking=True)
+    outs = pipe.run(y, z, [r.view(torch.uint16) for r in row])
+    orc = Oracle(tf.params)
+    for s in (0, 13, 35):
+        o = orc.run(tf.y[s], tf.z[s], tf.row[s])
+        compare_sector(outs[s], o, orc, tf.row[s][o.order])
+    pipe.close()
+
+
+def test_pipeline_refuses_merge_and_shared_streams(pkg, cfg1_small):
+    """S8 crosses sectors and a group only knows its own: the pipeline refuses it (it used to run it per group, with
+    links over group boundaries missing and group-local sector numbers).  Any two groups on one stream are refused at
+    create, not only neighbouring ones."""
+    import ctypes as C
+    import torch
+    from paper_2208_07412_b200 import binding as B
+    tf = cfg1_small
+    pipe = pkg.Pipeline(tf.params, 2, max_clusters_group=tf.n_clusters)       # 2 x 18 sectors: group = TPC side
+    for mask, what in ((0xFF, B.OUT_ALL), (0x7F, B.OUT_ALL | B.OUT_MERGE), (0xFF, B.OUT_ALL | B.OUT_MERGE)):
+        with pytest.raises(pkg.TpccaError) as e:
+            pipe.run(tf.y, tf.z, tf.row, stage_mask=mask, what=what)
+        assert e.value.code == -1 and "MERGE" in str(e.value)
+    outs = pipe.run(tf.y, tf.z, tf.row, stage_mask=0x7F, what=B.OUT_ALL | B.OUT_SELECTION)   # still usable afterwards
+    assert sum(o.n_tracks for o in outs) > 1000 and all(o.merge is None for o in outs)
+    lib = pkg.load_library()
+    p, keep = B._make_params(tf.params)
+    a, b = torch.cuda.Stream(), torch.cuda.Stream()
+    nbytes = pipe.workspace_bytes_each                                         # sized for 18 sectors: enough for 12
+    ws = [torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda:0") for _ in range(3)]
+    wsp = (C.c_void_p * 3)(*[(w.data_ptr() + 255) // 256 * 256 for w in ws])
+    for order, ok in (((a, b, a), False), ((a, a, b), False), ((a, b, torch.cuda.Stream()), True)):
+        st = (C.c_void_p * 3)(*[x.cuda_stream for x in order])
+        h = C.c_void_p()
+        rc = lib.tpcca_pipeline_create(C.byref(p), 0, 3, st, wsp, nbytes, tf.n_clusters, 0, C.byref(h))
+        if ok:
+            assert rc == 0 and h.value
+            lib.tpcca_pipeline_destroy(h)
+        else:
+            assert rc == -1 and not h.value and "own stream" in lib.tpcca_pipeline_last_error(None).decode()
+    pipe.close()
+
+
+def test_timings_are_zero_for_stages_not_run(pkg, cfg1_small):
+    """tpcca_get_timings: a stage outside the run's mask reports exactly 0 (the events around it are recorded all the
+    same, microseconds apart)."""
+    tf = cfg1_small
+    trk = pkg.Tracker(tf.params, max_clusters=tf.n_clusters)
+    trk.load_timeframe(tf)
+    trk.run(0x03); trk.sync()
+    t = trk.timings()
+    assert t[0] > 0 and t[1] > 0 and t[5] > 0 and t[2] == t[3] == t[4] == t[6] == t[7] == t[8] == 0.0
+    trk.run(0x1C); trk.sync()                       # S3-S5 on top of the S1 / S2 outputs
+    t = trk.timings()
+    assert t[0] == t[1] == 0.0 and min(t[2:6]) > 0 and t[6] == t[7] == t[8] == 0.0
+    trk.run(0x7F); trk.sync()
+    t = trk.timings()
+    assert min(t[:8]) > 0 and t[8] == 0.0           # S8 not run: 0, not the gap between two event records
+    t1 = trk.timings(2)
+    assert t1[0] > 0 and t1[2] == 0.0               # the ring keeps each run's own mask
+    trk.close()
+
+
 def test_get_tracks_all_equals_per_sector(pkg, cfg1_small):
     tf = cfg1_small
     trk = run_gpu(pkg, tf)
@@ -614,7 +689,8 @@ def test_merge_config1_and_config4(pkg, cfg1_small):
         trk.sync()
         rep = compare_merge(trk, tf)
         assert rep["n_links"] > 0.2 * rep["n_selected"] and rep["n_chains"] > 0
-        assert trk.timings()[8] > 0.0
+        t = trk.timings()
+        assert all(v > 0.0 for v in t)           # every stage of mask 0xFF ran and was timed
         compare_timeframe(trk, tf, Oracle(tf.params), sectors=(0, 19))       # S1-S5 outputs untouched by S6-S8
         trk.close()
 
