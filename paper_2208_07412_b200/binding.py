@@ -479,6 +479,7 @@ class Pipeline:
         if not torch.cuda.is_available():
             raise TpccaError(-3, "no CUDA device: tpcca has no CPU path")
         self.n_sectors, self.n_rows, self.n_groups = int(params.n_sectors), int(params.n_rows), int(n_groups)
+        self._torch, self.device = torch, int(device)
         p, self._keep = _make_params(params)
         nbytes = C.c_size_t(0)
         rc = self._lib.tpcca_pipeline_workspace_bytes(C.byref(p), self.n_groups, int(max_clusters_group), int(max_start_hits_group),
@@ -527,6 +528,12 @@ class Pipeline:
         py = (C.c_void_p * ns)(*[ptr(a) for a in y]); pz = (C.c_void_p * ns)(*[ptr(a) for a in z])
         pr = (C.c_void_p * ns)(*[ptr(a) for a in row])
         views = (_View * ns)()
+        if dev:
+            # the groups copy the inputs on their own streams: order those copies after whatever the caller's current
+            # stream still has queued on the tensors (a kernel writing them, an asynchronous upload)
+            cur = self._torch.cuda.current_stream(self.device)
+            for s in self._streams:
+                s.wait_stream(cur)
         rc = self._lib.tpcca_pipeline_run(self._h, n, py, pz, pr, MEM_DEVICE if dev else MEM_HOST, int(stage_mask), int(what), views)
         if rc:
             raise TpccaError(rc, self._lib.tpcca_pipeline_last_error(self._h).decode())
