@@ -64,7 +64,10 @@ extern "C" {
 #define TPCCA_STAGE_START      0x08u
 #define TPCCA_STAGE_TRACKLETS  0x10u
 #define TPCCA_STAGE_ALL        0x1Fu   /* the five stages of the hot path (BASELINE.json:5)             */
-#define TPCCA_STAGE_SELECT     0x20u   /* S6 tracklet selector; needs S1-S5           */
+#define TPCCA_STAGE_SELECT     0x20u   /* S6 tracklet selector; needs S1-S5.  Limit: fewer than  */
+                                       /* 2^23 = 8 388 608 tracklets per sector (the ownership key holds the track   */
+                                       /* number in 23 bits); beyond, tpcca_sync reports TPCCA_E_WORKSPACE.  The 4e8  */
+                                       /* cluster time frame has about 0.9 M per sector.                            */
 #define TPCCA_STAGE_RESIDUALS  0x40u   /* S7 cluster residuals to the selected tracks; needs S1-S6 */
 #define TPCCA_STAGE_MERGE      0x80u   /* S8 cross-sector merging + chain refit; needs S1-S7       */
 

@@ -185,8 +185,9 @@ def compare_merge(tracker, tf, precision="f32") -> dict:
     from paper_2208_07412_b200 import binding as B
     res, mg = run_timeframe_merged(tf, precision)
     tot = dict(sectors=0, n_selected=0, n_links=0, n_chains=0, par_bit_exact=True, cov_bit_exact=True)
+    gm = [tracker.get_tracks(s, B.OUT_MERGE | B.OUT_SELECTION).merge for s in range(tf.n_sectors)]
     for s in range(tf.n_sectors):
-        g = tracker.get_tracks(s, B.OUT_MERGE | B.OUT_SELECTION).merge
+        g = gm[s]
         m = mg[s]
         rep = {}
         try:
@@ -202,15 +203,18 @@ def compare_merge(tracker, tf, precision="f32") -> dict:
                 _eq("mg_" + f, g[f][h], getattr(m, f), rep)
             _eq("mg_x_ref", g["x_ref"][h], m.x_ref.astype(np.float32), rep)
             _eq("mg_z_ref", g["z_ref"][h], m.z_ref.astype(np.float32), rep)
-            # the chain of every head, rebuilt from the GPU's links, equals the oracle's segment list
+            # the chain of every head, walked along the TRACKER's next links (gm, never the oracle's mg), equals the
+            # oracle's segment list
             for k, ih in enumerate(h):
                 segs = [(s, int(ih))]
-                while True:
+                while len(segs) <= 4 * tf.n_sectors:          # a cycle in the GPU's links would fail the comparison below
                     a, b = segs[-1]
-                    ma = mg[a]
-                    if ma.next_sec[b] < 0:
+                    ga = gm[a]
+                    if ga is None:
+                        raise ParityError(f"chain of head {ih} enters sector {a}, which delivered no S8 outputs")
+                    if ga["next_sec"][b] < 0:
                         break
-                    segs.append((int(ma.next_sec[b]), int(ma.next_trk[b])))
+                    segs.append((int(ga["next_sec"][b]), int(ga["next_trk"][b])))
                 want = list(zip(m.seg_sec[m.seg_offset[k]:m.seg_offset[k + 1]].tolist(), m.seg_trk[m.seg_offset[k]:m.seg_offset[k + 1]].tolist()))
                 if segs != want:
                     raise ParityError(f"chain of head {ih}: {segs} vs {want}")

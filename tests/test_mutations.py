@@ -1,16 +1,33 @@
-"""Mutation check of the oracle pins (not collected by pytest; run by hand: python tests/mutation_check.py [k ...]).
+"""Mutation check of the oracle pins: every one-line mutation of the oracle must fail at least one pin.
 
-Applies one-line mutations of the S5 decisions / constants to a COPY of oracle/tpcca_oracle.cpp under /tmp
-and runs tests/test_oracle_pins.py against each copy: every mutation must be CAUGHT by at least one pin
-(VERDICT r1, weak #1).  The oracle in the repository is never modified.  Last run: tests/MUTATIONS.md."""
-import os, shutil, subprocess, sys
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))   # repo root (this file lives in tests/)
+Each case copies oracle/, tpcsynth/ and tests/ to a temporary directory, changes ONE line of the copy of
+oracle/tpcca_oracle.cpp (a decision, a sign, a constant, a tie-break of S5-S8) and runs tests/test_oracle_pins.py
+on the copy: the run must FAIL.  A mutation that survives marks a decision no pin fixes.  The oracle in the
+repository is never modified.  Mutations 0-15: the S5 decisions and constants; 16-34: S6 (selector), S7
+(residuals), S8 (cross-sector merging).
+
+Slow (a rebuild of the oracle and a run of the pins per mutation, ~10 minutes in all): collected always, run only
+with `python -m pytest tests/test_mutations.py --slow` (tests/conftest.py).  Last full run: profiles/r3_mutations.md.
+"""
+import os
+import shutil
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
 def nth(s, old, new, k):
+    """s with the k-th (0-based) occurrence of `old` replaced by `new`."""
     i = -1
     for _ in range(k + 1):
         i = s.index(old, i + 1)
     return s[:i] + new + s[i + len(old):]
-M = [
+
+
+MUTATIONS = [
  ("B gap >=", lambda s: nth(s, "if (++gap > max_gap) break;", "if (++gap >= max_gap) break;", 0)),
  ("C gap >=", lambda s: nth(s, "if (++gap > max_gap) break;", "if (++gap >= max_gap) break;", 1)),
  ("A gate from 4th", lambda s: s.replace("if (s.n >= 2 && dist2(s, ym, zm) > gate) break;", "if (s.n >= 3 && dist2(s, ym, zm) > gate) break;")),
@@ -47,19 +64,35 @@ M = [
  ("S8 dy window strict", lambda s: s.replace("if (!(std::fabs(dy) <= A.mg_dy && ", "if (!(std::fabs(dy) < A.mg_dy && ")),
  ("S8 tie -> larger sector/track", lambda s: s.replace("    if (sec != b.sec) return sec < b.sec;\n    return trk < b.trk;", "    if (sec != b.sec) return sec > b.sec;\n    return trk > b.trk;")),
 ]
-src = open(os.path.join(ROOT, "oracle", "tpcca_oracle.cpp")).read()
-only = sys.argv[1:]
-for k, (name, fn) in enumerate(M):
-    if only and str(k) not in only: continue
-    d = f"/tmp/mut_{k}"
-    shutil.rmtree(d, ignore_errors=True)
-    os.makedirs(d)
+
+
+def run_pins_on_copy(tmp, mutate):
     for sub in ("oracle", "tpcsynth", "tests"):
-        shutil.copytree(os.path.join(ROOT, sub), os.path.join(d, sub), ignore=shutil.ignore_patterns("*.so", "__pycache__", "test_gpu*", "test_abi*", "test_multirank*"))
-    m = fn(src)
-    assert m != src, name
-    open(os.path.join(d, "oracle", "tpcca_oracle.cpp"), "w").write(m)
-    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_oracle_pins.py", "-q", "-x", "-p", "no:cacheprovider"], cwd=d, capture_output=True, text=True)
-    tail = [l for l in r.stdout.splitlines() if l.startswith("FAILED") or "passed" in l or "failed" in l]
-    print(f"[{k}] {name}: {'CAUGHT' if r.returncode else 'SURVIVES'} :: {' | '.join(tail)[:200]}", flush=True)
-    shutil.rmtree(d, ignore_errors=True)
+        shutil.copytree(os.path.join(ROOT, sub), os.path.join(tmp, sub),
+                        ignore=shutil.ignore_patterns("*.so", "__pycache__", "test_gpu*", "test_abi*", "test_multirank*",
+                                                      "test_zz*", "test_mutations*"))
+    path = os.path.join(tmp, "oracle", "tpcca_oracle.cpp")
+    src = open(path).read()
+    out = mutate(src)
+    open(path, "w").write(out)
+    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_oracle_pins.py", "-q", "-x", "-p", "no:cacheprovider"],
+                       cwd=str(tmp), capture_output=True, text=True)
+    tail = [l for l in r.stdout.splitlines() if l.startswith("FAILED") or " passed" in l or " failed" in l]
+    return src != out, r.returncode, " | ".join(tail)[:300]
+
+
+@pytest.mark.slow
+def test_unmutated_copy_passes(tmp_path):
+    """The harness itself: an unchanged copy passes every pin (so a failing mutated copy means the mutation)."""
+    changed, rc, tail = run_pins_on_copy(str(tmp_path), lambda s: s)
+    assert not changed and rc == 0, tail
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("k", range(len(MUTATIONS)), ids=[f"{k}-{m[0]}".replace(" ", "_") for k, m in enumerate(MUTATIONS)])
+def test_mutation_is_caught(tmp_path, k):
+    name, mutate = MUTATIONS[k]
+    changed, rc, tail = run_pins_on_copy(str(tmp_path), mutate)
+    assert changed, f"mutation '{name}' no longer applies: the oracle line it edits has changed"
+    assert rc != 0, f"mutation '{name}' SURVIVES every pin: {tail}"
+    print(f"[{k}] {name}: CAUGHT :: {tail}")
