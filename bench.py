@@ -202,9 +202,9 @@ def _oracle_timed_job(job):
 
 def _oracle_output_job(job):
     """Worker: the full OracleResult of one sector, S6 / S7 included, for the parity check (not timed)."""
-    params, y, z, row = job
+    params, y, z, row = job[:4]
     from oracle import Oracle
-    return Oracle(params).run(y, z, row, stage_mask=0x7F)
+    return Oracle(params).run(y, z, row, stage_mask=job[4] if len(job) > 4 else 0x7F)
 
 
 def merge_properties(trk, tf, B):
@@ -301,6 +301,81 @@ def cpu_baseline_and_parity(args, tf, trk):
         parity["links_differing"] += rep["links_differing"]
         parity["par_bit_exact"] = bool(parity["par_bit_exact"] and rep.get("par_bit_exact", True))
     return cpu, parity
+
+
+def footprint_leg(args, env, peaks):
+    """The footprint BASELINE.json:10 names for the headline workload ("about 4e8 clusters (~8 GB fp32 SoA)"): the
+    generator text of configs[3] yields 1.45e8 clusters ("discrepancy to carry forward"), so the
+    same recipe is run once more at mult_scale 2.75 (~4e8 clusters): W warm-ups + 3 timed steps of S1-S5 on
+    device-resident inputs, per-stage times, the S2 roofline fraction, and an element-by-element parity check of two
+    sectors (one per side) against the oracle.  Called after the main legs have released their contexts."""
+    import copy
+    import multiprocessing as mp
+    import tpcsynth
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from oracle import Oracle
+    from parity import compare_sector
+    B = env.B
+    a = copy.copy(args)
+    a.mult_scale = args.footprint_scale
+    t0 = time.time()
+    tf = tpcsynth.generate(a.config, seed=rank_seed(a.config, a.seed, 0), mult_scale=a.mult_scale)
+    gen_s = time.time() - t0
+    N = tf.n_clusters
+    sectors = [0, tf.n_sectors // 2] if tf.n_sectors > 1 else [0]
+    pool = mp.get_context("spawn").Pool(len(sectors))       # the oracle starts on its sectors while the GPU leg runs
+    orc_async = pool.map_async(_oracle_output_job, [(tf.params, tf.y[s], tf.z[s], tf.row[s], 0x1F) for s in sectors], chunksize=1)
+    trk = env.tracker(tf.params, N, N // 8 + 1024)
+    devin = [(env.to_device(env.pin(tf.y[s])), env.to_device(env.pin(tf.z[s])), env.to_device(env.pin_u16(tf.row[s])))
+             for s in range(tf.n_sectors)]
+    trk.reset()
+    for s, (y, z, r) in enumerate(devin):
+        trk.load_clusters(s, y, z, r, borrow=True)
+    for _ in range(args.warmup):
+        trk.run()
+    trk.sync()
+    steps = 3
+    ev0, ev1 = env.event(), env.event()
+    env.synchronize()
+    ev0.record()
+    for _ in range(steps):
+        trk.run()
+    ev1.record()
+    env.synchronize()
+    ms = ev0.elapsed_time(ev1) / steps
+    trk.sync()
+    stage_ms = np.mean([trk.timings(i) for i in range(steps)], axis=0)
+    counts = trk.counts()
+    s2_bytes = 16.0 * N + 4.0 * counts["n_bins"] * tf.n_sectors
+    s2_gbs = s2_bytes / (stage_ms[1] * 1e-3) / 1e9
+    res = dict(workload=workload_name(a, tf), n_clusters=N, soa_bytes=int(18 * N), steps=steps, warmup=args.warmup,
+               ms_per_step=ms, value=N / (ms * 1e-3), unit=UNIT, n_start=counts["n_start"], n_tracks=counts["n_tracks"],
+               stage_ms=dict(zip(("S1_grid", "S2_neighbours", "S3_clean", "S4_start", "S5_tracklets", "total"),
+                                 (round(float(v), 4) for v in stage_ms))),
+               roofline=dict(kernel="S2 neighbour finder", bound="hbm", achieved=s2_gbs, peak=peaks["hbm_gbs"], unit="GB/s",
+                             frac=s2_gbs / peaks["hbm_gbs"], algorithmic_bytes=s2_bytes),
+               generate_s=round(gen_s, 1))
+    parity = dict(sectors=sectors, n_clusters=0, n_tracks=0, links_differing=0, par_bit_exact=True, status="pass")
+    t0 = time.time()
+    outs = orc_async.get()
+    pool.close()
+    parity["oracle_wait_s"] = round(time.time() - t0, 1)
+    orc = Oracle(tf.params)
+    for s, o in zip(sectors, outs):
+        g = trk.get_tracks(s, B.OUT_ALL)
+        try:
+            rep = compare_sector(g, o, orc, tf.row[s][o.order])
+        except AssertionError as e:
+            parity.update(status="FAIL", error=f"sector {s}: {str(e)[:300]}")
+            break
+        parity["n_clusters"] += int(o.n); parity["n_tracks"] += int(o.n_tracks)
+        parity["links_differing"] += rep["links_differing"]
+        parity["par_bit_exact"] = bool(parity["par_bit_exact"] and rep.get("par_bit_exact", True))
+    res["parity"] = parity
+    trk.close()
+    devin.clear()
+    env.empty_cache()
+    return res
 
 
 # --------------------------------------------------------------------------------------------------
@@ -599,6 +674,19 @@ def run_tpcca(args, env_cls=CudaEnv):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu, parity = cpu_baseline_and_parity(args, tf, trk)
 
+    # ---- the ~4e8-cluster footprint BASELINE.json:10 names, as a short extra leg (rank 0, N = 1, default workload) ----
+    footprint = None
+    if (rank == 0 and world == 1 and args.footprint_scale > 0 and args.config == 3 and args.mult_scale == 1.0
+            and not args.no_cpu_baseline):
+        trk.close()
+        devin.clear(); host.clear()
+        hy = hz = hr = None
+        env.empty_cache()
+        try:
+            footprint = footprint_leg(args, env, peaks)
+        except env.oom_error as e:
+            footprint = dict(status="FAIL", error=f"out of memory: {str(e)[:200]}")
+
     if rank == 0:
         line = dict(
             metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
@@ -630,7 +718,7 @@ def run_tpcca(args, env_cls=CudaEnv):
                                             streaming_value=(n_all * e2e_n / (e2e_sel_stream_ms * 1e-3) if e2e_sel_stream_ms else None),
                                             streaming_ms_per_step=(e2e_sel_stream_ms / e2e_n if e2e_sel_stream_ms else None))),
             gpu_launches=int(launches_per_step * args.steps),
-            clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1),
+            clocks=clocks, cpu_baseline=cpu, parity=parity, generate_s=round(gen_s, 1), footprint_4e8=footprint,
         )
         print(json.dumps(line), flush=True)
     trk.close()
@@ -669,6 +757,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sectors", type=int, default=36, help="sectors the CPU baseline (the oracle) is timed on; default: all")
     ap.add_argument("--parity-sectors", type=int, default=8, help="sectors of the full-size parity check against the oracle")
+    ap.add_argument("--footprint-scale", type=float, default=2.75,
+                    help="mult_scale of the extra ~4e8-cluster footprint leg of the default workload (0: off)")
     ap.add_argument("--no-streaming", action="store_true", help="e2e with one context only")
     ap.add_argument("--pipeline-groups", type=int, default=3, help="sector groups of the tpcca_pipeline e2e leg (0/1: off)")
     ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts (time frames in flight) of the streaming e2e mode")

@@ -695,6 +695,77 @@ def test_merge_config1_and_config4(pkg, cfg1_small):
         trk.close()
 
 
+def _mirror_track(rows, y0, sign, z0=100.0):
+    """Clusters of one straight-ish track on rows [rows[0], rows[1]): y = sign * (y0 + eps_row) with dyadic eps, z = z0.
+    sign = -1 is the exact y mirror image (negation is exact in every operation of the filter); y0 = 0: y == 0."""
+    rows = np.arange(*rows)
+    eps = ((rows * 7) % 5 - 2) / 64.0 if y0 else 0.0
+    return rows.astype(np.uint16), (sign * (y0 + eps) * np.ones(len(rows))).astype(np.float32), np.full(len(rows), z0, np.float32)
+
+
+def test_merge_ties_through_real_clusters(pkg):
+    """The S8 tie-breaks of the CUDA path (the 64-bit atomicMin key order of k_mg_match), through real clusters.
+    Three sectors of one side with the identity as sector rotation: a track at y == 0 has two partner candidates that
+    are exact y-mirror images of each other (+-2 cm), so dy and ds tie bit for bit and the score ties; the definition
+    picks the smaller sector, then the smaller track.  Ties for next() (two upper candidates) and for
+    prev() (two lower candidates), within one neighbour sector and across the two neighbour sectors (either way round:
+    the kernel visits sector 2 before sector 0)."""
+    from oracle import run_timeframe_merged
+    from parity import compare_merge
+    P = tpcsynth.default_params(n_sectors=3).copy(sectors_per_side=3, sector_cos=1.0, sector_sin=0.0, mg_dy=4.0)
+    LO, UP = (5, 41), (43, 80)
+    #        centre track     first candidate   its mirror image    expected partner (sector, track)
+    cases = [((1, LO, 0.0, 1), (2, UP, 2.0, 1), (2, UP, 2.0, -1), "next", (2, 0)),
+             ((1, LO, 0.0, 1), (2, UP, 2.0, 1), (0, UP, 2.0, -1), "next", (0, 0)),
+             ((1, LO, 0.0, 1), (0, UP, 2.0, 1), (2, UP, 2.0, -1), "next", (0, 0)),
+             ((1, UP, 0.0, 1), (0, LO, 2.0, 1), (0, LO, 2.0, -1), "prev", (0, 0)),
+             ((1, UP, 0.0, 1), (0, LO, 2.0, 1), (2, LO, 2.0, -1), "prev", (0, 0)),
+             ((1, UP, 0.0, 1), (2, LO, 2.0, 1), (0, LO, 2.0, -1), "prev", (0, 0))]
+    for *placement, which, want in cases:
+        secs = [([], [], []) for _ in range(3)]
+        for sec, rows, y0, sign in placement:
+            r, y, z = _mirror_track(rows, y0, sign)
+            secs[sec][0].append(y); secs[sec][1].append(z); secs[sec][2].append(r)
+        cat = lambda l, dt: np.concatenate(l).astype(dt) if l else np.zeros(0, dt)
+        tf = ArrTF(P, [(cat(a, np.float32), cat(b, np.float32), cat(c, np.uint16)) for a, b, c in secs])
+        # the premise, on the oracle: the two candidates are fitted to exact mirror images, and the tie goes to `want`
+        res, mg = run_timeframe_merged(tf, "f32")
+        cand = [res[sec].par[res[sec].selected] for sec, *_ in placement[1:]]
+        both = np.concatenate(cand) if placement[1][0] != placement[2][0] else cand[0]
+        assert both.shape == (2, 5) and np.array_equal(both[0] * [-1, 1, -1, 1, -1], both[1]) and both[0, 0] != 0.0
+        m1 = mg[1]
+        got = (int(m1.next_sec[0]), int(m1.next_trk[0])) if which == "next" else (int(m1.prev_sec[0]), int(m1.prev_trk[0]))
+        assert got == want, (placement, got, want)
+        # the CUDA path makes the same choice (links bit-exact, chains and refits compared as everywhere)
+        trk = pkg.Tracker(P, max_clusters=tf.n_clusters, workspace_fill=WS_FILL)
+        trk.load_timeframe(tf)
+        trk.run(0xFF)
+        trk.sync()
+        rep = compare_merge(trk, tf)
+        assert rep["n_links"] == 1 and rep["n_chains"] == 1, rep
+        trk.close()
+
+
+def test_merge_full_occupancy_three_sectors(pkg):
+    """S8 against the oracle at the FULL occupancy of the time-frame configs (the bench checks S8 at full size by
+    properties only: the oracle's all-pairs matching is out of reach over 36 sectors x 128 orbits).  Three neighbouring
+    sectors of BASELINE.json configs[2] at full size (32 orbits at 50 kHz: the same clusters per cm of drift as
+    configs[3]), ~1.35 M clusters and ~19 k selected tracks each, as a three-sector side: ~2e9 pair tests in the oracle.
+    Links bit-exact, chains walked along the tracker's links, refits within 1e-4."""
+    from parity import compare_merge
+    full = tpcsynth.generate(2)
+    P = full.params.copy(n_sectors=3, sectors_per_side=3)
+    tf = ArrTF(P, [(full.y[s], full.z[s], full.row[s]) for s in (0, 1, 2)])
+    assert tf.n_clusters > 3_000_000
+    trk = pkg.Tracker(P, max_clusters=tf.n_clusters, workspace_fill=WS_FILL)
+    trk.load_timeframe(tf)
+    trk.run(0xFF)
+    trk.sync()
+    rep = compare_merge(trk, tf)
+    assert rep["n_selected"] > 50_000 and rep["n_links"] > 15_000 and rep["n_chains"] > 12_000, rep
+    trk.close()
+
+
 def test_merge_time_frame_and_degenerate_layouts(pkg):
     """Several collisions along the 128-orbit z axis (candidate index over 900+ z buckets); sector layouts without a
     neighbour relation (1 or 3 sectors: S8 is a no-op) and with two sectors per side."""
